@@ -1,0 +1,154 @@
+/* fs.h -- C ABI of the B200-native hot path of arXiv 1702.08734
+ * ("Billion-scale similarity search with GPUs"): per-query k-selection fused
+ * with distance computation.
+ *
+ * Citations "P:L<n>" are line numbers of the paper text.
+ *
+ * General conventions (the paper is silent on all of them):
+ *  - Every data pointer is a DEVICE pointer unless its comment says "host".
+ *    The caller owns all inputs, outputs and workspaces; the library owns only
+ *    the opaque fs_ivfpq object and the inverted lists inside it.
+ *  - Work is enqueued on the given stream (a cudaStream_t cast to void*; NULL is
+ *    the legacy default stream); outputs are valid once that stream is
+ *    synchronised.  The *_host entry points are the exception: they take HOST
+ *    pointers, copy in, run, copy out and synchronise before returning.
+ *  - Every function returns FS_OK or an error code; nothing throws or aborts
+ *    across the ABI.  Arguments are validated before any launch;
+ *    fs_last_error() gives a thread-local detail string for the last failure.
+ *  - Results are ascending by distance/value; ties by lower index/id.  When
+ *    fewer than k candidates exist the tail is (+INF, -1) (the +inf sentinel
+ *    convention of P:L220).  Distances are SQUARED L2 (D is squared, P:L52;
+ *    Eq. 7/10).
+ *  - Workspaces: if ws == NULL the library allocates and frees a stream-ordered
+ *    temporary itself; otherwise ws must hold at least the matching *_ws_bytes.
+ */
+#ifndef FS_H_
+#define FS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fs_ivfpq fs_ivfpq; /* opaque, library-owned */
+typedef void* fs_stream;          /* cudaStream_t */
+
+enum {
+  FS_OK = 0,
+  FS_EINVAL = 1,       /* bad argument (NULL pointer, negative size, ld < n, d % M != 0 ...) */
+  FS_EUNSUPPORTED = 2, /* outside the supported range (k > 1024, d too large ...) */
+  FS_ENOMEM = 3,       /* allocation failed or ws_bytes too small */
+  FS_ECUDA = 4,        /* a CUDA call failed; fs_last_error() has the CUDA string */
+  FS_ESTATE = 5        /* index not in the state the call needs (no quantizers ...) */
+};
+
+#define FS_MAX_K 1024 /* "it supports k <= 1024" */
+
+const char* fs_last_error(void);
+/* Library version and the SM architecture it was compiled for ("sm_100a"). */
+const char* fs_version(void);
+/* Number of kernel launches this thread's calls have enqueued since the last
+ * fs_reset_launch_count(); used by bench.py to fill "gpu_launches". */
+int64_t fs_launch_count(void);
+void fs_reset_launch_count(void);
+
+/* --------------------------------------------------------------------------
+ * k-selection (WarpSelect, section 4.2; k = 1 is a
+ * reduction; long rows by decomposition).
+ * For each of n_rows arrays [a_i], i = 0..n-1, the k lowest values ascending
+ * with their indices; ties broken by lower index, -0 == +0, NaN (not expected)
+ * orders after +INF.  Bit-exact: out_val holds the original fp32 bits.
+ *   rows     device fp32 [n_rows][ld], row-major, ld >= n
+ *   out_val  device fp32 [n_rows][k];  out_idx device int32 [n_rows][k]
+ *   1 <= k <= FS_MAX_K; n < 2^31; k > n pads with (+INF, -1).
+ * n_rows == 0 or n == 0 is valid (n == 0 writes only padding).
+ * ------------------------------------------------------------------------ */
+int fs_kselect(const float* rows, int64_t n_rows, int64_t n, int64_t ld, int k, float* out_val,
+               int32_t* out_idx, void* ws, size_t ws_bytes, fs_stream stream);
+size_t fs_kselect_ws_bytes(int64_t n_rows, int64_t n, int k);
+/* Same with HOST buffers (copies in and out, synchronises). */
+int fs_kselect_host(const float* rows_host, int64_t n_rows, int64_t n, int64_t ld, int k,
+                    float* out_val_host, int32_t* out_idx_host);
+
+/* --------------------------------------------------------------------------
+ * Exact squared-L2 k-NN (Eq. 1-2; computation layout 5.1):
+ * norms (B1), the -2<x,y> tile contraction (B2), "+||y||^2 then k-select" as the
+ * tile epilogue (B3: the nq x nb matrix never reaches HBM), merge of the partial
+ * lists of database chunks and "+||x||^2" (B4).
+ *   xq device fp32 [nq][d], xb device fp32 [nb][d], row-major, contiguous
+ *   out_dist device fp32 [nq][k] (full squared distance, clamped at 0)
+ *   out_ids  device int64 [nq][k]
+ *   1 <= k <= FS_MAX_K; 1 <= d <= 2048; nb < 2^31.
+ * Arithmetic: fp32 (FFMA) or 3xTF32-split tensor-core products with fp32
+ * accumulation; |dist - exact| <= 1e-4 (||x||^2 + ||y||^2).
+ * ------------------------------------------------------------------------ */
+int fs_flat_l2_knn(const float* xq, int64_t nq, const float* xb, int64_t nb, int d, int k,
+                   float* out_dist, int64_t* out_ids, void* ws, size_t ws_bytes,
+                   fs_stream stream);
+size_t fs_flat_l2_knn_ws_bytes(int64_t nq, int64_t nb, int d, int k);
+int fs_flat_l2_knn_host(const float* xq_host, int64_t nq, const float* xb_host, int64_t nb, int d,
+                        int k, float* out_dist_host, int64_t* out_ids_host);
+
+/* --------------------------------------------------------------------------
+ * IVFADC index with 8-bit residual product quantizer (Eq. 3-7, P:L59-90;
+ * layout 5.2-5.3, Alg. 4).
+ *   d % M == 0, 1 <= M <= 64, nlist >= 1, 256 codewords per
+ *   sub-quantizer; sub-vector m = dimensions [m*d/M, (m+1)*d/M).
+ * ------------------------------------------------------------------------ */
+int fs_ivfpq_create(fs_ivfpq** out, int d, int nlist, int M);
+int fs_ivfpq_destroy(fs_ivfpq* index);
+
+/* Quantizers: coarse centroids [nlist][d] and PQ codebooks [M][256][d/M], device
+ * fp32; copied in / out.  The oracle and the library share these arrays. */
+int fs_ivfpq_set_quantizers(fs_ivfpq* index, const float* coarse, const float* pq,
+                            fs_stream stream);
+int fs_ivfpq_get_quantizers(const fs_ivfpq* index, float* coarse, float* pq, fs_stream stream);
+
+/* k-means training of both quantizers on n device vectors x [n][d] (
+ * assignment = exact search with k = 1).  Off the parity path: the
+ * resulting arrays are what both sides use. */
+int fs_ivfpq_train(fs_ivfpq* index, const float* x, int64_t n, int niter, uint64_t seed,
+                   fs_stream stream);
+
+/* Add (D1-D3): coarse assignment q1(y) = argmin_c ||y - c||^2 by the flat
+ * kernel with k = 1, residual PQ encoding (Eq. 3; byte
+ * m = sub-quantizer m), append of (code, id) to list q1(y).
+ *   xb device fp32 [n][d]; ids device int64 [n] or NULL (ids ntotal..ntotal+n-1).
+ * Lists keep append order (ascending id when ids are added ascending).
+ * Needs exclusive access to the index. */
+int fs_ivfpq_add(fs_ivfpq* index, const float* xb, int64_t n, const int64_t* ids,
+                 fs_stream stream);
+
+/* Search (C1-C5, Alg. 4): coarse top-nprobe (Eq. 5), per-(query,
+ * list) lookup tables in shared memory (Eq. 10), inverted-list code
+ * scan with fused pass-1 selection, pass-2 merge to k and id
+ * resolution for the winners only.
+ *   xq device fp32 [nq][d]; 1 <= nprobe <= min(nlist, 1024); 1 <= k <= FS_MAX_K
+ *   out_dist device fp32 [nq][k] (squared ADC distance), out_ids device int64 [nq][k]
+ *   out_probed device int32 [nq][nprobe] ascending coarse distance, or NULL. */
+int fs_ivfpq_search(fs_ivfpq* index, const float* xq, int64_t nq, int nprobe, int k,
+                    float* out_dist, int64_t* out_ids, int32_t* out_probed, void* ws,
+                    size_t ws_bytes, fs_stream stream);
+size_t fs_ivfpq_search_ws_bytes(const fs_ivfpq* index, int64_t nq, int nprobe, int k);
+int fs_ivfpq_search_host(fs_ivfpq* index, const float* xq_host, int64_t nq, int nprobe, int k,
+                         float* out_dist_host, int64_t* out_ids_host);
+
+int64_t fs_ivfpq_ntotal(const fs_ivfpq* index);
+/* Total code bytes the probed lists of the last fs_ivfpq_search held
+ * (sum over (query, list) pairs of len * M): the scan's algorithmic bytes. */
+int64_t fs_ivfpq_last_scanned_codes(const fs_ivfpq* index);
+/* Read-only device views of one list, valid until the next add/destroy. */
+int fs_ivfpq_list(const fs_ivfpq* index, int list_no, const uint8_t** codes, const int64_t** ids,
+                  int64_t* len);
+/* The whole inverted file in CSR form, copied to caller buffers (device):
+ * offsets int64 [nlist+1], codes uint8 [ntotal][M], ids int64 [ntotal]; any of
+ * the three may be NULL. */
+int fs_ivfpq_export(const fs_ivfpq* index, int64_t* offsets, uint8_t* codes, int64_t* ids,
+                    fs_stream stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FS_H_ */
