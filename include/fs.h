@@ -28,6 +28,12 @@
 #include <stddef.h>
 #include <stdint.h>
 
+#if defined(__GNUC__)
+#define FS_API __attribute__((visibility("default")))
+#else
+#define FS_API
+#endif
+
 #ifdef __cplusplus
 extern "C" {
 #endif
@@ -46,13 +52,13 @@ enum {
 
 #define FS_MAX_K 1024 /* "it supports k <= 1024" */
 
-const char* fs_last_error(void);
+FS_API const char* fs_last_error(void);
 /* Library version and the SM architecture it was compiled for ("sm_100a"). */
-const char* fs_version(void);
+FS_API const char* fs_version(void);
 /* Number of kernel launches this thread's calls have enqueued since the last
  * fs_reset_launch_count(); used by bench.py to fill "gpu_launches". */
-int64_t fs_launch_count(void);
-void fs_reset_launch_count(void);
+FS_API int64_t fs_launch_count(void);
+FS_API void fs_reset_launch_count(void);
 
 /* --------------------------------------------------------------------------
  * k-selection (WarpSelect, section 4.2; k = 1 is a
@@ -65,11 +71,11 @@ void fs_reset_launch_count(void);
  *   1 <= k <= FS_MAX_K; n < 2^31; k > n pads with (+INF, -1).
  * n_rows == 0 or n == 0 is valid (n == 0 writes only padding).
  * ------------------------------------------------------------------------ */
-int fs_kselect(const float* rows, int64_t n_rows, int64_t n, int64_t ld, int k, float* out_val,
+FS_API int fs_kselect(const float* rows, int64_t n_rows, int64_t n, int64_t ld, int k, float* out_val,
                int32_t* out_idx, void* ws, size_t ws_bytes, fs_stream stream);
-size_t fs_kselect_ws_bytes(int64_t n_rows, int64_t n, int k);
+FS_API size_t fs_kselect_ws_bytes(int64_t n_rows, int64_t n, int k);
 /* Same with HOST buffers (copies in and out, synchronises). */
-int fs_kselect_host(const float* rows_host, int64_t n_rows, int64_t n, int64_t ld, int k,
+FS_API int fs_kselect_host(const float* rows_host, int64_t n_rows, int64_t n, int64_t ld, int k,
                     float* out_val_host, int32_t* out_idx_host);
 
 /* --------------------------------------------------------------------------
@@ -84,11 +90,11 @@ int fs_kselect_host(const float* rows_host, int64_t n_rows, int64_t n, int64_t l
  * Arithmetic: fp32 (FFMA) or 3xTF32-split tensor-core products with fp32
  * accumulation; |dist - exact| <= 1e-4 (||x||^2 + ||y||^2).
  * ------------------------------------------------------------------------ */
-int fs_flat_l2_knn(const float* xq, int64_t nq, const float* xb, int64_t nb, int d, int k,
+FS_API int fs_flat_l2_knn(const float* xq, int64_t nq, const float* xb, int64_t nb, int d, int k,
                    float* out_dist, int64_t* out_ids, void* ws, size_t ws_bytes,
                    fs_stream stream);
-size_t fs_flat_l2_knn_ws_bytes(int64_t nq, int64_t nb, int d, int k);
-int fs_flat_l2_knn_host(const float* xq_host, int64_t nq, const float* xb_host, int64_t nb, int d,
+FS_API size_t fs_flat_l2_knn_ws_bytes(int64_t nq, int64_t nb, int d, int k);
+FS_API int fs_flat_l2_knn_host(const float* xq_host, int64_t nq, const float* xb_host, int64_t nb, int d,
                         int k, float* out_dist_host, int64_t* out_ids_host);
 
 /* --------------------------------------------------------------------------
@@ -97,19 +103,19 @@ int fs_flat_l2_knn_host(const float* xq_host, int64_t nq, const float* xb_host, 
  *   d % M == 0, 1 <= M <= 64, nlist >= 1, 256 codewords per
  *   sub-quantizer; sub-vector m = dimensions [m*d/M, (m+1)*d/M).
  * ------------------------------------------------------------------------ */
-int fs_ivfpq_create(fs_ivfpq** out, int d, int nlist, int M);
-int fs_ivfpq_destroy(fs_ivfpq* index);
+FS_API int fs_ivfpq_create(fs_ivfpq** out, int d, int nlist, int M);
+FS_API int fs_ivfpq_destroy(fs_ivfpq* index);
 
 /* Quantizers: coarse centroids [nlist][d] and PQ codebooks [M][256][d/M], device
  * fp32; copied in / out.  The oracle and the library share these arrays. */
-int fs_ivfpq_set_quantizers(fs_ivfpq* index, const float* coarse, const float* pq,
+FS_API int fs_ivfpq_set_quantizers(fs_ivfpq* index, const float* coarse, const float* pq,
                             fs_stream stream);
-int fs_ivfpq_get_quantizers(const fs_ivfpq* index, float* coarse, float* pq, fs_stream stream);
+FS_API int fs_ivfpq_get_quantizers(const fs_ivfpq* index, float* coarse, float* pq, fs_stream stream);
 
 /* k-means training of both quantizers on n device vectors x [n][d] (
  * assignment = exact search with k = 1).  Off the parity path: the
  * resulting arrays are what both sides use. */
-int fs_ivfpq_train(fs_ivfpq* index, const float* x, int64_t n, int niter, uint64_t seed,
+FS_API int fs_ivfpq_train(fs_ivfpq* index, const float* x, int64_t n, int niter, uint64_t seed,
                    fs_stream stream);
 
 /* Add (D1-D3): coarse assignment q1(y) = argmin_c ||y - c||^2 by the flat
@@ -118,7 +124,7 @@ int fs_ivfpq_train(fs_ivfpq* index, const float* x, int64_t n, int niter, uint64
  *   xb device fp32 [n][d]; ids device int64 [n] or NULL (ids ntotal..ntotal+n-1).
  * Lists keep append order (ascending id when ids are added ascending).
  * Needs exclusive access to the index. */
-int fs_ivfpq_add(fs_ivfpq* index, const float* xb, int64_t n, const int64_t* ids,
+FS_API int fs_ivfpq_add(fs_ivfpq* index, const float* xb, int64_t n, const int64_t* ids,
                  fs_stream stream);
 
 /* Search (C1-C5, Alg. 4): coarse top-nprobe (Eq. 5), per-(query,
@@ -128,24 +134,24 @@ int fs_ivfpq_add(fs_ivfpq* index, const float* xb, int64_t n, const int64_t* ids
  *   xq device fp32 [nq][d]; 1 <= nprobe <= min(nlist, 1024); 1 <= k <= FS_MAX_K
  *   out_dist device fp32 [nq][k] (squared ADC distance), out_ids device int64 [nq][k]
  *   out_probed device int32 [nq][nprobe] ascending coarse distance, or NULL. */
-int fs_ivfpq_search(fs_ivfpq* index, const float* xq, int64_t nq, int nprobe, int k,
+FS_API int fs_ivfpq_search(fs_ivfpq* index, const float* xq, int64_t nq, int nprobe, int k,
                     float* out_dist, int64_t* out_ids, int32_t* out_probed, void* ws,
                     size_t ws_bytes, fs_stream stream);
-size_t fs_ivfpq_search_ws_bytes(const fs_ivfpq* index, int64_t nq, int nprobe, int k);
-int fs_ivfpq_search_host(fs_ivfpq* index, const float* xq_host, int64_t nq, int nprobe, int k,
+FS_API size_t fs_ivfpq_search_ws_bytes(const fs_ivfpq* index, int64_t nq, int nprobe, int k);
+FS_API int fs_ivfpq_search_host(fs_ivfpq* index, const float* xq_host, int64_t nq, int nprobe, int k,
                          float* out_dist_host, int64_t* out_ids_host);
 
-int64_t fs_ivfpq_ntotal(const fs_ivfpq* index);
+FS_API int64_t fs_ivfpq_ntotal(const fs_ivfpq* index);
 /* Total code bytes the probed lists of the last fs_ivfpq_search held
  * (sum over (query, list) pairs of len * M): the scan's algorithmic bytes. */
-int64_t fs_ivfpq_last_scanned_codes(const fs_ivfpq* index);
+FS_API int64_t fs_ivfpq_last_scanned_codes(const fs_ivfpq* index);
 /* Read-only device views of one list, valid until the next add/destroy. */
-int fs_ivfpq_list(const fs_ivfpq* index, int list_no, const uint8_t** codes, const int64_t** ids,
+FS_API int fs_ivfpq_list(const fs_ivfpq* index, int list_no, const uint8_t** codes, const int64_t** ids,
                   int64_t* len);
 /* The whole inverted file in CSR form, copied to caller buffers (device):
  * offsets int64 [nlist+1], codes uint8 [ntotal][M], ids int64 [ntotal]; any of
  * the three may be NULL. */
-int fs_ivfpq_export(const fs_ivfpq* index, int64_t* offsets, uint8_t* codes, int64_t* ids,
+FS_API int fs_ivfpq_export(const fs_ivfpq* index, int64_t* offsets, uint8_t* codes, int64_t* ids,
                     fs_stream stream);
 
 #ifdef __cplusplus

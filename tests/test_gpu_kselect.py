@@ -1,0 +1,112 @@
+"""GPU parity: fs_kselect (through the C ABI) vs the oracle, bit-exact in values
+and indices (BASELINE.json: "ties broken by lower index")."""
+import numpy as np
+import pytest
+import torch
+
+import datagen
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+K_ALL = [1, 2, 31, 32, 33, 64, 100, 128, 200, 256, 500, 512, 1000, 1024]
+
+
+def run(rows_np, k, n=None):
+    import paper_1702_08734_b200 as fs
+    rows = torch.from_numpy(rows_np).cuda()
+    val, idx = fs.kselect(rows, k, n=n)
+    torch.cuda.synchronize()
+    return val.cpu().numpy(), idx.cpu().numpy()
+
+
+def assert_exact(rows_np, k, n=None):
+    ev, ei = oracle.kselect(rows_np, k, n=n)
+    gv, gi = run(rows_np, k, n=n)
+    bad = np.nonzero((gi != ei).any(1) | (gv.view(np.uint32) != ev.view(np.uint32)).any(1))[0]
+    assert bad.size == 0, "rows %s differ (k=%d); first: got %s want %s" % (
+        bad[:5], k, gi[bad[0]][:8], ei[bad[0]][:8])
+
+
+@pytest.mark.parametrize("k", K_ALL)
+def test_random_rows_ragged(k):
+    # several 128-element groups, the 4x unrolled body, a vector tail and a scalar tail
+    rows = datagen.kselect_rows(0, 37, 2000 + 3, duplicates=False)
+    assert_exact(rows, k)
+
+
+@pytest.mark.parametrize("k", [1, 32, 128, 1024])
+def test_cfg2_shaped_rows_with_duplicates(k):
+    """cfg2 shape (rows of 16 384) on the rows that carry duplicated runs plus plain ones."""
+    dup, _ = datagen.kselect_dup_rows(0, 10000)
+    sel = list(np.nonzero(dup)[0][:6]) + [0, 1, 2]
+    rows = np.concatenate([datagen.kselect_rows(int(r), 1, 16384) for r in sel])
+    assert_exact(rows, k)
+
+
+@pytest.mark.parametrize("n", [0, 1, 3, 4, 5, 31, 32, 33, 127, 128, 129, 511, 513])
+def test_small_n_and_padding(n):
+    rng = np.random.default_rng(n)
+    rows = rng.integers(0, 5, size=(9, max(n, 1))).astype(np.float32)[:, :max(n, 1)]
+    for k in (1, 4, 32, 40, 300):
+        assert_exact(rows, k, n=n)
+
+
+def test_structured_rows():
+    n = 5000
+    asc = np.arange(n, dtype=np.float32)
+    rows = np.stack([asc, asc[::-1].copy(), np.full(n, 2.5, np.float32),
+                     (np.arange(n) % 7).astype(np.float32), -asc])
+    for k in (1, 10, 128, 1024):
+        assert_exact(rows, k)
+
+
+def test_special_values():
+    rng = np.random.default_rng(0)
+    rows = rng.standard_normal((6, 700)).astype(np.float32)
+    rows[0, ::3] = 0.0
+    rows[0, 1::3] = -0.0
+    rows[1, ::5] = np.inf
+    rows[2, ::4] = -np.inf
+    rows[3, :] = np.inf
+    rows[4, 10:20] = np.nan
+    rows[5, :] = np.nan
+    for k in (1, 5, 64, 700, 1024):
+        assert_exact(rows, k)
+
+
+def test_row_stride_and_misaligned_base():
+    """ld > n and rows that do not start on a 16-byte boundary."""
+    import paper_1702_08734_b200 as fs
+    rng = np.random.default_rng(1)
+    big = rng.random((11, 1003), dtype=np.float32)
+    t = torch.from_numpy(big).cuda()
+    for off, n in [(1, 1000), (2, 997), (3, 900)]:
+        view = t[:, off:off + n]
+        for k in (1, 50, 600):
+            gv, gi = fs.kselect(view, k)
+            ev, ei = oracle.kselect(np.ascontiguousarray(big[:, off:off + n]), k)
+            assert np.array_equal(gi.cpu().numpy(), ei)
+            assert np.array_equal(gv.cpu().numpy().view(np.uint32), ev.view(np.uint32))
+
+
+@pytest.mark.parametrize("k", [1, 100, 1024])
+def test_long_row_is_split(k):
+    """A4: a few long rows go through the chunked passes (P > 1)."""
+    rows = datagen.kselect_rows(50000, 3, 300_001, duplicates=False)
+    rows[1, ::2] = np.floor(rows[1, ::2] * 16) / 16  # ties across chunks
+    assert_exact(rows, k)
+
+
+def test_host_entry_point_and_errors():
+    import paper_1702_08734_b200 as fs
+    rows = datagen.kselect_rows(7, 5, 3000)
+    v, i = fs.kselect_host(rows, 17)
+    ev, ei = oracle.kselect(rows, 17)
+    assert np.array_equal(i, ei) and np.array_equal(v.view(np.uint32), ev.view(np.uint32))
+    t = torch.from_numpy(rows).cuda()
+    with pytest.raises(fs.FsError):
+        fs.kselect(t, 0)
+    with pytest.raises(fs.FsError):
+        fs.kselect(t, 1025)
+    assert fs.kselect(t[:0], 5)[0].shape == (0, 5)
