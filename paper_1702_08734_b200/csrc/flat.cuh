@@ -1,0 +1,33 @@
+// flat.cuh -- internal interface of the exact-search engine (flat.cu), used by
+// the public fs_flat_l2_knn and by the IVFPQ coarse quantizer / add path.
+#pragma once
+
+#include "common.cuh"
+#include "select.cuh"
+
+namespace fs {
+
+struct FlatPlan {
+  int kclass;    // queue class: K = 32 << kclass
+  int K;
+  int S;         // database splits (partial queues per query)
+  int64_t chunk; // database vectors per split
+  size_t off_ynorm, off_xnorm, off_W, bytes;  // workspace layout
+};
+
+FlatPlan flat_plan(int64_t nq, int64_t nb, int d, int k);
+
+// ||row||^2 for n rows of x [n][d] (B1).
+int launch_row_norms(const float* x, int64_t n, int d, float* out, cudaStream_t s);
+
+// Exact k-NN on device buffers.  ynorm_opt: precomputed ||y||^2 [nb] or NULL.
+// ws must hold flat_plan(...).bytes.  nq > 0, nb > 0.
+int flat_knn_device(const float* xq, int64_t nq, const float* xb, int64_t nb, int d, int k,
+                    const float* ynorm_opt, float* out_dist, int64_t* out_ids, void* ws,
+                    cudaStream_t s);
+
+// B4: S partial queues per query -> k results (+||x||^2 if xnorm != NULL).
+int launch_flat_finish(const uint64_t* Wg, int64_t nq, int S, int k, const float* xnorm,
+                       float* out_dist, int64_t* out_ids, cudaStream_t s);
+
+}  // namespace fs

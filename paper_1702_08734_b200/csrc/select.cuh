@@ -122,13 +122,16 @@ __host__ __device__ constexpr int warp_select_smem_keys() {
 }
 
 // Sort one warp's batch of cnt (<= 32*NB) candidate keys in buf and merge it
-// into the warp queue W (NQ keys per lane, lane-stride, ascending).  Returns the
-// new threshold W[K-1].  Deliberately NOT inlined: one copy of the networks per
-// (NQ, NB); W is passed through lane-private memory (NQ loads + NQ stores per
-// call against the ~10^3 instructions of the networks).  Warp-collective.
+// into the warp queue W (32*NQ keys, lane-stride, ascending): this lane's r-th
+// key is Wmem[r * wstride] (wstride = 1 for a lane-private array, 32 for a
+// shared/global array addressed as base + lane).  Returns the new threshold
+// W[K-1].  Deliberately NOT inlined: one copy of the networks per (NQ, NB); W
+// goes through memory (NQ loads + NQ stores per call against the ~10^3
+// instructions of the networks).  Warp-collective.
 template <int NQ, int NB>
-__device__ __noinline__ uint64_t warp_flush(uint64_t* __restrict__ Wmem, uint64_t* buf, int cnt) {
+__device__ __noinline__ uint64_t warp_flush(uint64_t* Wmem, int wstride, uint64_t* buf, int cnt) {
   const int lane = threadIdx.x & 31;
+  constexpr int NM = NB < NQ ? NB : NQ;  // batch registers that can reach the queue
   __syncwarp();
   uint64_t B[NB];
 #pragma unroll
@@ -147,26 +150,46 @@ __device__ __noinline__ uint64_t warp_flush(uint64_t* __restrict__ Wmem, uint64_
   __syncwarp();
   uint64_t W[NQ];
 #pragma unroll
-  for (int r = 0; r < NQ; ++r) W[r] = Wmem[r];
-  // half-cleaner against the reversed batch: W[K-1-i] = min(W[K-1-i], B[i]), i < C
+  for (int r = 0; r < NQ; ++r) W[r] = Wmem[r * wstride];
+  // half-cleaner against the reversed batch: W[K-1-i] = min(W[K-1-i], B[i]), i < min(C, K)
 #pragma unroll
-  for (int r = 0; r < NB; ++r) {
+  for (int r = 0; r < NM; ++r) {
     const int i = r * 32 + (31 - lane);
     W[NQ - 1 - r] = umin64(W[NQ - 1 - r], buf[i + (i >> 4)]);
   }
   __syncwarp();
   merge_lane_stride<NQ>(W, lane);
 #pragma unroll
-  for (int r = 0; r < NQ; ++r) Wmem[r] = W[r];
+  for (int r = 0; r < NQ; ++r) Wmem[r * wstride] = W[r];
   return __shfl_sync(kFull, W[NQ - 1], 31);
+}
+
+// Queue-length class of k: K = 32 << kclass >= k.
+__host__ __device__ inline int k_class(int k) {
+  int c = 0;
+  while ((32 << c) < k) ++c;
+  return c;
+}
+
+// Run-time dispatch for kernels whose body does not depend on the queue length
+// (the fused distance kernels): batch of 64 candidates (NB = 2).
+__device__ __forceinline__ uint64_t warp_flush_b64(int kclass, uint64_t* Wmem, int wstride,
+                                                    uint64_t* buf, int cnt) {
+  switch (kclass) {
+    case 0: return warp_flush<1, 2>(Wmem, wstride, buf, cnt);
+    case 1: return warp_flush<2, 2>(Wmem, wstride, buf, cnt);
+    case 2: return warp_flush<4, 2>(Wmem, wstride, buf, cnt);
+    case 3: return warp_flush<8, 2>(Wmem, wstride, buf, cnt);
+    case 4: return warp_flush<16, 2>(Wmem, wstride, buf, cnt);
+    default: return warp_flush<32, 2>(Wmem, wstride, buf, cnt);
+  }
 }
 
 // Per-warp selection state.  K = 32*NQ >= k is the queue length, C = 32*NB the
 // candidate batch.  All member functions are warp-collective (full mask).
 template <int NQ, int NB>
 struct WarpSelect {
-  static_assert(NB <= NQ, "batch larger than the queue is never useful");
-  static constexpr int K = 32 * NQ;
+    static constexpr int K = 32 * NQ;
   static constexpr int C = 32 * NB;
 
   uint64_t W[NQ];    // lane-stride, ascending; kSentinelKey marks empty slots
@@ -201,7 +224,7 @@ struct WarpSelect {
     if (cnt > C - 32) flush();
   }
   __device__ __forceinline__ void flush() {
-    thr = warp_flush<NQ, NB>(W, buf, cnt);
+    thr = warp_flush<NQ, NB>(W, 1, buf, cnt);
     thr_val = key_val(thr);
     cnt = 0;
   }

@@ -1,0 +1,110 @@
+"""GPU parity: fs_flat_l2_knn (through the C ABI) vs the exact-search oracle.
+
+Acceptance (BASELINE.json north_star): for every returned
+(dist, id): |dist - D(j,id)| <= 1e-4 (||x_j||^2 + ||y_id||^2); D(j,id) <= oracle's
+k-th distance + that tolerance; ids distinct and in range; distances ascending;
+equal returned distances have ascending ids.  On integer-valued data (cfg3)
+fp32 arithmetic is exact and the result must equal the oracle bit for bit.
+"""
+import numpy as np
+import pytest
+import torch
+
+import datagen
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-4
+
+
+def run(xq, xb, k):
+    import paper_1702_08734_b200 as fs
+    d, i = fs.flat_l2_knn(torch.from_numpy(xq).cuda(), torch.from_numpy(xb).cuda(), k)
+    torch.cuda.synchronize()
+    return d.cpu().numpy(), i.cpu().numpy()
+
+
+def check_acceptance(xq, xb, k, gd, gi, od64):
+    nq, nb = xq.shape[0], xb.shape[0]
+    kk = min(k, nb)
+    xn = (xq.astype(np.float64) ** 2).sum(1)
+    yn = (xb.astype(np.float64) ** 2).sum(1)
+    assert np.all(gi[:, kk:] == -1) and np.all(np.isposinf(gd[:, kk:]))
+    ids = gi[:, :kk]
+    assert ids.min() >= 0 and ids.max() < nb
+    assert all(len(set(r.tolist())) == kk for r in ids), "duplicate ids"
+    exact = oracle.pair_l2(xq, xb, ids)
+    tol = TOL * (xn[:, None] + yn[ids])
+    assert np.all(np.abs(gd[:, :kk].astype(np.float64) - exact) <= tol), "distance off"
+    assert np.all(exact <= od64[:, kk - 1:kk] + tol), "returned id is not a k-NN within tolerance"
+    dd = np.diff(gd[:, :kk], axis=1)
+    assert np.all(dd >= 0), "not ascending"
+    same = dd == 0
+    assert np.all(np.diff(ids, axis=1)[same] > 0), "ties not by ascending id"
+
+
+def test_cfg1_tiny_full():
+    """BASELINE.json configs[0]: nb=8192, nq=64, d=64, ~N(0,1), seed 0, k=10."""
+    xb = datagen.gaussian_vectors(0, 8192, 64)
+    xq = datagen.gaussian_vectors(8192, 64, 64)
+    od, oi, od64 = oracle.flat_l2_knn(xq, xb, 10, want64=True)
+    gd, gi = run(xq, xb, 10)
+    check_acceptance(xq, xb, 10, gd, gi, od64)
+    assert (gi == oi).mean() > 0.999  # real-valued data: ids agree except at rounding near-ties
+
+
+@pytest.mark.parametrize("nq,nb,d,k", [
+    (1, 1, 1, 1), (3, 5, 2, 3), (65, 129, 3, 7), (70, 1000, 17, 32), (130, 3001, 64, 33),
+    (64, 2500, 128, 100), (33, 777, 96, 128), (17, 5000, 100, 1024), (200, 4099, 24, 1),
+    (5, 300, 130, 400),
+])
+def test_shapes_real_valued(nq, nb, d, k):
+    rng = np.random.default_rng(nq * 7 + nb)
+    xb = rng.standard_normal((nb, d)).astype(np.float32)
+    xq = rng.standard_normal((nq, d)).astype(np.float32)
+    _, _, od64 = oracle.flat_l2_knn(xq, xb, k, want64=True)
+    gd, gi = run(xq, xb, k)
+    check_acceptance(xq, xb, k, gd, gi, od64)
+
+
+@pytest.mark.parametrize("k", [1, 10, 100])
+def test_cfg3_shaped_integer_data_bit_exact(k):
+    """cfg3 recipe at reduced size: integer data -> bit-exact ids and distances,
+    exact ties resolved by lower id (many with few distinct values)."""
+    xb = datagen.sift_like(0, 20000)
+    xq = datagen.sift_like(1_000_000, 150)
+    xb[5000:5040] = xb[100:140]  # exact duplicates -> exact ties
+    od, oi = oracle.flat_l2_knn(xq, xb, k)
+    gd, gi = run(xq, xb, k)
+    assert np.array_equal(gi, oi)
+    assert np.array_equal(gd.view(np.uint32), od.view(np.uint32))
+
+
+def test_handworked_and_duplicates():
+    xb = np.array([[0, 0], [3, 4], [6, 8], [3, 4], [-3, 4]], np.float32)
+    xq = np.array([[0, 0], [3, 4]], np.float32)
+    gd, gi = run(xq, xb, 3)
+    assert gi.tolist() == [[0, 1, 3], [1, 3, 0]] and gd.tolist() == [[0, 25, 25], [0, 0, 25]]
+    gd, gi = run(xq, xb, 7)  # k > nb pads
+    assert gi[:, 5:].tolist() == [[-1, -1], [-1, -1]] and np.all(np.isposinf(gd[:, 5:]))
+
+
+def test_empty_and_errors():
+    import paper_1702_08734_b200 as fs
+    xq = torch.zeros((4, 8), device="cuda")
+    d, i = fs.flat_l2_knn(xq, torch.zeros((0, 8), device="cuda"), 3)
+    assert np.all(i.cpu().numpy() == -1) and np.all(np.isposinf(d.cpu().numpy()))
+    d, i = fs.flat_l2_knn(xq[:0], torch.zeros((5, 8), device="cuda"), 3)
+    assert d.shape == (0, 3)
+    with pytest.raises(fs.FsError):
+        fs.flat_l2_knn(xq, torch.zeros((5, 8), device="cuda"), 2000)
+
+
+def test_host_entry_point():
+    import paper_1702_08734_b200 as fs
+    xb = datagen.sift_like(0, 3000)
+    xq = datagen.sift_like(1_000_000, 20)
+    gd, gi = fs.flat_l2_knn_host(xq, xb, 10)
+    od, oi = oracle.flat_l2_knn(xq, xb, 10)
+    assert np.array_equal(gi, oi) and np.array_equal(gd, od)
