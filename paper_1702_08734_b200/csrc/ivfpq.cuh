@@ -1,0 +1,76 @@
+// ivfpq.cuh -- the IVFADC index object behind fs_ivfpq_* (include/fs.h) and the
+// internal interfaces between its translation units:
+//   ivfpq.cu        object life cycle, quantizers, add (D1-D3), export, C ABI
+//   ivfpq_search.cu search (C1-C5): LUT + list scan + pass-1 selection, pass 2
+//   ivfpq_train.cu  k-means training of both quantizers
+#pragma once
+
+#include <vector>
+
+#include "common.cuh"
+
+namespace fs {
+
+// Device buffer owned by the index (cudaMalloc / cudaFree), grown geometrically.
+struct DevBuf {
+  void* p = nullptr;
+  size_t cap = 0;
+  // Make room for `bytes`, keeping the first `keep` bytes.  Synchronises `s`.
+  int ensure(size_t bytes, size_t keep, cudaStream_t s);
+  void release();
+  template <typename T>
+  T* as() const { return static_cast<T*>(p); }
+};
+
+}  // namespace fs
+
+// The opaque object of include/fs.h.
+struct fs_ivfpq {
+  int d = 0, nlist = 0, M = 0, dsub = 0;
+  bool have_quantizers = false;
+  fs::DevBuf coarse;  // [nlist][d] fp32
+  fs::DevBuf cnorm;   // [nlist] fp32: ||c||^2 (B1 of the coarse search, precomputed)
+  fs::DevBuf pq;      // [M][256][dsub] fp32
+
+  // Finalised inverted file, CSR over list number (codes and
+  // ids in separate arrays, each list contiguous, append order kept).
+  int64_t n_csr = 0;
+  fs::DevBuf offsets;  // int64 [nlist+1]
+  fs::DevBuf codes;    // uint8 [n_csr][M]
+  fs::DevBuf ids;      // int64 [n_csr]
+  std::vector<int64_t> offsets_host;
+
+  // Vectors added since the last finalise, in arrival order.
+  int64_t n_staged = 0;
+  fs::DevBuf st_list;   // uint32 [n_staged]
+  fs::DevBuf st_codes;  // uint8 [n_staged][M]
+  fs::DevBuf st_ids;    // int64 [n_staged]
+
+  // Code bytes scanned by the last search (device counter, read lazily).
+  fs::DevBuf scanned;  // unsigned long long [1]
+
+  int64_t ntotal() const { return n_csr + n_staged; }
+};
+
+namespace fs {
+
+// Group staged vectors into the CSR lists (stable: append order kept).
+int ivfpq_finalise(fs_ivfpq* ix, cudaStream_t s);
+
+// D2: residual PQ encoding of n vectors with known coarse assignment.
+int launch_pq_encode(const fs_ivfpq* ix, const float* y, int64_t n, const int64_t* assign,
+                     uint8_t* codes_out, uint32_t* list_out, cudaStream_t s);
+
+// Generic Lloyd k-means on device data x [n][d] -> cent [K][d] (ivfpq_train.cu).
+int kmeans_device(const float* x, int64_t n, int d, int K, int niter, uint64_t seed, float* cent,
+                  cudaStream_t s);
+// Nearest centroid of each x (k = 1 exact search, chunked): assign int64 [n].
+int assign_nearest(const float* x, int64_t n, const float* cent, const float* cent_norm, int K,
+                   int d, int64_t* assign, cudaStream_t s);
+
+int ivfpq_search_device(fs_ivfpq* ix, const float* xq, int64_t nq, int nprobe, int k,
+                        float* out_dist, int64_t* out_ids, int32_t* out_probed, void* ws,
+                        cudaStream_t s);
+size_t ivfpq_search_ws(const fs_ivfpq* ix, int64_t nq, int nprobe, int k);
+
+}  // namespace fs

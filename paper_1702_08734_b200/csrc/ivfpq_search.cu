@@ -1,0 +1,274 @@
+// ivfpq_search.cu -- fs_ivfpq_search: Alg. 4, SURVEY 8a rows C1-C5.
+//
+//   C1 coarse quantizer  L_IVF = tau-argmin_c ||x - c||^2 (Eq. 5): the
+//                        exact-search engine over the centroids with k = nprobe
+//   C2 lookup tables     per (query, probed list): r = x - c_L,
+//                        T_m[c] = ||r^m - B[m][c]||^2 (Eq. 10), built in
+//                        SHARED memory by the CTA that scans the list (P:L317 has a
+//                        separate kernel write them to global memory; here they never
+//                        leave the SM)
+//   C3 list scan         dist = sum_m T_m[code_m] over the list's codes, streamed
+//                        from HBM (Alg. 4)
+//   C4 pass-1 selection  fused: every warp k-selects the distances it produces in a
+//                        register queue; a CTA covers a GROUP of G probed lists of
+//                        one query, so one partial list of k leaves the SM per group
+//                        (the paper writes all distances out first, and
+//                        found the fused form <= 15 % faster on Maxwell)
+//   C5 pass-2 + ids      the groups' partial lists are selected again to k; int64
+//                        ids are fetched for the winners only
+#include "flat.cuh"
+#include "ivfpq.cuh"
+#include "select.cuh"
+
+namespace fs {
+
+namespace {
+
+constexpr int SCAN_WARPS = 8;
+constexpr int SCAN_THREADS = SCAN_WARPS * 32;
+
+struct ScanArgs {
+  const float* xq;
+  const float* coarse;
+  const float* pq;
+  const int64_t* probe_ids;  // [nq][nprobe], ascending coarse distance
+  const int64_t* offsets;    // [nlist+1]
+  const uint8_t* codes;      // [ntotal][M]
+  uint64_t* Wg;              // [nq][ngroups][K] partial queues (keys: distance, CSR position)
+  unsigned long long* scanned;
+  int32_t* out_probed;       // [nq][nprobe] or NULL
+  int d, M, dsub, nprobe, G, ngroups, k;
+};
+
+// Shared memory: r[d] | T[M][256] | per-warp batches | merge area [SCAN_WARPS][K]
+template <int NQ>
+__global__ void __launch_bounds__(SCAN_THREADS) ivfpq_scan_kernel(const ScanArgs a) {
+  extern __shared__ __align__(16) unsigned char scan_smem[];
+  constexpr int K = 32 * NQ;
+  constexpr int NB = 2;
+  float* r = reinterpret_cast<float*>(scan_smem);
+  float* T = r + ((a.d + 3) & ~3);
+  uint64_t* bufs = reinterpret_cast<uint64_t*>(T + a.M * 256);
+  uint64_t* merge = bufs + SCAN_WARPS * warp_select_smem_keys<NB>();
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int64_t q = blockIdx.x / a.ngroups;
+  const int g = (int)(blockIdx.x - q * a.ngroups);
+  const int p_begin = g * a.G;
+  const int p_end = (p_begin + a.G) < a.nprobe ? (p_begin + a.G) : a.nprobe;
+  const int M = a.M, dsub = a.dsub, d = a.d;
+
+  WarpSelect<NQ, NB> sel;
+  sel.init(bufs + warp * warp_select_smem_keys<NB>(), lane);
+  unsigned long long bytes = 0;
+
+  for (int p = p_begin; p < p_end; ++p) {
+    const int64_t L = a.probe_ids[q * a.nprobe + p];
+    if (a.out_probed && tid == 0) a.out_probed[q * a.nprobe + p] = (int32_t)L;
+    if (L < 0) continue;  // fewer than nprobe centroids: cannot happen (nprobe <= nlist)
+    const int64_t lb = a.offsets[L], le = a.offsets[L + 1];
+    const int64_t len = le - lb;
+    if (len == 0) continue;  // empty lists are probed and contribute nothing
+    __syncthreads();         // previous list's table is no longer read
+    // C2: residual and tables
+    for (int j = tid; j < d; j += SCAN_THREADS) r[j] = a.xq[q * d + j] - a.coarse[L * d + j];
+    __syncthreads();
+    for (int e = tid; e < M * 256; e += SCAN_THREADS) {
+      const int m = e >> 8;
+      const float* b = a.pq + (int64_t)e * dsub;
+      const float* rm = r + m * dsub;
+      float acc = 0.f;
+      for (int j = 0; j < dsub; ++j) {
+        const float t = rm[j] - b[j];
+        acc = fmaf(t, t, acc);
+      }
+      T[e] = acc;
+    }
+    __syncthreads();
+    // C3 + C4: scan and select
+    bytes += (unsigned long long)len * M;
+    const uint8_t* cl = a.codes + lb * M;
+    for (int64_t v0 = 0; v0 < len; v0 += SCAN_THREADS) {
+      const int64_t v = v0 + tid;
+      const bool ok = v < len;
+      float dist = 0.f;
+      if (ok) {
+        const uint8_t* cv = cl + v * M;
+        if ((M & 3) == 0) {
+          const uint32_t* cw = reinterpret_cast<const uint32_t*>(cv);
+          for (int w = 0; w < (M >> 2); ++w) {
+            const uint32_t c = cw[w];
+            const float* Tw = T + (w << 10);
+            dist += Tw[c & 255u];
+            dist += Tw[256 + ((c >> 8) & 255u)];
+            dist += Tw[512 + ((c >> 16) & 255u)];
+            dist += Tw[768 + (c >> 24)];
+          }
+        } else {
+          for (int m = 0; m < M; ++m) dist += T[(m << 8) + cv[m]];
+        }
+      }
+      const uint64_t key = make_key(dist, (uint32_t)(lb + v));
+      sel.push(ok && sel.maybe(dist) && sel.wants(key), key);
+    }
+  }
+  sel.finish();
+  if (tid == 0 && bytes) atomicAdd(a.scanned, bytes);
+
+  // merge the warps' queues: warp 0 selects again over SCAN_WARPS * K keys
+  __syncthreads();
+#pragma unroll
+  for (int rr = 0; rr < NQ; ++rr) merge[warp * K + rr * 32 + lane] = sel.W[rr];
+  __syncthreads();
+  if (warp == 0) {
+    sel.reset();
+    for (int e0 = 0; e0 < SCAN_WARPS * K; e0 += 32) {
+      const uint64_t key = merge[e0 + lane];
+      sel.push(key < sel.thr, key);
+    }
+    sel.finish();
+    uint64_t* W = a.Wg + (int64_t)blockIdx.x * K;
+#pragma unroll
+    for (int rr = 0; rr < NQ; ++rr) W[rr * 32 + lane] = sel.W[rr];
+  }
+}
+
+// C5 second half: positions -> ids; entries with bitwise-equal distance are put
+// in ascending id order (positions order them by list and append order, which is
+// ascending id only inside a list filled in ascending id order).  One warp per query.
+__global__ void __launch_bounds__(128)
+    ivfpq_resolve_kernel(float* __restrict__ dist, int64_t* __restrict__ ids_io,
+                         const int64_t* __restrict__ ids, int64_t nq, int k) {
+  extern __shared__ __align__(16) unsigned char res_smem[];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int64_t q = (int64_t)blockIdx.x * 4 + warp;
+  if (q >= nq) return;
+  int64_t* sid = reinterpret_cast<int64_t*>(res_smem) + (size_t)warp * k;
+  float* sd = reinterpret_cast<float*>(reinterpret_cast<int64_t*>(res_smem) + (size_t)4 * k) +
+              (size_t)warp * k;
+  for (int i = lane; i < k; i += 32) {
+    const int64_t pos = ids_io[q * k + i];
+    sid[i] = pos < 0 ? -1 : ids[pos];
+    sd[i] = dist[q * k + i];
+  }
+  __syncwarp();
+  for (int i = lane; i < k; i += 32) {
+    const float di = sd[i];
+    const int64_t id = sid[i];
+    int rank = i;
+    if (id >= 0) {
+      int s = i, e = i;
+      while (s > 0 && sd[s - 1] == di && sid[s - 1] >= 0) --s;
+      while (e + 1 < k && sd[e + 1] == di && sid[e + 1] >= 0) ++e;
+      if (e > s) {
+        rank = s;
+        for (int j = s; j <= e; ++j) rank += (sid[j] < id) || (sid[j] == id && j < i);
+      }
+    }
+    ids_io[q * k + rank] = id;
+  }
+}
+
+struct SearchPlan {
+  int G, ngroups, K;
+  FlatPlan coarse;
+  size_t off_cdist, off_cids, off_W, bytes;
+};
+
+SearchPlan search_plan(const fs_ivfpq* ix, int64_t nq, int nprobe, int k) {
+  SearchPlan p;
+  p.K = 32 << k_class(k);
+  // enough CTAs to fill the GPU twice over, but never more groups than probes
+  const int64_t target = (int64_t)sm_count() * 4;
+  int64_t ng = nq > 0 ? ceil_div(target, nq) : 1;
+  if (ng > nprobe) ng = nprobe;
+  if (ng < 1) ng = 1;
+  p.G = (int)ceil_div(nprobe, ng);
+  p.ngroups = (int)ceil_div(nprobe, p.G);
+  p.coarse = flat_plan(nq, ix->nlist, ix->d, nprobe);
+  size_t o = align_up(p.coarse.bytes, 256);
+  p.off_cdist = o;
+  o += align_up((size_t)nq * nprobe * sizeof(float), 256);
+  p.off_cids = o;
+  o += align_up((size_t)nq * nprobe * sizeof(int64_t), 256);
+  p.off_W = o;
+  o += align_up((size_t)nq * p.ngroups * p.K * sizeof(uint64_t), 256);
+  p.bytes = o;
+  return p;
+}
+
+template <int NQ>
+int launch_scan(const ScanArgs& a, int64_t nq, cudaStream_t s) {
+  constexpr int K = 32 * NQ;
+  const size_t smem = (size_t)(((a.d + 3) & ~3) + a.M * 256) * sizeof(float) +
+                      (size_t)(SCAN_WARPS * warp_select_smem_keys<2>() + SCAN_WARPS * K) * sizeof(uint64_t);
+  if (smem > 227 * 1024) return set_error(FS_EUNSUPPORTED, "fs_ivfpq_search: shared memory (%zu B) exceeds 227 KB", smem);
+  static size_t attr_smem = 0;
+  if (smem > attr_smem) {
+    FS_CUDA(cudaFuncSetAttribute(ivfpq_scan_kernel<NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    attr_smem = smem;
+  }
+  const int64_t grid = nq * a.ngroups;
+  if (grid > 0x7fffffffLL) return set_error(FS_EUNSUPPORTED, "fs_ivfpq_search: nq * groups too large");
+  ivfpq_scan_kernel<NQ><<<(unsigned)grid, SCAN_THREADS, smem, s>>>(a);
+  FS_LAUNCHED();
+  return FS_OK;
+}
+
+}  // namespace
+
+size_t ivfpq_search_ws(const fs_ivfpq* ix, int64_t nq, int nprobe, int k) {
+  return search_plan(ix, nq, nprobe, k).bytes;
+}
+
+int ivfpq_search_device(fs_ivfpq* ix, const float* xq, int64_t nq, int nprobe, int k,
+                        float* out_dist, int64_t* out_ids, int32_t* out_probed, void* ws,
+                        cudaStream_t s) {
+  const SearchPlan p = search_plan(ix, nq, nprobe, k);
+  char* w = static_cast<char*>(ws);
+  float* cdist = reinterpret_cast<float*>(w + p.off_cdist);
+  int64_t* cids = reinterpret_cast<int64_t*>(w + p.off_cids);
+  uint64_t* Wg = reinterpret_cast<uint64_t*>(w + p.off_W);
+  int rc;
+  // C1
+  rc = flat_knn_device(xq, nq, ix->coarse.as<float>(), ix->nlist, ix->d, nprobe,
+                       ix->cnorm.as<float>(), cdist, cids, w, s);
+  if (rc != FS_OK) return rc;
+  FS_CUDA(cudaMemsetAsync(ix->scanned.p, 0, sizeof(unsigned long long), s));
+  // C2-C4
+  ScanArgs a;
+  a.xq = xq;
+  a.coarse = ix->coarse.as<float>();
+  a.pq = ix->pq.as<float>();
+  a.probe_ids = cids;
+  a.offsets = ix->offsets.as<int64_t>();
+  a.codes = ix->codes.as<uint8_t>();
+  a.Wg = Wg;
+  a.scanned = ix->scanned.as<unsigned long long>();
+  a.out_probed = out_probed;
+  a.d = ix->d;
+  a.M = ix->M;
+  a.dsub = ix->dsub;
+  a.nprobe = nprobe;
+  a.G = p.G;
+  a.ngroups = p.ngroups;
+  a.k = k;
+  switch (k_class(k)) {
+    case 0: rc = launch_scan<1>(a, nq, s); break;
+    case 1: rc = launch_scan<2>(a, nq, s); break;
+    case 2: rc = launch_scan<4>(a, nq, s); break;
+    case 3: rc = launch_scan<8>(a, nq, s); break;
+    case 4: rc = launch_scan<16>(a, nq, s); break;
+    default: rc = launch_scan<32>(a, nq, s); break;
+  }
+  if (rc != FS_OK) return rc;
+  // C5
+  rc = launch_flat_finish(Wg, nq, p.ngroups, k, nullptr, out_dist, out_ids, s);
+  if (rc != FS_OK) return rc;
+  const size_t smem = (size_t)4 * k * (sizeof(int64_t) + sizeof(float));
+  ivfpq_resolve_kernel<<<(unsigned)ceil_div(nq, 4), 128, smem, s>>>(out_dist, out_ids,
+                                                                    ix->ids.as<int64_t>(), nq, k);
+  FS_LAUNCHED();
+  return FS_OK;
+}
+
+}  // namespace fs
