@@ -1,0 +1,435 @@
+#!/usr/bin/env python
+"""bench.py -- measures the hot path of arXiv 1702.08734 on B200 through the C ABI.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--skip-also] [--ivfpq-nb NB]
+
+Headline (BASELINE.json configs[1], "k-select GB/s as % HBM peak"): one STEP is
+fs_kselect over the whole cfg2 batch -- 10 000 rows x 16 384 fp32 ~U[0,1) (1 % of
+rows with duplicated runs) at k = 1, 32, 128 and 1024, plus one row of 2^27 values at
+k = 1024.  value = algorithmic bytes (4 B per input element +
+8 B per output element) of all ranks / step time, inputs resident
+in HBM; e2e = the same step through fs_kselect_host from pinned HOST buffers, copies
+inside the timed region.  Inputs (1.19 GB per rank) are larger than the 126 MB L2.
+
+"also" (same JSON line): fs_flat_l2_knn on cfg3 (nb = 10^6, nq = 10^4, d = 128, SIFT-like
+integers, k = 1, 10, 100; rows B1-B4) in queries/s, and fs_ivfpq_search on a REDUCED
+cfg4-shaped index (rows C1-C5; the full 10^8-vector build does not fit a default run;
+see profiles/ for the full-size runs) in queries/s and code-scan GB/s.
+
+With N > 1 (torchrun) every rank runs the same step on its own rows (the path
+partitions by row/query: no data-path collective): weak scaling, time = max
+over ranks, value = sum of bytes / that time.
+
+--impl reference times the CPU oracle (oracle/, as it stands) on a bounded sample of
+the same workload on the host cores; rank 0 only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "k-NN queries/s (flat L2, IVFPQ) at oracle match; k-select GB/s as % HBM peak"
+N_ROWS, N_COLS, KS = 10_000, 16_384, (1, 32, 128, 1024)
+BIG_N, BIG_K = 1 << 27, 1024
+WORKLOAD = ("cfg2: fs_kselect on 10000x16384 fp32 U[0,1) rows (1% duplicate-run rows) at "
+            "k in {1,32,128,1024} + one row of 2^27 at k=1024")
+
+
+def step_bytes() -> int:
+    b = 0
+    for k in KS:
+        b += 4 * N_ROWS * N_COLS + 8 * N_ROWS * k
+    return b + 4 * BIG_N + 8 * BIG_K
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            j = json.load(f)
+        return dict(hbm=float(j["hbm_gbs"]), bf16=float(j["bf16_tflops"]),
+                    bf16_sustained=float(j.get("bf16_tflops_sustained", j["bf16_tflops"])),
+                    source="measured (MEASURED_PEAKS.json)")
+    return dict(hbm=6650.0, bf16=1590.0, bf16_sustained=1400.0, source="fallback (B200_PROFILING.md)")
+
+
+# ----------------------------------------------------------------------------
+class ClockSampler:
+    """SM clock and throttle reasons sampled (NVML) while the timed region runs."""
+
+    def __init__(self, index: int):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def _run(self):
+        nv = self.nv
+        names = {
+            "sw_power_cap": getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4),
+            "hw_slowdown": getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8),
+            "sw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20),
+            "hw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40),
+            "hw_power_brake": getattr(nv, "nvmlClocksEventReasonHwPowerBrakeSlowdown", 0x80),
+        }
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    m = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    m = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for n, bit in names.items():
+                    if m & bit:
+                        self.reasons.add(n)
+            except Exception:
+                pass
+            time.sleep(0.02)
+
+    def start(self):
+        if self.nv is not None:
+            self._stop.clear()
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+
+    def stop(self):
+        if self._thr is not None:
+            self._stop.set()
+            self._thr.join()
+            self._thr = None
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unavailable"]}
+        s = sorted(self.samples)
+        return {"sm_mhz": s[len(s) // 2], "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(s)}
+
+
+# ----------------------------------------------------------------------------
+def run_reference(args):
+    """The oracle on the host cores, same metric and config; bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import numpy as np
+    import datagen
+    import oracle
+    oracle.build()
+    rows_per_step, big_slice = 256, 1 << 21
+    rows = datagen.kselect_rows(0, rows_per_step, N_COLS)
+    big = datagen.kselect_rows(10**6, 1, big_slice, duplicates=False)
+    sample_bytes = sum(4 * rows.size + 8 * rows_per_step * k for k in KS) + 4 * big.size + 8 * BIG_K
+
+    def step():
+        for k in KS:
+            oracle.kselect(rows, k)
+        oracle.kselect(big, BIG_K)
+
+    for _ in range(args.warmup):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step()
+    dt = (time.perf_counter() - t0) / max(args.steps, 1)
+    gbs = sample_bytes / dt / 1e9
+    sample = ("per step: oracle.kselect (full sort per row) on %d of the %d rows at k in {1,32,128,1024} "
+              "+ the first 2^21 of the 2^27-value row at k=1024" % (rows_per_step, N_ROWS))
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": gbs, "unit": "GB/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic (seeded, datagen/)",
+        "config": {"workload": WORKLOAD, "sample": sample},
+        "cpu_baseline": {"value": gbs, "unit": "GB/s", "cores": oracle.num_threads(), "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": gbs, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+# ----------------------------------------------------------------------------
+def cpu_baseline():
+    """The oracle as it stands on the host cores, bounded sample of the headline workload."""
+    import datagen
+    import oracle
+    n_rows, big_slice = 2000, 1 << 23
+    rows = datagen.kselect_rows(0, n_rows, N_COLS)
+    big = datagen.kselect_rows(10**6, 1, big_slice, duplicates=False)
+    oracle.kselect(rows[:8], 32)  # load the library
+    t0 = time.perf_counter()
+    for k in KS:
+        oracle.kselect(rows, k)
+    oracle.kselect(big, BIG_K)
+    dt = time.perf_counter() - t0
+    b = sum(4 * rows.size + 8 * n_rows * k for k in KS) + 4 * big.size + 8 * BIG_K
+    return {"value": b / dt / 1e9, "unit": "GB/s", "cores": oracle.num_threads(), "kind": "oracle",
+            "seconds": dt,
+            "sample": "oracle.kselect (full sort per row, OpenMP over rows) on the first %d of %d rows "
+                      "at k in {1,32,128,1024} + the first 2^23 of the 2^27-value row at k=1024"
+                      % (n_rows, N_ROWS)}
+
+
+def event_pair():
+    import torch
+    return torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+
+def timed(fn, reps, warm=1):
+    """Best and median ms over reps, CUDA events on the current stream."""
+    import torch
+    for _ in range(warm):
+        fn()
+    torch.cuda.synchronize()
+    ts = []
+    for _ in range(reps):
+        a, b = event_pair()
+        a.record()
+        fn()
+        b.record()
+        torch.cuda.synchronize()
+        ts.append(a.elapsed_time(b))
+    ts.sort()
+    return ts[0], ts[len(ts) // 2]
+
+
+def also_flat(fs, gt, pk):
+    import torch
+    nb, nq, d = 1_000_000, 10_000, 128
+    xb = gt.sift_like(0, nb)
+    xq = gt.sift_like(nb, nq)
+    out = {"workload": "cfg3: nb=1e6, nq=1e4, d=128 SIFT-like integer fp32", "engine": fs.flat_engine(),
+           "flop_per_call": 2.0 * nb * nq * d}
+    for k in (1, 10, 100):
+        ws = torch.empty(fs.flat_l2_knn_ws_bytes(nq, nb, d, k), dtype=torch.uint8, device="cuda")
+        od = torch.empty((nq, k), dtype=torch.float32, device="cuda")
+        oi = torch.empty((nq, k), dtype=torch.int64, device="cuda")
+        best, med = timed(lambda: fs.flat_l2_knn(xq, xb, k, out_dist=od, out_ids=oi, ws=ws), 3)
+        out["k%d" % k] = {"ms": med, "queries_per_s": nq / med * 1e3, "tflops": 2.0 * nb * nq * d / med / 1e9}
+    del xb, xq
+    return out
+
+
+def also_ivfpq(fs, gt, pk, nb):
+    import torch
+    d, M, nq, k = 96, 16, 10_000, 100
+    nlist = max(64, min(65_536, int(2 ** round(__import__("math").log2(max(nb // 1526, 64))))))
+    ntrain = min(nb, max(256, min(1_000_000, 16 * nlist)))
+    t0 = time.perf_counter()
+    ix = fs.IvfPq(d, nlist, M)
+    ix.train(gt.deep_like(0, ntrain), niter=10, seed=0)
+    torch.cuda.synchronize()
+    t_train = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    chunk = 1 << 22
+    for b in range(0, nb, chunk):
+        ix.add(gt.deep_like(b, min(chunk, nb - b)))
+    xq = gt.deep_like(nb, nq)
+    ix.search(xq[:8], 1, 1)  # finalise the lists
+    torch.cuda.synchronize()
+    t_add = time.perf_counter() - t0
+    out = {"workload": "cfg4-shaped, REDUCED: nb=%d deep-like d=96, nlist=%d, M=16, nq=1e4, k=100" % (nb, nlist),
+           "train_s": t_train, "add_s": t_add, "add_vectors_per_s": nb / t_add}
+    od = torch.empty((nq, k), dtype=torch.float32, device="cuda")
+    oi = torch.empty((nq, k), dtype=torch.int64, device="cuda")
+    for nprobe in (16, 64, 256):
+        if nprobe > nlist:
+            continue
+        ws = torch.empty(ix.search_ws_bytes(nq, nprobe, k), dtype=torch.uint8, device="cuda")
+        best, med = timed(lambda: ix.search(xq, nprobe, k, out_dist=od, out_ids=oi, ws=ws), 3)
+        codes = ix.last_scanned_codes
+        out["nprobe%d" % nprobe] = {"ms": med, "queries_per_s": nq / med * 1e3, "code_bytes": codes,
+                                    "code_GBps_whole_search": codes / med / 1e6,
+                                    "frac_hbm_whole_search": codes / med / 1e6 / pk["hbm"]}
+    ix.close()
+    return out
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    import paper_1702_08734_b200 as fs
+    from datagen import gen_torch as gt
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    fs.lib()  # fail loudly if libfs.so is missing
+    pk = peaks()
+
+    # this rank's rows: distinct rows per rank (weak scaling)
+    rows = gt.kselect_rows(rank * N_ROWS, N_ROWS, N_COLS)
+    big = gt.kselect_rows(10**6 + rank, 1, BIG_N, duplicates=False)
+    outs = {k: (torch.empty((N_ROWS, k), dtype=torch.float32, device="cuda"),
+                torch.empty((N_ROWS, k), dtype=torch.int32, device="cuda")) for k in KS}
+    bout = (torch.empty((1, BIG_K), dtype=torch.float32, device="cuda"),
+            torch.empty((1, BIG_K), dtype=torch.int32, device="cuda"))
+    wsb = max([fs.kselect_ws_bytes(N_ROWS, N_COLS, k) for k in KS] + [fs.kselect_ws_bytes(1, BIG_N, BIG_K), 16])
+    ws = torch.empty(wsb, dtype=torch.uint8, device="cuda")
+    calls = [("k%d" % k, (lambda k=k: fs.kselect(rows, k, out_val=outs[k][0], out_idx=outs[k][1], ws=ws)),
+              4 * N_ROWS * N_COLS + 8 * N_ROWS * k) for k in KS]
+    calls.append(("bigrow_k1024", lambda: fs.kselect(big, BIG_K, out_val=bout[0], out_idx=bout[1], ws=ws),
+                  4 * BIG_N + 8 * BIG_K))
+    per_call = {name: [] for name, _, _ in calls}
+
+    def step(record=False):
+        for name, fn, _ in calls:
+            if record:
+                a, b = event_pair()
+                a.record()
+                fn()
+                b.record()
+                per_call[name].append((a, b))
+            else:
+                fn()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    sampler = ClockSampler(local)
+    barrier()
+    fs.reset_launch_count()
+    sampler.start()
+    t0, t1 = event_pair()
+    t0.record()
+    for _ in range(args.steps):
+        step(record=True)
+    t1.record()
+    barrier()
+    sampler.stop()
+    launches = fs.launch_count()
+    ms = t0.elapsed_time(t1)
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    ms_per_step = ms / args.steps
+    value = world * step_bytes() / (ms_per_step * 1e-3) / 1e9
+
+    # per-call device time (launch + its pass-2 launches), dominant call -> roofline
+    call_ms = {n: float(np.mean([a.elapsed_time(b) for a, b in ev])) for n, ev in per_call.items()}
+    call_bytes = {n: b for n, _, b in calls}
+    dom = max(call_ms, key=call_ms.get)
+    ach = call_bytes[dom] / call_ms[dom] / 1e6
+    roofline = {"bound": "hbm", "kernel": "kselect_warp_kernel (%s call)" % dom, "achieved": ach,
+                "peak": pk["hbm"], "unit": "GB/s", "frac": ach / pk["hbm"], "traffic": None,
+                "peak_source": pk["source"] + ", burst copy figure",
+                "per_call": {n: {"ms": call_ms[n], "GBps": call_bytes[n] / call_ms[n] / 1e6,
+                                 "frac": call_bytes[n] / call_ms[n] / 1e6 / pk["hbm"],
+                                 "share_of_step": call_ms[n] / sum(call_ms.values())} for n in call_ms},
+                "step_frac": value / world / pk["hbm"]}
+    tr = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tr):
+        try:
+            with open(tr) as f:
+                roofline["traffic"] = json.load(f).get(dom)
+        except Exception:
+            pass
+
+    # e2e: the same step through the host entry points, pinned host buffers
+    e2e_steps = max(1, min(args.steps, 2))
+    h_rows = torch.empty((N_ROWS, N_COLS), dtype=torch.float32, pin_memory=True)
+    h_rows.copy_(rows)
+    h_big = torch.empty((1, BIG_N), dtype=torch.float32, pin_memory=True)
+    h_big.copy_(big)
+    h_out = {k: (torch.empty((N_ROWS, k), dtype=torch.float32, pin_memory=True),
+                 torch.empty((N_ROWS, k), dtype=torch.int32, pin_memory=True)) for k in KS}
+    h_bout = (torch.empty((1, BIG_K), dtype=torch.float32, pin_memory=True),
+              torch.empty((1, BIG_K), dtype=torch.int32, pin_memory=True))
+    torch.cuda.synchronize()
+
+    def e2e_step():
+        for k in KS:
+            fs.kselect_host(h_rows, k, out_val=h_out[k][0], out_idx=h_out[k][1])
+        fs.kselect_host(h_big, BIG_K, out_val=h_bout[0], out_idx=h_bout[1])
+
+    e2e_step()
+    barrier()
+    w0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        e2e_step()
+    barrier()
+    e2e_s = (time.perf_counter() - w0) / e2e_steps
+    if world > 1:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    h2d = len(KS) * 4 * N_ROWS * N_COLS + 4 * BIG_N
+    d2h = sum(8 * N_ROWS * k for k in KS) + 8 * BIG_K
+    e2e = {"value": world * step_bytes() / e2e_s / 1e9, "unit": "GB/s", "h2d_bytes_per_step": h2d,
+           "d2h_bytes_per_step": d2h, "ms_per_step": e2e_s * 1e3, "steps": e2e_steps,
+           "api": "fs_kselect_host (pinned host buffers; cudaMalloc, H2D, kernels, D2H, free per call)"}
+    # spot-check the e2e results against the device-path results
+    assert torch.equal(h_out[32][1][:64], outs[32][1][:64].cpu()), "host and device paths disagree"
+    del h_rows, h_big, rows, big
+
+    line = {
+        "metric": METRIC, "value": value, "unit": "GB/s", "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic (seeded counter-based generator, datagen/; stands in for the paper's random rows, P:L377)",
+        "config": {"workload": WORKLOAD, "rows_per_gpu": N_ROWS, "algorithmic_bytes_per_step_per_gpu": step_bytes(),
+                   "l2": "inputs (1.19 GB per GPU) larger than the 126 MB L2", "parallelism": "rows split over ranks, no collective"},
+        "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+    }
+    if rank == 0 and world == 1:
+        if not args.skip_also:
+            torch.cuda.empty_cache()
+            also = {}
+            try:
+                also["flat_l2_knn"] = also_flat(fs, gt, pk)
+                torch.cuda.empty_cache()
+                also["ivfpq_search"] = also_ivfpq(fs, gt, pk, args.ivfpq_nb)
+            except Exception as e:  # the headline stands on its own
+                also["error"] = repr(e)
+            line["also"] = also
+        line["cpu_baseline"] = cpu_baseline()
+    if rank == 0:
+        print(json.dumps(line))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--skip-also", action="store_true")
+    ap.add_argument("--ivfpq-nb", type=int, default=10_000_000)
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -55,6 +55,9 @@ enum {
 FS_API const char* fs_last_error(void);
 /* Library version and the SM architecture it was compiled for ("sm_100a"). */
 FS_API const char* fs_version(void);
+/* Which engine fs_flat_l2_knn's contraction runs on in this build:
+ * "ffma-fp32" (CUDA cores) or "tcgen05-3xtf32" (tensor cores, split operands). */
+FS_API const char* fs_flat_engine(void);
 /* Number of kernel launches this thread's calls have enqueued since the last
  * fs_reset_launch_count(); used by bench.py to fill "gpu_launches". */
 FS_API int64_t fs_launch_count(void);

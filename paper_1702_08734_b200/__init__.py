@@ -50,6 +50,7 @@ def lib():
         L = ctypes.CDLL(LIB_PATH)
         L.fs_last_error.restype = ctypes.c_char_p
         L.fs_version.restype = ctypes.c_char_p
+        L.fs_flat_engine.restype = ctypes.c_char_p
         L.fs_launch_count.restype = _i64
         L.fs_reset_launch_count.restype = None
         for name in ("fs_kselect_ws_bytes", "fs_flat_l2_knn_ws_bytes", "fs_ivfpq_search_ws_bytes"):
@@ -79,6 +80,10 @@ def _dev(t: torch.Tensor, dtype, name: str) -> torch.Tensor:
 
 def _ptr(t):
     return _vp(0 if t is None else t.data_ptr())
+
+
+def flat_engine() -> str:
+    return lib().fs_flat_engine().decode()
 
 
 def launch_count() -> int:
@@ -118,15 +123,28 @@ def kselect(rows: torch.Tensor, k: int, n: int | None = None, out_val=None, out_
     return out_val, out_idx
 
 
-def kselect_host(rows, k: int):
-    """fs_kselect_host: same through HOST buffers (numpy fp32 [n_rows, n])."""
+def _host_ptr(a, dtype_np, dtype_t, name):
+    """Address of a contiguous HOST buffer: numpy array or CPU torch tensor (pinned or not)."""
     import numpy as np
-    rows = np.ascontiguousarray(rows, dtype=np.float32)
+    if isinstance(a, torch.Tensor):
+        if a.is_cuda or a.dtype != dtype_t or not a.is_contiguous():
+            raise ValueError("%s must be a contiguous CPU tensor of %s" % (name, dtype_t))
+        return a, a.data_ptr()
+    a = np.ascontiguousarray(a, dtype=dtype_np)
+    return a, a.ctypes.data
+
+
+def kselect_host(rows, k: int, out_val=None, out_idx=None):
+    """fs_kselect_host: same through HOST buffers (numpy or CPU torch fp32 [n_rows, n]);
+    the library copies in, runs and copies out.  Outputs are numpy unless given."""
+    import numpy as np
+    rows, rp = _host_ptr(rows, np.float32, torch.float32, "rows")
     n_rows, n = rows.shape
-    val = np.empty((n_rows, k), np.float32)
-    idx = np.empty((n_rows, k), np.int32)
-    _check(lib().fs_kselect_host(_vp(rows.ctypes.data), _i64(n_rows), _i64(n), _i64(n), _int(k),
-                                 _vp(val.ctypes.data), _vp(idx.ctypes.data)))
+    val = np.empty((n_rows, k), np.float32) if out_val is None else out_val
+    idx = np.empty((n_rows, k), np.int32) if out_idx is None else out_idx
+    val, vp = _host_ptr(val, np.float32, torch.float32, "out_val")
+    idx, ip = _host_ptr(idx, np.int32, torch.int32, "out_idx")
+    _check(lib().fs_kselect_host(_vp(rp), _i64(n_rows), _i64(n), _i64(n), _int(k), _vp(vp), _vp(ip)))
     return val, idx
 
 
@@ -153,16 +171,18 @@ def flat_l2_knn(xq: torch.Tensor, xb: torch.Tensor, k: int, out_dist=None, out_i
     return out_dist, out_ids
 
 
-def flat_l2_knn_host(xq, xb, k: int):
+def flat_l2_knn_host(xq, xb, k: int, out_dist=None, out_ids=None):
+    """fs_flat_l2_knn_host: HOST buffers in and out (numpy or CPU torch tensors)."""
     import numpy as np
-    xq = np.ascontiguousarray(xq, dtype=np.float32)
-    xb = np.ascontiguousarray(xb, dtype=np.float32)
+    xq, qp = _host_ptr(xq, np.float32, torch.float32, "xq")
+    xb, bp = _host_ptr(xb, np.float32, torch.float32, "xb")
     nq, d = xq.shape
-    dist = np.empty((nq, k), np.float32)
-    ids = np.empty((nq, k), np.int64)
-    _check(lib().fs_flat_l2_knn_host(_vp(xq.ctypes.data), _i64(nq), _vp(xb.ctypes.data),
-                                     _i64(xb.shape[0]), _int(d), _int(k), _vp(dist.ctypes.data),
-                                     _vp(ids.ctypes.data)))
+    dist = np.empty((nq, k), np.float32) if out_dist is None else out_dist
+    ids = np.empty((nq, k), np.int64) if out_ids is None else out_ids
+    dist, dp = _host_ptr(dist, np.float32, torch.float32, "out_dist")
+    ids, ip = _host_ptr(ids, np.int64, torch.int64, "out_ids")
+    _check(lib().fs_flat_l2_knn_host(_vp(qp), _i64(nq), _vp(bp), _i64(xb.shape[0]), _int(d), _int(k),
+                                     _vp(dp), _vp(ip)))
     return dist, ids
 
 
@@ -237,14 +257,15 @@ class IvfPq:
                                      _stream()))
         return (out_dist, out_ids, probed) if want_probed else (out_dist, out_ids)
 
-    def search_host(self, xq, nprobe: int, k: int):
+    def search_host(self, xq, nprobe: int, k: int, out_dist=None, out_ids=None):
         import numpy as np
-        xq = np.ascontiguousarray(xq, dtype=np.float32)
+        xq, qp = _host_ptr(xq, np.float32, torch.float32, "xq")
         nq = xq.shape[0]
-        dist = np.empty((nq, k), np.float32)
-        ids = np.empty((nq, k), np.int64)
-        _check(lib().fs_ivfpq_search_host(self._h, _vp(xq.ctypes.data), _i64(nq), _int(nprobe),
-                                          _int(k), _vp(dist.ctypes.data), _vp(ids.ctypes.data)))
+        dist = np.empty((nq, k), np.float32) if out_dist is None else out_dist
+        ids = np.empty((nq, k), np.int64) if out_ids is None else out_ids
+        dist, dp = _host_ptr(dist, np.float32, torch.float32, "out_dist")
+        ids, ip = _host_ptr(ids, np.int64, torch.int64, "out_ids")
+        _check(lib().fs_ivfpq_search_host(self._h, _vp(qp), _i64(nq), _int(nprobe), _int(k), _vp(dp), _vp(ip)))
         return dist, ids
 
     def export(self):

@@ -408,6 +408,8 @@ int flat_validate(const void* xq, int64_t nq, const void* xb, int64_t nb, int d,
 
 extern "C" {
 
+const char* fs_flat_engine(void) { return "ffma-fp32"; }
+
 size_t fs_flat_l2_knn_ws_bytes(int64_t nq, int64_t nb, int d, int k) {
   if (nq < 0 || nb < 0 || d < 1 || k < 1 || k > FS_MAX_K) return 0;
   return fs::flat_plan(nq, nb, d, k).bytes;
