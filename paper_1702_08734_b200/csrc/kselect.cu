@@ -12,6 +12,7 @@
 // of "lane j reads a_{32i+j}"), four groups in flight per lane.
 #include "common.cuh"
 #include "select.cuh"
+#include "tselect.cuh"
 
 namespace fs {
 
@@ -37,10 +38,14 @@ __device__ __forceinline__ float4 ld_stream4(const float* p) {
 }
 
 // ---------------------------------------------------------------------------
-// General k: one warp per (row, chunk).
+// General k: one warp per (row, chunk); threshold-filtered selection (tselect.cuh).
 // ---------------------------------------------------------------------------
-template <int NQ, int NB, int WARPS>
-__global__ void __launch_bounds__(WARPS * 32) kselect_warp_kernel(const KSelArgs a) {
+template <int NQ>
+__global__ void __launch_bounds__(TSelCfg<NQ>::WARPS * 32) kselect_warp_kernel(const KSelArgs a) {
+  constexpr int WARPS = TSelCfg<NQ>::WARPS;
+  constexpr int LCAP = TSelCfg<NQ>::LCAP;
+  constexpr int U = 8;          // 128-bit loads in flight per lane
+  constexpr int SAMPLE = 1024;  // elements of the row used to place the first bound
   extern __shared__ __align__(16) uint64_t smem_keys[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int64_t item = (int64_t)blockIdx.x * WARPS + warp;
@@ -55,100 +60,132 @@ __global__ void __launch_bounds__(WARPS * 32) kselect_warp_kernel(const KSelArgs
   const int32_t* pi = a.in_idx ? a.in_idx + row * a.ld + start : nullptr;
   const uint32_t base = (uint32_t)start;
 
-  WarpSelect<NQ, NB> q;
-  q.init(smem_keys + warp * warp_select_smem_keys<NB>(), lane);
-
-  // One element per lane with explicit validity (head, tail, and the indexed pass).
-  auto scalar_round = [&](int64_t e) {
-    bool ok = e < len;
-    float v = 0.f;
-    uint32_t idx = 0;
-    if (ok) {
-      v = p[e];
-      if (pi) {
-        const int32_t t = pi[e];
-        ok = t >= 0;
-        idx = (uint32_t)t;
-      } else {
-        idx = base + (uint32_t)e;
-      }
-    }
-    const uint64_t key = make_key(v, idx);
-    q.push(ok && q.maybe(v) && q.wants(key), key);
-  };
+  TSel<NQ> q;
+  q.init(smem_keys + (size_t)warp * (32 * LCAP), lane);
 
   if (pi) {
-    for (int64_t e0 = 0; e0 < len; e0 += 32) scalar_round(e0 + lane);
+    // pass >= 2: (value, index) pairs in arbitrary index order; index -1 = padding
+    for (int64_t e0 = 0; e0 < len; e0 += 32) {
+      const int64_t e = e0 + lane;
+      bool ok = e < len;
+      float v = 0.f;
+      int32_t t = -1;
+      if (ok) {
+        v = p[e];
+        t = pi[e];
+      }
+      q.push(ok && t >= 0, v, (uint32_t)t);
+      if (q.crowded()) q.flush(false);
+    }
+    q.flush(false);
   } else {
-    // peel to 16-byte alignment
     int64_t head = (4 - (int)(((uintptr_t)p >> 2) & 3)) & 3;
     if (head > len) head = len;
-    if (head) scalar_round(lane < head ? lane : len);
     const float* pv = p + head;
     const int64_t nvec = (len - head) >> 2;
     const uint32_t vbase = base + (uint32_t)head;
+    const int64_t done = head + (nvec << 2);
+    // elements of the sample that should pass so that ~MSTAR of the chunk do
+    float rho = (float)TSelCfg<NQ>::MSTAR * (float)SAMPLE / (float)(len > 0 ? len : 1);
+    if (rho < 12.f) rho = 12.f;
+    const int rho_lo = (int)rho, rho_hi = (int)(rho * 1.25f) + 1;
+    const bool can_sample = nvec >= U * 32 && rho_hi < SAMPLE / 2;
+    const int64_t want = a.k < len ? a.k : len;
 
-    auto consume = [&](const float4& x, int64_t v) {
-      const bool any = q.maybe(x.x) | q.maybe(x.y) | q.maybe(x.z) | q.maybe(x.w);
-      if (__any_sync(kFull, any)) {
-        const uint32_t i0 = vbase + (uint32_t)(v << 2);
-        const float xs[4] = {x.x, x.y, x.z, x.w};
-#pragma unroll 1
-        for (int t = 0; t < 4; ++t) {
-          const float xv = t == 0 ? xs[0] : t == 1 ? xs[1] : t == 2 ? xs[2] : xs[3];
-          const uint64_t key = make_key(xv, i0 + t);
-          q.push(q.maybe(xv) && q.wants(key), key);
-        }
-      }
+    auto push4 = [&](const float4& x, int64_t v, bool ok) {
+      const uint32_t i0 = vbase + (uint32_t)(v << 2);
+      q.push(ok, x.x, i0);
+      q.push(ok, x.y, i0 + 1);
+      q.push(ok, x.z, i0 + 2);
+      q.push(ok, x.w, i0 + 3);
     };
 
-    constexpr int U = 4;
-    int64_t v0 = 0;
-    for (; v0 + U * 32 <= nvec; v0 += U * 32) {
-      float4 x[U];
+#pragma unroll 1
+    for (int attempt = 0; attempt < 2; ++attempt) {
+      const bool sampled = attempt == 0 && can_sample;
+      q.reset();
+      if (head) q.push(lane < head, lane < head ? p[lane] : 0.f, base + lane);
+      if (sampled) {
+        // counting bisection in the order image over the first SAMPLE elements:
+        // find o with rho_lo <= #(v <= o) <= rho_hi.  No call while x[] is live.
+        float4 x[U];
 #pragma unroll
-      for (int u = 0; u < U; ++u) x[u] = ld_stream4(pv + ((v0 + u * 32 + lane) << 2));
+        for (int u = 0; u < U; ++u) x[u] = ld_stream4(pv + ((int64_t)(u * 32 + lane) << 2));
+        uint32_t lo = 0u, hi = 0xFF800000u, pick = 0xFF800000u;
 #pragma unroll 1
-      for (int u = 0; u < U; ++u) {
-        const float4 xu = u == 0 ? x[0] : u == 1 ? x[1] : u == 2 ? x[2] : x[3];
-        consume(xu, v0 + u * 32 + lane);
+        for (int it = 0; it < 34 && hi - lo > 1u; ++it) {
+          const uint32_t mid = lo + ((hi - lo) >> 1);
+          const float tf = ord_f32(mid);
+          int cme = 0;
+#pragma unroll
+          for (int u = 0; u < U; ++u)
+            cme += (x[u].x <= tf) + (x[u].y <= tf) + (x[u].z <= tf) + (x[u].w <= tf);
+          const int cw = __reduce_add_sync(kFull, cme);
+          if (cw < rho_lo) {
+            lo = mid;
+          } else {
+            hi = mid;
+            pick = mid;
+            if (cw <= rho_hi) break;
+          }
+        }
+        q.set_sampled_bound(pick);
       }
-    }
-    for (; v0 < nvec; v0 += 32) {
-      const int64_t v = v0 + lane;
-      const bool ok = v < nvec;
-      float4 x = make_float4(0.f, 0.f, 0.f, 0.f);
-      if (ok) x = ld_stream4(pv + (v << 2));
-      const uint32_t i0 = vbase + (uint32_t)(v << 2);
-#pragma unroll 1
-      for (int t = 0; t < 4; ++t) {
-        const float xv = t == 0 ? x.x : t == 1 ? x.y : t == 2 ? x.z : x.w;
-        const uint64_t key = make_key(xv, i0 + t);
-        q.push(ok && q.maybe(xv) && q.wants(key), key);
+      // Stream.  A batch stops early when a lane queue runs full; the restore
+      // step is called at ONE site where no loaded data is live, and the batch
+      // restarts behind the last 128-bit group that was consumed.
+      int64_t v0 = 0;
+      while (v0 + U * 32 <= nvec) {
+        float4 x[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) x[u] = ld_stream4(pv + ((v0 + u * 32 + lane) << 2));
+        int used = U;
+        bool full = false;
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+          if (!full) {
+            push4(x[u], v0 + u * 32 + lane, true);
+            full = q.crowded();
+            if (full) used = u + 1;
+          }
+        }
+        v0 += used * 32;
+        if (full) q.flush(true);
       }
+      for (; v0 < nvec; v0 += 32) {
+        const int64_t v = v0 + lane;
+        const bool ok = v < nvec;
+        float4 x = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (ok) x = ld_stream4(pv + (v << 2));
+        push4(x, v, ok);
+        if (q.crowded()) q.flush(true);
+      }
+      if (done < len) {
+        const bool ok = done + lane < len;
+        q.push(ok, ok ? p[done + lane] : 0.f, base + (uint32_t)(done + lane));
+      }
+      q.flush(true);
+      // the sampled bound let fewer than k elements through: scan again with the
+      // adaptive bound only (exact in every case)
+      if (!sampled || q.exact || q.total >= want) break;
     }
-    const int64_t done = head + (nvec << 2);
-    if (done < len) scalar_round(done + lane);
   }
-  q.finish();
 
-  // A3: W is the answer; element i = r*32 + lane.
+  // A3: buf[swz<NQ>(i)] is the i-th smallest key.  The value is rebuilt from the
+  // key's order image, except for the two images that are not injective (+-0 and
+  // NaN), which are re-read from the row so that the original bits come back.
   const float* g = a.gather + row * a.gather_ld;
   float* ov = a.out_val + item * a.k;
   int32_t* oi = a.out_idx + item * a.k;
-#pragma unroll
-  for (int r = 0; r < NQ; ++r) {
-    const int i = r * 32 + lane;
-    if (i < a.k) {
-      const uint64_t key = q.W[r];
-      if (key == kSentinelKey) {
-        ov[i] = __uint_as_float(0x7F800000u);
-        oi[i] = -1;
-      } else {
-        const uint32_t idx = key_idx(key);
-        ov[i] = g[idx];
-        oi[i] = (int32_t)idx;
-      }
+  for (int i = lane; i < a.k; i += 32) {
+    const uint64_t key = q.buf[swz<NQ>(i)];
+    if (key == kSentinelKey) {
+      ov[i] = __uint_as_float(0x7F800000u);
+      oi[i] = -1;
+    } else {
+      const uint32_t idx = key_idx(key), o = (uint32_t)(key >> 32);
+      ov[i] = (o == 0x80000000u || o == 0xFFFFFFFFu) ? g[idx] : ord_f32(o);
+      oi[i] = (int32_t)idx;
     }
   }
 }
@@ -276,14 +313,23 @@ int plan_passes(int64_t n_rows, int64_t n, int k, Pass* out) {
   return np;
 }
 
-template <int NQ, int NB>
+template <int NQ>
 int launch_warp(const KSelArgs& a, cudaStream_t s) {
+  constexpr int WARPS = TSelCfg<NQ>::WARPS;
   const int64_t items = a.n_rows * a.P;
   if (items == 0) return FS_OK;
-  const size_t smem = (size_t)kWarpsPerCta * warp_select_smem_keys<NB>() * sizeof(uint64_t);
-  const int64_t grid = ceil_div(items, kWarpsPerCta);
+  const size_t smem = (size_t)WARPS * 32 * TSelCfg<NQ>::LCAP * sizeof(uint64_t);
+  static bool attr_done = false;
+  if (!attr_done) {
+    FS_CUDA(cudaFuncSetAttribute(kselect_warp_kernel<NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)smem));
+    FS_CUDA(cudaFuncSetAttribute(kselect_warp_kernel<NQ>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                                 cudaSharedmemCarveoutMaxShared));
+    attr_done = true;
+  }
+  const int64_t grid = ceil_div(items, WARPS);
   if (grid > 0x7fffffffLL) return set_error(FS_EUNSUPPORTED, "too many rows for one launch");
-  kselect_warp_kernel<NQ, NB, kWarpsPerCta><<<(unsigned)grid, kWarpsPerCta * 32, smem, s>>>(a);
+  kselect_warp_kernel<NQ><<<(unsigned)grid, WARPS * 32, smem, s>>>(a);
   FS_LAUNCHED();
   return FS_OK;
 }
@@ -299,12 +345,12 @@ int launch_pass(const KSelArgs& a, cudaStream_t s) {
     FS_LAUNCHED();
     return FS_OK;
   }
-  if (k <= 32) return launch_warp<1, 1>(a, s);
-  if (k <= 64) return launch_warp<2, 2>(a, s);
-  if (k <= 128) return launch_warp<4, 4>(a, s);
-  if (k <= 256) return launch_warp<8, 8>(a, s);
-  if (k <= 512) return launch_warp<16, 8>(a, s);
-  return launch_warp<32, 8>(a, s);
+  if (k <= 32) return launch_warp<1>(a, s);
+  if (k <= 64) return launch_warp<2>(a, s);
+  if (k <= 128) return launch_warp<4>(a, s);
+  if (k <= 256) return launch_warp<8>(a, s);
+  if (k <= 512) return launch_warp<16>(a, s);
+  return launch_warp<32>(a, s);
 }
 
 int validate(const void* rows, int64_t n_rows, int64_t n, int64_t ld, int k, const void* ov,
