@@ -291,6 +291,16 @@ def run_ours(args):
               4 * N_ROWS * N_COLS + 8 * N_ROWS * k) for k in KS]
     calls.append(("bigrow_k1024", lambda: fs.kselect(big, BIG_K, out_val=bout[0], out_idx=bout[1], ws=ws),
                   4 * BIG_N + 8 * BIG_K))
+    if args.case:  # profiling aid: only the named call(s) of the step, no e2e / also / cpu legs
+        calls = [c for c in calls if c[0] in args.case.split(",")]
+        for _ in range(max(args.warmup, 1)):
+            for _, fn, _ in calls:
+                fn()
+        torch.cuda.synchronize()
+        for name, fn, nbytes in calls:
+            best, med = timed(fn, max(args.steps, 1), warm=0)
+            print(json.dumps({"case": name, "ms": med, "GBps": nbytes / med / 1e6, "frac": nbytes / med / 1e6 / pk["hbm"]}))
+        return
     per_call = {name: [] for name, _, _ in calls}
 
     def step(record=False):
@@ -424,6 +434,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--skip-also", action="store_true")
     ap.add_argument("--ivfpq-nb", type=int, default=10_000_000)
+    ap.add_argument("--case", default="", help="comma list of k1,k32,k128,k1024,bigrow_k1024: time only these calls")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
