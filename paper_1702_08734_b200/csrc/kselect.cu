@@ -1,15 +1,23 @@
 // kselect.cu -- fs_kselect: batched k-selection.
 //
-//   A1 stream + first-level filter   kselect_warp_kernel main loop
-//   A2 restore invariants            warp_flush<NQ,NB> in select.cuh
-//   A3 output                        final flush + gather of the original bits
-//   A4 long rows                     rows are cut into P chunks, one warp each; the
-//                                    P*k partial results are selected again
+//   A1 stream + first-level filter   kselect_stream_kernel main loop
+//   A2 restore invariants            tsel_flush in tselect.cuh
+//   A3 output                        final sort + gather of the original bits
+//   A4 long rows                     rows are cut into P chunks; every chunk
+//                                    keeps its k smallest keys, the largest of the
+//                                    chunks' j-th smallest keys (j = ceil(k/(P-1)))
+//                                    bounds the row's k-th key from above, only keys
+//                                    under that bound are gathered and selected again
 //   A5 k = 1                         kselect_k1_kernel: min/argmin reduction
 //
-// One warp owns one work item (a row, or a chunk of a row); lane j reads elements
-// 4j..4j+3 of each 128-element group with one 128-bit load (the vectorised form
-// of "lane j reads a_{32i+j}"), four groups in flight per lane.
+// One warp owns one work item (a row, or a chunk of a row).  Warps are persistent:
+// warp w takes items w, w + W, ...  The 16-byte aligned body of each item reaches
+// the warp through a private ring of 2 KB segments in shared memory filled by
+// cp.async.bulk (the TMA bulk-copy engine) and tracked by mbarriers, so several
+// segments per warp are in flight whatever the register budget, and the ring runs
+// ahead across item boundaries (the next row is already arriving while the current
+// one is being selected).  "Lane j reads a_{32i+j}" becomes: lane j reads
+// elements 4j..4j+3 of each 128-element group with one 128-bit shared-memory load.
 #include "common.cuh"
 #include "select.cuh"
 #include "tselect.cuh"
@@ -17,168 +25,163 @@
 namespace fs {
 
 struct KSelArgs {
-  const float* vals;     // [n_rows][ld] values to select from
-  const int32_t* in_idx; // optional [n_rows][ld]: index each value stands for (pass >= 2); -1 = skip
+  const float* vals;  // [n_rows][ld]
   int64_t n_rows, n, ld;
-  int P;                 // chunks per row
-  int64_t chunk;         // elements per chunk (multiple of 4)
-  const float* gather;   // original rows: out_val = gather[row*gather_ld + idx]
-  int64_t gather_ld;
-  float* out_val;        // [n_rows][P][k]
-  int32_t* out_idx;
+  int P;              // chunks per row
+  int64_t chunk;      // elements per chunk (multiple of 4)
   int k;
+  float* out_val;     // P == 1: [n_rows][k]
+  int32_t* out_idx;
+  uint64_t* out_keys;  // P > 1: [n_rows][P][k] sorted keys, sentinel padded
+  uint64_t* heads;     // P > 1: [n_rows][P-1][jth] the jth smallest keys of every chunk but the last
+  int jth;             // ceil(k / (P - 1))
+  unsigned int* work;  // item counter of the persistent warps (zero before the launch)
 };
 
-__device__ __forceinline__ float4 ld_stream4(const float* p) {
-  float4 r;
-  asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];"
-               : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w)
-               : "l"(p));
-  return r;
+// ---- mbarrier / bulk-copy PTX --------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+  return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      "WAIT_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra DONE_%=;\n\t"
+      "bra WAIT_%=;\n\t"
+      "DONE_%=:\n\t"
+      "}" ::"r"(smem_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+// global -> shared bulk copy (16-byte aligned, size a multiple of 16), completion on bar
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+          smem_u32(dst)),
+      "l"(src), "r"(bytes), "r"(smem_u32(bar))
+      : "memory");
 }
 
-// ---------------------------------------------------------------------------
-// General k: one warp per (row, chunk); threshold-filtered selection (tselect.cuh).
-// ---------------------------------------------------------------------------
-template <int NQ>
-__global__ void __launch_bounds__(TSelCfg<NQ>::WARPS * 32) kselect_warp_kernel(const KSelArgs a) {
-  constexpr int WARPS = TSelCfg<NQ>::WARPS;
-  constexpr int LCAP = TSelCfg<NQ>::LCAP;
-  constexpr int U = 8;          // 128-bit loads in flight per lane
-  constexpr int SAMPLE = 1024;  // elements of the row used to place the first bound
-  extern __shared__ __align__(16) uint64_t smem_keys[];
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int64_t item = (int64_t)blockIdx.x * WARPS + warp;
-  if (item >= a.n_rows * a.P) return;
-  const int64_t row = item / a.P;
-  const int c = (int)(item - row * a.P);
-  const int64_t start = (int64_t)c * a.chunk;
+constexpr int kSeg = 512;    // floats per ring segment (2 KB)
+constexpr int kStages = 4;   // ring depth per warp
+constexpr int kSample = 1024;
+
+struct ItemDesc {
+  const float* p;   // first element of the item
+  int64_t len;      // elements
+  int64_t row;
+  int c;            // chunk number
+  uint32_t base;    // index of p[0] in the row
+  int head;         // scalars before the aligned body
+  int64_t nvec;     // float4 in the body
+  int nseg;         // ring segments of the body
+};
+
+__device__ __forceinline__ ItemDesc decode_item(const KSelArgs& a, int64_t item) {
+  ItemDesc d;
+  d.row = item / a.P;
+  d.c = (int)(item - d.row * a.P);
+  const int64_t start = (int64_t)d.c * a.chunk;
   int64_t len = a.n - start;
   if (len > a.chunk) len = a.chunk;
   if (len < 0) len = 0;
-  const float* p = a.vals + row * a.ld + start;
-  const int32_t* pi = a.in_idx ? a.in_idx + row * a.ld + start : nullptr;
-  const uint32_t base = (uint32_t)start;
+  d.len = len;
+  d.p = a.vals + d.row * a.ld + start;
+  d.base = (uint32_t)start;
+  int64_t head = (4 - (int)(((uintptr_t)d.p >> 2) & 3)) & 3;
+  if (head > len) head = len;
+  d.head = (int)head;
+  d.nvec = (len - head) >> 2;
+  d.nseg = (int)((d.nvec + (kSeg / 4 - 1)) / (kSeg / 4));
+  return d;
+}
 
-  TSel<NQ> q;
-  q.init(smem_keys + (size_t)warp * (32 * LCAP), lane);
+// Per-warp ring: the producer side runs ahead of the consumer, at most into the
+// item after the one being consumed.  Items are handed out dynamically (one atomic
+// per item), so a late or slow warp never holds a fixed share of the work.
+struct Ring {
+  float* data;     // [kStages][kSeg]
+  uint64_t* bar;   // [kStages]
+  uint32_t issued, consumed;
+  int64_t c_item;  // item being consumed
+  int64_t n_item;  // the item after it (-1: not drawn yet)
+  int64_t p_item;  // item the producer is issuing (c_item or n_item)
+  const float* p_ptr;  // next segment of p_item
+  int p_left;          // float4 of p_item not yet issued
+};
 
-  if (pi) {
-    // pass >= 2: (value, index) pairs in arbitrary index order; index -1 = padding
-    for (int64_t e0 = 0; e0 < len; e0 += 32) {
-      const int64_t e = e0 + lane;
-      bool ok = e < len;
-      float v = 0.f;
-      int32_t t = -1;
-      if (ok) {
-        v = p[e];
-        t = pi[e];
-      }
-      q.push(ok && t >= 0, v, (uint32_t)t);
-      if (q.crowded()) q.flush(false);
-    }
-    q.flush(false);
-  } else {
-    int64_t head = (4 - (int)(((uintptr_t)p >> 2) & 3)) & 3;
-    if (head > len) head = len;
-    const float* pv = p + head;
-    const int64_t nvec = (len - head) >> 2;
-    const uint32_t vbase = base + (uint32_t)head;
-    const int64_t done = head + (nvec << 2);
-    // elements of the sample that should pass so that ~MSTAR of the chunk do
-    float rho = (float)TSelCfg<NQ>::MSTAR * (float)SAMPLE / (float)(len > 0 ? len : 1);
-    if (rho < 12.f) rho = 12.f;
-    const int rho_lo = (int)rho, rho_hi = (int)(rho * 1.25f) + 1;
-    const bool can_sample = nvec >= U * 32 && rho_hi < SAMPLE / 2;
-    const int64_t want = a.k < len ? a.k : len;
+__device__ __forceinline__ int64_t draw_item(const KSelArgs& a, int64_t n_warps, int lane) {
+  unsigned int t = 0;
+  if (lane == 0) t = atomicAdd(a.work, 1u);
+  t = __shfl_sync(kFull, t, 0);
+  return (int64_t)t + n_warps;
+}
 
-    auto push4 = [&](const float4& x, int64_t v, bool ok) {
-      const uint32_t i0 = vbase + (uint32_t)(v << 2);
-      q.push(ok, x.x, i0);
-      q.push(ok, x.y, i0 + 1);
-      q.push(ok, x.z, i0 + 2);
-      q.push(ok, x.w, i0 + 3);
-    };
+__device__ __forceinline__ void ring_point(const KSelArgs& a, Ring& r, int64_t n_items) {
+  r.p_left = 0;
+  if (r.p_item < n_items) {
+    const ItemDesc d = decode_item(a, r.p_item);
+    r.p_ptr = d.p + d.head;
+    r.p_left = (int)d.nvec;
+  }
+}
 
-#pragma unroll 1
-    for (int attempt = 0; attempt < 2; ++attempt) {
-      const bool sampled = attempt == 0 && can_sample;
-      q.reset();
-      if (head) q.push(lane < head, lane < head ? p[lane] : 0.f, base + lane);
-      if (sampled) {
-        // counting bisection in the order image over the first SAMPLE elements:
-        // find o with rho_lo <= #(v <= o) <= rho_hi.  No call while x[] is live.
-        float4 x[U];
-#pragma unroll
-        for (int u = 0; u < U; ++u) x[u] = ld_stream4(pv + ((int64_t)(u * 32 + lane) << 2));
-        uint32_t lo = 0u, hi = 0xFF800000u, pick = 0xFF800000u;
-#pragma unroll 1
-        for (int it = 0; it < 34 && hi - lo > 1u; ++it) {
-          const uint32_t mid = lo + ((hi - lo) >> 1);
-          const float tf = ord_f32(mid);
-          int cme = 0;
-#pragma unroll
-          for (int u = 0; u < U; ++u)
-            cme += (x[u].x <= tf) + (x[u].y <= tf) + (x[u].z <= tf) + (x[u].w <= tf);
-          const int cw = __reduce_add_sync(kFull, cme);
-          if (cw < rho_lo) {
-            lo = mid;
-          } else {
-            hi = mid;
-            pick = mid;
-            if (cw <= rho_hi) break;
-          }
-        }
-        q.set_sampled_bound(pick);
+// Issue bulk copies until the ring is full or the producer may not advance.
+// All lanes keep the cursor (uniform); lane 0 issues.
+__device__ __forceinline__ void ring_fill(const KSelArgs& a, Ring& r, int64_t n_items, int64_t n_warps,
+                                          int lane) {
+  while (r.issued - r.consumed < (uint32_t)kStages) {
+    if (r.p_left > 0) {
+      const int slot = (int)(r.issued % kStages);
+      const int n4 = r.p_left < kSeg / 4 ? r.p_left : kSeg / 4;
+      if (lane == 0) {
+        mbar_expect_tx(r.bar + slot, (uint32_t)n4 * 16u);
+        bulk_g2s(r.data + slot * kSeg, r.p_ptr, (uint32_t)n4 * 16u, r.bar + slot);
       }
-      // Stream.  A batch stops early when a lane queue runs full; the restore
-      // step is called at ONE site where no loaded data is live, and the batch
-      // restarts behind the last 128-bit group that was consumed.
-      int64_t v0 = 0;
-      while (v0 + U * 32 <= nvec) {
-        float4 x[U];
-#pragma unroll
-        for (int u = 0; u < U; ++u) x[u] = ld_stream4(pv + ((v0 + u * 32 + lane) << 2));
-        int used = U;
-        bool full = false;
-#pragma unroll
-        for (int u = 0; u < U; ++u) {
-          if (!full) {
-            push4(x[u], v0 + u * 32 + lane, true);
-            full = q.crowded();
-            if (full) used = u + 1;
-          }
-        }
-        v0 += used * 32;
-        if (full) q.flush(true);
-      }
-      for (; v0 < nvec; v0 += 32) {
-        const int64_t v = v0 + lane;
-        const bool ok = v < nvec;
-        float4 x = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (ok) x = ld_stream4(pv + (v << 2));
-        push4(x, v, ok);
-        if (q.crowded()) q.flush(true);
-      }
-      if (done < len) {
-        const bool ok = done + lane < len;
-        q.push(ok, ok ? p[done + lane] : 0.f, base + (uint32_t)(done + lane));
-      }
-      q.flush(true);
-      // the sampled bound let fewer than k elements through: scan again with the
-      // adaptive bound only (exact in every case)
-      if (!sampled || q.exact || q.total >= want) break;
+      ++r.issued;
+      r.p_ptr += kSeg;
+      r.p_left -= n4;
+    } else if (r.p_item == r.c_item && r.c_item < n_items) {
+      r.n_item = draw_item(a, n_warps, lane);
+      r.p_item = r.n_item;
+      ring_point(a, r, n_items);
+    } else {
+      break;
     }
   }
+}
 
-  // A3: buf[swz<NQ>(i)] is the i-th smallest key.  The value is rebuilt from the
-  // key's order image, except for the two images that are not injective (+-0 and
-  // NaN), which are re-read from the row so that the original bits come back.
-  const float* g = a.gather + row * a.gather_ld;
-  float* ov = a.out_val + item * a.k;
-  int32_t* oi = a.out_idx + item * a.k;
-  for (int i = lane; i < a.k; i += 32) {
-    const uint64_t key = q.buf[swz<NQ>(i)];
+// ---------------------------------------------------------------------------
+// General k: persistent warps, one item at a time, threshold-filtered selection.
+// ---------------------------------------------------------------------------
+template <int NQ>
+struct StreamSmem {
+  static constexpr int WARPS = TSelCfg<NQ>::WARPS;
+  static constexpr int LCAP = TSelCfg<NQ>::LCAP;
+  static constexpr size_t ring_bytes = (size_t)kStages * kSeg * sizeof(float);
+  static constexpr size_t queue_bytes = (size_t)32 * LCAP * sizeof(uint64_t);
+  static constexpr size_t scratch_bytes = sel_scratch_bytes<TSelCfg<NQ>::RB>();
+  static constexpr size_t per_warp = ring_bytes + queue_bytes + scratch_bytes;
+  static constexpr size_t total = per_warp * WARPS + (size_t)WARPS * kStages * sizeof(uint64_t);
+};
+
+// Writes the k winners of one item/row, sorted: values + indices (final) or keys.
+template <int NQ>
+__device__ __forceinline__ void write_sorted(const uint64_t* buf, int k, int lane, const float* g,
+                                             float* ov, int32_t* oi) {
+  // the value is rebuilt from the key's order image, except for the two images that are
+  // not injective (+-0 and NaN), which are re-read from the row (original bits, A3)
+  for (int i = lane; i < k; i += 32) {
+    const uint64_t key = buf[swz<NQ>(i)];
     if (key == kSentinelKey) {
       ov[i] = __uint_as_float(0x7F800000u);
       oi[i] = -1;
@@ -190,167 +193,464 @@ __global__ void __launch_bounds__(TSelCfg<NQ>::WARPS * 32) kselect_warp_kernel(c
   }
 }
 
+template <int NQ>
+__global__ void __launch_bounds__(TSelCfg<NQ>::WARPS * 32) kselect_stream_kernel(const KSelArgs a) {
+  using SM = StreamSmem<NQ>;
+  constexpr int WARPS = SM::WARPS;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  unsigned char* mine = smem_raw + (size_t)warp * SM::per_warp;
+  Ring ring;
+  ring.data = reinterpret_cast<float*>(mine);
+  uint64_t* qbuf = reinterpret_cast<uint64_t*>(mine + SM::ring_bytes);
+  uint32_t* scratch = reinterpret_cast<uint32_t*>(mine + SM::ring_bytes + SM::queue_bytes);
+  ring.bar = reinterpret_cast<uint64_t*>(smem_raw + SM::per_warp * WARPS) + warp * kStages;
+  if (lane == 0) {
+#pragma unroll
+    for (int s = 0; s < kStages; ++s) mbar_init(ring.bar + s, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncwarp();
+
+  const int64_t n_items = a.n_rows * a.P;
+  const int64_t n_warps = (int64_t)gridDim.x * WARPS;
+  ring.issued = ring.consumed = 0;
+  ring.c_item = (int64_t)blockIdx.x * WARPS + warp;
+  ring.n_item = -1;
+  ring.p_item = ring.c_item;
+  ring_point(a, ring, n_items);
+  ring_fill(a, ring, n_items, n_warps, lane);
+
+  TSel<NQ> q;
+  q.init(qbuf, scratch, lane, a.k);
+
+  while (ring.c_item < n_items) {
+    const int64_t item = ring.c_item;
+    const ItemDesc d = decode_item(a, item);
+    const uint32_t vbase = d.base + (uint32_t)d.head;
+    const int64_t want = a.k < d.len ? a.k : d.len;
+    q.reset();
+    if (d.head) q.push(lane < d.head, lane < d.head ? d.p[lane] : 0.f, d.base + lane);
+
+    // sampled bound: counting bisection in the order image over the first kSample
+    // elements of the body (two ring segments): find o with rho_lo <= #(v <= o) <= rho_hi
+    const float rho = sample_target(a.k, kSample, d.len);
+    const int rho_lo = (int)rho + 1, rho_hi = rho_lo + (rho_lo >> 3) + 2;
+    const bool sampled = d.nvec >= kSample / 4 && rho_hi < kSample / 2;
+    if (sampled) {
+      const int s0 = (int)(ring.consumed % kStages), s1 = (int)((ring.consumed + 1) % kStages);
+      mbar_wait(ring.bar + s0, (ring.consumed / kStages) & 1u);
+      mbar_wait(ring.bar + s1, ((ring.consumed + 1) / kStages) & 1u);
+      float4 x[8];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        x[u] = reinterpret_cast<const float4*>(ring.data + s0 * kSeg)[u * 32 + lane];
+        x[4 + u] = reinterpret_cast<const float4*>(ring.data + s1 * kSeg)[u * 32 + lane];
+      }
+      uint32_t lo = 0u, hi = 0xFF800000u, pick = 0xFF800000u;
+#pragma unroll 1
+      for (int it = 0; it < 34 && hi - lo > 1u; ++it) {
+        const uint32_t mid = lo + ((hi - lo) >> 1);
+        const float tf = ord_f32(mid);
+        int cme = 0;
+#pragma unroll
+        for (int u = 0; u < 8; ++u)
+          cme += (x[u].x <= tf) + (x[u].y <= tf) + (x[u].z <= tf) + (x[u].w <= tf);
+        const int cw = __reduce_add_sync(kFull, cme);
+        if (cw < rho_lo) {
+          lo = mid;
+        } else {
+          hi = mid;
+          pick = mid;
+          if (cw <= rho_hi) break;
+        }
+      }
+      q.set_sampled_bound(pick);
+    }
+
+    // A1: stream the body segment by segment
+    const int nseg = d.nseg;
+#pragma unroll 1
+    for (int seg = 0; seg < nseg; ++seg) {
+      const int slot = (int)(ring.consumed % kStages);
+      mbar_wait(ring.bar + slot, (ring.consumed / kStages) & 1u);
+      const int left = (int)d.nvec - seg * (kSeg / 4);
+      const float4* sp = reinterpret_cast<const float4*>(ring.data + slot * kSeg) + lane;
+      const uint32_t ib = vbase + (uint32_t)seg * kSeg + (uint32_t)lane * 4u;
+      if (left >= kSeg / 4) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const float4 x = sp[u * 32];
+          const uint32_t i0 = ib + u * 128;
+          if (q.crowded(4)) q.flush(true);
+          q.push(true, x.x, i0);
+          q.push(true, x.y, i0 + 1);
+          q.push(true, x.z, i0 + 2);
+          q.push(true, x.w, i0 + 3);
+        }
+      } else {
+#pragma unroll 1
+        for (int u = 0; u < 4; ++u) {
+          const bool ok = u * 32 + lane < left;
+          float4 x = make_float4(0.f, 0.f, 0.f, 0.f);
+          if (ok) x = sp[u * 32];
+          const uint32_t i0 = ib + u * 128;
+          if (q.crowded(4)) q.flush(true);
+          q.push(ok, x.x, i0);
+          q.push(ok, x.y, i0 + 1);
+          q.push(ok, x.z, i0 + 2);
+          q.push(ok, x.w, i0 + 3);
+        }
+      }
+      __syncwarp();  // every lane is done with the slot before it is refilled
+      ++ring.consumed;
+      ring_fill(a, ring, n_items, n_warps, lane);
+    }
+    {  // scalar tail
+      const int64_t done = d.head + (d.nvec << 2);
+      if (done < d.len) {
+        if (q.crowded(1)) q.flush(true);
+        const bool ok = done + lane < d.len;
+        q.push(ok, ok ? d.p[done + lane] : 0.f, d.base + (uint32_t)(done + lane));
+      }
+    }
+    q.flush(true);
+    if (sampled && !q.exact && q.total < want) {
+      // the sampled bound let fewer than k elements through (~4 sigma): scan again with
+      // the paper's adaptive bound only (exact in every case; plain loads)
+      q.reset();
+#pragma unroll 1
+      for (int64_t e0 = 0; e0 < d.len; e0 += 128) {
+        float v[4];
+        bool ok[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const int64_t e = e0 + u * 32 + lane;
+          ok[u] = e < d.len;
+          v[u] = ok[u] ? d.p[e] : 0.f;
+        }
+        if (q.crowded(4)) q.flush(true);
+#pragma unroll
+        for (int u = 0; u < 4; ++u) q.push(ok[u], v[u], d.base + (uint32_t)(e0 + u * 32 + lane));
+      }
+      q.flush(true);
+    }
+
+    // A3 / A4 output.  Chunked rows (P > 1) write keys: the sorted winners, whose
+    // first `heads` entries also go to the row's head list for the bound of step 2.
+    sort_block<NQ>(q.buf, q.total);
+    if (a.P == 1) {
+      write_sorted<NQ>(q.buf, a.k, lane, a.vals + d.row * a.ld, a.out_val + d.row * a.k,
+                       a.out_idx + d.row * a.k);
+    } else {
+      uint64_t* ok = a.out_keys + item * a.k;
+      for (int i = lane; i < a.k; i += 32) ok[i] = q.buf[swz<NQ>(i)];
+      if (d.c != a.P - 1) {
+        uint64_t* hd = a.heads + (d.row * (a.P - 1) + d.c) * a.jth;
+        for (int i = lane; i < a.jth; i += 32) hd[i] = q.buf[swz<NQ>(i)];
+      }
+    }
+    __syncwarp();
+
+    // next item
+    if (ring.n_item < 0) ring.n_item = draw_item(a, n_warps, lane);
+    ring.c_item = ring.n_item;
+    ring.n_item = -1;
+    if (ring.p_item != ring.c_item) {
+      ring.p_item = ring.c_item;
+      ring_point(a, ring, n_items);
+    }
+    ring_fill(a, ring, n_items, n_warps, lane);
+  }
+}
+
 // ---------------------------------------------------------------------------
 // k = 1: min / argmin reduction on packed keys, one warp per (row, chunk).
 // ---------------------------------------------------------------------------
+__device__ __forceinline__ float4 ld_stream4(const float* p) {
+  float4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];"
+               : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w)
+               : "l"(p));
+  return r;
+}
+
 template <int WARPS>
 __global__ void __launch_bounds__(WARPS * 32) kselect_k1_kernel(const KSelArgs a) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int64_t item = (int64_t)blockIdx.x * WARPS + warp;
   if (item >= a.n_rows * a.P) return;
-  const int64_t row = item / a.P;
-  const int c = (int)(item - row * a.P);
-  const int64_t start = (int64_t)c * a.chunk;
-  int64_t len = a.n - start;
-  if (len > a.chunk) len = a.chunk;
-  if (len < 0) len = 0;
-  const float* p = a.vals + row * a.ld + start;
-  const int32_t* pi = a.in_idx ? a.in_idx + row * a.ld + start : nullptr;
-  const uint32_t base = (uint32_t)start;
+  const ItemDesc d = decode_item(a, item);
+  const float* p = d.p;
   uint64_t best = kSentinelKey;
-
-  if (pi) {
-    for (int64_t e = lane; e < len; e += 32) {
-      const int32_t t = pi[e];
-      if (t >= 0) best = umin64(best, make_key(p[e], (uint32_t)t));
-    }
-  } else {
-    int64_t head = (4 - (int)(((uintptr_t)p >> 2) & 3)) & 3;
-    if (head > len) head = len;
-    if (lane < head) best = umin64(best, make_key(p[lane], base + lane));
-    const float* pv = p + head;
-    const int64_t nvec = (len - head) >> 2;
-    const uint32_t vbase = base + (uint32_t)head;
-    // Per lane a running float minimum decides whether the exact key compare is
-    // needed at all: "!(v > m)" is true for v <= m and for NaN.
-    float m = __uint_as_float(0x7FFFFFFFu);
-    auto take = [&](float v, uint32_t idx) {
-      if (!(v > m)) {
-        const uint64_t key = make_key(v, idx);
-        if (key < best) {
-          best = key;
-          m = key_val(key);
-        }
-      }
-    };
-    constexpr int U = 4;
-    int64_t v0 = 0;
-    for (; v0 + U * 32 <= nvec; v0 += U * 32) {
-      float4 x[U];
-#pragma unroll
-      for (int u = 0; u < U; ++u) x[u] = ld_stream4(pv + ((v0 + u * 32 + lane) << 2));
-#pragma unroll
-      for (int u = 0; u < U; ++u) {
-        const uint32_t i0 = vbase + (uint32_t)((v0 + u * 32 + lane) << 2);
-        take(x[u].x, i0);
-        take(x[u].y, i0 + 1);
-        take(x[u].z, i0 + 2);
-        take(x[u].w, i0 + 3);
+  if (lane < d.head) best = umin64(best, make_key(p[lane], d.base + lane));
+  const float* pv = p + d.head;
+  const int64_t nvec = d.nvec;
+  const uint32_t vbase = d.base + (uint32_t)d.head;
+  // Per lane a running float minimum decides whether the exact key compare is
+  // needed at all: "!(v > m)" is true for v <= m and for NaN.
+  float m = __uint_as_float(0x7FFFFFFFu);
+  auto take = [&](float v, uint32_t idx) {
+    if (!(v > m)) {
+      const uint64_t key = make_key(v, idx);
+      if (key < best) {
+        best = key;
+        m = key_val(key);
       }
     }
-    for (int64_t v = v0 + lane; v < nvec; v += 32) {
-      const float4 x = ld_stream4(pv + (v << 2));
-      const uint32_t i0 = vbase + (uint32_t)(v << 2);
-      take(x.x, i0);
-      take(x.y, i0 + 1);
-      take(x.z, i0 + 2);
-      take(x.w, i0 + 3);
+  };
+  constexpr int U = 4;
+  int64_t v0 = 0;
+  for (; v0 + U * 32 <= nvec; v0 += U * 32) {
+    float4 x[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) x[u] = ld_stream4(pv + ((v0 + u * 32 + lane) << 2));
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const uint32_t i0 = vbase + (uint32_t)((v0 + u * 32 + lane) << 2);
+      take(x[u].x, i0);
+      take(x[u].y, i0 + 1);
+      take(x[u].z, i0 + 2);
+      take(x[u].w, i0 + 3);
     }
-    const int64_t done = head + (nvec << 2);
-    if (done + lane < len) take(p[done + lane], base + (uint32_t)(done + lane));
   }
+  for (int64_t v = v0 + lane; v < nvec; v += 32) {
+    const float4 x = ld_stream4(pv + (v << 2));
+    const uint32_t i0 = vbase + (uint32_t)(v << 2);
+    take(x.x, i0);
+    take(x.y, i0 + 1);
+    take(x.z, i0 + 2);
+    take(x.w, i0 + 3);
+  }
+  const int64_t done = d.head + (nvec << 2);
+  if (done + lane < d.len) take(p[done + lane], d.base + (uint32_t)(done + lane));
 #pragma unroll
   for (int s = 16; s >= 1; s >>= 1) best = umin64(best, shfl_xor64(best, s));
   if (lane == 0) {
-    if (best == kSentinelKey) {
+    if (a.P > 1) {
+      a.out_keys[item] = best;
+      if (d.c != a.P - 1) a.heads[d.row * (a.P - 1) + d.c] = best;
+    } else if (best == kSentinelKey) {
       a.out_val[item] = __uint_as_float(0x7F800000u);
       a.out_idx[item] = -1;
     } else {
       const uint32_t idx = key_idx(best);
-      a.out_val[item] = a.gather[row * a.gather_ld + idx];
+      a.out_val[item] = a.vals[d.row * a.ld + idx];
       a.out_idx[item] = (int32_t)idx;
     }
   }
 }
 
 // ---------------------------------------------------------------------------
-// Host side: plan of passes (A4) and launches.
+// A4, steps 2-4.  Step 2: the row's bound = the k-th smallest of the chunks' head
+// keys (every chunk but the last contributes its jth smallest, (P-1)*jth >= k of
+// them: real elements of the row, so their k-th smallest is >= the row's k-th
+// smallest).  Step 3: gather the chunk winners under the bound.  Step 4: select.
+// Steps 2 and 4 are the same kernel: one warp per row over a list of keys.
 // ---------------------------------------------------------------------------
-namespace {
-
-constexpr int kWarpsPerCta = 4;
-
-struct Pass {
-  int64_t n;  // elements per row entering this pass
-  int P;      // chunks per row
-  int64_t chunk;
-};
-
-// Rows are cut into chunks until one warp per row is enough to occupy the GPU or
-// a chunk would fall under max(4096, 8k) elements (below that the k outputs per
-// chunk dominate).  Returns the passes; the last one has P == 1.
-int plan_passes(int64_t n_rows, int64_t n, int k, Pass* out) {
-  const int64_t target_items = (int64_t)sm_count() * 16;
-  const int64_t min_chunk = k * 8 > 4096 ? (int64_t)k * 8 : 4096;
-  int np = 0;
-  while (np < 7) {
-    int64_t P = 1;
-    if (n_rows < target_items && n >= 2 * min_chunk) {
-      P = ceil_div(target_items, n_rows);
-      const int64_t pmax = n / min_chunk;
-      if (P > pmax) P = pmax;
-      if (P < 1) P = 1;
-    }
-    int64_t chunk = ceil_div(n, P);
-    chunk = (chunk + 3) / 4 * 4;
-    if (chunk < 4) chunk = 4;
-    P = n > 0 ? ceil_div(n, chunk) : 1;
-    out[np++] = Pass{n, (int)P, chunk};
-    if (P == 1) break;
-    n = P * k;
+__global__ void __launch_bounds__(256)
+    kselect_prune_kernel(const uint64_t* __restrict__ keys, int64_t n_lists, int P, int k,
+                         const unsigned long long* __restrict__ bound, uint64_t* __restrict__ cand,
+                         unsigned int* __restrict__ count) {
+  // a warp takes 256 consecutive keys of one list (lists are sorted: stop at the first miss)
+  const int lane = threadIdx.x & 31;
+  const int parts = (k + 255) / 256;
+  const int64_t w = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
+  const int64_t list = w / parts;
+  if (list >= n_lists) return;
+  const int i_begin = (int)(w - list * parts) * 256;
+  const int i_end = i_begin + 256 < k ? i_begin + 256 : k;
+  const int64_t row = list / P;
+  const uint64_t B = bound[row];
+  uint64_t* out = cand + row * ((int64_t)P * k);
+  for (int i0 = i_begin; i0 < i_end; i0 += 32) {
+    const int i = i0 + lane;
+    uint64_t key = kSentinelKey;
+    if (i < i_end) key = keys[list * k + i];
+    const bool keep = key != kSentinelKey && key <= B;
+    const unsigned b = __ballot_sync(kFull, keep);
+    if (b == 0u) break;
+    unsigned int pos = 0;
+    if (lane == 0) pos = atomicAdd(count + row, (unsigned int)__popc(b));
+    pos = __shfl_sync(kFull, pos, 0);
+    if (keep) out[pos + __popc(b & ((1u << lane) - 1u))] = key;
+    if (b != kFull) break;
   }
-  if (out[np - 1].P != 1) out[np++] = Pass{n, 1, (n + 3) / 4 * 4 > 4 ? (n + 3) / 4 * 4 : 4};
-  return np;
 }
 
 template <int NQ>
-int launch_warp(const KSelArgs& a, cudaStream_t s) {
-  constexpr int WARPS = TSelCfg<NQ>::WARPS;
+__global__ void __launch_bounds__(128)
+    kselect_keys_kernel(const uint64_t* __restrict__ src, const unsigned int* __restrict__ count,
+                        int64_t n_fixed, int64_t n_rows, int64_t cap, int k,
+                        const float* __restrict__ rows, int64_t ld, float* __restrict__ out_val,
+                        int32_t* __restrict__ out_idx, unsigned long long* __restrict__ bound_out) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  constexpr int LCAP = TSelCfg<NQ>::LCAP;
+  constexpr size_t per_warp = (size_t)32 * LCAP * sizeof(uint64_t) + sel_scratch_bytes<TSelCfg<NQ>::RB>();
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int64_t row = (int64_t)blockIdx.x * 4 + warp;
+  if (row >= n_rows) return;
+  unsigned char* mine = smem_raw + (size_t)warp * per_warp;
+  TSel<NQ> q;
+  q.init(reinterpret_cast<uint64_t*>(mine),
+         reinterpret_cast<uint32_t*>(mine + (size_t)32 * LCAP * sizeof(uint64_t)), lane, k);
+  const uint64_t* c = src + row * cap;
+  const int64_t n = count ? (int64_t)count[row] : n_fixed;
+#pragma unroll 1
+  for (int64_t e0 = 0; e0 < n; e0 += 128) {
+    uint64_t key[4];
+    bool ok[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int64_t e = e0 + u * 32 + lane;
+      ok[u] = e < n;
+      key[u] = ok[u] ? c[e] : kSentinelKey;
+    }
+    if (q.crowded(4)) q.flush(false);
+#pragma unroll
+    for (int u = 0; u < 4; ++u) q.push(ok[u] && key[u] != kSentinelKey, key_val(key[u]), key_idx(key[u]));
+  }
+  q.flush(false);
+  if (bound_out) {
+    if (lane == 0) bound_out[row] = q.total >= k ? q.thr_key : kSentinelKey;
+    return;
+  }
+  sort_block<NQ>(q.buf, q.total);
+  write_sorted<NQ>(q.buf, k, lane, rows + row * ld, out_val + row * k, out_idx + row * k);
+}
+
+// ---------------------------------------------------------------------------
+// Host side: plan (A4) and launches.
+// ---------------------------------------------------------------------------
+namespace {
+
+constexpr int kWarpsPerCtaK1 = 4;
+constexpr int kResidentWarpsPerSm = 12;  // planning estimate; the grid uses the real occupancy
+
+struct Plan {
+  int P;          // chunks per row
+  int64_t chunk;  // elements per chunk (multiple of 4)
+  int jth;        // head keys per chunk: ceil(k / (P - 1))
+  size_t off_work, off_keys, off_heads, off_cand, off_bound, off_count, bytes;  // workspace layout
+};
+
+// Rows are cut into chunks only when there are too few rows to occupy the GPU, and
+// never below max(4096, 8k) elements per chunk (below that the k outputs per chunk
+// dominate).  One chunk per resident warp.
+Plan make_plan(int64_t n_rows, int64_t n, int k) {
+  Plan p;
+  const int64_t resident = (int64_t)sm_count() * kResidentWarpsPerSm;
+  const int64_t min_chunk = k * 8 > 4096 ? (int64_t)k * 8 : 4096;
+  int64_t P = 1;
+  if (n_rows > 0 && n_rows * 2 <= resident && n >= 2 * min_chunk) {
+    P = resident / n_rows;
+    const int64_t pmax = n / min_chunk;
+    if (P > pmax) P = pmax;
+    if (P < 1) P = 1;
+  }
+  int64_t chunk = ceil_div(n > 0 ? n : 1, P);
+  chunk = (chunk + 3) / 4 * 4;
+  P = n > 0 ? ceil_div(n, chunk) : 1;
+  p.P = (int)P;
+  p.chunk = chunk;
+  p.jth = P > 1 ? (int)ceil_div(k, P - 1) : 1;
+  size_t o = 0;
+  p.off_work = o;
+  o += 256;
+  p.off_bound = o;
+  if (P > 1) o += align_up((size_t)n_rows * sizeof(unsigned long long), 256);
+  p.off_count = o;
+  if (P > 1) o += align_up((size_t)n_rows * sizeof(unsigned int), 256);
+  p.off_keys = o;
+  if (P > 1) o += align_up((size_t)n_rows * P * k * sizeof(uint64_t), 256);
+  p.off_heads = o;
+  if (P > 1) o += align_up((size_t)n_rows * (P - 1) * p.jth * sizeof(uint64_t), 256);
+  p.off_cand = o;
+  if (P > 1) o += align_up((size_t)n_rows * P * k * sizeof(uint64_t), 256);
+  p.bytes = o;
+  return p;
+}
+
+template <int NQ>
+int launch_stream(const KSelArgs& a, cudaStream_t s) {
+  using SM = StreamSmem<NQ>;
   const int64_t items = a.n_rows * a.P;
   if (items == 0) return FS_OK;
-  const size_t smem = (size_t)WARPS * 32 * TSelCfg<NQ>::LCAP * sizeof(uint64_t);
-  static bool attr_done = false;
-  if (!attr_done) {
-    FS_CUDA(cudaFuncSetAttribute(kselect_warp_kernel<NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)smem));
-    FS_CUDA(cudaFuncSetAttribute(kselect_warp_kernel<NQ>, cudaFuncAttributePreferredSharedMemoryCarveout,
+  static int ctas_per_sm = 0;
+  if (ctas_per_sm == 0) {
+    FS_CUDA(cudaFuncSetAttribute(kselect_stream_kernel<NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)SM::total));
+    FS_CUDA(cudaFuncSetAttribute(kselect_stream_kernel<NQ>, cudaFuncAttributePreferredSharedMemoryCarveout,
                                  cudaSharedmemCarveoutMaxShared));
-    attr_done = true;
+    int occ = 0;
+    FS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kselect_stream_kernel<NQ>, SM::WARPS * 32,
+                                                          SM::total));
+    ctas_per_sm = occ > 0 ? occ : 1;
   }
-  const int64_t grid = ceil_div(items, WARPS);
-  if (grid > 0x7fffffffLL) return set_error(FS_EUNSUPPORTED, "too many rows for one launch");
-  kselect_warp_kernel<NQ><<<(unsigned)grid, WARPS * 32, smem, s>>>(a);
+  int64_t grid = ceil_div(items, SM::WARPS);
+  const int64_t cap = (int64_t)sm_count() * ctas_per_sm;
+  if (grid > cap) grid = cap;
+  kselect_stream_kernel<NQ><<<(unsigned)grid, SM::WARPS * 32, SM::total, s>>>(a);
   FS_LAUNCHED();
   return FS_OK;
 }
 
-int launch_pass(const KSelArgs& a, cudaStream_t s) {
-  const int k = a.k;
-  if (k == 1) {
+struct KeysArgs {
+  const uint64_t* src;
+  const unsigned int* count;  // per-row length, or NULL: n_fixed
+  int64_t n_fixed, n_rows, cap;
+  int k;
+  const float* rows;
+  int64_t ld;
+  float* out_val;
+  int32_t* out_idx;
+  unsigned long long* bound_out;  // not NULL: write only the k-th smallest key
+};
+
+template <int NQ>
+int launch_keys(const KeysArgs& g, cudaStream_t s) {
+  const size_t smem = 4 * ((size_t)32 * TSelCfg<NQ>::LCAP * sizeof(uint64_t) + sel_scratch_bytes<TSelCfg<NQ>::RB>());
+  static bool attr_done = false;
+  if (!attr_done) {
+    FS_CUDA(cudaFuncSetAttribute(kselect_keys_kernel<NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)smem));
+    attr_done = true;
+  }
+  kselect_keys_kernel<NQ><<<(unsigned)ceil_div(g.n_rows, 4), 128, smem, s>>>(
+      g.src, g.count, g.n_fixed, g.n_rows, g.cap, g.k, g.rows, g.ld, g.out_val, g.out_idx, g.bound_out);
+  FS_LAUNCHED();
+  return FS_OK;
+}
+
+#define FS_KCLASS_DISPATCH(k, CALL)          \
+  do {                                       \
+    if ((k) <= 32) return CALL(1);           \
+    if ((k) <= 64) return CALL(2);           \
+    if ((k) <= 128) return CALL(4);          \
+    if ((k) <= 256) return CALL(8);          \
+    if ((k) <= 512) return CALL(16);         \
+    return CALL(32);                         \
+  } while (0)
+
+int launch_level1(const KSelArgs& a, cudaStream_t s) {
+  if (a.k == 1) {
     const int64_t items = a.n_rows * a.P;
     if (items == 0) return FS_OK;
-    const int64_t grid = ceil_div(items, kWarpsPerCta);
+    const int64_t grid = ceil_div(items, kWarpsPerCtaK1);
     if (grid > 0x7fffffffLL) return set_error(FS_EUNSUPPORTED, "too many rows for one launch");
-    kselect_k1_kernel<kWarpsPerCta><<<(unsigned)grid, kWarpsPerCta * 32, 0, s>>>(a);
+    kselect_k1_kernel<kWarpsPerCtaK1><<<(unsigned)grid, kWarpsPerCtaK1 * 32, 0, s>>>(a);
     FS_LAUNCHED();
     return FS_OK;
   }
-  if (k <= 32) return launch_warp<1>(a, s);
-  if (k <= 64) return launch_warp<2>(a, s);
-  if (k <= 128) return launch_warp<4>(a, s);
-  if (k <= 256) return launch_warp<8>(a, s);
-  if (k <= 512) return launch_warp<16>(a, s);
-  return launch_warp<32>(a, s);
+#define FS_CALL(NQ) launch_stream<NQ>(a, s)
+  FS_KCLASS_DISPATCH(a.k, FS_CALL);
+#undef FS_CALL
+}
+
+int launch_keys_any(const KeysArgs& g, cudaStream_t s) {
+#define FS_CALL(NQ) launch_keys<NQ>(g, s)
+  FS_KCLASS_DISPATCH(g.k, FS_CALL);
+#undef FS_CALL
 }
 
 int validate(const void* rows, int64_t n_rows, int64_t n, int64_t ld, int k, const void* ov,
@@ -367,53 +667,61 @@ int validate(const void* rows, int64_t n_rows, int64_t n, int64_t ld, int k, con
 }  // namespace
 
 // Selection over device rows; also used by the flat and IVFPQ drivers.
-size_t kselect_ws_bytes(int64_t n_rows, int64_t n, int k) {
-  Pass ps[8];
-  const int np = plan_passes(n_rows, n, k, ps);
-  size_t tot = 0;
-  for (int i = 0; i + 1 < np; ++i)
-    tot += align_up((size_t)n_rows * ps[i].P * k * sizeof(float), 256) +
-           align_up((size_t)n_rows * ps[i].P * k * sizeof(int32_t), 256);
-  return tot;
-}
+size_t kselect_ws_bytes(int64_t n_rows, int64_t n, int k) { return make_plan(n_rows, n, k).bytes; }
 
 int kselect_device(const float* rows, int64_t n_rows, int64_t n, int64_t ld, int k, float* out_val,
                    int32_t* out_idx, void* ws, cudaStream_t s) {
-  Pass ps[8];
-  const int np = plan_passes(n_rows, n, k, ps);
+  const Plan p = make_plan(n_rows, n, k);
   char* w = static_cast<char*>(ws);
-  const float* cur_val = rows;
-  const int32_t* cur_idx = nullptr;
-  int64_t cur_ld = ld;
-  for (int i = 0; i < np; ++i) {
-    KSelArgs a;
-    a.vals = cur_val;
-    a.in_idx = cur_idx;
-    a.n_rows = n_rows;
-    a.n = ps[i].n;
-    a.ld = cur_ld;
-    a.P = ps[i].P;
-    a.chunk = ps[i].chunk;
-    a.gather = rows;
-    a.gather_ld = ld;
-    a.k = k;
-    const bool last = (i == np - 1);
-    if (last) {
-      a.out_val = out_val;
-      a.out_idx = out_idx;
-    } else {
-      a.out_val = reinterpret_cast<float*>(w);
-      w += align_up((size_t)n_rows * ps[i].P * k * sizeof(float), 256);
-      a.out_idx = reinterpret_cast<int32_t*>(w);
-      w += align_up((size_t)n_rows * ps[i].P * k * sizeof(int32_t), 256);
-    }
-    const int rc = launch_pass(a, s);
-    if (rc != FS_OK) return rc;
-    cur_val = a.out_val;
-    cur_idx = a.out_idx;
-    cur_ld = (int64_t)ps[i].P * k;
-  }
-  return FS_OK;
+  KSelArgs a;
+  a.vals = rows;
+  a.n_rows = n_rows;
+  a.n = n;
+  a.ld = ld;
+  a.P = p.P;
+  a.chunk = p.chunk;
+  a.k = k;
+  a.out_val = out_val;
+  a.out_idx = out_idx;
+  a.out_keys = nullptr;
+  a.heads = nullptr;
+  a.jth = p.jth;
+  a.work = reinterpret_cast<unsigned int*>(w + p.off_work);
+  // work counter, and for chunked rows bound + count (adjacent): one memset
+  FS_CUDA(cudaMemsetAsync(w, 0, p.off_keys, s));
+  if (p.P == 1) return launch_level1(a, s);
+  a.out_keys = reinterpret_cast<uint64_t*>(w + p.off_keys);
+  a.heads = reinterpret_cast<uint64_t*>(w + p.off_heads);
+  unsigned long long* bound = reinterpret_cast<unsigned long long*>(w + p.off_bound);
+  unsigned int* count = reinterpret_cast<unsigned int*>(w + p.off_count);
+  uint64_t* cand = reinterpret_cast<uint64_t*>(w + p.off_cand);
+  int rc = launch_level1(a, s);  // step 1: per-chunk winners
+  if (rc != FS_OK) return rc;
+  KeysArgs g;
+  g.src = a.heads;  // step 2: bound = k-th smallest head key
+  g.count = nullptr;
+  g.n_fixed = (int64_t)(p.P - 1) * p.jth;
+  g.n_rows = n_rows;
+  g.cap = g.n_fixed;
+  g.k = k;
+  g.rows = rows;
+  g.ld = ld;
+  g.out_val = nullptr;
+  g.out_idx = nullptr;
+  g.bound_out = bound;
+  if ((rc = launch_keys_any(g, s)) != FS_OK) return rc;
+  const int64_t n_lists = n_rows * p.P;  // step 3: gather under the bound
+  const int64_t warps = n_lists * ((k + 255) / 256);
+  kselect_prune_kernel<<<(unsigned)ceil_div(warps, 8), 256, 0, s>>>(a.out_keys, n_lists, p.P, k, bound, cand,
+                                                                    count);
+  FS_LAUNCHED();
+  g.src = cand;  // step 4: select among the gathered keys
+  g.count = count;
+  g.cap = (int64_t)p.P * k;
+  g.out_val = out_val;
+  g.out_idx = out_idx;
+  g.bound_out = nullptr;
+  return launch_keys_any(g, s);
 }
 
 }  // namespace fs

@@ -2,23 +2,30 @@
 //
 // Contract = the paper's WarpSelect: after any prefix of the input the
 // state holds the k smallest (value, index) keys seen.  The mechanism is re-cut for
-// B200, where the instruction budget per streamed element is small (~20 lane
-// instructions at 60 % of HBM peak) and shared memory is large:
+// B200, where the instruction budget per streamed element is small (~35 warp
+// instructions per 32 elements at 60 % of HBM peak) and shared memory is large:
 //
 //   * first-level filter: ONE float compare per element against the
 //     current bound, exactly as in the paper; an accepted element is appended to
 //     a LANE-PRIVATE queue in shared memory (slot (j, lane) -> word j*32+lane:
 //     the "thread queue" of P:L218, but LCAP-deep and outside the register file),
 //     with no ballot, shuffle or branch on the hot path;
-//   * restore step: only when some lane's queue is full (rare) or at
-//     the end of the row.  The ragged queues are compacted in place, sorted in
-//     blocks of <= 1024 keys with a bitonic network on registers in BLOCKED layout
-//     (15 cross-lane steps for any size; power-of-two sizes with sentinel padding
-//     instead of the odd-size networks of Alg. 1-2) and min-merged to the k
-//     smallest; the k-th key becomes the new exact bound;
+//   * restore step: only when some lane's queue is nearly full (rare)
+//     or at the end of the row.  The ragged queues are compacted in place and the
+//     exact k-th smallest key is found by RADIX SELECTION (6-bit digits, lane-
+//     private 16-bit counters in shared memory: no atomics, no bank conflicts);
+//     the k winners are compacted again and the k-th key becomes the new bound.
+//     No sorting network runs here: the paper's sort+merge of thread queues and
+//     warp queue (Alg. 1-3) is replaced by counting, which is O(m) with a small
+//     constant and a small code footprint (the unrolled networks of a k = 1024
+//     queue do not fit the instruction cache, profiles/r01);
+//   * output: ONE bitonic network on registers (blocked layout, 15
+//     cross-lane steps for any size; power-of-two sizes with sentinel padding
+//     instead of the odd-size networks of Alg. 1-2) sorts the k winners at the
+//     very end of the row;
 //   * the initial bound is not +inf: the first 1024 elements of the row are used
 //     as a sample, and a counting bisection on them picks a value that about
-//     m* = 1.5k..6k elements of the whole row are expected to pass, so a typical
+//     m* = 1.25k..6k elements of the whole row are expected to pass, so a typical
 //     row needs exactly one restore step.  If fewer than k elements passed, the
 //     row is scanned again with the paper's adaptive bound (+inf start); the
 //     result is exact either way.
@@ -31,7 +38,7 @@
 
 namespace fs {
 
-// ---- sorting networks on registers, blocked layout (element e = lane*NB + r) ----
+// ---- sorting network on registers, blocked layout (element e = lane*NB + r) ----
 // Bitonic sort in the "flip" form: a merge stage of size sz first compares e with
 // e ^ (sz - 1) (the mirrored element of the other sorted half), then runs the usual
 // half-cleaners e <-> e ^ j, j = sz/4 .. 1.  Every comparator then points the same
@@ -44,14 +51,12 @@ __device__ __forceinline__ void cmpex_up(uint64_t& a, uint64_t& b) {
 }
 
 template <int NB>
-__device__ __forceinline__ void local_halfcleaners(uint64_t (&B)[NB], int jmax) {
+__device__ __forceinline__ void local_halfcleaners(uint64_t (&B)[NB]) {
 #pragma unroll
   for (int j = NB / 2; j >= 1; j >>= 1) {
-    if (j <= jmax) {
 #pragma unroll
-      for (int r = 0; r < NB; ++r)
-        if ((r & j) == 0) cmpex_up(B[r], B[r | j]);
-    }
+    for (int r = 0; r < NB; ++r)
+      if ((r & j) == 0) cmpex_up(B[r], B[r | j]);
   }
 }
 
@@ -97,23 +102,8 @@ __device__ __forceinline__ void sort_blocked_rt(uint64_t (&B)[NB], int lane) {
         B[r] = low ? umin64(B[r], o) : umax64(B[r], o);
       }
     }
-    local_halfcleaners<NB>(B, NB / 2);
+    local_halfcleaners<NB>(B);
   }
-}
-
-// B bitonic over all 32*NB elements (blocked) -> ascending.
-template <int NB>
-__device__ __forceinline__ void merge_blocked_rt(uint64_t (&B)[NB], int lane) {
-#pragma unroll 1
-  for (int lj = 16; lj >= 1; lj >>= 1) {
-    const bool low = (lane & lj) == 0;
-#pragma unroll
-    for (int r = 0; r < NB; ++r) {
-      const uint64_t o = shfl_xor64(B[r], lj);
-      B[r] = low ? umin64(B[r], o) : umax64(B[r], o);
-    }
-  }
-  local_halfcleaners<NB>(B, NB / 2);
 }
 
 // Conflict-free placement of a blocked array in shared memory without padding:
@@ -149,75 +139,143 @@ __device__ __noinline__ void sort_block(uint64_t* base, int n) {
   __syncwarp();
 }
 
-// MAXN: largest n the caller can have (prunes the tiers that get instantiated).
-template <int MAXN>
-__device__ __forceinline__ int sort_block_any(uint64_t* base, int n) {  // returns log2(NB)
-  if (MAXN <= 32 || n <= 32) { sort_block<1>(base, n); return 0; }
-  if (MAXN <= 64 || n <= 64) { sort_block<2>(base, n); return 1; }
-  if (MAXN <= 128 || n <= 128) { sort_block<4>(base, n); return 2; }
-  if (MAXN <= 256 || n <= 256) { sort_block<8>(base, n); return 3; }
-  if (MAXN <= 512 || n <= 512) { sort_block<16>(base, n); return 4; }
-  sort_block<32>(base, n);
-  return 5;
-}
+// ---- radix selection -------------------------------------------------------------
+// Scratch of one warp: 2^RB bins x 32 lanes x 16-bit counters, also used as a 64-key
+// staging area.  Counter of (bin d, lane l) lives in 32-bit word
+// (d >> 1) * 32 + l, half (d & 1): a lane only ever touches its own words (no
+// races, no atomics) and the 32 lanes of an access hit 32 different banks.
+// RB = digit width: 6 bits (4 KB of counters) for the large queue classes, 5 bits
+// (2 KB) for the small ones, where shared memory per warp decides the occupancy.
+template <int RB>
+constexpr int sel_scratch_bytes() { return (1 << RB) * 32 * 2; }
 
-// buf[0..m) dense keys -> buf[swz<NQ>(i)], i < K = 32*NQ: the K smallest ascending
-// (sentinel padded).  Needs room for ceil(m/BLK) blocks of BLK keys.  Returns the
-// K-th key (kSentinelKey if m < K).  Warp-collective.
-template <int NQ, int CAP>
-__device__ __noinline__ uint64_t select_topk(uint64_t* buf, int m) {
-  // sort-block size: 512 keys (16 per lane) keeps the register count of the whole
-  // call tree at 128 for k <= 512; only the k = 1024 class sorts 1024 at a time
-  constexpr int LBLK = NQ == 32 ? 10 : 9;
-  constexpr int BLK = 1 << LBLK;
-  constexpr int K = 32 * NQ;
-  constexpr int LQ = NQ == 1 ? 0 : NQ == 2 ? 1 : NQ == 4 ? 2 : NQ == 8 ? 3 : NQ == 16 ? 4 : 5;
+// One counting pass over keys[0..m): among the keys whose bits [dec, 64) equal
+// those of prefix (all keys when dec >= 64), histogram the digit (key >> s) & 63
+// (s >= dec - 6, so the digit covers every undecided bit above s; decided bits that
+// fall into it are the same for all counted keys) and locate the digit holding the
+// rank-th smallest (rank 1-based).  Returns the digit; below = keys in smaller
+// digits, cnt = keys in that digit.  Warp-collective.
+template <int RB>
+__device__ __forceinline__ int radix_pass(const uint64_t* keys, int m, uint64_t prefix, int s, int dec,
+                                          int rank, uint32_t* scratch, int& below, int& cnt) {
   const int lane = threadIdx.x & 31;
-  const int nblk = m > BLK ? ((m + BLK - 1) >> LBLK) : 1;
-  int tiers = 0;  // log2(NB) of block b in bits [4b, 4b+4)
-#pragma unroll 1
-  for (int b = 0; b < nblk; ++b) {
-    int nb = m - (b << LBLK);
-    if (nb > BLK) nb = BLK;
-    tiers |= sort_block_any<(CAP < BLK ? CAP : BLK)>(buf + (b << LBLK), nb) << (4 * b);
-  }
-  const int t0 = tiers & 15;
-  if (nblk == 1 && t0 == LQ) return buf[swz<NQ>(K - 1)];
-  uint64_t W[NQ];
+  constexpr int kRadixBins = 1 << RB;
 #pragma unroll
-  for (int r = 0; r < NQ; ++r) {
-    const int i = lane * NQ + r;
-    W[r] = (i < (32 << t0)) ? buf[swz_rt(t0, i)] : kSentinelKey;
-  }
-#pragma unroll 1
-  for (int b = 1; b < nblk; ++b) {
-    const uint64_t* bb = buf + (b << LBLK);
-    const int t = (tiers >> (4 * b)) & 15;
-#pragma unroll
-    for (int r = 0; r < NQ; ++r) {
-      const int p = K - 1 - (lane * NQ + r);
-      const uint64_t o = (p < (32 << t)) ? bb[swz_rt(t, p)] : kSentinelKey;
-      W[r] = umin64(W[r], o);
+  for (int t = 0; t < kRadixBins / 2; ++t) scratch[t * 32 + lane] = 0u;
+  __syncwarp();
+  uint16_t* h16 = reinterpret_cast<uint16_t*>(scratch);
+  for (int i = lane; i < m; i += 32) {
+    const uint64_t key = keys[i];
+    const bool in = dec >= 64 || ((key ^ prefix) >> dec) == 0;
+    if (in) {
+      const uint32_t d = (uint32_t)(key >> s) & (kRadixBins - 1);
+      uint16_t* h = h16 + ((((d >> 1) * 32 + lane) << 1) | (d & 1));
+      *h = (uint16_t)(*h + 1);
     }
-    merge_blocked_rt<NQ>(W, lane);
   }
   __syncwarp();
+  // lane L owns digits 2L and 2L+1: sum word row L over the 32 source lanes (rotated: no conflicts)
+  uint32_t acc = 0;
+  if (lane < kRadixBins / 2) {
+#pragma unroll 8
+    for (int t = 0; t < 32; ++t) acc += scratch[lane * 32 + ((lane + t) & 31)];
+  }
+  const int c0 = (int)(acc & 0xFFFFu), c1 = (int)(acc >> 16);
+  int incl = c0 + c1;
 #pragma unroll
-  for (int r = 0; r < NQ; ++r) buf[swz<NQ>(lane * NQ + r)] = W[r];
+  for (int o = 1; o < 32; o <<= 1) {
+    const int v = __shfl_up_sync(kFull, incl, o);
+    if (lane >= o) incl += v;
+  }
+  const int excl = incl - (c0 + c1);
+  const bool mine = excl < rank && rank <= incl;
+  const unsigned who = __ballot_sync(kFull, mine);
+  const int src = __ffs(who) - 1;  // exactly one lane when 1 <= rank <= (keys counted)
+  int d, b, c;
+  if (rank <= excl + c0) {
+    d = 2 * lane;
+    b = excl;
+    c = c0;
+  } else {
+    d = 2 * lane + 1;
+    b = excl + c0;
+    c = c1;
+  }
+  d = __shfl_sync(kFull, d, src);
+  below = __shfl_sync(kFull, b, src);
+  cnt = __shfl_sync(kFull, c, src);
   __syncwarp();
-  return __shfl_sync(kFull, W[NQ - 1], 31);
+  return d;
 }
 
-// Per-class sizes: LCAP = depth of each lane queue (capacity 32*LCAP keys, a
-// multiple of the 1024-key sort block where it exceeds one), MSTAR = number of
-// elements the sampled bound is aimed to let through.
+// Exact rank-th smallest (1-based, 1 <= rank <= m) of the DISTINCT keys[0..m).
+// diff = OR over i of (keys[i] ^ keys[0]) (bits in which the keys differ at all).
+// Warp-collective; scratch = kSelScratchBytes of this warp.
+template <int RB>
+__device__ __noinline__ uint64_t radix_select_kth(const uint64_t* keys, int m, int rank, uint64_t diff,
+                                                  uint32_t* scratch) {
+  const int lane = threadIdx.x & 31;
+  if (diff == 0) return keys[0];  // m == 1 (keys are distinct)
+  const int top = 63 - __clzll((long long)diff);
+  constexpr int kRadixBits = RB;
+  int s = top - (kRadixBits - 1);
+  if (s < 0) s = 0;
+  uint64_t prefix = keys[0];  // bits above `top` are common to all keys
+  prefix = (top >= 63) ? 0ull : (prefix >> (top + 1)) << (top + 1);
+  int dec = 64;  // lowest decided bit; the common bits above `top` need no test
+  while (true) {
+    int below, cnt;
+    const int d = radix_pass<RB>(keys, m, prefix, s, dec, rank, scratch, below, cnt);
+    dec = s;
+    rank -= below;
+    prefix |= (uint64_t)d << s;
+    if (s == 0) return prefix;
+    if (cnt <= 64) {
+      // stage the <= 64 keys of the digit, sort them, take the rank-th
+      uint64_t* st = reinterpret_cast<uint64_t*>(scratch);
+      int n = 0;
+      for (int i0 = 0; i0 < m; i0 += 32) {
+        const int i = i0 + lane;
+        uint64_t key = 0;
+        bool in = false;
+        if (i < m) {
+          key = keys[i];
+          in = ((key ^ prefix) >> s) == 0;
+        }
+        const unsigned b = __ballot_sync(kFull, in);
+        if (in) st[n + __popc(b & ((1u << lane) - 1u))] = key;
+        n += __popc(b);
+      }
+      __syncwarp();
+      sort_block<2>(st, n);
+      const uint64_t r = st[swz<2>(rank - 1)];
+      __syncwarp();
+      return r;
+    }
+    s -= kRadixBits;
+    if (s < 0) s = 0;
+  }
+}
+
+// Per-class sizes: LCAP = depth of each lane queue (capacity 32*LCAP keys; sized for
+// the mean + 4 sigma of a lane's share of the sampled bound's m*, see sample_target),
+// RB = radix digit width, WARPS per CTA.
 template <int NQ> struct TSelCfg;
-template <> struct TSelCfg<1> { static constexpr int LCAP = 16, MSTAR = 192, WARPS = 4; };
-template <> struct TSelCfg<2> { static constexpr int LCAP = 32, MSTAR = 288, WARPS = 4; };
-template <> struct TSelCfg<4> { static constexpr int LCAP = 32, MSTAR = 448, WARPS = 4; };
-template <> struct TSelCfg<8> { static constexpr int LCAP = 48, MSTAR = 704, WARPS = 4; };
-template <> struct TSelCfg<16> { static constexpr int LCAP = 64, MSTAR = 960, WARPS = 2; };
-template <> struct TSelCfg<32> { static constexpr int LCAP = 96, MSTAR = 1536, WARPS = 1; };
+template <> struct TSelCfg<1> { static constexpr int LCAP = 28, RB = 5, WARPS = 1; };
+template <> struct TSelCfg<2> { static constexpr int LCAP = 32, RB = 5, WARPS = 1; };
+template <> struct TSelCfg<4> { static constexpr int LCAP = 36, RB = 5, WARPS = 1; };
+template <> struct TSelCfg<8> { static constexpr int LCAP = 48, RB = 5, WARPS = 1; };
+template <> struct TSelCfg<16> { static constexpr int LCAP = 60, RB = 6, WARPS = 1; };
+template <> struct TSelCfg<32> { static constexpr int LCAP = 72, RB = 6, WARPS = 1; };
+
+// How many of the S sample elements the sampled bound should let through so that at
+// least k of the len elements pass with ~4 sigma confidence: the count c of sample
+// elements under a value has standard deviation ~sqrt(c), so c - 4 sqrt(c) >= k S/len.
+__device__ __forceinline__ float sample_target(int k, int S, int64_t len) {
+  const float c0 = (float)k * (float)S / (float)(len > 0 ? len : 1);
+  const float r = 0.5f * (4.f + sqrtf(16.f + 4.f * c0));
+  return r * r;
+}
 
 __device__ __forceinline__ float ord_next_up(uint32_t o) {
   // smallest float strictly above the value with order image o; NaN ("accept
@@ -226,16 +284,18 @@ __device__ __forceinline__ float ord_next_up(uint32_t o) {
 }
 
 struct TSelFlushOut {
-  uint64_t kth;  // K-th smallest key (kSentinelKey if fewer than K survive)
-  int m;         // keys that entered the selection
+  uint64_t kth;  // k-th smallest key (kSentinelKey if fewer than k survive)
+  int m;         // keys kept: min(k, keys that entered the selection)
 };
 
-// Compacts the ragged lane queues of one warp in place (rows [0, wrows) hold keys
-// already, the rest raw (bits, index) pairs), drops what the exact bound excludes,
-// and selects: on return buf[swz<NQ>(i)], i < K, are the K smallest ascending.
-// A free function taking values so that the caller's state stays in registers.
-template <int NQ>
-__device__ __noinline__ TSelFlushOut tsel_flush(uint64_t* buf, int cnt, int wrows, uint64_t thr_key) {
+// Restore step.  Compacts the ragged lane queues of one warp in place (rows
+// [0, wrows) hold keys already, the rest raw (bits, index) pairs), drops what the
+// exact bound excludes, and selects: on return buf[0..out.m) are the k smallest
+// keys (dense, unordered).  A free function taking values so that the caller's
+// state stays in registers.  Warp-collective.
+template <int RB>
+__device__ __noinline__ TSelFlushOut tsel_flush(uint64_t* buf, uint32_t* scratch, int cnt, int wrows,
+                                                uint64_t thr_key, int k) {
   const int lane = threadIdx.x & 31;
   const unsigned lt = (1u << lane) - 1u;
   int maxc = cnt;
@@ -245,6 +305,7 @@ __device__ __noinline__ TSelFlushOut tsel_flush(uint64_t* buf, int cnt, int wrow
     maxc = o > maxc ? o : maxc;
   }
   int m = 0;
+  uint64_t first = 0, diff = 0;
   for (int j = 0; j < maxc; ++j) {
     bool valid = j < cnt;
     uint64_t key = kSentinelKey;
@@ -254,33 +315,72 @@ __device__ __noinline__ TSelFlushOut tsel_flush(uint64_t* buf, int cnt, int wrow
       valid = key != kSentinelKey && key <= thr_key;
     }
     const unsigned b = __ballot_sync(kFull, valid);  // also orders this row's reads before the writes
-    if (valid) buf[m + __popc(b & lt)] = key;
-    m += __popc(b);
+    if (b != 0u) {
+      if (m == 0) first = __shfl_sync(kFull, key, __ffs(b) - 1);
+      if (valid) {
+        buf[m + __popc(b & lt)] = key;
+        diff |= key ^ first;
+      }
+      m += __popc(b);
+    }
     __syncwarp();
   }
   TSelFlushOut out;
-  out.kth = select_topk<NQ, 32 * TSelCfg<NQ>::LCAP>(buf, m);
-  out.m = m;
+  if (m <= k) {
+    out.kth = (m == k && m > 0) ? 0ull : kSentinelKey;
+    out.m = m;
+    if (m == k && m > 0) {  // all kept: the bound is their maximum
+      uint64_t mx = 0;
+      for (int i = lane; i < m; i += 32) mx = umax64(mx, buf[i]);
+#pragma unroll
+      for (int s = 16; s >= 1; s >>= 1) mx = umax64(mx, shfl_xor64(mx, s));
+      out.kth = mx;
+    }
+    return out;
+  }
+  const uint32_t dlo = __reduce_or_sync(kFull, (uint32_t)diff);
+  const uint32_t dhi = __reduce_or_sync(kFull, (uint32_t)(diff >> 32));
+  const uint64_t kth = radix_select_kth<RB>(buf, m, k, ((uint64_t)dhi << 32) | dlo, scratch);
+  // keep the keys <= kth (exactly k of them: keys are distinct)
+  int w = 0;
+  for (int i0 = 0; i0 < m; i0 += 32) {
+    const int i = i0 + lane;
+    uint64_t key = 0;
+    bool keep = false;
+    if (i < m) {
+      key = buf[i];
+      keep = key <= kth;
+    }
+    const unsigned b = __ballot_sync(kFull, keep);
+    if (keep) buf[w + __popc(b & lt)] = key;
+    w += __popc(b);
+    __syncwarp();
+  }
+  out.kth = kth;
+  out.m = w;
   return out;
 }
 
 template <int NQ>
 struct TSel {
-  static constexpr int K = 32 * NQ;
   static constexpr int LCAP = TSelCfg<NQ>::LCAP;
 
-  uint64_t* buf;     // this warp's 32*LCAP slots
-  uint64_t thr_key;  // exact bound once `exact`; kSentinelKey before
-  float thr_x;       // an element enters iff !(v >= thr_x)
-  int cnt;           // entries in this lane's queue (rows [0, wrows) are shared, see flush)
-  int wrows;         // rows that already hold keys (the current top-K), 0 or NQ
-  int total;         // valid keys after the last flush (<= K)
+  uint64_t* buf;      // this warp's 32*LCAP slots
+  uint32_t* scratch;  // this warp's sel_scratch_bytes<RB>()
+  uint64_t thr_key;   // exact bound once `exact`; kSentinelKey before
+  float thr_x;        // an element enters iff !(v >= thr_x)
+  int cnt;            // entries in this lane's queue (rows [0, wrows) are shared, see flush)
+  int wrows;          // rows that already hold keys (the current top-k)
+  int total;          // valid keys after the last flush (<= k)
+  int k;
   int lane;
-  bool exact;        // thr_key is the K-th smallest key of everything seen so far
+  bool exact;         // thr_key is the k-th smallest key of everything seen so far
 
-  __device__ __forceinline__ void init(uint64_t* b, int lane_) {
+  __device__ __forceinline__ void init(uint64_t* b, uint32_t* sc, int lane_, int k_) {
     buf = b;
+    scratch = sc;
     lane = lane_;
+    k = k_;
     reset();
   }
   __device__ __forceinline__ void reset() {
@@ -300,21 +400,25 @@ struct TSel {
       ++cnt;
     }
   }
-  __device__ __forceinline__ bool crowded() const { return __any_sync(kFull, cnt > LCAP - 4); }
+  // room for `need` more entries in every lane?
+  __device__ __forceinline__ bool crowded(int need) const { return __any_sync(kFull, cnt > LCAP - need); }
 
   // Restore step.  monotone: every future element has a larger index than all
   // elements seen so far, so ties with the bound can never win (strict bound).
   __device__ __forceinline__ void flush(bool monotone) {
-    const TSelFlushOut o = tsel_flush<NQ>(buf, cnt, wrows, thr_key);
-    total = o.m < K ? o.m : K;
-    if (o.m >= K) {
+    const TSelFlushOut o = tsel_flush<TSelCfg<NQ>::RB>(buf, scratch, cnt, wrows, thr_key, k);
+    total = o.m;
+    if (o.m >= k) {
       thr_key = o.kth;
       exact = true;
       const uint32_t ov = (uint32_t)(o.kth >> 32);
       thr_x = monotone ? ord_f32(ov) : ord_next_up(ov);
     }
-    wrows = NQ;
-    cnt = NQ;
+    // the kept keys occupy rows [0, wrows); pad the last row with sentinels
+    wrows = (o.m + 31) >> 5;
+    if (wrows * 32 - 32 + lane >= o.m && wrows > 0) buf[(wrows - 1) * 32 + lane] = kSentinelKey;
+    cnt = wrows;
+    __syncwarp();
   }
 };
 
