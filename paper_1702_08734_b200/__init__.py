@@ -18,7 +18,7 @@ import re
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libfs.so")
+LIB_PATH = os.environ.get("FS_LIB_PATH") or os.path.join(_HERE, "libfs.so")  # override: A/B builds
 HEADER_PATH = os.path.join(os.path.dirname(_HERE), "include", "fs.h")
 _lib = None
 

@@ -32,7 +32,7 @@ struct KSelArgs {
   int k;
   float* out_val;     // P == 1: [n_rows][k]
   int32_t* out_idx;
-  uint64_t* out_keys;  // P > 1: [n_rows][P][k] sorted keys, sentinel padded
+  uint64_t* out_keys;  // P > 1: [n_rows][P][k] keys, sentinel padded (sorted unless jth == 1)
   uint64_t* heads;     // P > 1: [n_rows][P-1][jth] the jth smallest keys of every chunk but the last
   int jth;             // ceil(k / (P - 1))
   unsigned int* work;  // item counter of the persistent warps (zero before the launch)
@@ -71,8 +71,14 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
       : "memory");
 }
 
-constexpr int kSeg = 512;    // floats per ring segment (2 KB)
-constexpr int kStages = 4;   // ring depth per warp
+#ifndef FS_KSEG
+#define FS_KSEG 512
+#endif
+#ifndef FS_KSTAGES
+#define FS_KSTAGES 2
+#endif
+constexpr int kSeg = FS_KSEG;    // floats per ring segment (2 KB)
+constexpr int kStages = FS_KSTAGES;   // ring depth per warp
 constexpr int kSample = 1024;
 
 struct ItemDesc {
@@ -247,10 +253,35 @@ __global__ void __launch_bounds__(TSelCfg<NQ>::WARPS * 32) kselect_stream_kernel
         x[u] = reinterpret_cast<const float4*>(ring.data + s0 * kSeg)[u * 32 + lane];
         x[4 + u] = reinterpret_cast<const float4*>(ring.data + s1 * kSeg)[u * 32 + lane];
       }
-      uint32_t lo = 0u, hi = 0xFF800000u, pick = 0xFF800000u;
+      // bracket [lo, hi] in the order image with counts (clo < rho_lo, chi > rho_hi);
+      // probes interpolate linearly in the value domain (3 of 4 steps) or bisect the
+      // order image (every 4th step: guarantees termination)
+      float mn = x[0].x, mx = x[0].x;
+#pragma unroll
+      for (int u = 0; u < 8; ++u) {
+        mn = fminf(fminf(mn, x[u].x), fminf(fminf(x[u].y, x[u].z), x[u].w));
+        mx = fmaxf(fmaxf(mx, x[u].x), fmaxf(fmaxf(x[u].y, x[u].z), x[u].w));
+      }
+#pragma unroll
+      for (int sft = 16; sft >= 1; sft >>= 1) {
+        mn = fminf(mn, __shfl_xor_sync(kFull, mn, sft));
+        mx = fmaxf(mx, __shfl_xor_sync(kFull, mx, sft));
+      }
+      uint32_t lo = f32_ord(mn), hi = f32_ord(mx), pick = 0xFF800000u;
+      lo = lo > 0u ? lo - 1u : 0u;
+      if (hi > 0xFF800000u) hi = 0xFF800000u;  // NaN in the sample: +inf image is the widest bound
+      int clo = 0, chi = kSample;
+      const float target = 0.5f * (float)(rho_lo + rho_hi);
+      if (!(mn == mn) || !(mx == mx) || hi <= lo) hi = lo;  // degenerate: keep pick = +inf
 #pragma unroll 1
-      for (int it = 0; it < 34 && hi - lo > 1u; ++it) {
-        const uint32_t mid = lo + ((hi - lo) >> 1);
+      for (int it = 0; it < 48 && hi - lo > 1u; ++it) {
+        uint32_t mid = lo + ((hi - lo) >> 1);
+        if ((it & 3) != 3) {
+          const float vlo = ord_f32(lo), vhi = ord_f32(hi);
+          const float t = vlo + (vhi - vlo) * ((target - (float)clo) / (float)(chi - clo));
+          const uint32_t m2 = f32_ord(t);
+          if (t == t && m2 > lo && m2 < hi) mid = m2;
+        }
         const float tf = ord_f32(mid);
         int cme = 0;
 #pragma unroll
@@ -259,12 +290,15 @@ __global__ void __launch_bounds__(TSelCfg<NQ>::WARPS * 32) kselect_stream_kernel
         const int cw = __reduce_add_sync(kFull, cme);
         if (cw < rho_lo) {
           lo = mid;
+          clo = cw;
         } else {
           hi = mid;
+          chi = cw;
           pick = mid;
           if (cw <= rho_hi) break;
         }
       }
+      if (pick == 0xFF800000u && hi < 0xFF800000u && hi > lo) pick = hi;  // window never hit: hi passes >= rho_lo
       q.set_sampled_bound(pick);
     }
 
@@ -275,32 +309,38 @@ __global__ void __launch_bounds__(TSelCfg<NQ>::WARPS * 32) kselect_stream_kernel
       const int slot = (int)(ring.consumed % kStages);
       mbar_wait(ring.bar + slot, (ring.consumed / kStages) & 1u);
       const int left = (int)d.nvec - seg * (kSeg / 4);
-      const float4* sp = reinterpret_cast<const float4*>(ring.data + slot * kSeg) + lane;
+      const float* sf = ring.data + slot * kSeg + lane * 4;
       const uint32_t ib = vbase + (uint32_t)seg * kSeg + (uint32_t)lane * 4u;
+      // first-level filter: one compare per element, results in a 16-bit mask
+      const float thr = q.thr_x;
+      uint32_t mask = 0u;
       if (left >= kSeg / 4) {
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
-          const float4 x = sp[u * 32];
-          const uint32_t i0 = ib + u * 128;
-          if (q.crowded(4)) q.flush(true);
-          q.push(true, x.x, i0);
-          q.push(true, x.y, i0 + 1);
-          q.push(true, x.z, i0 + 2);
-          q.push(true, x.w, i0 + 3);
+          const float4 x = *reinterpret_cast<const float4*>(sf + u * 128);
+          mask |= (!(x.x >= thr) ? 1u : 0u) << (4 * u);
+          mask |= (!(x.y >= thr) ? 2u : 0u) << (4 * u);
+          mask |= (!(x.z >= thr) ? 4u : 0u) << (4 * u);
+          mask |= (!(x.w >= thr) ? 8u : 0u) << (4 * u);
         }
       } else {
 #pragma unroll 1
         for (int u = 0; u < 4; ++u) {
-          const bool ok = u * 32 + lane < left;
-          float4 x = make_float4(0.f, 0.f, 0.f, 0.f);
-          if (ok) x = sp[u * 32];
-          const uint32_t i0 = ib + u * 128;
-          if (q.crowded(4)) q.flush(true);
-          q.push(ok, x.x, i0);
-          q.push(ok, x.y, i0 + 1);
-          q.push(ok, x.z, i0 + 2);
-          q.push(ok, x.w, i0 + 3);
+          if (u * 32 + lane < left) {
+            const float4 x = *reinterpret_cast<const float4*>(sf + u * 128);
+            mask |= ((!(x.x >= thr) ? 1u : 0u) | (!(x.y >= thr) ? 2u : 0u) | (!(x.z >= thr) ? 4u : 0u) |
+                     (!(x.w >= thr) ? 8u : 0u))
+                    << (4 * u);
+          }
         }
+      }
+      // accepted elements (few) move from the ring slot to the lane queue
+      if (__any_sync(kFull, q.cnt + __popc(mask) > TSel<NQ>::LCAP)) q.flush(true);
+      while (mask) {
+        const int b2 = __ffs(mask) - 1;
+        mask &= mask - 1u;
+        const int off = (b2 >> 2) * 128 + (b2 & 3);
+        q.push_raw(sf[off], ib + (uint32_t)off);
       }
       __syncwarp();  // every lane is done with the slot before it is refilled
       ++ring.consumed;
@@ -316,7 +356,7 @@ __global__ void __launch_bounds__(TSelCfg<NQ>::WARPS * 32) kselect_stream_kernel
     }
     q.flush(true);
     if (sampled && !q.exact && q.total < want) {
-      // the sampled bound let fewer than k elements through (~4 sigma): scan again with
+      // the sampled bound let fewer than k elements through (~3 sigma): scan again with
       // the paper's adaptive bound only (exact in every case; plain loads)
       q.reset();
 #pragma unroll 1
@@ -338,16 +378,30 @@ __global__ void __launch_bounds__(TSelCfg<NQ>::WARPS * 32) kselect_stream_kernel
 
     // A3 / A4 output.  Chunked rows (P > 1) write keys: the sorted winners, whose
     // first `heads` entries also go to the row's head list for the bound of step 2.
-    sort_block<NQ>(q.buf, q.total);
-    if (a.P == 1) {
-      write_sorted<NQ>(q.buf, a.k, lane, a.vals + d.row * a.ld, a.out_val + d.row * a.k,
-                       a.out_idx + d.row * a.k);
-    } else {
+    if (a.P > 1 && a.jth == 1) {
+      // many chunks: the head is the chunk's smallest key, the winners stay unsorted
       uint64_t* ok = a.out_keys + item * a.k;
-      for (int i = lane; i < a.k; i += 32) ok[i] = q.buf[swz<NQ>(i)];
-      if (d.c != a.P - 1) {
-        uint64_t* hd = a.heads + (d.row * (a.P - 1) + d.c) * a.jth;
-        for (int i = lane; i < a.jth; i += 32) hd[i] = q.buf[swz<NQ>(i)];
+      uint64_t mn = kSentinelKey;
+      for (int i = lane; i < a.k; i += 32) {
+        const uint64_t key = i < q.total ? q.buf[i] : kSentinelKey;
+        ok[i] = key;
+        mn = umin64(mn, key);
+      }
+#pragma unroll
+      for (int sft = 16; sft >= 1; sft >>= 1) mn = umin64(mn, shfl_xor64(mn, sft));
+      if (lane == 0 && d.c != a.P - 1) a.heads[d.row * (a.P - 1) + d.c] = mn;
+    } else {
+      sort_block_inl<NQ>(q.buf, q.total);
+      if (a.P == 1) {
+        write_sorted<NQ>(q.buf, a.k, lane, a.vals + d.row * a.ld, a.out_val + d.row * a.k,
+                         a.out_idx + d.row * a.k);
+      } else {
+        uint64_t* ok = a.out_keys + item * a.k;
+        for (int i = lane; i < a.k; i += 32) ok[i] = q.buf[swz<NQ>(i)];
+        if (d.c != a.P - 1) {
+          uint64_t* hd = a.heads + (d.row * (a.P - 1) + d.c) * a.jth;
+          for (int i = lane; i < a.jth; i += 32) hd[i] = q.buf[swz<NQ>(i)];
+        }
       }
     }
     __syncwarp();
@@ -452,7 +506,7 @@ __global__ void __launch_bounds__(256)
     kselect_prune_kernel(const uint64_t* __restrict__ keys, int64_t n_lists, int P, int k,
                          const unsigned long long* __restrict__ bound, uint64_t* __restrict__ cand,
                          unsigned int* __restrict__ count) {
-  // a warp takes 256 consecutive keys of one list (lists are sorted: stop at the first miss)
+  // a warp takes 256 consecutive keys of one list
   const int lane = threadIdx.x & 31;
   const int parts = (k + 255) / 256;
   const int64_t w = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
@@ -469,12 +523,11 @@ __global__ void __launch_bounds__(256)
     if (i < i_end) key = keys[list * k + i];
     const bool keep = key != kSentinelKey && key <= B;
     const unsigned b = __ballot_sync(kFull, keep);
-    if (b == 0u) break;
+    if (b == 0u) continue;
     unsigned int pos = 0;
     if (lane == 0) pos = atomicAdd(count + row, (unsigned int)__popc(b));
     pos = __shfl_sync(kFull, pos, 0);
     if (keep) out[pos + __popc(b & ((1u << lane) - 1u))] = key;
-    if (b != kFull) break;
   }
 }
 
@@ -525,7 +578,21 @@ __global__ void __launch_bounds__(128)
 namespace {
 
 constexpr int kWarpsPerCtaK1 = 4;
-constexpr int kResidentWarpsPerSm = 12;  // planning estimate; the grid uses the real occupancy
+// Planning estimate of the resident warps per SM of a queue class (shared memory
+// per warp decides it); the grid itself uses the real occupancy.
+template <int NQ>
+constexpr int resident_est() {
+  return (int)((227 * 1024) / (StreamSmem<NQ>::total + 1024));
+}
+int resident_warps_per_sm(int k) {
+  if (k == 1) return 16;
+  if (k <= 32) return resident_est<1>();
+  if (k <= 64) return resident_est<2>();
+  if (k <= 128) return resident_est<4>();
+  if (k <= 256) return resident_est<8>();
+  if (k <= 512) return resident_est<16>();
+  return resident_est<32>();
+}
 
 struct Plan {
   int P;          // chunks per row
@@ -539,7 +606,7 @@ struct Plan {
 // dominate).  One chunk per resident warp.
 Plan make_plan(int64_t n_rows, int64_t n, int k) {
   Plan p;
-  const int64_t resident = (int64_t)sm_count() * kResidentWarpsPerSm;
+  const int64_t resident = (int64_t)sm_count() * resident_warps_per_sm(k);
   const int64_t min_chunk = k * 8 > 4096 ? (int64_t)k * 8 : 4096;
   int64_t P = 1;
   if (n_rows > 0 && n_rows * 2 <= resident && n >= 2 * min_chunk) {

@@ -124,6 +124,21 @@ __device__ __forceinline__ int swz(int e) {
 // Sort base[0..n) (dense, any order; n <= 32*NB) -> base[swz<NB>(e)] = e-th
 // smallest, sentinel-padded to 32*NB.  Warp-collective.
 template <int NB>
+__device__ __forceinline__ void sort_block_inl(uint64_t* base, int n) {
+  const int lane = threadIdx.x & 31;
+  uint64_t B[NB];
+#pragma unroll
+  for (int r = 0; r < NB; ++r) {
+    const int e = r * 32 + lane;
+    B[r] = e < n ? base[e] : kSentinelKey;
+  }
+  __syncwarp();
+  sort_blocked_rt<NB>(B, lane);
+#pragma unroll
+  for (int r = 0; r < NB; ++r) base[swz<NB>(lane * NB + r)] = B[r];
+  __syncwarp();
+}
+template <int NB>
 __device__ __noinline__ void sort_block(uint64_t* base, int n) {
   const int lane = threadIdx.x & 31;
   uint64_t B[NB];
@@ -269,11 +284,11 @@ template <> struct TSelCfg<16> { static constexpr int LCAP = 60, RB = 6, WARPS =
 template <> struct TSelCfg<32> { static constexpr int LCAP = 72, RB = 6, WARPS = 1; };
 
 // How many of the S sample elements the sampled bound should let through so that at
-// least k of the len elements pass with ~4 sigma confidence: the count c of sample
-// elements under a value has standard deviation ~sqrt(c), so c - 4 sqrt(c) >= k S/len.
+// least k of the len elements pass with ~3 sigma confidence: the count c of sample
+// elements under a value has standard deviation ~sqrt(c), so c - 3 sqrt(c) >= k S/len.
 __device__ __forceinline__ float sample_target(int k, int S, int64_t len) {
   const float c0 = (float)k * (float)S / (float)(len > 0 ? len : 1);
-  const float r = 0.5f * (4.f + sqrtf(16.f + 4.f * c0));
+  const float r = 0.5f * (3.f + sqrtf(9.f + 4.f * c0));
   return r * r;
 }
 
@@ -305,7 +320,7 @@ __device__ __noinline__ TSelFlushOut tsel_flush(uint64_t* buf, uint32_t* scratch
     maxc = o > maxc ? o : maxc;
   }
   int m = 0;
-  uint64_t first = 0, diff = 0;
+  uint64_t kor = 0ull, kand = ~0ull;
   for (int j = 0; j < maxc; ++j) {
     bool valid = j < cnt;
     uint64_t key = kSentinelKey;
@@ -315,14 +330,12 @@ __device__ __noinline__ TSelFlushOut tsel_flush(uint64_t* buf, uint32_t* scratch
       valid = key != kSentinelKey && key <= thr_key;
     }
     const unsigned b = __ballot_sync(kFull, valid);  // also orders this row's reads before the writes
-    if (b != 0u) {
-      if (m == 0) first = __shfl_sync(kFull, key, __ffs(b) - 1);
-      if (valid) {
-        buf[m + __popc(b & lt)] = key;
-        diff |= key ^ first;
-      }
-      m += __popc(b);
+    if (valid) {
+      buf[m + __popc(b & lt)] = key;
+      kor |= key;
+      kand &= key;
     }
+    m += __popc(b);
     __syncwarp();
   }
   TSelFlushOut out;
@@ -338,9 +351,11 @@ __device__ __noinline__ TSelFlushOut tsel_flush(uint64_t* buf, uint32_t* scratch
     }
     return out;
   }
-  const uint32_t dlo = __reduce_or_sync(kFull, (uint32_t)diff);
-  const uint32_t dhi = __reduce_or_sync(kFull, (uint32_t)(diff >> 32));
-  const uint64_t kth = radix_select_kth<RB>(buf, m, k, ((uint64_t)dhi << 32) | dlo, scratch);
+  // bits in which the keys differ at all: set in some key and clear in some key
+  const uint32_t olo = __reduce_or_sync(kFull, (uint32_t)kor), ohi = __reduce_or_sync(kFull, (uint32_t)(kor >> 32));
+  const uint32_t alo = __reduce_and_sync(kFull, (uint32_t)kand), ahi = __reduce_and_sync(kFull, (uint32_t)(kand >> 32));
+  const uint64_t diff = (((uint64_t)ohi << 32) | olo) & ~(((uint64_t)ahi << 32) | alo);
+  const uint64_t kth = radix_select_kth<RB>(buf, m, k, diff, scratch);
   // keep the keys <= kth (exactly k of them: keys are distinct)
   int w = 0;
   for (int i0 = 0; i0 < m; i0 += 32) {
@@ -399,6 +414,10 @@ struct TSel {
       buf[cnt * 32 + lane] = ((uint64_t)idx << 32) | __float_as_uint(v);  // raw (bits, index)
       ++cnt;
     }
+  }
+  __device__ __forceinline__ void push_raw(float v, uint32_t idx) {  // caller checked the bound and the room
+    buf[cnt * 32 + lane] = ((uint64_t)idx << 32) | __float_as_uint(v);
+    ++cnt;
   }
   // room for `need` more entries in every lane?
   __device__ __forceinline__ bool crowded(int need) const { return __any_sync(kFull, cnt > LCAP - need); }
