@@ -278,6 +278,11 @@ def run_ours(args):
     fs.lib()  # fail loudly if libfs.so is missing
     pk = peaks()
 
+    if args.case in ("flat", "ivfpq"):  # profiling aid: only that "also" leg
+        out = also_flat(fs, gt, pk) if args.case == "flat" else also_ivfpq(fs, gt, pk, args.ivfpq_nb)
+        print(json.dumps({"case": args.case, **out}))
+        return
+
     # this rank's rows: distinct rows per rank (weak scaling)
     rows = gt.kselect_rows(rank * N_ROWS, N_ROWS, N_COLS)
     big = gt.kselect_rows(10**6 + rank, 1, BIG_N, duplicates=False)
@@ -434,7 +439,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--skip-also", action="store_true")
     ap.add_argument("--ivfpq-nb", type=int, default=10_000_000)
-    ap.add_argument("--case", default="", help="comma list of k1,k32,k128,k1024,bigrow_k1024: time only these calls")
+    ap.add_argument("--case", default="", help="comma list of k1,k32,k128,k1024,bigrow_k1024 (time only these calls), or flat / ivfpq (only that leg)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -345,13 +345,17 @@ FlatPlan flat_plan(int64_t nq, int64_t nb, int d, int k) {
   p.off_xnorm = align_up((size_t)nb * sizeof(float), 256);
   p.off_W = p.off_xnorm + align_up((size_t)nq * sizeof(float), 256);
   p.bytes = p.off_W + align_up((size_t)nq * p.S * p.K * sizeof(uint64_t), 256);
-  (void)d;
+  if (flat_tc_supported(d) && nq > 0 && nb > 0) {  // the tensor-core engine lays out its own workspace
+    const size_t tb = flat_tc_plan(nq, nb, d, k).bytes;
+    if (tb > p.bytes) p.bytes = tb;
+  }
   return p;
 }
 
 int flat_knn_device(const float* xq, int64_t nq, const float* xb, int64_t nb, int d, int k,
                     const float* ynorm_opt, float* out_dist, int64_t* out_ids, void* ws,
                     cudaStream_t s) {
+  if (flat_tc_supported(d)) return flat_knn_tc_device(xq, nq, xb, nb, d, k, out_dist, out_ids, ws, s);
   const FlatPlan p = flat_plan(nq, nb, d, k);
   char* w = static_cast<char*>(ws);
   float* ynorm = reinterpret_cast<float*>(w + p.off_ynorm);
@@ -408,7 +412,9 @@ int flat_validate(const void* xq, int64_t nq, const void* xb, int64_t nb, int d,
 
 extern "C" {
 
-const char* fs_flat_engine(void) { return "ffma-fp32"; }
+const char* fs_flat_engine(void) {
+  return fs::flat_tc_supported(128) ? "tcgen05-3xtf32 (d % 32 == 0, d <= 128; ffma-fp32 otherwise)" : "ffma-fp32";
+}
 
 size_t fs_flat_l2_knn_ws_bytes(int64_t nq, int64_t nb, int d, int k) {
   if (nq < 0 || nb < 0 || d < 1 || k < 1 || k > FS_MAX_K) return 0;

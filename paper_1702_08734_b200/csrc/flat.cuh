@@ -26,6 +26,18 @@ int flat_knn_device(const float* xq, int64_t nq, const float* xb, int64_t nb, in
                     const float* ynorm_opt, float* out_dist, int64_t* out_ids, void* ws,
                     cudaStream_t s);
 
+// Tensor-core engine (flat_tc.cu): tcgen05 / TMEM / TMA, 3xTF32 split operands.
+struct FlatTcPlan {
+  int kclass, K, S, qtiles, grid, KB, nstage;
+  int64_t chunk;
+  size_t smem;
+  size_t off_ynorm, off_xnorm, off_flag, off_gbound, off_W, off_cbuf, off_qhi, off_qlo, off_bhi, off_blo, bytes;
+};
+bool flat_tc_supported(int d);  // d % 32 == 0, 32 <= d <= 128, not disabled by FS_FLAT_ENGINE=ffma
+FlatTcPlan flat_tc_plan(int64_t nq, int64_t nb, int d, int k);
+int flat_knn_tc_device(const float* xq, int64_t nq, const float* xb, int64_t nb, int d, int k, float* out_dist,
+                       int64_t* out_ids, void* ws, cudaStream_t s);
+
 // B4: S partial queues per query -> k results (+||x||^2 if xnorm != NULL).
 int launch_flat_finish(const uint64_t* Wg, int64_t nq, int S, int k, const float* xnorm,
                        float* out_dist, int64_t* out_ids, cudaStream_t s);

@@ -1,0 +1,482 @@
+// flat_tc.cu -- tensor-core engine of fs_flat_l2_knn:
+// the -2<x,y> contraction on tcgen05 tensor cores with the accumulator
+// in TMEM, operands staged by TMA, and the "+||y||^2 then k-select" step run
+// by the epilogue warps straight from TMEM: the nq x nb matrix never reaches HBM.
+//
+// Precision (reading F-5): every fp32 operand is split as x = hi + lo with
+// hi = x truncated to TF32 (10 explicit mantissa bits) and lo = (x - hi) truncated to
+// TF32; the tile accumulates hi*hi + lo*hi + hi*lo in fp32 ("3xTF32", ~2^-21 relative).
+// A pre-pass writes the hi / lo planes (and the squared norms, B1) once per call; if it
+// finds lo == 0 everywhere (e.g. small-integer data such as cfg3) the kernel issues the
+// hi*hi products only, which is then exact -- a checked dispatch, never a guess.
+//
+// Kernel shape: persistent CTAs (one per SM), 192 threads:
+//   warp 0      TMA producer   query tile (128 rows, resident per work item) and a ring
+//                              of database stages (256 rows x 32 columns x fp32 = 32 KB)
+//   warp 1      MMA issuer     tcgen05.mma kind::tf32, M=128 N=256 K=8, two 256-column
+//                              accumulators in TMEM (ping-pong with the epilogue)
+//   warps 2-5   epilogue       thread = TMEM lane = query row: tcgen05.ld, d' = ||y||^2 -
+//                              2 acc, compare with the row's bound; the rare survivors go
+//                              to a per-row candidate buffer, merged into the row's queue
+//                              by the whole warp (warp_flush of select.cuh)
+// Work item = (database split s, query tile): items are ordered split-major, so CTAs that
+// run at the same time read the same part of the database (L2 reuse), and a query's
+// bound found in earlier splits (gbound) prunes the later ones.
+#include <cuda.h>
+
+#include <cstdlib>
+#include <cstring>
+
+#include "flat.cuh"
+#include "sm100.cuh"
+
+namespace fs {
+
+namespace {
+
+constexpr int BM = 128;                      // query rows per tile (MMA M)
+constexpr int BN = 256;                      // database rows per tile (MMA N)
+constexpr int BK = 32;                       // fp32 columns per stage = 128 bytes (swizzle span)
+constexpr int A_KB_BYTES = BM * BK * 4;      // 16 KB
+constexpr int B_STAGE_BYTES = BN * BK * 4;   // 32 KB
+constexpr int MAX_STAGES = 4;
+constexpr int TC_THREADS = 192;
+constexpr int CBS = 72;                      // candidate-buffer stride per row (64 + padding of warp_flush<*,2>)
+constexpr int SMEM_LIMIT = 227 * 1024;
+
+struct TcArgs {
+  int64_t nq, nb;
+  int d, KB, k, kclass, K;
+  int S, qtiles, nstage;
+  int64_t chunk;               // database rows per split (multiple of BN)
+  const float* ynorm;          // [>= nb rounded up to BN]
+  uint64_t* Wg;                // [nq][S][K]
+  unsigned int* gbound;        // [nq] order image of the best known k-th distance
+  uint64_t* cbuf;              // [gridDim.x][BM][CBS]
+  const unsigned int* lo_flag; // != 0: lo planes are not all zero (3xTF32)
+};
+
+// ---------------------------------------------------------------------------
+// B1 + operand split: hi / lo planes and squared norms, one warp per vector.
+// ---------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+    split_norm_kernel(const float* __restrict__ x, int64_t n, int d, float* __restrict__ hi,
+                      float* __restrict__ lo, float* __restrict__ norm, unsigned int* __restrict__ flag) {
+  const int lane = threadIdx.x & 31;
+  const int64_t row = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
+  if (row >= n) return;
+  const float* p = x + row * d;
+  float s = 0.f;
+  bool any = false;
+  for (int c = lane; c < d; c += 32) {
+    const float v = p[c];
+    s = fmaf(v, v, s);
+    const float h = __uint_as_float(__float_as_uint(v) & 0xFFFFE000u);
+    const float l = __uint_as_float(__float_as_uint(v - h) & 0xFFFFE000u);
+    hi[row * d + c] = h;
+    lo[row * d + c] = l;
+    any |= (l != 0.f);
+  }
+#pragma unroll
+  for (int m = 16; m >= 1; m >>= 1) s += __shfl_xor_sync(kFull, s, m);
+  if (lane == 0) norm[row] = s;
+  if (__any_sync(kFull, any) && lane == 0) atomicOr(flag, 1u);
+}
+
+// ---------------------------------------------------------------------------
+// B2 + B3: the tile kernel.
+// ---------------------------------------------------------------------------
+struct Pipe {
+  int stage;
+  uint32_t phase;
+  __device__ __forceinline__ void advance(int nstage) {
+    if (++stage == nstage) {
+      stage = 0;
+      phase ^= 1u;
+    }
+  }
+};
+
+__global__ void __launch_bounds__(TC_THREADS, 1)
+    flat_tc_kernel(const __grid_constant__ CUtensorMap map_a_hi, const __grid_constant__ CUtensorMap map_a_lo,
+                   const __grid_constant__ CUtensorMap map_b_hi, const __grid_constant__ CUtensorMap map_b_lo,
+                   const TcArgs a) {
+  extern __shared__ unsigned char smem_dyn[];
+  // operand tiles need 1024-byte alignment (128-byte swizzle atoms of 8 rows)
+  unsigned char* smem = smem_dyn + ((1024u - (sm100::smem_addr(smem_dyn) & 1023u)) & 1023u);
+  unsigned char* sA_hi = smem;
+  unsigned char* sA_lo = sA_hi + (size_t)a.KB * A_KB_BYTES;
+  unsigned char* sB = sA_lo + (size_t)a.KB * A_KB_BYTES;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(sB + (size_t)a.nstage * B_STAGE_BYTES);
+  uint64_t* full = bars;                    // [MAX_STAGES]
+  uint64_t* empty = bars + MAX_STAGES;      // [MAX_STAGES]
+  uint64_t* tfull = bars + 2 * MAX_STAGES;  // [2]
+  uint64_t* tempty = tfull + 2;             // [2]
+  uint64_t* a_full = tempty + 2;
+  uint64_t* a_empty = a_full + 1;
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(a_empty + 1);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < MAX_STAGES; ++i) {
+      sm100::mbar_init(full + i, 1);
+      sm100::mbar_init(empty + i, 1);
+    }
+    for (int i = 0; i < 2; ++i) {
+      sm100::mbar_init(tfull + i, 1);
+      sm100::mbar_init(tempty + i, 4);
+    }
+    sm100::mbar_init(a_full, 1);
+    sm100::mbar_init(a_empty, 1);
+    sm100::fence_mbar_init();
+    sm100::tma_prefetch_desc(&map_a_hi);
+    sm100::tma_prefetch_desc(&map_a_lo);
+    sm100::tma_prefetch_desc(&map_b_hi);
+    sm100::tma_prefetch_desc(&map_b_lo);
+  }
+  if (warp == 1) sm100::tmem_alloc(tmem_slot, 512);
+  sm100::tc_fence_before();
+  __syncthreads();
+  sm100::tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+  const bool split = *a.lo_flag != 0u;
+  const int64_t n_items = (int64_t)a.S * a.qtiles;
+  const int KB = a.KB, nstage = a.nstage;
+
+  if (warp == 0) {
+    // ===== TMA producer =====
+    if (lane == 0) {
+      Pipe pp{0, 0u};
+      int it = 0;
+      for (int64_t item = blockIdx.x; item < n_items; item += gridDim.x, ++it) {
+        const int s = (int)(item / a.qtiles), qt = (int)(item - (int64_t)s * a.qtiles);
+        const int64_t b_begin = (int64_t)s * a.chunk;
+        const int64_t b_end = b_begin + a.chunk < a.nb ? b_begin + a.chunk : a.nb;
+        const int ntiles = (int)((b_end - b_begin + BN - 1) / BN);
+        if (it > 0) sm100::mbar_wait(a_empty, (uint32_t)(it - 1) & 1u);  // previous item's MMAs are done with A
+        sm100::mbar_expect_tx(a_full, (uint32_t)(KB * A_KB_BYTES * (split ? 2 : 1)));
+        for (int kb = 0; kb < KB; ++kb) {
+          sm100::tma_load_2d(sA_hi + kb * A_KB_BYTES, &map_a_hi, kb * BK, qt * BM, a_full);
+          if (split) sm100::tma_load_2d(sA_lo + kb * A_KB_BYTES, &map_a_lo, kb * BK, qt * BM, a_full);
+        }
+        for (int t = 0; t < ntiles; ++t) {
+          const int row0 = (int)(b_begin + (int64_t)t * BN);
+          for (int kb = 0; kb < KB; ++kb) {
+            for (int pl = 0; pl < (split ? 2 : 1); ++pl) {
+              sm100::mbar_wait(empty + pp.stage, pp.phase ^ 1u);
+              sm100::mbar_expect_tx(full + pp.stage, (uint32_t)B_STAGE_BYTES);
+              sm100::tma_load_2d(sB + (size_t)pp.stage * B_STAGE_BYTES, pl ? &map_b_lo : &map_b_hi, kb * BK, row0,
+                                 full + pp.stage);
+              pp.advance(nstage);
+            }
+          }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===== MMA issuer =====
+    if (lane == 0) {
+      constexpr uint32_t idesc = sm100::make_idesc_tf32(BM, BN);
+      Pipe pc{0, 0u};
+      uint32_t tile_count = 0;
+      int it = 0;
+      for (int64_t item = blockIdx.x; item < n_items; item += gridDim.x, ++it) {
+        const int s = (int)(item / a.qtiles);
+        const int64_t b_begin = (int64_t)s * a.chunk;
+        const int64_t b_end = b_begin + a.chunk < a.nb ? b_begin + a.chunk : a.nb;
+        const int ntiles = (int)((b_end - b_begin + BN - 1) / BN);
+        sm100::mbar_wait(a_full, (uint32_t)it & 1u);
+        sm100::tc_fence_after();
+        for (int t = 0; t < ntiles; ++t, ++tile_count) {
+          const uint32_t as = tile_count & 1u;
+          sm100::mbar_wait(tempty + as, ((tile_count >> 1) & 1u) ^ 1u);  // epilogue drained this accumulator
+          sm100::tc_fence_after();
+          const uint32_t d_tmem = tmem_base + as * BN;
+          for (int kb = 0; kb < KB; ++kb) {
+            const uint64_t da_hi = sm100::make_kmajor_sw128_desc(sm100::smem_addr(sA_hi + kb * A_KB_BYTES));
+            const uint64_t da_lo = sm100::make_kmajor_sw128_desc(sm100::smem_addr(sA_lo + kb * A_KB_BYTES));
+            // stage with the hi plane of the database: hi*hi (+ lo*hi)
+            sm100::mbar_wait(full + pc.stage, pc.phase);
+            sm100::tc_fence_after();
+            uint64_t db = sm100::make_kmajor_sw128_desc(sm100::smem_addr(sB + (size_t)pc.stage * B_STAGE_BYTES));
+#pragma unroll
+            for (int ks = 0; ks < BK / 8; ++ks)  // K = 8 per MMA = 32 bytes = 2 descriptor units
+              sm100::mma_tf32_ss(d_tmem, da_hi + 2 * ks, db + 2 * ks, idesc, (kb | ks) != 0 ? 1u : 0u);
+            if (split) {
+#pragma unroll
+              for (int ks = 0; ks < BK / 8; ++ks) sm100::mma_tf32_ss(d_tmem, da_lo + 2 * ks, db + 2 * ks, idesc, 1u);
+            }
+            sm100::mma_commit(empty + pc.stage);
+            pc.advance(nstage);
+            if (split) {  // stage with the lo plane: hi*lo
+              sm100::mbar_wait(full + pc.stage, pc.phase);
+              sm100::tc_fence_after();
+              db = sm100::make_kmajor_sw128_desc(sm100::smem_addr(sB + (size_t)pc.stage * B_STAGE_BYTES));
+#pragma unroll
+              for (int ks = 0; ks < BK / 8; ++ks) sm100::mma_tf32_ss(d_tmem, da_hi + 2 * ks, db + 2 * ks, idesc, 1u);
+              sm100::mma_commit(empty + pc.stage);
+              pc.advance(nstage);
+            }
+          }
+          sm100::mma_commit(tfull + as);
+        }
+        sm100::mma_commit(a_empty);
+      }
+    }
+  } else {
+    // ===== epilogue: B3 =====
+    const int quarter = warp & 3;  // TMEM lanes 32*quarter .. +31 belong to this warp
+    const int row = quarter * 32 + lane;
+    const int K = a.K;
+    uint64_t* cb_warp = a.cbuf + ((size_t)blockIdx.x * BM + quarter * 32) * CBS;
+    uint64_t* cb = cb_warp + (size_t)lane * CBS;
+    uint32_t tile_count = 0;
+    for (int64_t item = blockIdx.x; item < n_items; item += gridDim.x) {
+      const int s = (int)(item / a.qtiles), qt = (int)(item - (int64_t)s * a.qtiles);
+      const int64_t b_begin = (int64_t)s * a.chunk;
+      const int64_t b_end = b_begin + a.chunk < a.nb ? b_begin + a.chunk : a.nb;
+      const int ntiles = (int)((b_end - b_begin + BN - 1) / BN);
+      const int64_t q_warp = (int64_t)qt * BM + quarter * 32;
+      const int64_t q = q_warp + lane;
+      const bool valid = q < a.nq;
+      // queues of this warp's rows start empty
+      for (int r = 0; r < 32; ++r) {
+        if (q_warp + r < a.nq) {
+          uint64_t* W = a.Wg + ((q_warp + r) * a.S + s) * K;
+          for (int i = lane; i < K; i += 32) W[i] = kSentinelKey;
+        }
+      }
+      // start from the best bound other splits have published (inclusive)
+      const uint64_t thr0 = valid ? (((uint64_t)a.gbound[q] << 32) | 0xFFFFFFFFull) : 0ull;
+      uint64_t thr_key = thr0;
+      float thr_val = valid ? ord_f32((uint32_t)(thr0 >> 32)) : __uint_as_float(0xFF800000u);
+      int cnt = 0;
+      __syncwarp();
+
+      auto flush_rows = [&](bool need) {
+        unsigned m = __ballot_sync(kFull, need);
+        while (m) {
+          const int r = __ffs(m) - 1;
+          m &= m - 1u;
+          const int rcnt = __shfl_sync(kFull, cnt, r);
+          const uint64_t nt = warp_flush_b64(a.kclass, a.Wg + ((q_warp + r) * a.S + s) * K + lane, 32,
+                                             cb_warp + (size_t)r * CBS, rcnt);
+          if (lane == r) {
+            thr_key = nt < thr0 ? nt : thr0;
+            thr_val = key_val(thr_key);
+            cnt = 0;
+          }
+        }
+      };
+
+      for (int t = 0; t < ntiles; ++t, ++tile_count) {
+        const uint32_t as = tile_count & 1u;
+        const int64_t col0 = b_begin + (int64_t)t * BN;
+        const int ncols = (int)(b_end - col0 < BN ? b_end - col0 : BN);
+        sm100::mbar_wait(tfull + as, (tile_count >> 1) & 1u);
+        sm100::tc_fence_after();
+        const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + as * BN;
+#pragma unroll 1
+        for (int cg = 0; cg < BN / 32; ++cg) {
+          uint32_t v[32];
+          sm100::tmem_ld32(taddr + cg * 32, v);
+          float4 yn[8];
+          const float4* ynp = reinterpret_cast<const float4*>(a.ynorm + col0 + cg * 32);
+#pragma unroll
+          for (int j = 0; j < 8; ++j) yn[j] = __ldg(ynp + j);
+          sm100::tmem_ld_wait();
+          const uint32_t cbase = (uint32_t)col0 + cg * 32;
+          const int climit = ncols - cg * 32;  // columns of this group that exist
+#pragma unroll
+          for (int j = 0; j < 32; ++j) {
+            const float y = j % 4 == 0 ? yn[j / 4].x : j % 4 == 1 ? yn[j / 4].y : j % 4 == 2 ? yn[j / 4].z : yn[j / 4].w;
+            const float dp = fmaf(-2.f, __uint_as_float(v[j]), y);
+            if (!(dp > thr_val)) {  // rare
+              const uint64_t key = make_key(dp, cbase + j);
+              if (j < climit && key < thr_key) cb[cnt++] = key;
+            }
+          }
+          flush_rows(cnt > 32);
+        }
+        // accumulator drained
+        sm100::tc_fence_before();
+        __syncwarp();
+        if (lane == 0) sm100::mbar_arrive(tempty + as);
+      }
+      flush_rows(cnt > 0);
+      __syncwarp();
+      // publish this split's k-th distance as a bound for the splits still to run
+      if (valid) {
+        const uint64_t kth = a.Wg[(q * a.S + s) * K + (a.k - 1)];
+        if (kth != kSentinelKey) atomicMin(a.gbound + q, (unsigned int)(kth >> 32));
+      }
+    }
+  }
+  // teardown
+  sm100::tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    sm100::tc_fence_after();
+    sm100::tmem_dealloc(tmem_base, 512);
+  }
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------
+// Host side
+// ---------------------------------------------------------------------------
+namespace {
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_tiled_fn() {
+  static EncodeTiledFn fn = nullptr;
+  static bool tried = false;
+  if (!tried) {
+    tried = true;
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+        qres == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<EncodeTiledFn>(p);
+    cudaGetLastError();
+  }
+  return fn;
+}
+
+// 2-D fp32 row-major [rows][d] tensor, box = box_rows x 32 columns, 128-byte swizzle,
+// out-of-range rows read as zeros.
+int make_map(CUtensorMap* m, const float* base, int64_t rows, int d, int box_rows) {
+  EncodeTiledFn fn = encode_tiled_fn();
+  if (!fn) return set_error(FS_ECUDA, "cuTensorMapEncodeTiled is not available");
+  const cuuint64_t dims[2] = {(cuuint64_t)d, (cuuint64_t)(rows > 0 ? rows : 1)};
+  const cuuint64_t strides[1] = {(cuuint64_t)d * sizeof(float)};
+  const cuuint32_t box[2] = {(cuuint32_t)BK, (cuuint32_t)box_rows};
+  const cuuint32_t estr[2] = {1, 1};
+  const CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(base), dims, strides, box, estr,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return set_error(FS_ECUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r);
+  return FS_OK;
+}
+
+}  // namespace
+
+bool flat_tc_supported(int d) {
+  static int forced_off = -1;
+  if (forced_off < 0) {
+    const char* e = getenv("FS_FLAT_ENGINE");
+    forced_off = (e && strcmp(e, "ffma") == 0) ? 1 : 0;
+  }
+  return !forced_off && d % BK == 0 && d >= BK && d <= 128;
+}
+
+FlatTcPlan flat_tc_plan(int64_t nq, int64_t nb, int d, int k) {
+  FlatTcPlan p;
+  p.kclass = k_class(k);
+  p.K = 32 << p.kclass;
+  p.qtiles = (int)ceil_div(nq, BM);
+  const int64_t nt = ceil_div(nb > 0 ? nb : 1, BN);
+  const int64_t sms = sm_count();
+  // database splits: fill whole waves of CTAs with as few partial queues as possible
+  int64_t best_S = 1;
+  double best = -1.0;
+  const int64_t max_S = nt < 64 ? nt : 64;
+  for (int64_t S = 1; S <= max_S; ++S) {
+    const int64_t per = ceil_div(nt, S);
+    const int64_t realS = ceil_div(nt, per);
+    const int64_t items = realS * p.qtiles;
+    const int64_t g = items < sms ? items : sms;
+    const double eff = (double)items / (double)(ceil_div(items, g) * g) * ((double)g / (double)sms);
+    const double score = eff - 0.002 * (double)realS;
+    if (score > best) {
+      best = score;
+      best_S = realS;
+    }
+  }
+  const int64_t per = ceil_div(nt, best_S);
+  p.chunk = per * BN;
+  p.S = (int)ceil_div(nb > 0 ? nb : 1, p.chunk);
+  const int64_t items = (int64_t)p.S * p.qtiles;
+  p.grid = (int)(items < sms ? items : sms);
+  p.KB = d / BK;
+  const int fixed = 2 * p.KB * A_KB_BYTES + 1024 /*alignment*/ + 256 /*barriers*/;
+  int st = (SMEM_LIMIT - fixed) / B_STAGE_BYTES;
+  p.nstage = st > MAX_STAGES ? MAX_STAGES : st;
+  p.smem = (size_t)fixed + (size_t)p.nstage * B_STAGE_BYTES;
+  size_t o = 0;
+  auto take = [&](size_t bytes) {
+    const size_t at = o;
+    o += align_up(bytes, 256);
+    return at;
+  };
+  p.off_ynorm = take((size_t)(nb + 2 * BN) * sizeof(float));
+  p.off_xnorm = take((size_t)(nq + 1) * sizeof(float));
+  p.off_flag = take(256);
+  p.off_gbound = take((size_t)(nq + 1) * sizeof(unsigned int));
+  p.off_W = take((size_t)nq * p.S * p.K * sizeof(uint64_t));
+  p.off_cbuf = take((size_t)sms * BM * CBS * sizeof(uint64_t));
+  p.off_qhi = take((size_t)nq * d * sizeof(float));
+  p.off_qlo = take((size_t)nq * d * sizeof(float));
+  p.off_bhi = take((size_t)nb * d * sizeof(float));
+  p.off_blo = take((size_t)nb * d * sizeof(float));
+  p.bytes = o;
+  return p;
+}
+
+int flat_knn_tc_device(const float* xq, int64_t nq, const float* xb, int64_t nb, int d, int k, float* out_dist,
+                       int64_t* out_ids, void* ws, cudaStream_t s) {
+  const FlatTcPlan p = flat_tc_plan(nq, nb, d, k);
+  if (p.nstage < 2) return set_error(FS_EUNSUPPORTED, "flat tensor-core engine: d = %d leaves no room for the stage ring", d);
+  char* w = static_cast<char*>(ws);
+  float* ynorm = reinterpret_cast<float*>(w + p.off_ynorm);
+  float* xnorm = reinterpret_cast<float*>(w + p.off_xnorm);
+  unsigned int* flag = reinterpret_cast<unsigned int*>(w + p.off_flag);
+  unsigned int* gbound = reinterpret_cast<unsigned int*>(w + p.off_gbound);
+  float* qhi = reinterpret_cast<float*>(w + p.off_qhi);
+  float* qlo = reinterpret_cast<float*>(w + p.off_qlo);
+  float* bhi = reinterpret_cast<float*>(w + p.off_bhi);
+  float* blo = reinterpret_cast<float*>(w + p.off_blo);
+  FS_CUDA(cudaMemsetAsync(flag, 0, 256, s));
+  FS_CUDA(cudaMemsetAsync(gbound, 0xFF, (size_t)nq * sizeof(unsigned int), s));  // +inf image and above: no bound
+  split_norm_kernel<<<(unsigned)ceil_div(nb, 8), 256, 0, s>>>(xb, nb, d, bhi, blo, ynorm, flag);
+  FS_LAUNCHED();
+  split_norm_kernel<<<(unsigned)ceil_div(nq, 8), 256, 0, s>>>(xq, nq, d, qhi, qlo, xnorm, flag);
+  FS_LAUNCHED();
+
+  CUtensorMap ma_hi, ma_lo, mb_hi, mb_lo;
+  int rc;
+  if ((rc = make_map(&ma_hi, qhi, nq, d, BM)) != FS_OK || (rc = make_map(&ma_lo, qlo, nq, d, BM)) != FS_OK ||
+      (rc = make_map(&mb_hi, bhi, nb, d, BN)) != FS_OK || (rc = make_map(&mb_lo, blo, nb, d, BN)) != FS_OK)
+    return rc;
+  TcArgs a;
+  a.nq = nq;
+  a.nb = nb;
+  a.d = d;
+  a.KB = p.KB;
+  a.k = k;
+  a.kclass = p.kclass;
+  a.K = p.K;
+  a.S = p.S;
+  a.qtiles = p.qtiles;
+  a.nstage = p.nstage;
+  a.chunk = p.chunk;
+  a.ynorm = ynorm;
+  a.Wg = reinterpret_cast<uint64_t*>(w + p.off_W);
+  a.gbound = gbound;
+  a.cbuf = reinterpret_cast<uint64_t*>(w + p.off_cbuf);
+  a.lo_flag = flag;
+  static size_t attr_smem = 0;
+  if (p.smem > attr_smem) {
+    FS_CUDA(cudaFuncSetAttribute(flat_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem));
+    attr_smem = p.smem;
+  }
+  flat_tc_kernel<<<(unsigned)p.grid, TC_THREADS, p.smem, s>>>(ma_hi, ma_lo, mb_hi, mb_lo, a);
+  FS_LAUNCHED();
+  return launch_flat_finish(a.Wg, nq, p.S, k, xnorm, out_dist, out_ids, s);
+}
+
+}  // namespace fs
