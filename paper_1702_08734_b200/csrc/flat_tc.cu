@@ -10,12 +10,12 @@
 // finds lo == 0 everywhere (e.g. small-integer data such as cfg3) the kernel issues the
 // hi*hi products only, which is then exact -- a checked dispatch, never a guess.
 //
-// Kernel shape: persistent CTAs (one per SM), 192 threads:
+// Kernel shape: persistent CTAs (one per SM), 320 threads:
 //   warp 0      TMA producer   query tile (128 rows, resident per work item) and a ring
 //                              of database stages (256 rows x 32 columns x fp32 = 32 KB)
 //   warp 1      MMA issuer     tcgen05.mma kind::tf32, M=128 N=256 K=8, two 256-column
 //                              accumulators in TMEM (ping-pong with the epilogue)
-//   warps 2-5   epilogue       thread = TMEM lane = query row: tcgen05.ld, d' = ||y||^2 -
+//   warps 2-9   epilogue       two warpgroups, each on half of the tile's columns; thread = TMEM lane = query row: tcgen05.ld, d' = ||y||^2 -
 //                              2 acc, compare with the row's bound; the rare survivors go
 //                              to a per-row candidate buffer, merged into the row's queue
 //                              by the whole warp (warp_flush of select.cuh)
@@ -29,6 +29,7 @@
 
 #include "flat.cuh"
 #include "sm100.cuh"
+#include "tselect.cuh"
 
 namespace fs {
 
@@ -40,19 +41,23 @@ constexpr int BK = 32;                       // fp32 columns per stage = 128 byt
 constexpr int A_KB_BYTES = BM * BK * 4;      // 16 KB
 constexpr int B_STAGE_BYTES = BN * BK * 4;   // 32 KB
 constexpr int MAX_STAGES = 4;
-constexpr int TC_THREADS = 192;
-constexpr int CBS = 72;                      // candidate-buffer stride per row (64 + padding of warp_flush<*,2>)
+constexpr int EPI_GROUPS = 2;                 // epilogue warpgroups; group g takes columns [g*128, g*128+128) of a tile
+constexpr int TC_THREADS = 64 + EPI_GROUPS * 128;
+constexpr int EPI_RB = 5;                     // radix digit width of the epilogue selection (2 KB of counters per warp)
+constexpr int SCRATCH_BYTES = EPI_GROUPS * 4 * (1 << EPI_RB) * 64;  // 8 warps x 2 KB
 constexpr int SMEM_LIMIT = 227 * 1024;
 
 struct TcArgs {
   int64_t nq, nb;
   int d, KB, k, kclass, K;
-  int S, qtiles, nstage;
+  int S, qtiles;
+  int cap;                     // keys per row buffer: max(256, 2K)
+  int smem_bytes;              // dynamic shared memory of the launch
   int64_t chunk;               // database rows per split (multiple of BN)
   const float* ynorm;          // [>= nb rounded up to BN]
-  uint64_t* Wg;                // [nq][S][K]
+  uint64_t* Wg;                // [nq][S * EPI_GROUPS][K]
   unsigned int* gbound;        // [nq] order image of the best known k-th distance
-  uint64_t* cbuf;              // [gridDim.x][BM][CBS]
+  uint64_t* cbuf;              // [gridDim.x][EPI_GROUPS][BM][cap]: winners so far, then new candidates
   const unsigned int* lo_flag; // != 0: lo planes are not all zero (3xTF32)
 };
 
@@ -104,10 +109,10 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
   extern __shared__ unsigned char smem_dyn[];
   // operand tiles need 1024-byte alignment (128-byte swizzle atoms of 8 rows)
   unsigned char* smem = smem_dyn + ((1024u - (sm100::smem_addr(smem_dyn) & 1023u)) & 1023u);
-  unsigned char* sA_hi = smem;
-  unsigned char* sA_lo = sA_hi + (size_t)a.KB * A_KB_BYTES;
-  unsigned char* sB = sA_lo + (size_t)a.KB * A_KB_BYTES;
-  uint64_t* bars = reinterpret_cast<uint64_t*>(sB + (size_t)a.nstage * B_STAGE_BYTES);
+  const bool split = *a.lo_flag != 0u;
+  const int KB = a.KB;
+  // carve: barriers | selection scratch | A hi (| A lo) | ring of B stages (as many as fit, <= 4)
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem);
   uint64_t* full = bars;                    // [MAX_STAGES]
   uint64_t* empty = bars + MAX_STAGES;      // [MAX_STAGES]
   uint64_t* tfull = bars + 2 * MAX_STAGES;  // [2]
@@ -115,6 +120,12 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
   uint64_t* a_full = tempty + 2;
   uint64_t* a_empty = a_full + 1;
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(a_empty + 1);
+  unsigned char* scratch_all = smem + 1024;
+  unsigned char* sA_hi = scratch_all + SCRATCH_BYTES;
+  unsigned char* sA_lo = sA_hi + (size_t)KB * A_KB_BYTES;
+  unsigned char* sB = sA_lo + (split ? (size_t)KB * A_KB_BYTES : 0);
+  int nstage = (int)((smem_dyn + a.smem_bytes - sB) / B_STAGE_BYTES);
+  if (nstage > MAX_STAGES) nstage = MAX_STAGES;
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   if (threadIdx.x == 0) {
@@ -124,7 +135,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
     }
     for (int i = 0; i < 2; ++i) {
       sm100::mbar_init(tfull + i, 1);
-      sm100::mbar_init(tempty + i, 4);
+      sm100::mbar_init(tempty + i, 4 * EPI_GROUPS);
     }
     sm100::mbar_init(a_full, 1);
     sm100::mbar_init(a_empty, 1);
@@ -139,9 +150,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
   __syncthreads();
   sm100::tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
-  const bool split = *a.lo_flag != 0u;
   const int64_t n_items = (int64_t)a.S * a.qtiles;
-  const int KB = a.KB, nstage = a.nstage;
 
   if (warp == 0) {
     // ===== TMA producer =====
@@ -226,10 +235,12 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
   } else {
     // ===== epilogue: B3 =====
     const int quarter = warp & 3;  // TMEM lanes 32*quarter .. +31 belong to this warp
-    const int row = quarter * 32 + lane;
-    const int K = a.K;
-    uint64_t* cb_warp = a.cbuf + ((size_t)blockIdx.x * BM + quarter * 32) * CBS;
-    uint64_t* cb = cb_warp + (size_t)lane * CBS;
+    const int eg = (warp - 2) >> 2;  // epilogue group: its own columns, candidate buffers and partial queues
+    const int K = a.K, k = a.k, cap = a.cap;
+    const int SQ = a.S * EPI_GROUPS;  // partial queues per query
+    uint32_t* scratch = reinterpret_cast<uint32_t*>(scratch_all + (size_t)(warp - 2) * sel_scratch_bytes<EPI_RB>());
+    uint64_t* cb_warp = a.cbuf + (((size_t)blockIdx.x * EPI_GROUPS + eg) * BM + quarter * 32) * cap;
+    uint64_t* cb = cb_warp + (size_t)lane * cap;
     uint32_t tile_count = 0;
     for (int64_t item = blockIdx.x; item < n_items; item += gridDim.x) {
       const int s = (int)(item / a.qtiles), qt = (int)(item - (int64_t)s * a.qtiles);
@@ -239,32 +250,52 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
       const int64_t q_warp = (int64_t)qt * BM + quarter * 32;
       const int64_t q = q_warp + lane;
       const bool valid = q < a.nq;
-      // queues of this warp's rows start empty
-      for (int r = 0; r < 32; ++r) {
-        if (q_warp + r < a.nq) {
-          uint64_t* W = a.Wg + ((q_warp + r) * a.S + s) * K;
-          for (int i = lane; i < K; i += 32) W[i] = kSentinelKey;
-        }
-      }
       // start from the best bound other splits have published (inclusive)
       const uint64_t thr0 = valid ? (((uint64_t)a.gbound[q] << 32) | 0xFFFFFFFFull) : 0ull;
       uint64_t thr_key = thr0;
       float thr_val = valid ? ord_f32((uint32_t)(thr0 >> 32)) : __uint_as_float(0xFF800000u);
-      int cnt = 0;
+      int cnt = 0;  // keys in this row's buffer: the winners so far, then new candidates
       __syncwarp();
 
+      // Restore step for the rows that ask for it: the whole warp selects the k
+      // smallest of the row's buffer by radix counting (tselect.cuh), in place.
       auto flush_rows = [&](bool need) {
-        unsigned m = __ballot_sync(kFull, need);
-        while (m) {
-          const int r = __ffs(m) - 1;
-          m &= m - 1u;
-          const int rcnt = __shfl_sync(kFull, cnt, r);
-          const uint64_t nt = warp_flush_b64(a.kclass, a.Wg + ((q_warp + r) * a.S + s) * K + lane, 32,
-                                             cb_warp + (size_t)r * CBS, rcnt);
+        unsigned todo = __ballot_sync(kFull, need);
+        while (todo) {
+          const int r = __ffs(todo) - 1;
+          todo &= todo - 1u;
+          const int m = __shfl_sync(kFull, cnt, r);
+          if (m < k) continue;
+          uint64_t* buf = cb_warp + (size_t)r * cap;
+          __syncwarp();
+          uint64_t kor = 0ull, kand = ~0ull;
+          for (int i = lane; i < m; i += 32) {
+            const uint64_t key = buf[i];
+            kor |= key;
+            kand &= key;
+          }
+          const uint32_t olo = __reduce_or_sync(kFull, (uint32_t)kor), ohi = __reduce_or_sync(kFull, (uint32_t)(kor >> 32));
+          const uint32_t alo = __reduce_and_sync(kFull, (uint32_t)kand), ahi = __reduce_and_sync(kFull, (uint32_t)(kand >> 32));
+          const uint64_t diff = (((uint64_t)ohi << 32) | olo) & ~(((uint64_t)ahi << 32) | alo);
+          const uint64_t kth = radix_select_kth<EPI_RB>(buf, m, k, diff, scratch);
+          int w = 0;
+          for (int i0 = 0; i0 < m; i0 += 32) {  // keep the keys <= kth: exactly k (keys are distinct)
+            const int i = i0 + lane;
+            uint64_t key = 0;
+            bool keep = false;
+            if (i < m) {
+              key = buf[i];
+              keep = key <= kth;
+            }
+            const unsigned b = __ballot_sync(kFull, keep);
+            if (keep) buf[w + __popc(b & ((1u << lane) - 1u))] = key;
+            w += __popc(b);
+          }
+          __syncwarp();
           if (lane == r) {
-            thr_key = nt < thr0 ? nt : thr0;
+            thr_key = kth < thr0 ? kth : thr0;
             thr_val = key_val(thr_key);
-            cnt = 0;
+            cnt = k;
           }
         }
       };
@@ -277,7 +308,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
         sm100::tc_fence_after();
         const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + as * BN;
 #pragma unroll 1
-        for (int cg = 0; cg < BN / 32; ++cg) {
+        for (int cg = eg * (BN / 32 / EPI_GROUPS); cg < (eg + 1) * (BN / 32 / EPI_GROUPS); ++cg) {
           uint32_t v[32];
           sm100::tmem_ld32(taddr + cg * 32, v);
           float4 yn[8];
@@ -287,29 +318,46 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
           sm100::tmem_ld_wait();
           const uint32_t cbase = (uint32_t)col0 + cg * 32;
           const int climit = ncols - cg * 32;  // columns of this group that exist
+          // first-level filter: one FFMA and one compare per element, results in a mask
+          uint32_t mask = 0u;
 #pragma unroll
           for (int j = 0; j < 32; ++j) {
             const float y = j % 4 == 0 ? yn[j / 4].x : j % 4 == 1 ? yn[j / 4].y : j % 4 == 2 ? yn[j / 4].z : yn[j / 4].w;
             const float dp = fmaf(-2.f, __uint_as_float(v[j]), y);
-            if (!(dp > thr_val)) {  // rare
-              const uint64_t key = make_key(dp, cbase + j);
-              if (j < climit && key < thr_key) cb[cnt++] = key;
-            }
+            v[j] = __float_as_uint(dp);
+            mask |= (!(dp > thr_val) ? 1u : 0u) << j;
           }
-          flush_rows(cnt > 32);
+          if (climit < 32) mask &= climit > 0 ? (0xFFFFFFFFu >> (32 - climit)) : 0u;
+          while (mask) {  // rare survivors: exact key test, append to the row's buffer
+            const int j = __ffs(mask) - 1;
+            mask &= mask - 1u;
+            float dp = 0.f;
+#pragma unroll
+            for (int jj = 0; jj < 32; ++jj)
+              if (jj == j) dp = __uint_as_float(v[jj]);
+            const uint64_t key = make_key(dp, cbase + j);
+            if (key < thr_key) cb[cnt++] = key;
+          }
+          flush_rows(cnt > cap - 32);
         }
         // accumulator drained
         sm100::tc_fence_before();
         __syncwarp();
         if (lane == 0) sm100::mbar_arrive(tempty + as);
       }
-      flush_rows(cnt > 0);
+      flush_rows(cnt >= k);
       __syncwarp();
-      // publish this split's k-th distance as a bound for the splits still to run
-      if (valid) {
-        const uint64_t kth = a.Wg[(q * a.S + s) * K + (a.k - 1)];
-        if (kth != kSentinelKey) atomicMin(a.gbound + q, (unsigned int)(kth >> 32));
+      // the row's partial queue for B4 (unordered winners, sentinel padded), and this
+      // split's k-th distance as a bound for the splits still to run
+      for (int r = 0; r < 32; ++r) {
+        if (q_warp + r >= a.nq) break;
+        const int m = __shfl_sync(kFull, cnt, r);
+        const uint64_t* buf = cb_warp + (size_t)r * cap;
+        uint64_t* W = a.Wg + ((q_warp + r) * SQ + s * EPI_GROUPS + eg) * K;
+        for (int i = lane; i < K; i += 32) W[i] = i < m ? buf[i] : kSentinelKey;
       }
+      if (valid && cnt >= k && thr_key < thr0) atomicMin(a.gbound + q, (unsigned int)(thr_key >> 32));
+      __syncwarp();
     }
   }
   // teardown
@@ -403,10 +451,13 @@ FlatTcPlan flat_tc_plan(int64_t nq, int64_t nb, int d, int k) {
   const int64_t items = (int64_t)p.S * p.qtiles;
   p.grid = (int)(items < sms ? items : sms);
   p.KB = d / BK;
-  const int fixed = 2 * p.KB * A_KB_BYTES + 1024 /*alignment*/ + 256 /*barriers*/;
+  p.cap = 2 * p.K > 256 ? 2 * p.K : 256;
+  // the kernel carves the ring at run time (the lo plane of the query tile is only
+  // resident in 3xTF32 mode); worst case = with the lo plane
+  const int fixed = 1024 /*alignment*/ + 1024 /*barriers*/ + SCRATCH_BYTES + 2 * p.KB * A_KB_BYTES;
   int st = (SMEM_LIMIT - fixed) / B_STAGE_BYTES;
   p.nstage = st > MAX_STAGES ? MAX_STAGES : st;
-  p.smem = (size_t)fixed + (size_t)p.nstage * B_STAGE_BYTES;
+  p.smem = SMEM_LIMIT;
   size_t o = 0;
   auto take = [&](size_t bytes) {
     const size_t at = o;
@@ -417,8 +468,8 @@ FlatTcPlan flat_tc_plan(int64_t nq, int64_t nb, int d, int k) {
   p.off_xnorm = take((size_t)(nq + 1) * sizeof(float));
   p.off_flag = take(256);
   p.off_gbound = take((size_t)(nq + 1) * sizeof(unsigned int));
-  p.off_W = take((size_t)nq * p.S * p.K * sizeof(uint64_t));
-  p.off_cbuf = take((size_t)sms * BM * CBS * sizeof(uint64_t));
+  p.off_W = take((size_t)nq * p.S * EPI_GROUPS * p.K * sizeof(uint64_t));
+  p.off_cbuf = take((size_t)sms * EPI_GROUPS * BM * p.cap * sizeof(uint64_t));
   p.off_qhi = take((size_t)nq * d * sizeof(float));
   p.off_qlo = take((size_t)nq * d * sizeof(float));
   p.off_bhi = take((size_t)nb * d * sizeof(float));
@@ -462,7 +513,8 @@ int flat_knn_tc_device(const float* xq, int64_t nq, const float* xb, int64_t nb,
   a.K = p.K;
   a.S = p.S;
   a.qtiles = p.qtiles;
-  a.nstage = p.nstage;
+  a.cap = p.cap;
+  a.smem_bytes = (int)p.smem;
   a.chunk = p.chunk;
   a.ynorm = ynorm;
   a.Wg = reinterpret_cast<uint64_t*>(w + p.off_W);
@@ -476,7 +528,7 @@ int flat_knn_tc_device(const float* xq, int64_t nq, const float* xb, int64_t nb,
   }
   flat_tc_kernel<<<(unsigned)p.grid, TC_THREADS, p.smem, s>>>(ma_hi, ma_lo, mb_hi, mb_lo, a);
   FS_LAUNCHED();
-  return launch_flat_finish(a.Wg, nq, p.S, k, xnorm, out_dist, out_ids, s);
+  return launch_flat_finish(a.Wg, nq, p.S * EPI_GROUPS, k, xnorm, out_dist, out_ids, s);
 }
 
 }  // namespace fs
