@@ -41,6 +41,7 @@ constexpr int BK = 32;                       // fp32 columns per stage = 128 byt
 constexpr int A_KB_BYTES = BM * BK * 4;      // 16 KB
 constexpr int B_STAGE_BYTES = BN * BK * 4;   // 32 KB
 constexpr int MAX_STAGES = 4;
+constexpr int YN_RING = 4;                    // ||y||^2 tiles (1 KB each) in flight ahead of the epilogue
 constexpr int EPI_GROUPS = 2;                 // epilogue warpgroups; group g takes columns [g*128, g*128+128) of a tile
 constexpr int TC_THREADS = 64 + EPI_GROUPS * 128;
 constexpr int EPI_RB = 5;                     // radix digit width of the epilogue selection (2 KB of counters per warp)
@@ -119,8 +120,11 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
   uint64_t* tempty = tfull + 2;             // [2]
   uint64_t* a_full = tempty + 2;
   uint64_t* a_empty = a_full + 1;
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(a_empty + 1);
-  unsigned char* scratch_all = smem + 1024;
+  uint64_t* yfull = a_empty + 1;            // [YN_RING]
+  uint64_t* yempty = yfull + YN_RING;       // [YN_RING]
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(yempty + YN_RING);
+  float* s_yn = reinterpret_cast<float*>(smem + 1024);  // [YN_RING][BN]
+  unsigned char* scratch_all = smem + 1024 + YN_RING * BN * 4;
   unsigned char* sA_hi = scratch_all + SCRATCH_BYTES;
   unsigned char* sA_lo = sA_hi + (size_t)KB * A_KB_BYTES;
   unsigned char* sB = sA_lo + (split ? (size_t)KB * A_KB_BYTES : 0);
@@ -139,6 +143,10 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
     }
     sm100::mbar_init(a_full, 1);
     sm100::mbar_init(a_empty, 1);
+    for (int i = 0; i < YN_RING; ++i) {
+      sm100::mbar_init(yfull + i, 1);
+      sm100::mbar_init(yempty + i, 4 * EPI_GROUPS);
+    }
     sm100::fence_mbar_init();
     sm100::tma_prefetch_desc(&map_a_hi);
     sm100::tma_prefetch_desc(&map_a_lo);
@@ -157,6 +165,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
     if (lane == 0) {
       Pipe pp{0, 0u};
       int it = 0;
+      uint32_t ptile = 0;
       for (int64_t item = blockIdx.x; item < n_items; item += gridDim.x, ++it) {
         const int s = (int)(item / a.qtiles), qt = (int)(item - (int64_t)s * a.qtiles);
         const int64_t b_begin = (int64_t)s * a.chunk;
@@ -168,8 +177,14 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
           sm100::tma_load_2d(sA_hi + kb * A_KB_BYTES, &map_a_hi, kb * BK, qt * BM, a_full);
           if (split) sm100::tma_load_2d(sA_lo + kb * A_KB_BYTES, &map_a_lo, kb * BK, qt * BM, a_full);
         }
-        for (int t = 0; t < ntiles; ++t) {
+        for (int t = 0; t < ntiles; ++t, ++ptile) {
           const int row0 = (int)(b_begin + (int64_t)t * BN);
+          {  // the tile's ||y||^2 values for the epilogue
+            const uint32_t ys = ptile % YN_RING;
+            sm100::mbar_wait(yempty + ys, ((ptile / YN_RING) & 1u) ^ 1u);
+            sm100::mbar_expect_tx(yfull + ys, BN * 4);
+            sm100::bulk_load(s_yn + ys * BN, a.ynorm + row0, BN * 4, yfull + ys);
+          }
           for (int kb = 0; kb < KB; ++kb) {
             for (int pl = 0; pl < (split ? 2 : 1); ++pl) {
               sm100::mbar_wait(empty + pp.stage, pp.phase ^ 1u);
@@ -307,22 +322,29 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
         sm100::mbar_wait(tfull + as, (tile_count >> 1) & 1u);
         sm100::tc_fence_after();
         const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + as * BN;
-#pragma unroll 1
-        for (int cg = eg * (BN / 32 / EPI_GROUPS); cg < (eg + 1) * (BN / 32 / EPI_GROUPS); ++cg) {
-          uint32_t v[32];
-          sm100::tmem_ld32(taddr + cg * 32, v);
-          float4 yn[8];
-          const float4* ynp = reinterpret_cast<const float4*>(a.ynorm + col0 + cg * 32);
+        // this group's 128 columns in four blocks of 32; ||y||^2 comes from the shared-memory
+        // tile the producer staged (the TMEM load is not pipelined: its destination
+        // registers must not be touched before tcgen05.wait::ld)
+        constexpr int NBLK = BN / 32 / EPI_GROUPS;
+        const int cg0 = eg * NBLK;
+        uint32_t v[32];
+        const uint32_t ys = tile_count % YN_RING;
+        sm100::mbar_wait(yfull + ys, (tile_count / YN_RING) & 1u);
+        const float4* ynp = reinterpret_cast<const float4*>(s_yn + ys * BN + cg0 * 32);
 #pragma unroll
-          for (int j = 0; j < 8; ++j) yn[j] = __ldg(ynp + j);
+        for (int i = 0; i < NBLK; ++i) {
+          flush_rows(cnt > cap - 32);
+          sm100::tmem_ld32(taddr + (cg0 + i) * 32, v);
           sm100::tmem_ld_wait();
+          const int cg = cg0 + i;
           const uint32_t cbase = (uint32_t)col0 + cg * 32;
-          const int climit = ncols - cg * 32;  // columns of this group that exist
+          const int climit = ncols - cg * 32;  // columns of this block that exist
           // first-level filter: one FFMA and one compare per element, results in a mask
           uint32_t mask = 0u;
 #pragma unroll
           for (int j = 0; j < 32; ++j) {
-            const float y = j % 4 == 0 ? yn[j / 4].x : j % 4 == 1 ? yn[j / 4].y : j % 4 == 2 ? yn[j / 4].z : yn[j / 4].w;
+            const float4 y4 = ynp[i * 8 + j / 4];
+            const float y = j % 4 == 0 ? y4.x : j % 4 == 1 ? y4.y : j % 4 == 2 ? y4.z : y4.w;
             const float dp = fmaf(-2.f, __uint_as_float(v[j]), y);
             v[j] = __float_as_uint(dp);
             mask |= (!(dp > thr_val) ? 1u : 0u) << j;
@@ -338,12 +360,14 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
             const uint64_t key = make_key(dp, cbase + j);
             if (key < thr_key) cb[cnt++] = key;
           }
-          flush_rows(cnt > cap - 32);
         }
         // accumulator drained
         sm100::tc_fence_before();
         __syncwarp();
-        if (lane == 0) sm100::mbar_arrive(tempty + as);
+        if (lane == 0) {
+          sm100::mbar_arrive(tempty + as);
+          sm100::mbar_arrive(yempty + ys);
+        }
       }
       flush_rows(cnt >= k);
       __syncwarp();
@@ -454,7 +478,7 @@ FlatTcPlan flat_tc_plan(int64_t nq, int64_t nb, int d, int k) {
   p.cap = 2 * p.K > 256 ? 2 * p.K : 256;
   // the kernel carves the ring at run time (the lo plane of the query tile is only
   // resident in 3xTF32 mode); worst case = with the lo plane
-  const int fixed = 1024 /*alignment*/ + 1024 /*barriers*/ + SCRATCH_BYTES + 2 * p.KB * A_KB_BYTES;
+  const int fixed = 1024 /*alignment*/ + 1024 /*barriers*/ + YN_RING * BN * 4 + SCRATCH_BYTES + 2 * p.KB * A_KB_BYTES;
   int st = (SMEM_LIMIT - fixed) / B_STAGE_BYTES;
   p.nstage = st > MAX_STAGES ? MAX_STAGES : st;
   p.smem = SMEM_LIMIT;
