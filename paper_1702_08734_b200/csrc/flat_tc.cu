@@ -23,6 +23,9 @@
 // run at the same time read the same part of the database (L2 reuse), and a query's
 // bound found in earlier splits (gbound) prunes the later ones.
 #include <cuda.h>
+#ifndef FS_TC_EXP
+#define FS_TC_EXP 0  // 1 / 2: timing experiments (epilogue without filter / without TMEM loads); never shipped
+#endif
 
 #include <cstdlib>
 #include <cstring>
@@ -41,6 +44,8 @@ constexpr int BK = 32;                       // fp32 columns per stage = 128 byt
 constexpr int A_KB_BYTES = BM * BK * 4;      // 16 KB
 constexpr int B_STAGE_BYTES = BN * BK * 4;   // 32 KB
 constexpr int MAX_STAGES = 4;
+constexpr int CLUSTER = 2;                    // CTAs per cluster: same database tiles, different query tiles;
+                                              // each loads 1/CLUSTER of a database stage and multicasts it
 constexpr int YN_RING = 4;                    // ||y||^2 tiles (1 KB each) in flight ahead of the epilogue
 constexpr int EPI_GROUPS = 2;                 // epilogue warpgroups; group g takes columns [g*128, g*128+128) of a tile
 constexpr int TC_THREADS = 64 + EPI_GROUPS * 128;
@@ -52,6 +57,7 @@ struct TcArgs {
   int64_t nq, nb;
   int d, KB, k, kclass, K;
   int S, qtiles;
+  int qgroups;                 // ceil(qtiles / CLUSTER): work item = (split, group of CLUSTER query tiles)
   int cap;                     // keys per row buffer: max(256, 2K)
   int smem_bytes;              // dynamic shared memory of the launch
   int64_t chunk;               // database rows per split (multiple of BN)
@@ -135,7 +141,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
   if (threadIdx.x == 0) {
     for (int i = 0; i < MAX_STAGES; ++i) {
       sm100::mbar_init(full + i, 1);
-      sm100::mbar_init(empty + i, 1);
+      sm100::mbar_init(empty + i, CLUSTER);  // the MMA warps of all CTAs of the cluster release a stage
     }
     for (int i = 0; i < 2; ++i) {
       sm100::mbar_init(tfull + i, 1);
@@ -156,9 +162,13 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
   if (warp == 1) sm100::tmem_alloc(tmem_slot, 512);
   sm100::tc_fence_before();
   __syncthreads();
+  if (CLUSTER > 1) sm100::cluster_sync_all();  // peers' barriers are initialised before anything lands on them
   sm100::tc_fence_after();
+  const uint32_t crank = CLUSTER > 1 ? sm100::cluster_ctarank() : 0u;
+  const int64_t cluster_id = blockIdx.x / CLUSTER, n_clusters = gridDim.x / CLUSTER;
+  constexpr uint16_t kAllCtas = (uint16_t)((1u << CLUSTER) - 1u);
   const uint32_t tmem_base = *tmem_slot;
-  const int64_t n_items = (int64_t)a.S * a.qtiles;
+  const int64_t n_items = (int64_t)a.S * a.qgroups;
 
   if (warp == 0) {
     // ===== TMA producer =====
@@ -166,8 +176,8 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
       Pipe pp{0, 0u};
       int it = 0;
       uint32_t ptile = 0;
-      for (int64_t item = blockIdx.x; item < n_items; item += gridDim.x, ++it) {
-        const int s = (int)(item / a.qtiles), qt = (int)(item - (int64_t)s * a.qtiles);
+      for (int64_t item = cluster_id; item < n_items; item += n_clusters, ++it) {
+        const int s = (int)(item / a.qgroups), qt = (int)(item - (int64_t)s * a.qgroups) * CLUSTER + (int)crank;
         const int64_t b_begin = (int64_t)s * a.chunk;
         const int64_t b_end = b_begin + a.chunk < a.nb ? b_begin + a.chunk : a.nb;
         const int ntiles = (int)((b_end - b_begin + BN - 1) / BN);
@@ -187,10 +197,17 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
           }
           for (int kb = 0; kb < KB; ++kb) {
             for (int pl = 0; pl < (split ? 2 : 1); ++pl) {
-              sm100::mbar_wait(empty + pp.stage, pp.phase ^ 1u);
+              sm100::mbar_wait(empty + pp.stage, pp.phase ^ 1u);  // free in every CTA of the cluster
               sm100::mbar_expect_tx(full + pp.stage, (uint32_t)B_STAGE_BYTES);
-              sm100::tma_load_2d(sB + (size_t)pp.stage * B_STAGE_BYTES, pl ? &map_b_lo : &map_b_hi, kb * BK, row0,
-                                 full + pp.stage);
+              if (CLUSTER > 1) {  // this CTA's share of the rows, delivered to all CTAs
+                constexpr int rows = BN / CLUSTER;
+                sm100::tma_load_2d_mc(sB + (size_t)pp.stage * B_STAGE_BYTES + (size_t)crank * rows * BK * 4,
+                                      pl ? &map_b_lo : &map_b_hi, kb * BK, row0 + (int)crank * rows, full + pp.stage,
+                                      kAllCtas);
+              } else {
+                sm100::tma_load_2d(sB + (size_t)pp.stage * B_STAGE_BYTES, pl ? &map_b_lo : &map_b_hi, kb * BK, row0,
+                                   full + pp.stage);
+              }
               pp.advance(nstage);
             }
           }
@@ -204,8 +221,8 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
       Pipe pc{0, 0u};
       uint32_t tile_count = 0;
       int it = 0;
-      for (int64_t item = blockIdx.x; item < n_items; item += gridDim.x, ++it) {
-        const int s = (int)(item / a.qtiles);
+      for (int64_t item = cluster_id; item < n_items; item += n_clusters, ++it) {
+        const int s = (int)(item / a.qgroups);
         const int64_t b_begin = (int64_t)s * a.chunk;
         const int64_t b_end = b_begin + a.chunk < a.nb ? b_begin + a.chunk : a.nb;
         const int ntiles = (int)((b_end - b_begin + BN - 1) / BN);
@@ -230,7 +247,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
 #pragma unroll
               for (int ks = 0; ks < BK / 8; ++ks) sm100::mma_tf32_ss(d_tmem, da_lo + 2 * ks, db + 2 * ks, idesc, 1u);
             }
-            sm100::mma_commit(empty + pc.stage);
+            if (CLUSTER > 1) sm100::mma_commit_mc(empty + pc.stage, kAllCtas); else sm100::mma_commit(empty + pc.stage);
             pc.advance(nstage);
             if (split) {  // stage with the lo plane: hi*lo
               sm100::mbar_wait(full + pc.stage, pc.phase);
@@ -238,7 +255,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
               db = sm100::make_kmajor_sw128_desc(sm100::smem_addr(sB + (size_t)pc.stage * B_STAGE_BYTES));
 #pragma unroll
               for (int ks = 0; ks < BK / 8; ++ks) sm100::mma_tf32_ss(d_tmem, da_hi + 2 * ks, db + 2 * ks, idesc, 1u);
-              sm100::mma_commit(empty + pc.stage);
+              if (CLUSTER > 1) sm100::mma_commit_mc(empty + pc.stage, kAllCtas); else sm100::mma_commit(empty + pc.stage);
               pc.advance(nstage);
             }
           }
@@ -257,8 +274,8 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
     uint64_t* cb_warp = a.cbuf + (((size_t)blockIdx.x * EPI_GROUPS + eg) * BM + quarter * 32) * cap;
     uint64_t* cb = cb_warp + (size_t)lane * cap;
     uint32_t tile_count = 0;
-    for (int64_t item = blockIdx.x; item < n_items; item += gridDim.x) {
-      const int s = (int)(item / a.qtiles), qt = (int)(item - (int64_t)s * a.qtiles);
+    for (int64_t item = cluster_id; item < n_items; item += n_clusters) {
+      const int s = (int)(item / a.qgroups), qt = (int)(item - (int64_t)s * a.qgroups) * CLUSTER + (int)crank;
       const int64_t b_begin = (int64_t)s * a.chunk;
       const int64_t b_end = b_begin + a.chunk < a.nb ? b_begin + a.chunk : a.nb;
       const int ntiles = (int)((b_end - b_begin + BN - 1) / BN);
@@ -325,40 +342,52 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
         // this group's 128 columns in four blocks of 32; ||y||^2 comes from the shared-memory
         // tile the producer staged (the TMEM load is not pipelined: its destination
         // registers must not be touched before tcgen05.wait::ld)
-        constexpr int NBLK = BN / 32 / EPI_GROUPS;
-        const int cg0 = eg * NBLK;
-        uint32_t v[32];
+        constexpr int BW = 64;  // columns per TMEM load
+        constexpr int NBLK = BN / BW / EPI_GROUPS;
+        const int cg0 = eg * NBLK;  // first block of this group
+        uint32_t v[BW];
         const uint32_t ys = tile_count % YN_RING;
         sm100::mbar_wait(yfull + ys, (tile_count / YN_RING) & 1u);
-        const float4* ynp = reinterpret_cast<const float4*>(s_yn + ys * BN + cg0 * 32);
-#pragma unroll
+        const float4* ynp = reinterpret_cast<const float4*>(s_yn + ys * BN + cg0 * BW);
+#pragma unroll 1
         for (int i = 0; i < NBLK; ++i) {
-          flush_rows(cnt > cap - 32);
-          sm100::tmem_ld32(taddr + (cg0 + i) * 32, v);
+          flush_rows(cnt > cap - BW);
+#if FS_TC_EXP == 2
+          continue;
+#endif
+          sm100::tmem_ld64(taddr + (cg0 + i) * BW, v);
           sm100::tmem_ld_wait();
-          const int cg = cg0 + i;
-          const uint32_t cbase = (uint32_t)col0 + cg * 32;
-          const int climit = ncols - cg * 32;  // columns of this block that exist
-          // first-level filter: one FFMA and one compare per element, results in a mask
-          uint32_t mask = 0u;
+#if FS_TC_EXP == 1
+          if (v[0] == 0x12345678u && v[63] == 0x9abcdef0u) cb[cnt++] = 0;  // keep the load alive
+          continue;
+#endif
+          const uint32_t cbase = (uint32_t)col0 + (cg0 + i) * BW;
+          const int climit = ncols - (cg0 + i) * BW;  // columns of this block that exist
+          // first-level filter: one FFMA and one compare per element, results in two masks
+          uint32_t mask[2] = {0u, 0u};
 #pragma unroll
-          for (int j = 0; j < 32; ++j) {
-            const float4 y4 = ynp[i * 8 + j / 4];
+          for (int j = 0; j < BW; ++j) {
+            const float4 y4 = ynp[i * (BW / 4) + j / 4];
             const float y = j % 4 == 0 ? y4.x : j % 4 == 1 ? y4.y : j % 4 == 2 ? y4.z : y4.w;
             const float dp = fmaf(-2.f, __uint_as_float(v[j]), y);
             v[j] = __float_as_uint(dp);
-            mask |= (!(dp > thr_val) ? 1u : 0u) << j;
+            mask[j >> 5] |= (!(dp > thr_val) ? 1u : 0u) << (j & 31);
           }
-          if (climit < 32) mask &= climit > 0 ? (0xFFFFFFFFu >> (32 - climit)) : 0u;
-          while (mask) {  // rare survivors: exact key test, append to the row's buffer
-            const int j = __ffs(mask) - 1;
-            mask &= mask - 1u;
-            float dp = 0.f;
 #pragma unroll
-            for (int jj = 0; jj < 32; ++jj)
-              if (jj == j) dp = __uint_as_float(v[jj]);
-            const uint64_t key = make_key(dp, cbase + j);
-            if (key < thr_key) cb[cnt++] = key;
+          for (int h = 0; h < 2; ++h) {
+            const int cl = climit - 32 * h;
+            uint32_t mk = mask[h];
+            if (cl < 32) mk &= cl > 0 ? (0xFFFFFFFFu >> (32 - cl)) : 0u;
+            while (mk) {  // rare survivors: exact key test, append to the row's buffer
+              const int j = __ffs(mk) - 1;
+              mk &= mk - 1u;
+              float dp = 0.f;
+#pragma unroll
+              for (int jj = 0; jj < 32; ++jj)
+                if (jj == j) dp = __uint_as_float(v[32 * h + jj]);
+              const uint64_t key = make_key(dp, cbase + 32 * h + j);
+              if (key < thr_key) cb[cnt++] = key;
+            }
           }
         }
         // accumulator drained
@@ -384,9 +413,10 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
       __syncwarp();
     }
   }
-  // teardown
+  // teardown (no CTA may exit while a peer can still write into it or arrive on its barriers)
   sm100::tc_fence_before();
   __syncthreads();
+  if (CLUSTER > 1) sm100::cluster_sync_all();
   if (warp == 1) {
     sm100::tc_fence_after();
     sm100::tmem_dealloc(tmem_base, 512);
@@ -453,6 +483,8 @@ FlatTcPlan flat_tc_plan(int64_t nq, int64_t nb, int d, int k) {
   p.qtiles = (int)ceil_div(nq, BM);
   const int64_t nt = ceil_div(nb > 0 ? nb : 1, BN);
   const int64_t sms = sm_count();
+  const int64_t qgroups = ceil_div(p.qtiles, CLUSTER), ncl = sms / CLUSTER;
+  p.qgroups = (int)qgroups;
   // database splits: fill whole waves of CTAs with as few partial queues as possible
   int64_t best_S = 1;
   double best = -1.0;
@@ -460,9 +492,9 @@ FlatTcPlan flat_tc_plan(int64_t nq, int64_t nb, int d, int k) {
   for (int64_t S = 1; S <= max_S; ++S) {
     const int64_t per = ceil_div(nt, S);
     const int64_t realS = ceil_div(nt, per);
-    const int64_t items = realS * p.qtiles;
-    const int64_t g = items < sms ? items : sms;
-    const double eff = (double)items / (double)(ceil_div(items, g) * g) * ((double)g / (double)sms);
+    const int64_t items = realS * qgroups;
+    const int64_t g = items < ncl ? items : ncl;
+    const double eff = (double)items / (double)(ceil_div(items, g) * g) * ((double)g / (double)ncl);
     const double score = eff - 0.002 * (double)realS;
     if (score > best) {
       best = score;
@@ -472,10 +504,10 @@ FlatTcPlan flat_tc_plan(int64_t nq, int64_t nb, int d, int k) {
   const int64_t per = ceil_div(nt, best_S);
   p.chunk = per * BN;
   p.S = (int)ceil_div(nb > 0 ? nb : 1, p.chunk);
-  const int64_t items = (int64_t)p.S * p.qtiles;
-  p.grid = (int)(items < sms ? items : sms);
+  const int64_t items = (int64_t)p.S * qgroups;
+  p.grid = (int)(items < ncl ? items : ncl) * CLUSTER;
   p.KB = d / BK;
-  p.cap = 2 * p.K > 256 ? 2 * p.K : 256;
+  p.cap = 2 * p.K > 256 ? 2 * p.K : 256;  // >= K + 64: a block appends at most 64 keys per row
   // the kernel carves the ring at run time (the lo plane of the query tile is only
   // resident in 3xTF32 mode); worst case = with the lo plane
   const int fixed = 1024 /*alignment*/ + 1024 /*barriers*/ + YN_RING * BN * 4 + SCRATCH_BYTES + 2 * p.KB * A_KB_BYTES;
@@ -525,7 +557,8 @@ int flat_knn_tc_device(const float* xq, int64_t nq, const float* xb, int64_t nb,
   CUtensorMap ma_hi, ma_lo, mb_hi, mb_lo;
   int rc;
   if ((rc = make_map(&ma_hi, qhi, nq, d, BM)) != FS_OK || (rc = make_map(&ma_lo, qlo, nq, d, BM)) != FS_OK ||
-      (rc = make_map(&mb_hi, bhi, nb, d, BN)) != FS_OK || (rc = make_map(&mb_lo, blo, nb, d, BN)) != FS_OK)
+      (rc = make_map(&mb_hi, bhi, nb, d, BN / CLUSTER)) != FS_OK ||
+      (rc = make_map(&mb_lo, blo, nb, d, BN / CLUSTER)) != FS_OK)
     return rc;
   TcArgs a;
   a.nq = nq;
@@ -537,6 +570,7 @@ int flat_knn_tc_device(const float* xq, int64_t nq, const float* xb, int64_t nb,
   a.K = p.K;
   a.S = p.S;
   a.qtiles = p.qtiles;
+  a.qgroups = p.qgroups;
   a.cap = p.cap;
   a.smem_bytes = (int)p.smem;
   a.chunk = p.chunk;
@@ -550,7 +584,19 @@ int flat_knn_tc_device(const float* xq, int64_t nq, const float* xb, int64_t nb,
     FS_CUDA(cudaFuncSetAttribute(flat_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem));
     attr_smem = p.smem;
   }
-  flat_tc_kernel<<<(unsigned)p.grid, TC_THREADS, p.smem, s>>>(ma_hi, ma_lo, mb_hi, mb_lo, a);
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)p.grid);
+  cfg.blockDim = dim3(TC_THREADS);
+  cfg.dynamicSmemBytes = p.smem;
+  cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = CLUSTER;
+  attr[0].val.clusterDim.y = 1;
+  attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  FS_CUDA(cudaLaunchKernelEx(&cfg, flat_tc_kernel, ma_hi, ma_lo, mb_hi, mb_lo, a));
   FS_LAUNCHED();
   return launch_flat_finish(a.Wg, nq, p.S * EPI_GROUPS, k, xnorm, out_dist, out_ids, s);
 }
