@@ -11,11 +11,11 @@
 // hi*hi products only, which is then exact -- a checked dispatch, never a guess.
 //
 // Kernel shape: persistent CTAs (one per SM), 320 threads:
-//   warp 0      TMA producer   query tile (128 rows, resident per work item) and a ring
+//   warp 8      TMA producer   query tile (128 rows, resident per work item) and a ring
 //                              of database stages (256 rows x 32 columns x fp32 = 32 KB)
-//   warp 1      MMA issuer     tcgen05.mma kind::tf32, M=128 N=256 K=8, two 256-column
+//   warp 9      MMA issuer     tcgen05.mma kind::tf32, M=128 N=256 K=8, two 256-column
 //                              accumulators in TMEM (ping-pong with the epilogue)
-//   warps 2-9   epilogue       two warpgroups, each on half of the tile's columns; thread = TMEM lane = query row: tcgen05.ld, d' = ||y||^2 -
+//   warps 0-7   epilogue       two warpgroups, each on half of the tile's columns; thread = TMEM lane = query row: tcgen05.ld, d' = ||y||^2 -
 //                              2 acc, compare with the row's bound; the rare survivors go
 //                              to a per-row candidate buffer, merged into the row's queue
 //                              by the whole warp (warp_flush of select.cuh)
@@ -46,11 +46,15 @@ constexpr int B_STAGE_BYTES = BN * BK * 4;   // 32 KB
 constexpr int MAX_STAGES = 4;
 constexpr int CLUSTER = 2;                    // CTAs per cluster: same database tiles, different query tiles;
                                               // each loads 1/CLUSTER of a database stage and multicasts it
-constexpr int YN_RING = 4;                    // ||y||^2 tiles (1 KB each) in flight ahead of the epilogue
+constexpr int YN_RING = 2;                    // ||y||^2 tiles (1 KB each) in flight ahead of the epilogue
 constexpr int EPI_GROUPS = 2;                 // epilogue warpgroups; group g takes columns [g*128, g*128+128) of a tile
 constexpr int TC_THREADS = 64 + EPI_GROUPS * 128;
-constexpr int EPI_RB = 5;                     // radix digit width of the epilogue selection (2 KB of counters per warp)
-constexpr int SCRATCH_BYTES = EPI_GROUPS * 4 * (1 << EPI_RB) * 64;  // 8 warps x 2 KB
+// Warp roles.  The two single-thread roles take the highest warp ids (the sub-partition
+// schedulers favour higher warp ids; a starved MMA issuer would idle the tensor pipe).
+constexpr int TMA_WARP = EPI_GROUPS * 4, MMA_WARP = EPI_GROUPS * 4 + 1;
+constexpr int EPI_RB = 4;                     // radix digit width of the epilogue selection (1 KB of counters per warp)
+constexpr int STAGE_KEYS = 256;               // row buffers up to this size are selected in shared memory
+constexpr int SCRATCH_BYTES = EPI_GROUPS * 4 * ((1 << EPI_RB) * 64 + STAGE_KEYS * 8);  // 8 warps x (1 KB + 2 KB)
 constexpr int SMEM_LIMIT = 227 * 1024;
 
 struct TcArgs {
@@ -58,7 +62,7 @@ struct TcArgs {
   int d, KB, k, kclass, K;
   int S, qtiles;
   int qgroups;                 // ceil(qtiles / CLUSTER): work item = (split, group of CLUSTER query tiles)
-  int cap;                     // keys per row buffer: max(256, 2K)
+  int cap;                     // keys per row buffer: K + 128
   int smem_bytes;              // dynamic shared memory of the launch
   int64_t chunk;               // database rows per split (multiple of BN)
   const float* ynorm;          // [>= nb rounded up to BN]
@@ -98,6 +102,19 @@ __global__ void __launch_bounds__(256)
 // ---------------------------------------------------------------------------
 // B2 + B3: the tile kernel.
 // ---------------------------------------------------------------------------
+// v[j] for a run-time j without 64 compare+select pairs: a jump table.
+#define FS_PICK_CASE(J) case J: r = v[J]; break;
+#define FS_PICK_8(B) FS_PICK_CASE(B) FS_PICK_CASE(B + 1) FS_PICK_CASE(B + 2) FS_PICK_CASE(B + 3) \
+  FS_PICK_CASE(B + 4) FS_PICK_CASE(B + 5) FS_PICK_CASE(B + 6) FS_PICK_CASE(B + 7)
+__device__ __forceinline__ uint32_t pick64(const uint32_t (&v)[64], int j) {
+  uint32_t r = 0u;
+  switch (j) {
+    FS_PICK_8(0) FS_PICK_8(8) FS_PICK_8(16) FS_PICK_8(24) FS_PICK_8(32) FS_PICK_8(40) FS_PICK_8(48) FS_PICK_8(56)
+    default: break;
+  }
+  return r;
+}
+
 struct Pipe {
   int stage;
   uint32_t phase;
@@ -159,7 +176,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
     sm100::tma_prefetch_desc(&map_b_hi);
     sm100::tma_prefetch_desc(&map_b_lo);
   }
-  if (warp == 1) sm100::tmem_alloc(tmem_slot, 512);
+  if (warp == MMA_WARP) sm100::tmem_alloc(tmem_slot, 512);
   sm100::tc_fence_before();
   __syncthreads();
   if (CLUSTER > 1) sm100::cluster_sync_all();  // peers' barriers are initialised before anything lands on them
@@ -170,7 +187,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
   const uint32_t tmem_base = *tmem_slot;
   const int64_t n_items = (int64_t)a.S * a.qgroups;
 
-  if (warp == 0) {
+  if (warp == TMA_WARP) {
     // ===== TMA producer =====
     if (lane == 0) {
       Pipe pp{0, 0u};
@@ -214,7 +231,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
         }
       }
     }
-  } else if (warp == 1) {
+  } else if (warp == MMA_WARP) {
     // ===== MMA issuer =====
     if (lane == 0) {
       constexpr uint32_t idesc = sm100::make_idesc_tf32(BM, BN);
@@ -267,10 +284,11 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
   } else {
     // ===== epilogue: B3 =====
     const int quarter = warp & 3;  // TMEM lanes 32*quarter .. +31 belong to this warp
-    const int eg = (warp - 2) >> 2;  // epilogue group: its own columns, candidate buffers and partial queues
+    const int eg = warp >> 2;  // epilogue group: its own columns, candidate buffers and partial queues
     const int K = a.K, k = a.k, cap = a.cap;
     const int SQ = a.S * EPI_GROUPS;  // partial queues per query
-    uint32_t* scratch = reinterpret_cast<uint32_t*>(scratch_all + (size_t)(warp - 2) * sel_scratch_bytes<EPI_RB>());
+    uint32_t* scratch = reinterpret_cast<uint32_t*>(scratch_all + (size_t)warp * (sel_scratch_bytes<EPI_RB>() + STAGE_KEYS * 8));
+    uint64_t* stage = reinterpret_cast<uint64_t*>(reinterpret_cast<unsigned char*>(scratch) + sel_scratch_bytes<EPI_RB>());
     uint64_t* cb_warp = a.cbuf + (((size_t)blockIdx.x * EPI_GROUPS + eg) * BM + quarter * 32) * cap;
     uint64_t* cb = cb_warp + (size_t)lane * cap;
     uint32_t tile_count = 0;
@@ -283,7 +301,9 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
       const int64_t q = q_warp + lane;
       const bool valid = q < a.nq;
       // start from the best bound other splits have published (inclusive)
-      const uint64_t thr0 = valid ? (((uint64_t)a.gbound[q] << 32) | 0xFFFFFFFFull) : 0ull;
+      uint32_t gb = valid ? a.gbound[q] : 0u;
+      if (gb > 0xFF800000u) gb = 0xFF800000u;  // no bound yet: +inf
+      const uint64_t thr0 = valid ? (((uint64_t)gb << 32) | 0xFFFFFFFFull) : 0ull;
       uint64_t thr_key = thr0;
       float thr_val = valid ? ord_f32((uint32_t)(thr0 >> 32)) : __uint_as_float(0xFF800000u);
       int cnt = 0;  // keys in this row's buffer: the winners so far, then new candidates
@@ -298,14 +318,20 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
           todo &= todo - 1u;
           const int m = __shfl_sync(kFull, cnt, r);
           if (m < k) continue;
-          uint64_t* buf = cb_warp + (size_t)r * cap;
+          uint64_t* gbuf = cb_warp + (size_t)r * cap;
           __syncwarp();
+          // small buffers are selected in shared memory (one coalesced read instead of a
+          // chain of dependent global round trips), the winners go back to the row buffer
+          const bool staged = m <= STAGE_KEYS;
+          uint64_t* buf = staged ? stage : gbuf;
           uint64_t kor = 0ull, kand = ~0ull;
           for (int i = lane; i < m; i += 32) {
-            const uint64_t key = buf[i];
+            const uint64_t key = gbuf[i];
+            if (staged) stage[i] = key;
             kor |= key;
             kand &= key;
           }
+          __syncwarp();
           const uint32_t olo = __reduce_or_sync(kFull, (uint32_t)kor), ohi = __reduce_or_sync(kFull, (uint32_t)(kor >> 32));
           const uint32_t alo = __reduce_and_sync(kFull, (uint32_t)kand), ahi = __reduce_and_sync(kFull, (uint32_t)(kand >> 32));
           const uint64_t diff = (((uint64_t)ohi << 32) | olo) & ~(((uint64_t)ahi << 32) | alo);
@@ -320,7 +346,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
               keep = key <= kth;
             }
             const unsigned b = __ballot_sync(kFull, keep);
-            if (keep) buf[w + __popc(b & ((1u << lane) - 1u))] = key;
+            if (keep) gbuf[w + __popc(b & ((1u << lane) - 1u))] = key;
             w += __popc(b);
           }
           __syncwarp();
@@ -363,30 +389,57 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
 #endif
           const uint32_t cbase = (uint32_t)col0 + (cg0 + i) * BW;
           const int climit = ncols - (cg0 + i) * BW;  // columns of this block that exist
-          // first-level filter: one FFMA and one compare per element, results in two masks
-          uint32_t mask[2] = {0u, 0u};
+          // first-level filter: d' = ||y||^2 - 2 acc, then the sign of thr - d' is
+          // shifted into a mask: FFMA + FADD + funnel shift per element (element j -> bit
+          // 31 - j, 1 = reject)
+          uint32_t rej[2] = {0u, 0u};
 #pragma unroll
           for (int j = 0; j < BW; ++j) {
             const float4 y4 = ynp[i * (BW / 4) + j / 4];
             const float y = j % 4 == 0 ? y4.x : j % 4 == 1 ? y4.y : j % 4 == 2 ? y4.z : y4.w;
             const float dp = fmaf(-2.f, __uint_as_float(v[j]), y);
             v[j] = __float_as_uint(dp);
-            mask[j >> 5] |= (!(dp > thr_val) ? 1u : 0u) << (j & 31);
+            rej[j >> 5] = __funnelshift_l(__float_as_uint(thr_val - dp), rej[j >> 5], 1);
           }
+          uint32_t mk[2];
 #pragma unroll
           for (int h = 0; h < 2; ++h) {
             const int cl = climit - 32 * h;
-            uint32_t mk = mask[h];
-            if (cl < 32) mk &= cl > 0 ? (0xFFFFFFFFu >> (32 - cl)) : 0u;
-            while (mk) {  // rare survivors: exact key test, append to the row's buffer
-              const int j = __ffs(mk) - 1;
-              mk &= mk - 1u;
-              float dp = 0.f;
+            mk[h] = __brev(~rej[h]);
+            if (cl < 32) mk[h] &= cl > 0 ? (0xFFFFFFFFu >> (32 - cl)) : 0u;
+          }
+          auto take = [&](float dp, uint32_t col) {  // exact key test, append to the row's buffer
+            const uint64_t key = make_key(dp, col);
+            if (key < thr_key) {
+              if (k == 1) {  // the queue is one register: the bound is always exact
+                thr_key = key;
+                thr_val = dp;
+                cb[0] = key;
+                cnt = 1;
+              } else {
+                cb[cnt++] = key;
+              }
+            }
+          };
+          // survivors (rare once the row has a bound): each lane walks its own mask; the
+          // register pick is a select tree, so the lanes of an iteration stay converged
 #pragma unroll
-              for (int jj = 0; jj < 32; ++jj)
-                if (jj == j) dp = __uint_as_float(v[32 * h + jj]);
-              const uint64_t key = make_key(dp, cbase + 32 * h + j);
-              if (key < thr_key) cb[cnt++] = key;
+          for (int h = 0; h < 2; ++h) {
+            uint32_t m2 = mk[h];
+            while (m2) {
+              const int j = __ffs(m2) - 1;
+              m2 &= m2 - 1u;
+              uint32_t t16[16], t8[8], t4[4], t2[2];
+#pragma unroll
+              for (int e = 0; e < 16; ++e) t16[e] = (j & 16) ? v[32 * h + 16 + e] : v[32 * h + e];
+#pragma unroll
+              for (int e = 0; e < 8; ++e) t8[e] = (j & 8) ? t16[8 + e] : t16[e];
+#pragma unroll
+              for (int e = 0; e < 4; ++e) t4[e] = (j & 4) ? t8[4 + e] : t8[e];
+#pragma unroll
+              for (int e = 0; e < 2; ++e) t2[e] = (j & 2) ? t4[2 + e] : t4[e];
+              const uint32_t pv = (j & 1) ? t2[1] : t2[0];
+              take(__uint_as_float(pv), cbase + 32 * h + j);
             }
           }
         }
@@ -398,10 +451,10 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
           sm100::mbar_arrive(yempty + ys);
         }
       }
-      flush_rows(cnt >= k);
+      flush_rows(cnt >= k);  // establishes the split's k-th distance (published below)
       __syncwarp();
-      // the row's partial queue for B4 (unordered winners, sentinel padded), and this
-      // split's k-th distance as a bound for the splits still to run
+      // the row's partial queue for B4 (unordered, sentinel padded), and this split's k-th
+      // distance (when a restore step has established it) as a bound for the splits to come
       for (int r = 0; r < 32; ++r) {
         if (q_warp + r >= a.nq) break;
         const int m = __shfl_sync(kFull, cnt, r);
@@ -417,7 +470,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
   sm100::tc_fence_before();
   __syncthreads();
   if (CLUSTER > 1) sm100::cluster_sync_all();
-  if (warp == 1) {
+  if (warp == MMA_WARP) {
     sm100::tc_fence_after();
     sm100::tmem_dealloc(tmem_base, 512);
   }
@@ -507,7 +560,7 @@ FlatTcPlan flat_tc_plan(int64_t nq, int64_t nb, int d, int k) {
   const int64_t items = (int64_t)p.S * qgroups;
   p.grid = (int)(items < ncl ? items : ncl) * CLUSTER;
   p.KB = d / BK;
-  p.cap = 2 * p.K > 256 ? 2 * p.K : 256;  // >= K + 64: a block appends at most 64 keys per row
+  p.cap = p.K + 128;  // the restore step runs when fewer than 64 more keys would fit
   // the kernel carves the ring at run time (the lo plane of the query tile is only
   // resident in 3xTF32 mode); worst case = with the lo plane
   const int fixed = 1024 /*alignment*/ + 1024 /*barriers*/ + YN_RING * BN * 4 + SCRATCH_BYTES + 2 * p.KB * A_KB_BYTES;
