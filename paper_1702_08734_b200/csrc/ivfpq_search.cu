@@ -18,6 +18,7 @@
 //                        ids are fetched for the winners only
 #include "flat.cuh"
 #include "ivfpq.cuh"
+#include "ivfpq_scan.cuh"
 #include "select.cuh"
 
 namespace fs {
@@ -26,19 +27,6 @@ namespace {
 
 constexpr int SCAN_WARPS = 8;
 constexpr int SCAN_THREADS = SCAN_WARPS * 32;
-
-struct ScanArgs {
-  const float* xq;
-  const float* coarse;
-  const float* pq;
-  const int64_t* probe_ids;  // [nq][nprobe], ascending coarse distance
-  const int64_t* offsets;    // [nlist+1]
-  const uint8_t* codes;      // [ntotal][M]
-  uint64_t* Wg;              // [nq][ngroups][K] partial queues (keys: distance, CSR position)
-  unsigned long long* scanned;
-  int32_t* out_probed;       // [nq][nprobe] or NULL
-  int d, M, dsub, nprobe, G, ngroups, k;
-};
 
 // Shared memory: r[d] | T[M][256] | per-warp batches | merge area [SCAN_WARPS][K]
 template <int NQ>
@@ -171,7 +159,7 @@ __global__ void __launch_bounds__(128)
 struct SearchPlan {
   int G, ngroups, K;
   FlatPlan coarse;
-  size_t off_cdist, off_cids, off_W, bytes;
+  size_t off_cdist, off_cids, off_W, off_work, bytes;
 };
 
 SearchPlan search_plan(const fs_ivfpq* ix, int64_t nq, int nprobe, int k) {
@@ -190,6 +178,8 @@ SearchPlan search_plan(const fs_ivfpq* ix, int64_t nq, int nprobe, int k) {
   o += align_up((size_t)nq * nprobe * sizeof(float), 256);
   p.off_cids = o;
   o += align_up((size_t)nq * nprobe * sizeof(int64_t), 256);
+  p.off_work = o;
+  o += 256;
   p.off_W = o;
   o += align_up((size_t)nq * p.ngroups * p.K * sizeof(uint64_t), 256);
   p.bytes = o;
@@ -252,6 +242,9 @@ int ivfpq_search_device(fs_ivfpq* ix, const float* xq, int64_t nq, int nprobe, i
   a.G = p.G;
   a.ngroups = p.ngroups;
   a.k = k;
+  if (scan2_supported(ix->d, ix->M, k))
+    rc = launch_scan2(a, nq, k, reinterpret_cast<unsigned int*>(w + p.off_work), s);
+  else
   switch (k_class(k)) {
     case 0: rc = launch_scan<1>(a, nq, s); break;
     case 1: rc = launch_scan<2>(a, nq, s); break;
