@@ -210,16 +210,30 @@ def timed(fn, reps, warm=1):
 def also_flat(fs, gt, pk):
     import torch
     nb, nq, d = 1_000_000, 10_000, 128
-    xb = gt.sift_like(0, nb)
-    xq = gt.sift_like(nb, nq)
+    tf32_peak = pk["bf16"] / 2.0  # dense TF32 = half the measured BF16 rate (B200_PROFILING.md nominal ratio)
     out = {"workload": "cfg3: nb=1e6, nq=1e4, d=128 SIFT-like integer fp32", "engine": fs.flat_engine(),
-           "flop_per_call": 2.0 * nb * nq * d}
-    for k in (1, 10, 100):
+           "flop_per_call": 2.0 * nb * nq * d, "tf32_peak_tflops": tf32_peak,
+           "note": "integer data: the lo planes are zero, the checked dispatch issues 1 TF32 product per MAC (exact); "
+                   "real-valued data issue 3 (3xTF32): see real_valued"}
+
+    def run(xq, xb, k, passes):
         ws = torch.empty(fs.flat_l2_knn_ws_bytes(nq, nb, d, k), dtype=torch.uint8, device="cuda")
         od = torch.empty((nq, k), dtype=torch.float32, device="cuda")
         oi = torch.empty((nq, k), dtype=torch.int64, device="cuda")
         best, med = timed(lambda: fs.flat_l2_knn(xq, xb, k, out_dist=od, out_ids=oi, ws=ws), 3)
-        out["k%d" % k] = {"ms": med, "queries_per_s": nq / med * 1e3, "tflops": 2.0 * nb * nq * d / med / 1e9}
+        tf = 2.0 * nb * nq * d / med / 1e9
+        return {"ms": med, "queries_per_s": nq / med * 1e3, "tflops": tf, "issued_tflops": passes * tf,
+                "tensor_frac": passes * tf / tf32_peak}
+
+    xb = gt.sift_like(0, nb)
+    xq = gt.sift_like(nb, nq)
+    for k in (1, 10, 100):
+        out["k%d" % k] = run(xq, xb, k, 1)
+    del xb, xq
+    torch.cuda.empty_cache()
+    xb = gt.gaussian_vectors(0, nb, d)
+    xq = gt.gaussian_vectors(nb, nq, d)
+    out["real_valued"] = {"workload": "same shape, i.i.d. ~N(0,1) fp32 (3xTF32 path)", "k10": run(xq, xb, 10, 3)}
     del xb, xq
     return out
 
@@ -265,6 +279,7 @@ def run_ours(args):
     import torch.distributed as dist
 
     import paper_1702_08734_b200 as fs
+    from paper_1702_08734_b200 import multirank as mr
     from datagen import gen_torch as gt
 
     rank = int(os.environ.get("RANK", "0"))
@@ -284,7 +299,7 @@ def run_ours(args):
         return
 
     # this rank's rows: distinct rows per rank (weak scaling)
-    rows = gt.kselect_rows(rank * N_ROWS, N_ROWS, N_COLS)
+    rows = gt.kselect_rows(mr.rank_rows(rank, N_ROWS)[0], N_ROWS, N_COLS)
     big = gt.kselect_rows(10**6 + rank, 1, BIG_N, duplicates=False)
     outs = {k: (torch.empty((N_ROWS, k), dtype=torch.float32, device="cuda"),
                 torch.empty((N_ROWS, k), dtype=torch.int32, device="cuda")) for k in KS}
@@ -338,20 +353,16 @@ def run_ours(args):
     barrier()
     sampler.stop()
     launches = fs.launch_count()
-    ms = t0.elapsed_time(t1)
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = mr.max_over_ranks(t0.elapsed_time(t1), "cuda")
     ms_per_step = ms / args.steps
-    value = world * step_bytes() / (ms_per_step * 1e-3) / 1e9
+    value = mr.job_throughput(step_bytes(), ms_per_step, world) / 1e9
 
     # per-call device time (launch + its pass-2 launches), dominant call -> roofline
     call_ms = {n: float(np.mean([a.elapsed_time(b) for a, b in ev])) for n, ev in per_call.items()}
     call_bytes = {n: b for n, _, b in calls}
     dom = max(call_ms, key=call_ms.get)
     ach = call_bytes[dom] / call_ms[dom] / 1e6
-    roofline = {"bound": "hbm", "kernel": "kselect_warp_kernel (%s call)" % dom, "achieved": ach,
+    roofline = {"bound": "hbm", "kernel": "kselect_stream_kernel (%s call)" % dom, "achieved": ach,
                 "peak": pk["hbm"], "unit": "GB/s", "frac": ach / pk["hbm"], "traffic": None,
                 "peak_source": pk["source"] + ", burst copy figure",
                 "per_call": {n: {"ms": call_ms[n], "GBps": call_bytes[n] / call_ms[n] / 1e6,
@@ -390,10 +401,7 @@ def run_ours(args):
         e2e_step()
     barrier()
     e2e_s = (time.perf_counter() - w0) / e2e_steps
-    if world > 1:
-        t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = mr.max_over_ranks(e2e_s, "cuda")
     h2d = len(KS) * 4 * N_ROWS * N_COLS + 4 * BIG_N
     d2h = sum(8 * N_ROWS * k for k in KS) + 8 * BIG_K
     e2e = {"value": world * step_bytes() / e2e_s / 1e9, "unit": "GB/s", "h2d_bytes_per_step": h2d,
