@@ -1,0 +1,136 @@
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times.
+
+The oracle cannot run the whole workloads in seconds, so (SURVEY 8c / the tier rules):
+  cfg2  all 10 000 x 16 384 rows go through fs_kselect exactly as in bench.py; a seeded
+        sample of rows (every duplicate-run pattern included) is compared bit for bit with
+        the oracle; the 2^27-element row is checked against the oracle applied to the
+        elements <= the k-th value (found with numpy's partition), which is the whole answer.
+  cfg3  nb = 10^6, nq = 10^4, d = 128 integer data through fs_flat_l2_knn as in bench.py; a
+        seeded sample of queries is compared bit for bit with the oracle.
+  cfg4  the 10^8-vector index does not fit a test run; a cfg4-shaped index of 2 * 10^6
+        vectors (same generator, same d / M / k / nprobe, nlist scaled) is built and searched
+        with nq = 2 000; a seeded query subset is checked by the oracle over the GPU-built
+        lists and a seeded sample of the add path is re-encoded by the oracle.
+Inputs come from datagen's torch twin on the device (bit-identical to the numpy generator,
+tests/test_datagen.py).
+"""
+import numpy as np
+import pytest
+import torch
+
+import datagen
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+
+def fsmod():
+    import paper_1702_08734_b200 as fs
+    return fs
+
+
+@pytest.mark.parametrize("k", [1, 32, 128, 1024])
+def test_cfg2_full_batch_sampled_rows(k):
+    from datagen import gen_torch as gt
+    fs = fsmod()
+    n_rows, n = 10_000, 16_384
+    rows = gt.kselect_rows(0, n_rows, n)
+    val, idx = fs.kselect(rows, k)
+    torch.cuda.synchronize()
+    dup, _ = datagen.kselect_dup_rows(0, n_rows)
+    rng = np.random.default_rng(k)
+    sample = np.unique(np.concatenate([np.nonzero(dup)[0][:24], rng.integers(0, n_rows, 72), [0, n_rows - 1]]))
+    host = rows[torch.from_numpy(sample).cuda()].cpu().numpy()
+    for j in range(3):  # device generator == numpy generator
+        assert np.array_equal(host[j], datagen.kselect_rows(int(sample[j]), 1, n)[0])
+    ev, ei = oracle.kselect(host, k)
+    gv, gi = val[torch.from_numpy(sample).cuda()].cpu().numpy(), idx[torch.from_numpy(sample).cuda()].cpu().numpy()
+    assert np.array_equal(gi, ei)
+    assert np.array_equal(gv.view(np.uint32), ev.view(np.uint32))
+    # properties on every row: ascending, values are the row's values at the indices
+    v, i = val.cpu().numpy(), idx.cpu().numpy()
+    assert np.all(np.diff(v, axis=1) >= 0)
+    got = torch.gather(rows, 1, idx.long()).cpu().numpy()
+    assert np.array_equal(got.view(np.uint32), v.view(np.uint32))
+    eq = np.diff(v, axis=1) == 0
+    assert np.all(np.diff(i, axis=1)[eq] > 0), "ties not by ascending index"
+
+
+def test_cfg2_long_row():
+    from datagen import gen_torch as gt
+    fs = fsmod()
+    n, k = 1 << 27, 1024
+    row = gt.kselect_rows(10**6, 1, n, duplicates=False)
+    val, idx = fs.kselect(row, k)
+    torch.cuda.synchronize()
+    host = row[0].cpu().numpy()
+    kth = np.partition(host, k - 1)[k - 1]            # independent library routine
+    cand = np.nonzero(host <= kth)[0]                 # every element that can be in the answer
+    assert k <= cand.size < 4 * k
+    ev, ei = oracle.kselect(host[cand][None, :], k)   # the oracle on the candidates = the answer
+    assert np.array_equal(idx[0].cpu().numpy(), cand[ei[0]].astype(np.int32))
+    assert np.array_equal(val[0].cpu().numpy().view(np.uint32), ev[0].view(np.uint32))
+
+
+@pytest.mark.parametrize("k", [1, 10, 100])
+def test_cfg3_full_sampled_queries(k):
+    from datagen import gen_torch as gt
+    fs = fsmod()
+    nb, nq = 1_000_000, 10_000
+    xb = gt.sift_like(0, nb)
+    xq = gt.sift_like(nb, nq)
+    gd, gi = fs.flat_l2_knn(xq, xb, k)
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(100 + k)
+    sample = np.unique(np.concatenate([rng.integers(0, nq, 14), [0, nq - 1]]))
+    xb_h = xb.cpu().numpy()
+    assert np.array_equal(xb_h[:64], datagen.sift_like(0, 64))
+    od, oi = oracle.flat_l2_knn(xq[torch.from_numpy(sample).cuda()].cpu().numpy(), xb_h, k)
+    s = torch.from_numpy(sample).cuda()
+    assert np.array_equal(gi[s].cpu().numpy(), oi)                       # integer data: exact
+    assert np.array_equal(gd[s].cpu().numpy().view(np.uint32), od.view(np.uint32))
+    d_all, i_all = gd.cpu().numpy(), gi.cpu().numpy()
+    assert np.all(np.diff(d_all, axis=1) >= 0) and i_all.min() >= 0 and i_all.max() < nb
+
+
+def test_cfg4_shaped_index():
+    from datagen import gen_torch as gt
+    from test_gpu_ivfpq import check_search
+    fs = fsmod()
+    d, M, nb, nlist, nq, k = 96, 16, 2_000_000, 2048, 2000, 100
+    ix = fs.IvfPq(d, nlist, M)
+    ix.train(gt.deep_like(0, 64 * nlist), niter=6, seed=0)
+    chunk = 1 << 19
+    for b in range(0, nb, chunk):
+        ix.add(gt.deep_like(b, min(chunk, nb - b)))
+    assert ix.ntotal == nb
+    coarse, pq = (t.cpu().numpy() for t in ix.get_quantizers())
+    offs, codes, lids = (t.cpu().numpy() for t in ix.export())
+    # structure: every id exactly once, lists in append (= ascending id) order
+    assert offs[0] == 0 and offs[-1] == nb and np.all(np.diff(offs) >= 0)
+    assert np.array_equal(np.sort(lids), np.arange(nb))
+    inner = np.ones(nb, bool)
+    inner[offs[1:-1][offs[1:-1] < nb]] = False
+    assert np.all(np.diff(lids)[inner[1:]] > 0)
+    # sampled add path: the oracle re-encodes seeded ids from regenerated vectors
+    rng = np.random.default_rng(7)
+    sid = np.unique(rng.integers(0, nb, 3000))
+    ys = np.concatenate([datagen.deep_like(int(i), 1) for i in sid[:400]])
+    sid = sid[:400]
+    olist, ocodes, cm, km = oracle.ivfpq_encode(coarse, pq, ys, margins=True)
+    pos = np.empty(nb, np.int64)
+    pos[lids] = np.arange(nb)
+    glist = np.searchsorted(offs, pos[sid], side="right") - 1
+    assert not ((glist != olist) & (cm >= 1e-5)).any()
+    same = glist == olist
+    assert not ((codes[pos[sid]] != ocodes) & (km >= 1e-5) & same[:, None]).any()
+    # search: whole batch as bench.py runs it, oracle on a seeded subset over the GPU-built lists
+    xq = gt.deep_like(10**8, nq)
+    for nprobe in (16, 64):
+        gd, gi = ix.search(xq, nprobe, k)
+        torch.cuda.synchronize()
+        sub = np.unique(rng.integers(0, nq, 24))
+        xs = xq[torch.from_numpy(sub).cuda()].cpu().numpy()
+        sd, si, _ = check_search(ix, coarse, pq, offs, codes, lids, xs, nprobe, k)
+        assert np.array_equal(si, gi[torch.from_numpy(sub).cuda()].cpu().numpy())  # batch == subset run
+    ix.close()
