@@ -167,7 +167,7 @@ def cpu_baseline():
     """The oracle as it stands on the host cores, bounded sample of the headline workload."""
     import datagen
     import oracle
-    n_rows, big_slice = 2000, 1 << 23
+    n_rows, big_slice = 10_000, 1 << 26
     rows = datagen.kselect_rows(0, n_rows, N_COLS)
     big = datagen.kselect_rows(10**6, 1, big_slice, duplicates=False)
     oracle.kselect(rows[:8], 32)  # load the library
@@ -180,7 +180,7 @@ def cpu_baseline():
     return {"value": b / dt / 1e9, "unit": "GB/s", "cores": oracle.num_threads(), "kind": "oracle",
             "seconds": dt,
             "sample": "oracle.kselect (full sort per row, OpenMP over rows) on the first %d of %d rows "
-                      "at k in {1,32,128,1024} + the first 2^23 of the 2^27-value row at k=1024"
+                      "at k in {1,32,128,1024} + the first 2^26 of the 2^27-value row at k=1024"
                       % (n_rows, N_ROWS)}
 
 

@@ -529,6 +529,18 @@ bool flat_tc_supported(int d) {
   return !forced_off && d % BK == 0 && d >= BK && d <= 128;
 }
 
+// Every extra split is one more partial queue per query (more survivors in the epilogue,
+// more keys in B4): weigh it against the wave quantisation of the MMA work.
+static double split_penalty(int kclass) {
+  static double forced = -1.0;
+  if (forced < 0.0) {
+    const char* e = getenv("FS_FLAT_SPLIT_PENALTY");  // tuning knob (A/B runs)
+    forced = e ? atof(e) : 0.0;
+  }
+  if (forced > 0.0) return forced;
+  return kclass == 0 ? 0.002 : 0.004;
+}
+
 FlatTcPlan flat_tc_plan(int64_t nq, int64_t nb, int d, int k) {
   FlatTcPlan p;
   p.kclass = k_class(k);
@@ -548,7 +560,7 @@ FlatTcPlan flat_tc_plan(int64_t nq, int64_t nb, int d, int k) {
     const int64_t items = realS * qgroups;
     const int64_t g = items < ncl ? items : ncl;
     const double eff = (double)items / (double)(ceil_div(items, g) * g) * ((double)g / (double)ncl);
-    const double score = eff - 0.002 * (double)realS;
+    const double score = eff - split_penalty(p.kclass) * (double)realS;
     if (score > best) {
       best = score;
       best_S = realS;

@@ -1,8 +1,7 @@
 // ivfpq_scan.cu -- the IVFPQ list scan, persistent form.
 //
-//   C2 lookup tables   per (query, probed list): r = x - c_L,
-//                      T_m[c] = ||r^m - B[m][c]||^2 = ||r^m||^2 - 2 <r^m, B[m][c]> + ||B[m][c]||^2
-//                      (Eq. 10), built in shared memory by the CTA that scans
+//   C2 lookup tables   per (query, probed list): r = x - c_L, T_m[c] = ||r^m - B[m][c]||^2
+//                      (Eq. 10; direct form), built in shared memory by the CTA that scans
 //                      the list from a codebook that is RESIDENT in shared memory
 //   C3 list scan       dist = sum_m T_m[code_m] (Alg. 4); one thread per
 //                      vector, one 8/16/32-byte load of its code
@@ -71,8 +70,7 @@ __device__ __forceinline__ void load_code(const uint8_t* p, uint32_t (&w)[MW]) {
   }
 }
 
-// Shared memory: cb [256][d+1] | bnorm [M][256] | lut [256][32] | r [d] + rn [M] |
-//                per-warp select batches | merge area [SW][K]
+// Shared memory: cb [256][d+1] | lut [2][256][32] | per-warp select batches | merge area [SW][K]
 template <int NQ, int M>
 __global__ void __launch_bounds__(ST, 1) ivfpq_scan2_kernel(const ScanArgs a, unsigned int* __restrict__ work,
                                                             int64_t n_items) {
@@ -81,36 +79,28 @@ __global__ void __launch_bounds__(ST, 1) ivfpq_scan2_kernel(const ScanArgs a, un
   constexpr int NB = 2;
   constexpr int MW = M / 4;
   constexpr int REP = 32 / M;
+  constexpr int DSUB_MAX = 16;
   const int d = a.d, dsub = a.dsub, dp = d + 1;
   float* cb = reinterpret_cast<float*>(smem_raw);  // codeword c of all sub-quantizers: cb[c * dp + m * dsub + j]
-  float* bnorm = cb + 256 * dp;                    // ||B[m][c]||^2 at bnorm[m * 256 + c]
-  float* lut = bnorm + M * 256;
-  float* r = lut + 256 * 32;
-  float* rn = r + ((d + 3) & ~3);
-  uint64_t* bufs = reinterpret_cast<uint64_t*>(rn + ((M + 3) & ~3));
+  float* lut0 = cb + 256 * dp;                     // two tables: the next one is built while slow warps still scan
+  uint64_t* bufs = reinterpret_cast<uint64_t*>(lut0 + 2 * 256 * 32);
   uint64_t* merge = bufs + SW * warp_select_smem_keys<NB>();
   __shared__ int s_item;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
-  // the codebook becomes resident: pq [M][256][dsub] -> cb, and its squared norms
+  // the codebook becomes resident: pq [M][256][dsub] -> cb
   for (int e = tid; e < M * 256; e += ST) {
     const int m = e >> 8, c = e & 255;
-    float s = 0.f;
-    for (int j = 0; j < dsub; ++j) {
-      const float v = a.pq[(int64_t)e * dsub + j];
-      cb[c * dp + m * dsub + j] = v;
-      s = fmaf(v, v, s);
-    }
-    bnorm[e] = s;
+    for (int j = 0; j < dsub; ++j) cb[c * dp + m * dsub + j] = a.pq[(int64_t)e * dsub + j];
   }
   __syncthreads();
 
   WarpSelect<NQ, NB> sel;
   sel.init(bufs + warp * warp_select_smem_keys<NB>(), lane);
   const int rot = lane % M;
-  // byte offset of this lane's bank at step s is ((s + lane) & 31) * 4
-  const int mylane = lane;
+  const int my_m = lane % M, my_cofs = lane / M;
   unsigned long long bytes = 0;
+  int which = 0;
 
   while (true) {
     __syncthreads();
@@ -131,30 +121,28 @@ __global__ void __launch_bounds__(ST, 1) ivfpq_scan2_kernel(const ScanArgs a, un
       const int64_t lb = a.offsets[L], le = a.offsets[L + 1];
       const int64_t len = le - lb;
       if (len == 0) continue;  // empty lists are probed and contribute nothing
-      __syncthreads();         // the previous list's table is no longer read
-      // C2: residual, its sub-vector norms, table
-      for (int j = tid; j < d; j += ST) r[j] = a.xq[q * d + j] - a.coarse[L * d + j];
-      __syncthreads();
-      if (tid < M) {
-        float s = 0.f;
-        for (int j = 0; j < dsub; ++j) s = fmaf(r[tid * dsub + j], r[tid * dsub + j], s);
-        rn[tid] = s;
-      }
-      __syncthreads();
-      // lane -> (sub-quantizer m = lane % M, codeword c0 + lane / M); the entry goes to the
-      // REP banks that hold table m
-      for (int c0 = warp * REP; c0 < 256; c0 += SW * REP) {
-        const int m = lane % M, c = c0 + lane / M;
-        const float* b = cb + c * dp + m * dsub;
-        const float* rm = r + m * dsub;
-        float dot = 0.f;
-        for (int j = 0; j < dsub; ++j) dot = fmaf(rm[j], b[j], dot);
-        float t = fmaf(-2.f, dot, rn[m] + bnorm[m * 256 + c]);
-        t = t > 0.f ? t : 0.f;  // the expanded form can round below zero
+      // C2: this lane's residual sub-vector r^m = (x - c_L)^m in registers, then its share of
+      // the table: entry (m = lane % M, c = c0 + lane / M) goes to the REP banks of table m
+      float* lut = lut0 + which * (256 * 32);
+      float rm[DSUB_MAX];
 #pragma unroll
-        for (int rep = 0; rep < REP; ++rep) lut[c * 32 + m + rep * M] = t;
+      for (int j = 0; j < DSUB_MAX; ++j)
+        rm[j] = j < dsub ? __ldg(a.xq + q * d + my_m * dsub + j) - __ldg(a.coarse + L * d + my_m * dsub + j) : 0.f;
+      for (int c0 = warp * REP; c0 < 256; c0 += SW * REP) {
+        const int c = c0 + my_cofs;
+        const float* b = cb + c * dp + my_m * dsub;
+        float t = 0.f;
+#pragma unroll
+        for (int j = 0; j < DSUB_MAX; ++j) {
+          if (j < dsub) {
+            const float df = rm[j] - b[j];
+            t = fmaf(df, df, t);
+          }
+        }
+#pragma unroll
+        for (int rep = 0; rep < REP; ++rep) lut[c * 32 + my_m + rep * M] = t;
       }
-      __syncthreads();
+      __syncthreads();  // table complete (and every warp is past the scan that used the other one)
       // C3 + C4: scan and select
       bytes += (unsigned long long)len * M;
       const uint8_t* cl = a.codes + lb * M;
@@ -170,7 +158,7 @@ __global__ void __launch_bounds__(ST, 1) ivfpq_scan2_kernel(const ScanArgs a, un
 #pragma unroll
           for (int s = 0; s < M; ++s) {
             const uint32_t c = (w[s >> 2] >> (8 * (s & 3))) & 255u;
-            dist += *reinterpret_cast<const float*>(lutb + c * 128 + (((s + mylane) & 31) << 2));
+            dist += *reinterpret_cast<const float*>(lutb + c * 128 + (((s + lane) & 31) << 2));
           }
         }
         const bool cand = ok && sel.maybe(dist);
@@ -179,6 +167,7 @@ __global__ void __launch_bounds__(ST, 1) ivfpq_scan2_kernel(const ScanArgs a, un
           sel.push(cand && sel.wants(key), key);
         }
       }
+      which ^= 1;
     }
     sel.finish();
 
@@ -205,7 +194,7 @@ __global__ void __launch_bounds__(ST, 1) ivfpq_scan2_kernel(const ScanArgs a, un
 template <int NQ, int M>
 size_t scan2_smem(int d) {
   constexpr int K = 32 * NQ;
-  return (size_t)(256 * (d + 1) + M * 256 + 256 * 32 + ((d + 3) & ~3) + ((M + 3) & ~3)) * sizeof(float) +
+  return (size_t)(256 * (d + 1) + 2 * 256 * 32) * sizeof(float) +
          (size_t)(SW * warp_select_smem_keys<2>() + SW * K) * sizeof(uint64_t);
 }
 
@@ -252,9 +241,10 @@ bool scan2_supported(int d, int M, int k) {
   if (!(M == 8 || M == 16 || M == 32)) return false;
   const int kc = k_class(k);
   if (kc > 3) return false;  // the merge area of larger queues does not fit beside the codebook
-  const size_t smem = (size_t)(256 * (d + 1) + M * 256 + 256 * 32 + d + M + 8) * sizeof(float) +
+  if (d / M > 16) return false;
+  const size_t smem = (size_t)(256 * (d + 1) + 2 * 256 * 32) * sizeof(float) +
                       (size_t)(SW * warp_select_smem_keys<2>() + SW * (32 << kc)) * sizeof(uint64_t);
-  return smem <= 200 * 1024;
+  return smem <= 224 * 1024;
 }
 
 int launch_scan2(const ScanArgs& a, int64_t nq, int k, unsigned int* work, cudaStream_t s) {
