@@ -256,7 +256,8 @@ def also_ivfpq(fs, gt, pk, nb):
     ix.search(xq[:8], 1, 1)  # finalise the lists
     torch.cuda.synchronize()
     t_add = time.perf_counter() - t0
-    out = {"workload": "cfg4-shaped, REDUCED: nb=%d deep-like d=96, nlist=%d, M=16, nq=1e4, k=100" % (nb, nlist),
+    out = {"workload": "cfg4%s: nb=%d deep-like d=96, nlist=%d, M=16, nq=1e4, k=100"
+                       % ("" if nb >= 100_000_000 else "-shaped, REDUCED", nb, nlist),
            "train_s": t_train, "add_s": t_add, "add_vectors_per_s": nb / t_add}
     od = torch.empty((nq, k), dtype=torch.float32, device="cuda")
     oi = torch.empty((nq, k), dtype=torch.int64, device="cuda")
