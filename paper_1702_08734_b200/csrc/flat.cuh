@@ -31,7 +31,7 @@ struct FlatTcPlan {
   int kclass, K, S, qtiles, qgroups, grid, KB, nstage, cap;
   int64_t chunk;
   size_t smem;
-  size_t off_ynorm, off_xnorm, off_flag, off_gbound, off_W, off_cbuf, off_qhi, off_qlo, off_bhi, off_blo, bytes;
+  size_t off_ynorm, off_xnorm, off_flag, off_gbound, off_hbound, off_hclaim, off_W, off_cbuf, off_qhi, off_qlo, off_bhi, off_blo, bytes;
 };
 bool flat_tc_supported(int d);  // d % 32 == 0, 32 <= d <= 128, not disabled by FS_FLAT_ENGINE=ffma
 FlatTcPlan flat_tc_plan(int64_t nq, int64_t nb, int d, int k);

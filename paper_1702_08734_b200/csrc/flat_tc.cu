@@ -55,6 +55,8 @@ constexpr int TMA_WARP = EPI_GROUPS * 4, MMA_WARP = EPI_GROUPS * 4 + 1;
 constexpr int EPI_RB = 4;                     // radix digit width of the epilogue selection (1 KB of counters per warp)
 constexpr int STAGE_KEYS = 256;               // row buffers up to this size are selected in shared memory
 constexpr int SCRATCH_BYTES = EPI_GROUPS * 4 * ((1 << EPI_RB) * 64 + STAGE_KEYS * 8);  // 8 warps x (1 KB + 2 KB)
+constexpr int HB_LEVELS = 3;                  // hierarchical bound: levels 1..3 (2, 4, 8 queues)
+constexpr int HB_SLOTS = 2 + 4 + 8;
 constexpr int SMEM_LIMIT = 227 * 1024;
 
 struct TcArgs {
@@ -68,6 +70,9 @@ struct TcArgs {
   const float* ynorm;          // [>= nb rounded up to BN]
   uint64_t* Wg;                // [nq][S * EPI_GROUPS][K]
   unsigned int* gbound;        // [nq] order image of the best known k-th distance
+  unsigned int* hbound;        // [nq][HB_SLOTS] level l (1..HB_LEVELS) holds the ceil(k / 2^l)-th smallest
+                               // distances of 2^l different finished partial queues (+inf image: empty)
+  unsigned int* hclaim;        // [nq][HB_LEVELS] slots handed out per level
   uint64_t* cbuf;              // [gridDim.x][EPI_GROUPS][BM][cap]: winners so far, then new candidates
   const unsigned int* lo_flag; // != 0: lo planes are not all zero (3xTF32)
 };
@@ -102,19 +107,6 @@ __global__ void __launch_bounds__(256)
 // ---------------------------------------------------------------------------
 // B2 + B3: the tile kernel.
 // ---------------------------------------------------------------------------
-// v[j] for a run-time j without 64 compare+select pairs: a jump table.
-#define FS_PICK_CASE(J) case J: r = v[J]; break;
-#define FS_PICK_8(B) FS_PICK_CASE(B) FS_PICK_CASE(B + 1) FS_PICK_CASE(B + 2) FS_PICK_CASE(B + 3) \
-  FS_PICK_CASE(B + 4) FS_PICK_CASE(B + 5) FS_PICK_CASE(B + 6) FS_PICK_CASE(B + 7)
-__device__ __forceinline__ uint32_t pick64(const uint32_t (&v)[64], int j) {
-  uint32_t r = 0u;
-  switch (j) {
-    FS_PICK_8(0) FS_PICK_8(8) FS_PICK_8(16) FS_PICK_8(24) FS_PICK_8(32) FS_PICK_8(40) FS_PICK_8(48) FS_PICK_8(56)
-    default: break;
-  }
-  return r;
-}
-
 struct Pipe {
   int stage;
   uint32_t phase;
@@ -302,6 +294,20 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
       const bool valid = q < a.nq;
       // start from the best bound other splits have published (inclusive)
       uint32_t gb = valid ? a.gbound[q] : 0u;
+      if (valid && k >= 8) {
+        // 2^l disjoint partial queues whose ceil(k / 2^l)-th smallest distances are all <= m hold
+        // >= k elements <= m together: m bounds the query's k-th distance (tighter than any
+        // single queue's own k-th once several splits have finished)
+        const unsigned int* hb = a.hbound + q * HB_SLOTS;
+        int o = 0;
+#pragma unroll
+        for (int l = 1; l <= HB_LEVELS; ++l) {
+          unsigned int mx = 0u;
+          for (int t = 0; t < (1 << l); ++t) mx = max(mx, hb[o + t]);
+          gb = min(gb, mx);
+          o += 1 << l;
+        }
+      }
       if (gb > 0xFF800000u) gb = 0xFF800000u;  // no bound yet: +inf
       const uint64_t thr0 = valid ? (((uint64_t)gb << 32) | 0xFFFFFFFFull) : 0ull;
       uint64_t thr_key = thr0;
@@ -311,7 +317,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
 
       // Restore step for the rows that ask for it: the whole warp selects the k
       // smallest of the row's buffer by radix counting (tselect.cuh), in place.
-      auto flush_rows = [&](bool need) {
+      auto flush_rows = [&](bool need, bool final) {
         unsigned todo = __ballot_sync(kFull, need);
         while (todo) {
           const int r = __ffs(todo) - 1;
@@ -336,6 +342,21 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
           const uint32_t alo = __reduce_and_sync(kFull, (uint32_t)kand), ahi = __reduce_and_sync(kFull, (uint32_t)(kand >> 32));
           const uint64_t diff = (((uint64_t)ohi << 32) | olo) & ~(((uint64_t)ahi << 32) | alo);
           const uint64_t kth = radix_select_kth<EPI_RB>(buf, m, k, diff, scratch);
+          if (final && staged && k >= 8) {
+            // publish this queue's ceil(k / 2^l)-th smallest distances (first come, first served)
+            int o = 0;
+#pragma unroll 1
+            for (int l = 1; l <= HB_LEVELS; ++l) {
+              const int rank = (k + (1 << l) - 1) >> l;
+              const uint64_t kv = radix_select_kth<EPI_RB>(buf, m, rank, diff, scratch);
+              if (lane == 0) {
+                const unsigned int slot = atomicAdd(a.hclaim + (q_warp + r) * HB_LEVELS + (l - 1), 1u);
+                if (slot < (1u << l)) a.hbound[(q_warp + r) * HB_SLOTS + o + slot] = (unsigned int)(kv >> 32);
+              }
+              o += 1 << l;
+            }
+            __syncwarp();
+          }
           int w = 0;
           for (int i0 = 0; i0 < m; i0 += 32) {  // keep the keys <= kth: exactly k (keys are distinct)
             const int i = i0 + lane;
@@ -377,7 +398,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
         const float4* ynp = reinterpret_cast<const float4*>(s_yn + ys * BN + cg0 * BW);
 #pragma unroll 1
         for (int i = 0; i < NBLK; ++i) {
-          flush_rows(cnt > cap - BW);
+          flush_rows(cnt > cap - BW, false);
 #if FS_TC_EXP == 2
           continue;
 #endif
@@ -451,7 +472,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
           sm100::mbar_arrive(yempty + ys);
         }
       }
-      flush_rows(cnt >= k);  // establishes the split's k-th distance (published below)
+      flush_rows(cnt >= k, true);  // establishes the split's k-th distance (published below)
       __syncwarp();
       // the row's partial queue for B4 (unordered, sentinel padded), and this split's k-th
       // distance (when a restore step has established it) as a bound for the splits to come
@@ -589,6 +610,8 @@ FlatTcPlan flat_tc_plan(int64_t nq, int64_t nb, int d, int k) {
   p.off_xnorm = take((size_t)(nq + 1) * sizeof(float));
   p.off_flag = take(256);
   p.off_gbound = take((size_t)(nq + 1) * sizeof(unsigned int));
+  p.off_hbound = take((size_t)(nq + 1) * HB_SLOTS * sizeof(unsigned int));
+  p.off_hclaim = take((size_t)(nq + 1) * HB_LEVELS * sizeof(unsigned int));
   p.off_W = take((size_t)nq * p.S * EPI_GROUPS * p.K * sizeof(uint64_t));
   p.off_cbuf = take((size_t)sms * EPI_GROUPS * BM * p.cap * sizeof(uint64_t));
   p.off_qhi = take((size_t)nq * d * sizeof(float));
@@ -613,7 +636,9 @@ int flat_knn_tc_device(const float* xq, int64_t nq, const float* xb, int64_t nb,
   float* bhi = reinterpret_cast<float*>(w + p.off_bhi);
   float* blo = reinterpret_cast<float*>(w + p.off_blo);
   FS_CUDA(cudaMemsetAsync(flag, 0, 256, s));
-  FS_CUDA(cudaMemsetAsync(gbound, 0xFF, (size_t)nq * sizeof(unsigned int), s));  // +inf image and above: no bound
+  // +inf image and above: no bound (gbound and hbound are adjacent); no slot handed out yet
+  FS_CUDA(cudaMemsetAsync(gbound, 0xFF, p.off_hclaim - p.off_gbound, s));
+  FS_CUDA(cudaMemsetAsync(w + p.off_hclaim, 0, (size_t)(nq + 1) * HB_LEVELS * sizeof(unsigned int), s));
   split_norm_kernel<<<(unsigned)ceil_div(nb, 8), 256, 0, s>>>(xb, nb, d, bhi, blo, ynorm, flag);
   FS_LAUNCHED();
   split_norm_kernel<<<(unsigned)ceil_div(nq, 8), 256, 0, s>>>(xq, nq, d, qhi, qlo, xnorm, flag);
@@ -642,6 +667,8 @@ int flat_knn_tc_device(const float* xq, int64_t nq, const float* xb, int64_t nb,
   a.ynorm = ynorm;
   a.Wg = reinterpret_cast<uint64_t*>(w + p.off_W);
   a.gbound = gbound;
+  a.hbound = reinterpret_cast<unsigned int*>(w + p.off_hbound);
+  a.hclaim = reinterpret_cast<unsigned int*>(w + p.off_hclaim);
   a.cbuf = reinterpret_cast<uint64_t*>(w + p.off_cbuf);
   a.lo_flag = flag;
   static size_t attr_smem = 0;
