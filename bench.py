@@ -238,11 +238,12 @@ def also_flat(fs, gt, pk):
     return out
 
 
-def also_ivfpq(fs, gt, pk, nb):
+def also_ivfpq(fs, gt, pk, nb, cfg5=False):
     import torch
-    d, M, nq, k = 96, 16, 10_000, 100
-    nlist = max(64, min(65_536, int(2 ** round(__import__("math").log2(max(nb // 1526, 64))))))
-    ntrain = min(nb, max(256, min(1_000_000, 16 * nlist)))
+    d, M, nq, k = 96, (8 if cfg5 else 16), 10_000, 100
+    per_list = 3815 if cfg5 else 1526
+    nlist = max(64, min(262_144 if cfg5 else 65_536, int(2 ** round(__import__("math").log2(max(nb // per_list, 64))))))
+    ntrain = min(nb, max(256, min(4_194_304 if cfg5 else 1_000_000, 16 * nlist)))
     t0 = time.perf_counter()
     ix = fs.IvfPq(d, nlist, M)
     ix.train(gt.deep_like(0, ntrain), niter=10, seed=0)
@@ -256,18 +257,20 @@ def also_ivfpq(fs, gt, pk, nb):
     ix.search(xq[:8], 1, 1)  # finalise the lists
     torch.cuda.synchronize()
     t_add = time.perf_counter() - t0
-    out = {"workload": "cfg4%s: nb=%d deep-like d=96, nlist=%d, M=16, nq=1e4, k=100"
-                       % ("" if nb >= 100_000_000 else "-shaped, REDUCED", nb, nlist),
+    out = {"workload": "cfg%d%s: nb=%d deep-like d=96, nlist=%d, M=%d, nq=1e4"
+                       % (5 if cfg5 else 4, "" if nb >= (10**9 if cfg5 else 10**8) else "-shaped, REDUCED", nb, nlist, M),
            "train_s": t_train, "add_s": t_add, "add_vectors_per_s": nb / t_add}
     od = torch.empty((nq, k), dtype=torch.float32, device="cuda")
     oi = torch.empty((nq, k), dtype=torch.int64, device="cuda")
-    for nprobe in (16, 64, 256):
+    for nprobe, k in (((32, 1), (32, 100), (128, 1), (128, 100)) if cfg5 else ((16, 100), (64, 100), (256, 100))):
         if nprobe > nlist:
             continue
         ws = torch.empty(ix.search_ws_bytes(nq, nprobe, k), dtype=torch.uint8, device="cuda")
+        od = torch.empty((nq, k), dtype=torch.float32, device="cuda")
+        oi = torch.empty((nq, k), dtype=torch.int64, device="cuda")
         best, med = timed(lambda: ix.search(xq, nprobe, k, out_dist=od, out_ids=oi, ws=ws), 3)
         codes = ix.last_scanned_codes
-        out["nprobe%d" % nprobe] = {"ms": med, "queries_per_s": nq / med * 1e3, "code_bytes": codes,
+        out[("nprobe%d_k%d" % (nprobe, k)) if cfg5 else ("nprobe%d" % nprobe)] = {"ms": med, "queries_per_s": nq / med * 1e3, "code_bytes": codes,
                                     "code_GBps_whole_search": codes / med / 1e6,
                                     "frac_hbm_whole_search": codes / med / 1e6 / pk["hbm"]}
     ix.close()
@@ -294,8 +297,9 @@ def run_ours(args):
     fs.lib()  # fail loudly if libfs.so is missing
     pk = peaks()
 
-    if args.case in ("flat", "ivfpq"):  # profiling aid: only that "also" leg
-        out = also_flat(fs, gt, pk) if args.case == "flat" else also_ivfpq(fs, gt, pk, args.ivfpq_nb)
+    if args.case in ("flat", "ivfpq", "ivfpq5"):  # profiling aid: only that "also" leg
+        out = also_flat(fs, gt, pk) if args.case == "flat" else also_ivfpq(fs, gt, pk, args.ivfpq_nb,
+                                                                         cfg5=args.case == "ivfpq5")
         print(json.dumps({"case": args.case, **out}))
         return
 
