@@ -71,6 +71,29 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
       : "memory");
 }
 
+// the same on 32-bit shared-memory addresses computed once per warp
+__device__ __forceinline__ void mbar_expect_tx_a(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait_a(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      "WAIT_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra DONE_%=;\n\t"
+      "bra WAIT_%=;\n\t"
+      "DONE_%=:\n\t"
+      "}" ::"r"(bar),
+      "r"(parity)
+      : "memory");
+}
+__device__ __forceinline__ void bulk_g2s_a(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+               "l"(src), "r"(bytes), "r"(bar)
+               : "memory");
+}
+
 #ifndef FS_KSEG
 #define FS_KSEG 512
 #endif
@@ -117,6 +140,7 @@ __device__ __forceinline__ ItemDesc decode_item(const KSelArgs& a, int64_t item)
 struct Ring {
   float* data;     // [kStages][kSeg]
   uint64_t* bar;   // [kStages]
+  uint32_t data_a, bar_a;  // the same as shared-memory addresses
   uint32_t issued, consumed;
   int64_t c_item;  // item being consumed
   int64_t n_item;  // the item after it (-1: not drawn yet)
@@ -150,8 +174,8 @@ __device__ __forceinline__ void ring_fill(const KSelArgs& a, Ring& r, int64_t n_
       const int slot = (int)(r.issued % kStages);
       const int n4 = r.p_left < kSeg / 4 ? r.p_left : kSeg / 4;
       if (lane == 0) {
-        mbar_expect_tx(r.bar + slot, (uint32_t)n4 * 16u);
-        bulk_g2s(r.data + slot * kSeg, r.p_ptr, (uint32_t)n4 * 16u, r.bar + slot);
+        mbar_expect_tx_a(r.bar_a + slot * 8, (uint32_t)n4 * 16u);
+        bulk_g2s_a(r.data_a + slot * (kSeg * 4), r.p_ptr, (uint32_t)n4 * 16u, r.bar_a + slot * 8);
       }
       ++r.issued;
       r.p_ptr += kSeg;
@@ -211,6 +235,8 @@ __global__ void __launch_bounds__(TSelCfg<NQ>::WARPS * 32) kselect_stream_kernel
   uint64_t* qbuf = reinterpret_cast<uint64_t*>(mine + SM::ring_bytes);
   uint32_t* scratch = reinterpret_cast<uint32_t*>(mine + SM::ring_bytes + SM::queue_bytes);
   ring.bar = reinterpret_cast<uint64_t*>(smem_raw + SM::per_warp * WARPS) + warp * kStages;
+  ring.data_a = smem_u32(ring.data);
+  ring.bar_a = smem_u32(ring.bar);
   if (lane == 0) {
 #pragma unroll
     for (int s = 0; s < kStages; ++s) mbar_init(ring.bar + s, 1);
@@ -307,7 +333,7 @@ __global__ void __launch_bounds__(TSelCfg<NQ>::WARPS * 32) kselect_stream_kernel
 #pragma unroll 1
     for (int seg = 0; seg < nseg; ++seg) {
       const int slot = (int)(ring.consumed % kStages);
-      mbar_wait(ring.bar + slot, (ring.consumed / kStages) & 1u);
+      mbar_wait_a(ring.bar_a + slot * 8, (ring.consumed / kStages) & 1u);
       const int left = (int)d.nvec - seg * (kSeg / 4);
       const float* sf = ring.data + slot * kSeg + lane * 4;
       const uint32_t ib = vbase + (uint32_t)seg * kSeg + (uint32_t)lane * 4u;
@@ -315,14 +341,18 @@ __global__ void __launch_bounds__(TSelCfg<NQ>::WARPS * 32) kselect_stream_kernel
       const float thr = q.thr_x;
       uint32_t mask = 0u;
       if (left >= kSeg / 4) {
+        // the sign of (bound - v) is funnel-shifted into the mask: one subtract and one shift per
+        // element (v equal to the bound and NaN pass as well: the restore step tests keys exactly)
+        uint32_t rej = 0u;
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
           const float4 x = *reinterpret_cast<const float4*>(sf + u * 128);
-          mask |= (!(x.x >= thr) ? 1u : 0u) << (4 * u);
-          mask |= (!(x.y >= thr) ? 2u : 0u) << (4 * u);
-          mask |= (!(x.z >= thr) ? 4u : 0u) << (4 * u);
-          mask |= (!(x.w >= thr) ? 8u : 0u) << (4 * u);
+          rej = __funnelshift_l(__float_as_uint(thr - x.x), rej, 1);
+          rej = __funnelshift_l(__float_as_uint(thr - x.y), rej, 1);
+          rej = __funnelshift_l(__float_as_uint(thr - x.z), rej, 1);
+          rej = __funnelshift_l(__float_as_uint(thr - x.w), rej, 1);
         }
+        mask = __brev(~rej) >> 16;  // element e = 4u + t back at bit e
       } else {
 #pragma unroll 1
         for (int u = 0; u < 4; ++u) {
