@@ -343,15 +343,16 @@ __global__ void __launch_bounds__(TSelCfg<NQ>::WARPS * 32) kselect_stream_kernel
       if (left >= kSeg / 4) {
         // the sign of (bound - v) is funnel-shifted into the mask: one subtract and one shift per
         // element (v equal to the bound and NaN pass as well: the restore step tests keys exactly)
-        uint32_t rej = 0u;
+        uint32_t rj[4];  // four independent chains (one per 128-bit load)
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
           const float4 x = *reinterpret_cast<const float4*>(sf + u * 128);
-          rej = __funnelshift_l(__float_as_uint(thr - x.x), rej, 1);
-          rej = __funnelshift_l(__float_as_uint(thr - x.y), rej, 1);
-          rej = __funnelshift_l(__float_as_uint(thr - x.z), rej, 1);
-          rej = __funnelshift_l(__float_as_uint(thr - x.w), rej, 1);
+          rj[u] = __float_as_uint(thr - x.x) >> 31;
+          rj[u] = __funnelshift_l(__float_as_uint(thr - x.y), rj[u], 1);
+          rj[u] = __funnelshift_l(__float_as_uint(thr - x.z), rj[u], 1);
+          rj[u] = __funnelshift_l(__float_as_uint(thr - x.w), rj[u], 1);
         }
+        const uint32_t rej = (rj[0] << 12) | (rj[1] << 8) | (rj[2] << 4) | rj[3];
         mask = __brev(~rej) >> 16;  // element e = 4u + t back at bit e
       } else {
 #pragma unroll 1
