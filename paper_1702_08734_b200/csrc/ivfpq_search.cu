@@ -16,6 +16,8 @@
 //                        found the fused form <= 15 % faster on Maxwell)
 //   C5 pass-2 + ids      the groups' partial lists are selected again to k; int64
 //                        ids are fetched for the winners only
+#include <cstdlib>
+
 #include "flat.cuh"
 #include "ivfpq.cuh"
 #include "ivfpq_scan.cuh"
@@ -29,7 +31,8 @@ constexpr int SCAN_WARPS = 8;
 constexpr int SCAN_THREADS = SCAN_WARPS * 32;
 
 // Shared memory: r[d] | T[M][256] | per-warp batches | merge area [SCAN_WARPS][K]
-template <int NQ>
+// MT = M when M is 8 or 16 (code loaded with one 8 / 16-byte load, lookups unrolled), else 0.
+template <int NQ, int MT>
 __global__ void __launch_bounds__(SCAN_THREADS) ivfpq_scan_kernel(const ScanArgs a) {
   extern __shared__ __align__(16) unsigned char scan_smem[];
   constexpr int K = 32 * NQ;
@@ -81,7 +84,23 @@ __global__ void __launch_bounds__(SCAN_THREADS) ivfpq_scan_kernel(const ScanArgs
       float dist = 0.f;
       if (ok) {
         const uint8_t* cv = cl + v * M;
-        if ((M & 3) == 0) {
+        if (MT == 8 || MT == 16) {
+          constexpr int CW = MT >= 4 ? MT / 4 : 1;
+          uint32_t cw[CW];
+          if (MT == 8) {
+            const uint2 t = *reinterpret_cast<const uint2*>(cv);
+            cw[0] = t.x;
+            cw[1] = t.y;
+          } else {
+            const uint4 t = *reinterpret_cast<const uint4*>(cv);
+            cw[0] = t.x;
+            cw[1] = t.y;
+            cw[CW - 2 < 0 ? 0 : CW - 2] = t.z;
+            cw[CW - 1] = t.w;
+          }
+#pragma unroll
+          for (int m = 0; m < MT; ++m) dist += T[(m << 8) + ((cw[(m >> 2) % CW] >> (8 * (m & 3))) & 255u)];
+        } else if ((M & 3) == 0) {
           const uint32_t* cw = reinterpret_cast<const uint32_t*>(cv);
           for (int w = 0; w < (M >> 2); ++w) {
             const uint32_t c = cw[w];
@@ -95,8 +114,11 @@ __global__ void __launch_bounds__(SCAN_THREADS) ivfpq_scan_kernel(const ScanArgs
           for (int m = 0; m < M; ++m) dist += T[(m << 8) + cv[m]];
         }
       }
-      const uint64_t key = make_key(dist, (uint32_t)(lb + v));
-      sel.push(ok && sel.maybe(dist) && sel.wants(key), key);
+      const bool cand = ok && sel.maybe(dist);
+      if (__any_sync(kFull, cand)) {  // the exact key is only built when some lane may have a winner
+        const uint64_t key = make_key(dist, (uint32_t)(lb + v));
+        sel.push(cand && sel.wants(key), key);
+      }
     }
   }
   sel.finish();
@@ -186,22 +208,35 @@ SearchPlan search_plan(const fs_ivfpq* ix, int64_t nq, int nprobe, int k) {
   return p;
 }
 
-template <int NQ>
-int launch_scan(const ScanArgs& a, int64_t nq, cudaStream_t s) {
+template <int NQ, int MT>
+int launch_scan_m(const ScanArgs& a, int64_t nq, cudaStream_t s) {
   constexpr int K = 32 * NQ;
   const size_t smem = (size_t)(((a.d + 3) & ~3) + a.M * 256) * sizeof(float) +
                       (size_t)(SCAN_WARPS * warp_select_smem_keys<2>() + SCAN_WARPS * K) * sizeof(uint64_t);
   if (smem > 227 * 1024) return set_error(FS_EUNSUPPORTED, "fs_ivfpq_search: shared memory (%zu B) exceeds 227 KB", smem);
   static size_t attr_smem = 0;
   if (smem > attr_smem) {
-    FS_CUDA(cudaFuncSetAttribute(ivfpq_scan_kernel<NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    FS_CUDA(cudaFuncSetAttribute(ivfpq_scan_kernel<NQ, MT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    // Leave part of the unified L1 / shared memory to L1: every CTA re-reads the PQ codebook
+    // (256 d floats, 96 KB at d = 96) for every table it builds; with the maximum shared-memory
+    // carve-out those reads all go to L2.
+    const char* e = getenv("FS_IVFPQ_CARVEOUT");
+    FS_CUDA(cudaFuncSetAttribute(ivfpq_scan_kernel<NQ, MT>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                                 e ? atoi(e) : 65));
     attr_smem = smem;
   }
   const int64_t grid = nq * a.ngroups;
   if (grid > 0x7fffffffLL) return set_error(FS_EUNSUPPORTED, "fs_ivfpq_search: nq * groups too large");
-  ivfpq_scan_kernel<NQ><<<(unsigned)grid, SCAN_THREADS, smem, s>>>(a);
+  ivfpq_scan_kernel<NQ, MT><<<(unsigned)grid, SCAN_THREADS, smem, s>>>(a);
   FS_LAUNCHED();
   return FS_OK;
+}
+
+template <int NQ>
+int launch_scan(const ScanArgs& a, int64_t nq, cudaStream_t s) {
+  if (a.M == 16) return launch_scan_m<NQ, 16>(a, nq, s);
+  if (a.M == 8) return launch_scan_m<NQ, 8>(a, nq, s);
+  return launch_scan_m<NQ, 0>(a, nq, s);
 }
 
 }  // namespace
