@@ -68,9 +68,32 @@ __global__ void __launch_bounds__(SCAN_THREADS) ivfpq_scan_kernel(const ScanArgs
       const float* b = a.pq + (int64_t)e * dsub;
       const float* rm = r + m * dsub;
       float acc = 0.f;
-      for (int j = 0; j < dsub; ++j) {
-        const float t = rm[j] - b[j];
-        acc = fmaf(t, t, acc);
+      if (dsub == 6) {  // d = 96, M = 16: three 8-byte loads (e * 24 bytes is 8-byte aligned)
+        const float2* b2 = reinterpret_cast<const float2*>(b);
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+          const float2 bb = __ldg(b2 + j);
+          const float t0 = rm[2 * j] - bb.x, t1 = rm[2 * j + 1] - bb.y;
+          acc = fmaf(t0, t0, acc);
+          acc = fmaf(t1, t1, acc);
+        }
+      } else if (dsub == 12) {  // d = 96, M = 8: three 16-byte loads
+        const float4* b4 = reinterpret_cast<const float4*>(b);
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+          const float4 bb = __ldg(b4 + j);
+          const float t0 = rm[4 * j] - bb.x, t1 = rm[4 * j + 1] - bb.y, t2 = rm[4 * j + 2] - bb.z,
+                      t3 = rm[4 * j + 3] - bb.w;
+          acc = fmaf(t0, t0, acc);
+          acc = fmaf(t1, t1, acc);
+          acc = fmaf(t2, t2, acc);
+          acc = fmaf(t3, t3, acc);
+        }
+      } else {
+        for (int j = 0; j < dsub; ++j) {
+          const float t = rm[j] - b[j];
+          acc = fmaf(t, t, acc);
+        }
       }
       T[e] = acc;
     }
