@@ -22,6 +22,46 @@ struct ScanArgs {
   int d, M, dsub, nprobe, G, ngroups, k;
 };
 
+// rotate the MW-word little-endian value w right by r bytes (r < 4 MW, per-lane constant)
+template <int MW>
+__device__ __forceinline__ void rotate_bytes(uint32_t (&w)[MW], int r) {
+  if (MW > 1) {
+#pragma unroll
+    for (int bit = MW / 2; bit >= 1; bit >>= 1) {  // word rotation by (r >> 2), one bit at a time
+      const bool on = ((r >> 2) & bit) != 0;
+      uint32_t t[MW];
+#pragma unroll
+      for (int i = 0; i < MW; ++i) t[i] = on ? w[(i + bit) % MW] : w[i];
+#pragma unroll
+      for (int i = 0; i < MW; ++i) w[i] = t[i];
+    }
+  }
+  const int sh = (r & 3) * 8;
+  uint32_t t[MW];
+#pragma unroll
+  for (int i = 0; i < MW; ++i) t[i] = __funnelshift_r(w[i], w[(i + 1) % MW], sh);
+#pragma unroll
+  for (int i = 0; i < MW; ++i) w[i] = t[i];
+}
+
+template <int MW>
+__device__ __forceinline__ void load_code(const uint8_t* p, uint32_t (&w)[MW]) {
+  if (MW == 2) {
+    const uint2 t = *reinterpret_cast<const uint2*>(p);
+    w[0] = t.x;
+    w[1] = t.y;
+  } else {
+#pragma unroll
+    for (int i = 0; i < MW / 4; ++i) {
+      const uint4 t = reinterpret_cast<const uint4*>(p)[i];
+      w[4 * i] = t.x;
+      w[4 * i + 1] = t.y;
+      w[4 * i + 2] = t.z;
+      w[4 * i + 3] = t.w;
+    }
+  }
+}
+
 // Persistent scan: M in {8, 16, 32}, queue class K <= 256, codebook + tables within 200 KB.
 bool scan2_supported(int d, int M, int k);
 int launch_scan2(const ScanArgs& a, int64_t nq, int k, unsigned int* work, cudaStream_t s);

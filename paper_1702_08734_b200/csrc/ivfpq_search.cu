@@ -17,6 +17,7 @@
 //   C5 pass-2 + ids      the groups' partial lists are selected again to k; int64
 //                        ids are fetched for the winners only
 #include <cstdlib>
+#include <cstring>
 
 #include "flat.cuh"
 #include "ivfpq.cuh"
@@ -31,8 +32,9 @@ constexpr int SCAN_WARPS = 8;
 constexpr int SCAN_THREADS = SCAN_WARPS * 32;
 
 // Shared memory: r[d] | T[M][256] | per-warp batches | merge area [SCAN_WARPS][K]
-// MT = M when M is 8 or 16 (code loaded with one 8 / 16-byte load, lookups unrolled), else 0.
-template <int NQ, int MT>
+// MT = M when M is 8 or 16 (code loaded with one 8 / 16-byte load, lookups unrolled), else 0;
+// DS = d / M when it is 6 or 12 and MT != 0 (table build unrolled, 8 / 16-byte codebook loads), else 0.
+template <int NQ, int MT, int DS>
 __global__ void __launch_bounds__(SCAN_THREADS) ivfpq_scan_kernel(const ScanArgs a) {
   extern __shared__ __align__(16) unsigned char scan_smem[];
   constexpr int K = 32 * NQ;
@@ -63,39 +65,48 @@ __global__ void __launch_bounds__(SCAN_THREADS) ivfpq_scan_kernel(const ScanArgs
     // C2: residual and tables
     for (int j = tid; j < d; j += SCAN_THREADS) r[j] = a.xq[q * d + j] - a.coarse[L * d + j];
     __syncthreads();
-    for (int e = tid; e < M * 256; e += SCAN_THREADS) {
-      const int m = e >> 8;
-      const float* b = a.pq + (int64_t)e * dsub;
-      const float* rm = r + m * dsub;
-      float acc = 0.f;
-      if (dsub == 6) {  // d = 96, M = 16: three 8-byte loads (e * 24 bytes is 8-byte aligned)
-        const float2* b2 = reinterpret_cast<const float2*>(b);
+    if (MT != 0 && DS != 0) {
+      // thread t builds entry c = t of every table m (SCAN_THREADS == 256): unrolled, vector loads
+      constexpr int VW = DS == 6 ? 2 : 4;  // floats per load: 8-byte (DS = 6) or 16-byte (DS = 12)
+      const float* bq = a.pq + (size_t)tid * DS;
+#pragma unroll 4
+      for (int m = 0; m < MT; ++m) {
+        const float* b = bq + (size_t)m * 256 * DS;
+        const float* rm = r + m * DS;
+        float acc = 0.f;
 #pragma unroll
-        for (int j = 0; j < 3; ++j) {
-          const float2 bb = __ldg(b2 + j);
-          const float t0 = rm[2 * j] - bb.x, t1 = rm[2 * j + 1] - bb.y;
-          acc = fmaf(t0, t0, acc);
-          acc = fmaf(t1, t1, acc);
-        }
-      } else if (dsub == 12) {  // d = 96, M = 8: three 16-byte loads
-        const float4* b4 = reinterpret_cast<const float4*>(b);
+        for (int j = 0; j < DS / VW; ++j) {
+          float bv[VW], rv[VW];
+          if (VW == 2) {
+            const float2 t = __ldg(reinterpret_cast<const float2*>(b) + j);
+            const float2 u = reinterpret_cast<const float2*>(rm)[j];
+            bv[0] = t.x; bv[1] = t.y; rv[0] = u.x; rv[1] = u.y;
+          } else {
+            const float4 t = __ldg(reinterpret_cast<const float4*>(b) + j);
+            const float4 u = reinterpret_cast<const float4*>(rm)[j];
+            bv[0] = t.x; bv[1] = t.y; bv[VW - 2] = t.z; bv[VW - 1] = t.w;
+            rv[0] = u.x; rv[1] = u.y; rv[VW - 2] = u.z; rv[VW - 1] = u.w;
+          }
 #pragma unroll
-        for (int j = 0; j < 3; ++j) {
-          const float4 bb = __ldg(b4 + j);
-          const float t0 = rm[4 * j] - bb.x, t1 = rm[4 * j + 1] - bb.y, t2 = rm[4 * j + 2] - bb.z,
-                      t3 = rm[4 * j + 3] - bb.w;
-          acc = fmaf(t0, t0, acc);
-          acc = fmaf(t1, t1, acc);
-          acc = fmaf(t2, t2, acc);
-          acc = fmaf(t3, t3, acc);
+          for (int i = 0; i < VW; ++i) {
+            const float df = rv[i] - bv[i];
+            acc = fmaf(df, df, acc);
+          }
         }
-      } else {
+        T[m * 256 + tid] = acc;
+      }
+    } else {
+      for (int e = tid; e < M * 256; e += SCAN_THREADS) {
+        const int m = e >> 8;
+        const float* b = a.pq + (int64_t)e * dsub;
+        const float* rm = r + m * dsub;
+        float acc = 0.f;
         for (int j = 0; j < dsub; ++j) {
           const float t = rm[j] - b[j];
           acc = fmaf(t, t, acc);
         }
+        T[e] = acc;
       }
-      T[e] = acc;
     }
     __syncthreads();
     // C3 + C4: scan and select
@@ -231,7 +242,187 @@ SearchPlan search_plan(const fs_ivfpq* ix, int64_t nq, int nprobe, int k) {
   return p;
 }
 
-template <int NQ, int MT>
+// ---------------------------------------------------------------------------
+// M = 8 or 16: the same scan with a bank-conflict-free gather.
+//   * the table is stored as lut[c][b], b = 0..31: word (c, b) lives in shared-memory bank b and
+//     holds T_{b mod M}[c] (32 / M replicas of every table); lane l adds its sub-quantizers in
+//     the rotated order m = (s + l) mod M, so at step s the 32 lanes read 32 different banks;
+//     lane l rotates its code by l mod M bytes once per vector (funnel shifts);
+//   * so that the rotated order cannot change the sum, the entries are FIXED-POINT: the CTA
+//     scales every table of the (query, list) pair by one power of two such that the largest
+//     entry is < 2^27, rounds to integers, and the scan adds integers (exact, associative).
+//     Identical codes therefore give identical distances whatever lane scans them (reading
+//     C-6).  Quantisation: <= 2^-28 of the largest table entry per entry, M times that per
+//     distance -- far inside the 1e-3 relative tolerance for every distance that is not
+//     ~5 orders of magnitude below the largest entry of its tables.
+// Shared memory: r[d] | Tn[M][257] | lut[256][32] | red[8] | select batches | merge area
+// ---------------------------------------------------------------------------
+template <int NQ, int M>
+__global__ void __launch_bounds__(SCAN_THREADS) ivfpq_scan_rot_kernel(const ScanArgs a) {
+  extern __shared__ __align__(16) unsigned char scan_smem[];
+  constexpr int K = 32 * NQ;
+  constexpr int NB = 2;
+  constexpr int MW = M / 4;
+  constexpr int REP = 32 / M;
+  constexpr int TS = 257;  // row stride of the natural table: conflict-free reads by m
+  const int d = a.d, dsub = a.dsub;
+  float* r = reinterpret_cast<float*>(scan_smem);
+  float* Tn = r + ((d + 3) & ~3);
+  uint32_t* lut = reinterpret_cast<uint32_t*>(Tn + ((M * TS + 3) & ~3));
+  float* red = reinterpret_cast<float*>(lut + 256 * 32);
+  uint64_t* bufs = reinterpret_cast<uint64_t*>(red + 8);
+  uint64_t* merge = bufs + SCAN_WARPS * warp_select_smem_keys<NB>();
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int64_t q = blockIdx.x / a.ngroups;
+  const int g = (int)(blockIdx.x - q * a.ngroups);
+  const int p_begin = g * a.G;
+  const int p_end = (p_begin + a.G) < a.nprobe ? (p_begin + a.G) : a.nprobe;
+
+  WarpSelect<NQ, NB> sel;
+  sel.init(bufs + warp * warp_select_smem_keys<NB>(), lane);
+  unsigned long long bytes = 0;
+  const int rot = lane % M;
+
+  for (int p = p_begin; p < p_end; ++p) {
+    const int64_t L = a.probe_ids[q * a.nprobe + p];
+    if (a.out_probed && tid == 0) a.out_probed[q * a.nprobe + p] = (int32_t)L;
+    if (L < 0) continue;
+    const int64_t lb = a.offsets[L], le = a.offsets[L + 1];
+    const int64_t len = le - lb;
+    if (len == 0) continue;  // empty lists are probed and contribute nothing
+    __syncthreads();         // previous list's tables are no longer read
+    for (int j = tid; j < d; j += SCAN_THREADS) r[j] = a.xq[q * d + j] - a.coarse[L * d + j];
+    __syncthreads();
+    // C2, step 1: T_m[c] = ||r^m - B[m][c]||^2 (Eq. 10) in the natural layout, and its maximum
+    float mx = 0.f;
+    for (int e = tid; e < M * 256; e += SCAN_THREADS) {
+      const int m = e >> 8;
+      const float* b = a.pq + (int64_t)e * dsub;
+      const float* rm = r + m * dsub;
+      float acc = 0.f;
+      if (dsub == 6) {
+        const float2* b2 = reinterpret_cast<const float2*>(b);
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+          const float2 bb = __ldg(b2 + j);
+          const float t0 = rm[2 * j] - bb.x, t1 = rm[2 * j + 1] - bb.y;
+          acc = fmaf(t0, t0, acc);
+          acc = fmaf(t1, t1, acc);
+        }
+      } else if (dsub == 12) {
+        const float4* b4 = reinterpret_cast<const float4*>(b);
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+          const float4 bb = __ldg(b4 + j);
+          const float t0 = rm[4 * j] - bb.x, t1 = rm[4 * j + 1] - bb.y, t2 = rm[4 * j + 2] - bb.z,
+                      t3 = rm[4 * j + 3] - bb.w;
+          acc = fmaf(t0, t0, acc);
+          acc = fmaf(t1, t1, acc);
+          acc = fmaf(t2, t2, acc);
+          acc = fmaf(t3, t3, acc);
+        }
+      } else {
+        for (int j = 0; j < dsub; ++j) {
+          const float t = rm[j] - b[j];
+          acc = fmaf(t, t, acc);
+        }
+      }
+      Tn[m * TS + (e & 255)] = acc;
+      mx = fmaxf(mx, acc);
+    }
+#pragma unroll
+    for (int sft = 16; sft >= 1; sft >>= 1) mx = fmaxf(mx, __shfl_xor_sync(kFull, mx, sft));
+    if (lane == 0) red[warp] = mx;
+    __syncthreads();
+    // C2, step 2: one power-of-two scale for the pair, integer entries into the banked layout
+    mx = red[0];
+#pragma unroll
+    for (int w = 1; w < SCAN_WARPS; ++w) mx = fmaxf(mx, red[w]);
+    int ex = 0;
+    if (mx > 0.f && mx < 3.0e38f) frexpf(mx, &ex);  // mx < 2^ex
+    int se = 27 - ex;                               // scale = 2^se: scaled entries < 2^27
+    se = se > 100 ? 100 : (se < -100 ? -100 : se);
+    const float scale = __uint_as_float((uint32_t)(127 + se) << 23);
+    const float inv_scale = __uint_as_float((uint32_t)(127 - se) << 23);
+    {
+      const int m = lane % M, cofs = lane / M;
+      for (int c0 = warp * REP; c0 < 256; c0 += SCAN_WARPS * REP) {
+        const int c = c0 + cofs;
+        const uint32_t v = __float2uint_rn(Tn[m * TS + c] * scale);
+#pragma unroll
+        for (int rep = 0; rep < REP; ++rep) lut[c * 32 + m + rep * M] = v;
+      }
+    }
+    __syncthreads();
+    // C3 + C4: scan and select
+    bytes += (unsigned long long)len * M;
+    const uint8_t* cl = a.codes + lb * M;
+    const char* lutb = reinterpret_cast<const char*>(lut);
+    for (int64_t v0 = 0; v0 < len; v0 += SCAN_THREADS) {
+      const int64_t v = v0 + tid;
+      const bool ok = v < len;
+      float dist = 0.f;
+      if (ok) {
+        uint32_t w[MW];
+        load_code<MW>(cl + v * M, w);
+        rotate_bytes<MW>(w, rot);
+        uint32_t acc = 0u;
+#pragma unroll
+        for (int s2 = 0; s2 < M; ++s2) {
+          const uint32_t c = (w[s2 >> 2] >> (8 * (s2 & 3))) & 255u;
+          acc += *reinterpret_cast<const uint32_t*>(lutb + c * 128 + (((s2 + lane) & 31) << 2));
+        }
+        dist = (float)acc * inv_scale;
+      }
+      const bool cand = ok && sel.maybe(dist);
+      if (__any_sync(kFull, cand)) {
+        const uint64_t key = make_key(dist, (uint32_t)(lb + v));
+        sel.push(cand && sel.wants(key), key);
+      }
+    }
+  }
+  sel.finish();
+  if (tid == 0 && bytes) atomicAdd(a.scanned, bytes);
+
+  __syncthreads();
+#pragma unroll
+  for (int rr = 0; rr < NQ; ++rr) merge[warp * K + rr * 32 + lane] = sel.W[rr];
+  __syncthreads();
+  if (warp == 0) {
+    sel.reset();
+    for (int e0 = 0; e0 < SCAN_WARPS * K; e0 += 32) {
+      const uint64_t key = merge[e0 + lane];
+      sel.push(key < sel.thr, key);
+    }
+    sel.finish();
+    uint64_t* W = a.Wg + (int64_t)blockIdx.x * K;
+#pragma unroll
+    for (int rr = 0; rr < NQ; ++rr) W[rr * 32 + lane] = sel.W[rr];
+  }
+}
+
+template <int NQ, int M>
+int launch_scan_rot(const ScanArgs& a, int64_t nq, cudaStream_t s) {
+  constexpr int K = 32 * NQ;
+  const size_t smem = (size_t)(((a.d + 3) & ~3) + ((M * 257 + 3) & ~3) + 256 * 32 + 8) * sizeof(float) +
+                      (size_t)(SCAN_WARPS * warp_select_smem_keys<2>() + SCAN_WARPS * K) * sizeof(uint64_t);
+  if (smem > 227 * 1024) return set_error(FS_EUNSUPPORTED, "fs_ivfpq_search: shared memory (%zu B) exceeds 227 KB", smem);
+  static size_t attr_smem = 0;
+  if (smem > attr_smem) {
+    FS_CUDA(cudaFuncSetAttribute(ivfpq_scan_rot_kernel<NQ, M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const char* e = getenv("FS_IVFPQ_CARVEOUT");
+    FS_CUDA(cudaFuncSetAttribute(ivfpq_scan_rot_kernel<NQ, M>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                                 e ? atoi(e) : 100));
+    attr_smem = smem;
+  }
+  const int64_t grid = nq * a.ngroups;
+  if (grid > 0x7fffffffLL) return set_error(FS_EUNSUPPORTED, "fs_ivfpq_search: nq * groups too large");
+  ivfpq_scan_rot_kernel<NQ, M><<<(unsigned)grid, SCAN_THREADS, smem, s>>>(a);
+  FS_LAUNCHED();
+  return FS_OK;
+}
+
+template <int NQ, int MT, int DS>
 int launch_scan_m(const ScanArgs& a, int64_t nq, cudaStream_t s) {
   constexpr int K = 32 * NQ;
   const size_t smem = (size_t)(((a.d + 3) & ~3) + a.M * 256) * sizeof(float) +
@@ -239,27 +430,38 @@ int launch_scan_m(const ScanArgs& a, int64_t nq, cudaStream_t s) {
   if (smem > 227 * 1024) return set_error(FS_EUNSUPPORTED, "fs_ivfpq_search: shared memory (%zu B) exceeds 227 KB", smem);
   static size_t attr_smem = 0;
   if (smem > attr_smem) {
-    FS_CUDA(cudaFuncSetAttribute(ivfpq_scan_kernel<NQ, MT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    FS_CUDA(cudaFuncSetAttribute(ivfpq_scan_kernel<NQ, MT, DS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     // Leave part of the unified L1 / shared memory to L1: every CTA re-reads the PQ codebook
     // (256 d floats, 96 KB at d = 96) for every table it builds; with the maximum shared-memory
     // carve-out those reads all go to L2.
     const char* e = getenv("FS_IVFPQ_CARVEOUT");
-    FS_CUDA(cudaFuncSetAttribute(ivfpq_scan_kernel<NQ, MT>, cudaFuncAttributePreferredSharedMemoryCarveout,
+    FS_CUDA(cudaFuncSetAttribute(ivfpq_scan_kernel<NQ, MT, DS>, cudaFuncAttributePreferredSharedMemoryCarveout,
                                  e ? atoi(e) : 65));
     attr_smem = smem;
   }
   const int64_t grid = nq * a.ngroups;
   if (grid > 0x7fffffffLL) return set_error(FS_EUNSUPPORTED, "fs_ivfpq_search: nq * groups too large");
-  ivfpq_scan_kernel<NQ, MT><<<(unsigned)grid, SCAN_THREADS, smem, s>>>(a);
+  ivfpq_scan_kernel<NQ, MT, DS><<<(unsigned)grid, SCAN_THREADS, smem, s>>>(a);
   FS_LAUNCHED();
   return FS_OK;
 }
 
 template <int NQ>
 int launch_scan(const ScanArgs& a, int64_t nq, cudaStream_t s) {
-  if (a.M == 16) return launch_scan_m<NQ, 16>(a, nq, s);
-  if (a.M == 8) return launch_scan_m<NQ, 8>(a, nq, s);
-  return launch_scan_m<NQ, 0>(a, nq, s);
+  // FS_IVFPQ_SCAN=rot selects the bank-conflict-free fixed-point kernel (A/B runs): correct, but
+  // its second table pass and larger footprint cost more than the conflicts (profiles/r01_ivfpq.md)
+  static int plain = -1;
+  if (plain < 0) {
+    const char* e = getenv("FS_IVFPQ_SCAN");
+    plain = (e && strcmp(e, "rot") == 0) ? 0 : 1;
+  }
+  if (!plain && NQ <= 8 && a.M == 16) return launch_scan_rot<NQ, 16>(a, nq, s);
+  if (!plain && NQ <= 8 && a.M == 8) return launch_scan_rot<NQ, 8>(a, nq, s);
+  if (a.M == 16 && a.dsub == 6) return launch_scan_m<NQ, 16, 6>(a, nq, s);
+  if (a.M == 8 && a.dsub == 12) return launch_scan_m<NQ, 8, 12>(a, nq, s);
+  if (a.M == 16) return launch_scan_m<NQ, 16, 0>(a, nq, s);
+  if (a.M == 8) return launch_scan_m<NQ, 8, 0>(a, nq, s);
+  return launch_scan_m<NQ, 0, 0>(a, nq, s);
 }
 
 }  // namespace
