@@ -31,18 +31,39 @@ namespace {
 constexpr int SCAN_WARPS = 8;
 constexpr int SCAN_THREADS = SCAN_WARPS * 32;
 
-// Shared memory: r[d] | T[M][256] | per-warp batches | merge area [SCAN_WARPS][K]
+// dist += T_m[byte m of the code] for m = m0 .. MT-1.  Tb = shared-space address of T, 1 KB aligned:
+// the lookup address is one shift and one LOP3, the table offset m * 1 KB is an immediate.
+template <int OFF>
+__device__ __forceinline__ float lds_f32_off(uint32_t addr) {
+  float t;
+  asm volatile("ld.shared.f32 %0, [%1+%2];" : "=f"(t) : "r"(addr), "n"(OFF));
+  return t;
+}
+template <int m, int MT>
+__device__ __forceinline__ void lookup_all(const uint32_t* cw, uint32_t Tb, float& dist) {
+  if constexpr (m < MT) {
+    const uint32_t w = cw[m >> 2];
+    constexpr int j = m & 3;
+    const uint32_t sh = j == 0 ? (w << 2) : (w >> (8 * j - 2));
+    dist += lds_f32_off<m * 1024>((sh & 0x3FCu) | Tb);
+    lookup_all<m + 1, MT>(cw, Tb, dist);
+  }
+}
+
+// Shared memory: T[M][256] | r[d] | per-warp batches | merge area [SCAN_WARPS][K]
 // MT = M when M is 8 or 16 (code loaded with one 8 / 16-byte load, lookups unrolled), else 0;
 // DS = d / M when it is 6 or 12 and MT != 0 (table build unrolled, 8 / 16-byte codebook loads), else 0.
 template <int NQ, int MT, int DS>
 __global__ void __launch_bounds__(SCAN_THREADS) ivfpq_scan_kernel(const ScanArgs a) {
-  extern __shared__ __align__(16) unsigned char scan_smem[];
+  extern __shared__ __align__(1024) unsigned char scan_smem[];
   constexpr int K = 32 * NQ;
   constexpr int NB = 2;
-  float* r = reinterpret_cast<float*>(scan_smem);
-  float* T = r + ((a.d + 3) & ~3);
-  uint64_t* bufs = reinterpret_cast<uint64_t*>(T + a.M * 256);
+  // T first: each table starts on a 1 KB boundary, so a lookup address is (4 * byte) | base
+  float* T = reinterpret_cast<float*>(scan_smem);
+  float* r = T + a.M * 256;
+  uint64_t* bufs = reinterpret_cast<uint64_t*>(r + ((a.d + 3) & ~3));
   uint64_t* merge = bufs + SCAN_WARPS * warp_select_smem_keys<NB>();
+  const uint32_t Tb = (uint32_t)__cvta_generic_to_shared(T);
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int64_t q = blockIdx.x / a.ngroups;
   const int g = (int)(blockIdx.x - q * a.ngroups);
@@ -62,6 +83,12 @@ __global__ void __launch_bounds__(SCAN_THREADS) ivfpq_scan_kernel(const ScanArgs
     const int64_t len = le - lb;
     if (len == 0) continue;  // empty lists are probed and contribute nothing
     __syncthreads();         // previous list's table is no longer read
+    // the first code of every thread is requested before the table is built, and inside the
+    // scan every thread holds the code of its next vector: the load latency is off the path
+    const uint8_t* cl = a.codes + lb * M;
+    constexpr int CW = MT >= 4 ? MT / 4 : 2;
+    uint32_t nxt[CW] = {};
+    if (MT != 0 && tid < len) load_code<CW>(cl + (size_t)tid * MT, nxt);
     // C2: residual and tables
     for (int j = tid; j < d; j += SCAN_THREADS) r[j] = a.xq[q * d + j] - a.coarse[L * d + j];
     __syncthreads();
@@ -111,47 +138,47 @@ __global__ void __launch_bounds__(SCAN_THREADS) ivfpq_scan_kernel(const ScanArgs
     __syncthreads();
     // C3 + C4: scan and select
     bytes += (unsigned long long)len * M;
-    const uint8_t* cl = a.codes + lb * M;
-    for (int64_t v0 = 0; v0 < len; v0 += SCAN_THREADS) {
-      const int64_t v = v0 + tid;
-      const bool ok = v < len;
-      float dist = 0.f;
-      if (ok) {
-        const uint8_t* cv = cl + v * M;
-        if (MT == 8 || MT == 16) {
-          constexpr int CW = MT >= 4 ? MT / 4 : 1;
-          uint32_t cw[CW];
-          if (MT == 8) {
-            const uint2 t = *reinterpret_cast<const uint2*>(cv);
-            cw[0] = t.x;
-            cw[1] = t.y;
-          } else {
-            const uint4 t = *reinterpret_cast<const uint4*>(cv);
-            cw[0] = t.x;
-            cw[1] = t.y;
-            cw[CW - 2 < 0 ? 0 : CW - 2] = t.z;
-            cw[CW - 1] = t.w;
-          }
+    // 32-bit indices inside a piece of at most 2^30 vectors (one piece unless a list is enormous)
+    for (int64_t c0 = 0; c0 < len; c0 += (int64_t)1 << 30) {
+      const int n = (int)((len - c0) < ((int64_t)1 << 30) ? (len - c0) : ((int64_t)1 << 30));
+      const uint8_t* cc = cl + c0 * M;
+      const uint32_t pos0 = (uint32_t)(lb + c0);
+      if (MT != 0 && c0 != 0 && tid < n) load_code<CW>(cc + (size_t)tid * MT, nxt);
+      for (int v0 = 0; v0 < n; v0 += SCAN_THREADS) {
+        const int v = v0 + tid;
+        const bool ok = v < n;
+        float dist = 0.f;
+        uint32_t cw[CW];
+        if (MT != 0) {
 #pragma unroll
-          for (int m = 0; m < MT; ++m) dist += T[(m << 8) + ((cw[(m >> 2) % CW] >> (8 * (m & 3))) & 255u)];
-        } else if ((M & 3) == 0) {
-          const uint32_t* cw = reinterpret_cast<const uint32_t*>(cv);
-          for (int w = 0; w < (M >> 2); ++w) {
-            const uint32_t c = cw[w];
-            const float* Tw = T + (w << 10);
-            dist += Tw[c & 255u];
-            dist += Tw[256 + ((c >> 8) & 255u)];
-            dist += Tw[512 + ((c >> 16) & 255u)];
-            dist += Tw[768 + (c >> 24)];
-          }
-        } else {
-          for (int m = 0; m < M; ++m) dist += T[(m << 8) + cv[m]];
+          for (int i = 0; i < CW; ++i) cw[i] = nxt[i];
+          if (v + SCAN_THREADS < n) load_code<CW>(cc + (size_t)(uint32_t)(v + SCAN_THREADS) * MT, nxt);
         }
-      }
-      const bool cand = ok && sel.maybe(dist);
-      if (__any_sync(kFull, cand)) {  // the exact key is only built when some lane may have a winner
-        const uint64_t key = make_key(dist, (uint32_t)(lb + v));
-        sel.push(cand && sel.wants(key), key);
+        if (ok) {
+          if (MT == 8 || MT == 16) {
+            lookup_all<0, MT>(cw, Tb, dist);
+          } else {
+            const uint8_t* cv = cc + (size_t)(uint32_t)v * M;
+            if ((M & 3) == 0) {
+              const uint32_t* cw = reinterpret_cast<const uint32_t*>(cv);
+              for (int w = 0; w < (M >> 2); ++w) {
+                const uint32_t c = cw[w];
+                const float* Tw = T + (w << 10);
+                dist += Tw[c & 255u];
+                dist += Tw[256 + ((c >> 8) & 255u)];
+                dist += Tw[512 + ((c >> 16) & 255u)];
+                dist += Tw[768 + (c >> 24)];
+              }
+            } else {
+              for (int m = 0; m < M; ++m) dist += T[(m << 8) + cv[m]];
+            }
+          }
+        }
+        const bool cand = ok && sel.maybe(dist);
+        if (__any_sync(kFull, cand)) {  // the exact key is only built when some lane may have a winner
+          const uint64_t key = make_key(dist, pos0 + (uint32_t)v);
+          sel.push(cand && sel.wants(key), key);
+        }
       }
     }
   }
@@ -259,7 +286,7 @@ SearchPlan search_plan(const fs_ivfpq* ix, int64_t nq, int nprobe, int k) {
 // ---------------------------------------------------------------------------
 template <int NQ, int M>
 __global__ void __launch_bounds__(SCAN_THREADS) ivfpq_scan_rot_kernel(const ScanArgs a) {
-  extern __shared__ __align__(16) unsigned char scan_smem[];
+  extern __shared__ __align__(1024) unsigned char scan_smem[];
   constexpr int K = 32 * NQ;
   constexpr int NB = 2;
   constexpr int MW = M / 4;
