@@ -13,6 +13,7 @@ struct ScanArgs {
   const float* xq;
   const float* coarse;
   const float* pq;
+  const float* pq_t;         // pq regrouped for vector loads (ivfpq_search.cu), or NULL
   const int64_t* probe_ids;  // [nq][nprobe], ascending coarse distance
   const int64_t* offsets;    // [nlist+1]
   const uint8_t* codes;      // [ntotal][M]
@@ -64,6 +65,7 @@ __device__ __forceinline__ void load_code(const uint8_t* p, uint32_t (&w)[MW]) {
 
 // Persistent scan: M in {8, 16, 32}, queue class K <= 256, codebook + tables within 200 KB.
 bool scan2_supported(int d, int M, int k);
+int scan2_queues_per_item();  // partial queues it writes per (query, list group): Wg is [nq][ngroups][that][K]
 int launch_scan2(const ScanArgs& a, int64_t nq, int k, unsigned int* work, cudaStream_t s);
 
 }  // namespace fs

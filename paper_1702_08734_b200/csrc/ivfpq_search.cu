@@ -74,6 +74,9 @@ __global__ void __launch_bounds__(SCAN_THREADS) ivfpq_scan_kernel(const ScanArgs
   WarpSelect<NQ, NB> sel;
   sel.init(bufs + warp * warp_select_smem_keys<NB>(), lane);
   unsigned long long bytes = 0;
+  // the CTA's K-th distance is <= every warp's K-th: the smallest one published bounds all warps
+  __shared__ uint32_t cta_bound;
+  if (tid == 0) cta_bound = 0x7F800000u;
 
   for (int p = p_begin; p < p_end; ++p) {
     const int64_t L = a.probe_ids[q * a.nprobe + p];
@@ -94,22 +97,24 @@ __global__ void __launch_bounds__(SCAN_THREADS) ivfpq_scan_kernel(const ScanArgs
     __syncthreads();
     if (MT != 0 && DS != 0) {
       // thread t builds entry c = t of every table m (SCAN_THREADS == 256): unrolled, vector loads
+      // a.pq_t: the codebook regrouped as [m][DS / VW][256 codewords][VW] so that the 32 lanes of a
+      // warp (32 consecutive codewords) read 32 consecutive 8 / 16-byte pieces: 2 / 4 wavefronts
+      // per load instead of the 6 / 12 lines a [m][c][DS] row layout touches
       constexpr int VW = DS == 6 ? 2 : 4;  // floats per load: 8-byte (DS = 6) or 16-byte (DS = 12)
-      const float* bq = a.pq + (size_t)tid * DS;
+      constexpr int NV = DS / VW;
 #pragma unroll 4
       for (int m = 0; m < MT; ++m) {
-        const float* b = bq + (size_t)m * 256 * DS;
         const float* rm = r + m * DS;
         float acc = 0.f;
 #pragma unroll
-        for (int j = 0; j < DS / VW; ++j) {
+        for (int j = 0; j < NV; ++j) {
           float bv[VW], rv[VW];
           if (VW == 2) {
-            const float2 t = __ldg(reinterpret_cast<const float2*>(b) + j);
+            const float2 t = __ldg(reinterpret_cast<const float2*>(a.pq_t) + (m * NV + j) * 256 + tid);
             const float2 u = reinterpret_cast<const float2*>(rm)[j];
             bv[0] = t.x; bv[1] = t.y; rv[0] = u.x; rv[1] = u.y;
           } else {
-            const float4 t = __ldg(reinterpret_cast<const float4*>(b) + j);
+            const float4 t = __ldg(reinterpret_cast<const float4*>(a.pq_t) + (m * NV + j) * 256 + tid);
             const float4 u = reinterpret_cast<const float4*>(rm)[j];
             bv[0] = t.x; bv[1] = t.y; bv[VW - 2] = t.z; bv[VW - 1] = t.w;
             rv[0] = u.x; rv[1] = u.y; rv[VW - 2] = u.z; rv[VW - 1] = u.w;
@@ -174,10 +179,13 @@ __global__ void __launch_bounds__(SCAN_THREADS) ivfpq_scan_kernel(const ScanArgs
             }
           }
         }
-        const bool cand = ok && sel.maybe(dist);
+        const float bound = fminf(sel.thr_val, __uint_as_float(*reinterpret_cast<volatile uint32_t*>(&cta_bound)));
+        const bool cand = ok && !(dist > bound);
         if (__any_sync(kFull, cand)) {  // the exact key is only built when some lane may have a winner
           const uint64_t key = make_key(dist, pos0 + (uint32_t)v);
+          const uint64_t thr_before = sel.thr;
           sel.push(cand && sel.wants(key), key);
+          if (sel.thr != thr_before && lane == 0) atomicMin(&cta_bound, __float_as_uint(sel.thr_val));
         }
       }
     }
@@ -239,10 +247,22 @@ __global__ void __launch_bounds__(128)
   }
 }
 
+// The codebook regrouped for the vectorised table build: pq [M][256][dsub] ->
+// pq_t [M][dsub / vw][256][vw] (a few hundred KB at most; redone per search, it is ~2 us).
+__global__ void pq_regroup_kernel(const float* __restrict__ pq, float* __restrict__ pq_t, int M, int dsub,
+                                  int vw) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= M * 256 * dsub) return;
+  const int m = i / (256 * dsub);
+  const int rem = i - m * 256 * dsub;
+  const int c = rem / dsub, j = rem - c * dsub;
+  pq_t[((m * (dsub / vw) + j / vw) * 256 + c) * vw + (j % vw)] = pq[i];
+}
+
 struct SearchPlan {
   int G, ngroups, K;
   FlatPlan coarse;
-  size_t off_cdist, off_cids, off_W, off_work, bytes;
+  size_t off_cdist, off_cids, off_W, off_work, off_pqt, bytes;
 };
 
 SearchPlan search_plan(const fs_ivfpq* ix, int64_t nq, int nprobe, int k) {
@@ -263,8 +283,11 @@ SearchPlan search_plan(const fs_ivfpq* ix, int64_t nq, int nprobe, int k) {
   o += align_up((size_t)nq * nprobe * sizeof(int64_t), 256);
   p.off_work = o;
   o += 256;
+  p.off_pqt = o;
+  o += align_up((size_t)256 * ix->d * sizeof(float), 256);
   p.off_W = o;
-  o += align_up((size_t)nq * p.ngroups * p.K * sizeof(uint64_t), 256);
+  const int qpi = scan2_supported(ix->d, ix->M, k) ? scan2_queues_per_item() : 1;
+  o += align_up((size_t)nq * p.ngroups * qpi * p.K * sizeof(uint64_t), 256);
   p.bytes = o;
   return p;
 }
@@ -516,6 +539,14 @@ int ivfpq_search_device(fs_ivfpq* ix, const float* xq, int64_t nq, int nprobe, i
   a.xq = xq;
   a.coarse = ix->coarse.as<float>();
   a.pq = ix->pq.as<float>();
+  a.pq_t = nullptr;
+  if ((ix->M == 16 && ix->dsub == 6) || (ix->M == 8 && ix->dsub == 12)) {
+    float* pq_t = reinterpret_cast<float*>(w + p.off_pqt);
+    const int n = 256 * ix->d;
+    pq_regroup_kernel<<<ceil_div(n, 256), 256, 0, s>>>(a.pq, pq_t, ix->M, ix->dsub, ix->dsub == 6 ? 2 : 4);
+    FS_LAUNCHED();
+    a.pq_t = pq_t;
+  }
   a.probe_ids = cids;
   a.offsets = ix->offsets.as<int64_t>();
   a.codes = ix->codes.as<uint8_t>();
@@ -529,7 +560,9 @@ int ivfpq_search_device(fs_ivfpq* ix, const float* xq, int64_t nq, int nprobe, i
   a.G = p.G;
   a.ngroups = p.ngroups;
   a.k = k;
-  if (scan2_supported(ix->d, ix->M, k))
+  const bool persistent = ix->ntotal() < ((int64_t)1 << 31) && scan2_supported(ix->d, ix->M, k);  // 32-bit list lengths
+  const int qpi = persistent ? scan2_queues_per_item() : 1;
+  if (persistent)
     rc = launch_scan2(a, nq, k, reinterpret_cast<unsigned int*>(w + p.off_work), s);
   else
   switch (k_class(k)) {
@@ -542,7 +575,7 @@ int ivfpq_search_device(fs_ivfpq* ix, const float* xq, int64_t nq, int nprobe, i
   }
   if (rc != FS_OK) return rc;
   // C5
-  rc = launch_flat_finish(Wg, nq, p.ngroups, k, nullptr, out_dist, out_ids, s);
+  rc = launch_flat_finish(Wg, nq, p.ngroups * qpi, k, nullptr, out_dist, out_ids, s);
   if (rc != FS_OK) return rc;
   const size_t smem = (size_t)4 * k * (sizeof(int64_t) + sizeof(float));
   ivfpq_resolve_kernel<<<(unsigned)ceil_div(nq, 4), 128, smem, s>>>(out_dist, out_ids,
