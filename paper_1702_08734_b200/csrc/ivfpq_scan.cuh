@@ -14,6 +14,8 @@ struct ScanArgs {
   const float* coarse;
   const float* pq;
   const float* pq_t;         // pq regrouped for vector loads (ivfpq_search.cu), or NULL
+  const float* pq_r;         // pq regrouped for the rotated fixed-point kernel, or NULL
+  const float* bmax;         // [M] max_c ||B[m][c]||, or NULL
   const int64_t* probe_ids;  // [nq][nprobe], ascending coarse distance
   const int64_t* offsets;    // [nlist+1]
   const uint8_t* codes;      // [ntotal][M]
@@ -21,6 +23,8 @@ struct ScanArgs {
   unsigned long long* scanned;
   int32_t* out_probed;       // [nq][nprobe] or NULL
   int d, M, dsub, nprobe, G, ngroups, k;
+  unsigned int* work;        // zeroed counter for the kernels that hand items out dynamically
+  bool len32;                // every list is shorter than 2^31 vectors
 };
 
 // rotate the MW-word little-endian value w right by r bytes (r < 4 MW, per-lane constant)
@@ -45,16 +49,18 @@ __device__ __forceinline__ void rotate_bytes(uint32_t (&w)[MW], int r) {
   for (int i = 0; i < MW; ++i) w[i] = t[i];
 }
 
+// One code = MW words.  Streaming loads (evict-first): the codes pass through L1 once, the
+// codebook that every table build re-reads should stay there.
 template <int MW>
 __device__ __forceinline__ void load_code(const uint8_t* p, uint32_t (&w)[MW]) {
   if (MW == 2) {
-    const uint2 t = *reinterpret_cast<const uint2*>(p);
+    const uint2 t = __ldcs(reinterpret_cast<const uint2*>(p));
     w[0] = t.x;
     w[1] = t.y;
   } else {
 #pragma unroll
     for (int i = 0; i < MW / 4; ++i) {
-      const uint4 t = reinterpret_cast<const uint4*>(p)[i];
+      const uint4 t = __ldcs(reinterpret_cast<const uint4*>(p) + i);
       w[4 * i] = t.x;
       w[4 * i + 1] = t.y;
       w[4 * i + 2] = t.z;

@@ -247,22 +247,42 @@ __global__ void __launch_bounds__(128)
   }
 }
 
-// The codebook regrouped for the vectorised table build: pq [M][256][dsub] ->
-// pq_t [M][dsub / vw][256][vw] (a few hundred KB at most; redone per search, it is ~2 us).
-__global__ void pq_regroup_kernel(const float* __restrict__ pq, float* __restrict__ pq_t, int M, int dsub,
-                                  int vw) {
+// The codebook regrouped for the vectorised table builds (a few hundred KB at most; redone per
+// search, it is ~2 us):
+//   pq_t [M][dsub / vw][256][vw]            thread c builds entry c of every table (float kernel)
+//   pq_r [256 / REP][dsub / vw][32][vw]     lane l = cofs * M + m builds entry (m, c0 + cofs) (rot kernel)
+//   bmax [M]                                max_c ||B[m][c]|| (bound of the fixed-point scale)
+__global__ void pq_regroup_kernel(const float* __restrict__ pq, float* __restrict__ pq_t, float* __restrict__ pq_r,
+                                  int M, int dsub, int vw) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= M * 256 * dsub) return;
   const int m = i / (256 * dsub);
   const int rem = i - m * 256 * dsub;
   const int c = rem / dsub, j = rem - c * dsub;
-  pq_t[((m * (dsub / vw) + j / vw) * 256 + c) * vw + (j % vw)] = pq[i];
+  const int nv = dsub / vw, rep = 32 / M;
+  pq_t[((m * nv + j / vw) * 256 + c) * vw + (j % vw)] = pq[i];
+  pq_r[(((c / rep) * nv + j / vw) * 32 + (c % rep) * M + m) * vw + (j % vw)] = pq[i];
+}
+
+__global__ void pq_bmax_kernel(const float* __restrict__ pq, float* __restrict__ bmax, int dsub) {
+  const int m = blockIdx.x, lane = threadIdx.x;  // one warp per sub-quantizer
+  float mx = 0.f;
+  for (int c = lane; c < 256; c += 32) {
+    float n = 0.f;
+    for (int j = 0; j < dsub; ++j) {
+      const float v = pq[((int64_t)m * 256 + c) * dsub + j];
+      n = fmaf(v, v, n);
+    }
+    mx = fmaxf(mx, n);
+  }
+  for (int sft = 16; sft >= 1; sft >>= 1) mx = fmaxf(mx, __shfl_xor_sync(kFull, mx, sft));
+  if (lane == 0) bmax[m] = sqrtf(mx);
 }
 
 struct SearchPlan {
   int G, ngroups, K;
   FlatPlan coarse;
-  size_t off_cdist, off_cids, off_W, off_work, off_pqt, bytes;
+  size_t off_cdist, off_cids, off_W, off_work, off_pqt, off_pqr, bytes;
 };
 
 SearchPlan search_plan(const fs_ivfpq* ix, int64_t nq, int nprobe, int k) {
@@ -285,6 +305,8 @@ SearchPlan search_plan(const fs_ivfpq* ix, int64_t nq, int nprobe, int k) {
   o += 256;
   p.off_pqt = o;
   o += align_up((size_t)256 * ix->d * sizeof(float), 256);
+  p.off_pqr = o;
+  o += align_up((size_t)256 * ix->d * sizeof(float), 256) + 256;  // + bmax[M]
   p.off_W = o;
   const int qpi = scan2_supported(ix->d, ix->M, k) ? scan2_queues_per_item() : 1;
   o += align_up((size_t)nq * p.ngroups * qpi * p.K * sizeof(uint64_t), 256);
@@ -293,34 +315,45 @@ SearchPlan search_plan(const fs_ivfpq* ix, int64_t nq, int nprobe, int k) {
 }
 
 // ---------------------------------------------------------------------------
-// M = 8 or 16: the same scan with a bank-conflict-free gather.
+// M = 8 or 16, dsub = 6 or 12: the same scan with a bank-conflict-free gather (FS_IVFPQ_SCAN=rot).
 //   * the table is stored as lut[c][b], b = 0..31: word (c, b) lives in shared-memory bank b and
 //     holds T_{b mod M}[c] (32 / M replicas of every table); lane l adds its sub-quantizers in
 //     the rotated order m = (s + l) mod M, so at step s the 32 lanes read 32 different banks;
 //     lane l rotates its code by l mod M bytes once per vector (funnel shifts);
-//   * so that the rotated order cannot change the sum, the entries are FIXED-POINT: the CTA
-//     scales every table of the (query, list) pair by one power of two such that the largest
-//     entry is < 2^27, rounds to integers, and the scan adds integers (exact, associative).
-//     Identical codes therefore give identical distances whatever lane scans them (reading
-//     C-6).  Quantisation: <= 2^-28 of the largest table entry per entry, M times that per
-//     distance -- far inside the 1e-3 relative tolerance for every distance that is not
-//     ~5 orders of magnitude below the largest entry of its tables.
-// Shared memory: r[d] | Tn[M][257] | lut[256][32] | red[8] | select batches | merge area
+//   * so that the rotated order cannot change the sum, the entries are FIXED-POINT: one power-of-two
+//     scale per (query, list) pair, from the bound (||r^m|| + max_c ||B[m][c]||)^2 >= every entry of
+//     T_m, makes every entry an integer < 2^27; the scan adds integers (exact, associative), so
+//     identical codes give identical distances whatever lane scans them (reading C-6).
+//     Quantisation: <= 2^-27 of the bound per entry, M times that per distance;
+//   * build: lane l of a warp computes entry (m = l mod M, c = c0 + l / M) from a codebook that
+//     pq_regroup_kernel lays out so that the warp's loads are 32 consecutive 8 / 16-byte pieces,
+//     and stores its 32 / M replicas in rotated replica order: loads coalesced, stores conflict-free.
+// Shared memory: lut[256][32] | r[d] | select batches | merge area
 // ---------------------------------------------------------------------------
-template <int NQ, int M>
-__global__ void __launch_bounds__(SCAN_THREADS) ivfpq_scan_rot_kernel(const ScanArgs a) {
+template <int s, int M>
+__device__ __forceinline__ void rot_gather(const uint32_t* w, const uint32_t* base, uint32_t& acc) {
+  if constexpr (s < M) {
+    const uint32_t c = __byte_perm(w[s >> 2], 0u, 0x4440u + (s & 3));  // byte s, zero-extended
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(base[s] + c * 128u));
+    acc += v;
+    rot_gather<s + 1, M>(w, base, acc);
+  }
+}
+
+template <int NQ, int M, int DS>
+__global__ void __launch_bounds__(SCAN_THREADS, 3) ivfpq_scan_rot_kernel(const ScanArgs a) {
   extern __shared__ __align__(1024) unsigned char scan_smem[];
   constexpr int K = 32 * NQ;
   constexpr int NB = 2;
   constexpr int MW = M / 4;
   constexpr int REP = 32 / M;
-  constexpr int TS = 257;  // row stride of the natural table: conflict-free reads by m
-  const int d = a.d, dsub = a.dsub;
-  float* r = reinterpret_cast<float*>(scan_smem);
-  float* Tn = r + ((d + 3) & ~3);
-  uint32_t* lut = reinterpret_cast<uint32_t*>(Tn + ((M * TS + 3) & ~3));
-  float* red = reinterpret_cast<float*>(lut + 256 * 32);
-  uint64_t* bufs = reinterpret_cast<uint64_t*>(red + 8);
+  constexpr int VW = DS == 6 ? 2 : 4;
+  constexpr int NV = DS / VW;
+  const int d = a.d;
+  uint32_t* lut = reinterpret_cast<uint32_t*>(scan_smem);
+  float* r = reinterpret_cast<float*>(lut + 256 * 32);
+  uint64_t* bufs = reinterpret_cast<uint64_t*>(r + ((d + 3) & ~3));
   uint64_t* merge = bufs + SCAN_WARPS * warp_select_smem_keys<NB>();
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int64_t q = blockIdx.x / a.ngroups;
@@ -331,103 +364,98 @@ __global__ void __launch_bounds__(SCAN_THREADS) ivfpq_scan_rot_kernel(const Scan
   WarpSelect<NQ, NB> sel;
   sel.init(bufs + warp * warp_select_smem_keys<NB>(), lane);
   unsigned long long bytes = 0;
+  __shared__ uint32_t cta_bound;
+  if (tid == 0) cta_bound = 0x7F800000u;
   const int rot = lane % M;
+  const int my_m = lane % M, cofs = lane / M;
+  const float my_bmax = a.bmax[my_m];
+  const uint32_t lutb = (uint32_t)__cvta_generic_to_shared(lut);
+  uint32_t base[M];
+#pragma unroll
+  for (int s = 0; s < M; ++s) base[s] = lutb + (((lane + s) & 31) << 2);
 
   for (int p = p_begin; p < p_end; ++p) {
     const int64_t L = a.probe_ids[q * a.nprobe + p];
     if (a.out_probed && tid == 0) a.out_probed[q * a.nprobe + p] = (int32_t)L;
     if (L < 0) continue;
     const int64_t lb = a.offsets[L], le = a.offsets[L + 1];
-    const int64_t len = le - lb;
-    if (len == 0) continue;  // empty lists are probed and contribute nothing
-    __syncthreads();         // previous list's tables are no longer read
+    const int64_t len64 = le - lb;
+    if (len64 == 0) continue;  // empty lists are probed and contribute nothing
+    const int len = (int)len64;  // the caller routes indexes of 2^31 vectors or more to the float kernel
+    __syncthreads();             // previous list's table is no longer read
+    const uint8_t* cl = a.codes + lb * M;
+    uint32_t nxt[MW] = {};
+    if (tid < len) load_code<MW>(cl + (size_t)tid * M, nxt);
     for (int j = tid; j < d; j += SCAN_THREADS) r[j] = a.xq[q * d + j] - a.coarse[L * d + j];
     __syncthreads();
-    // C2, step 1: T_m[c] = ||r^m - B[m][c]||^2 (Eq. 10) in the natural layout, and its maximum
-    float mx = 0.f;
-    for (int e = tid; e < M * 256; e += SCAN_THREADS) {
-      const int m = e >> 8;
-      const float* b = a.pq + (int64_t)e * dsub;
-      const float* rm = r + m * dsub;
-      float acc = 0.f;
-      if (dsub == 6) {
-        const float2* b2 = reinterpret_cast<const float2*>(b);
+    // C2: scale from the bound, then the fixed-point table (Eq. 10)
+    float rm[DS];
+    float n = 0.f;
 #pragma unroll
-        for (int j = 0; j < 3; ++j) {
-          const float2 bb = __ldg(b2 + j);
-          const float t0 = rm[2 * j] - bb.x, t1 = rm[2 * j + 1] - bb.y;
-          acc = fmaf(t0, t0, acc);
-          acc = fmaf(t1, t1, acc);
-        }
-      } else if (dsub == 12) {
-        const float4* b4 = reinterpret_cast<const float4*>(b);
-#pragma unroll
-        for (int j = 0; j < 3; ++j) {
-          const float4 bb = __ldg(b4 + j);
-          const float t0 = rm[4 * j] - bb.x, t1 = rm[4 * j + 1] - bb.y, t2 = rm[4 * j + 2] - bb.z,
-                      t3 = rm[4 * j + 3] - bb.w;
-          acc = fmaf(t0, t0, acc);
-          acc = fmaf(t1, t1, acc);
-          acc = fmaf(t2, t2, acc);
-          acc = fmaf(t3, t3, acc);
-        }
-      } else {
-        for (int j = 0; j < dsub; ++j) {
-          const float t = rm[j] - b[j];
-          acc = fmaf(t, t, acc);
-        }
-      }
-      Tn[m * TS + (e & 255)] = acc;
-      mx = fmaxf(mx, acc);
+    for (int j = 0; j < DS; ++j) {
+      rm[j] = r[my_m * DS + j];
+      n = fmaf(rm[j], rm[j], n);
     }
+    float u = sqrtf(n) + my_bmax;
+    u = u * u * 1.001f;  // >= every entry of T_m as the float code below computes it
 #pragma unroll
-    for (int sft = 16; sft >= 1; sft >>= 1) mx = fmaxf(mx, __shfl_xor_sync(kFull, mx, sft));
-    if (lane == 0) red[warp] = mx;
-    __syncthreads();
-    // C2, step 2: one power-of-two scale for the pair, integer entries into the banked layout
-    mx = red[0];
-#pragma unroll
-    for (int w = 1; w < SCAN_WARPS; ++w) mx = fmaxf(mx, red[w]);
+    for (int sft = 16; sft >= 1; sft >>= 1) u = fmaxf(u, __shfl_xor_sync(kFull, u, sft));
     int ex = 0;
-    if (mx > 0.f && mx < 3.0e38f) frexpf(mx, &ex);  // mx < 2^ex
-    int se = 27 - ex;                               // scale = 2^se: scaled entries < 2^27
+    if (u > 0.f && u < 3.0e38f) frexpf(u, &ex);  // u < 2^ex
+    int se = 27 - ex;                            // scaled entries < 2^27
     se = se > 100 ? 100 : (se < -100 ? -100 : se);
     const float scale = __uint_as_float((uint32_t)(127 + se) << 23);
     const float inv_scale = __uint_as_float((uint32_t)(127 - se) << 23);
-    {
-      const int m = lane % M, cofs = lane / M;
-      for (int c0 = warp * REP; c0 < 256; c0 += SCAN_WARPS * REP) {
-        const int c = c0 + cofs;
-        const uint32_t v = __float2uint_rn(Tn[m * TS + c] * scale);
+#pragma unroll 2
+    for (int c0 = warp * REP; c0 < 256; c0 += SCAN_WARPS * REP) {
+      const int c = c0 + cofs;
+      float t = 0.f;
 #pragma unroll
-        for (int rep = 0; rep < REP; ++rep) lut[c * 32 + m + rep * M] = v;
+      for (int jv = 0; jv < NV; ++jv) {
+        float bv[VW];
+        if (VW == 2) {
+          const float2 x = __ldg(reinterpret_cast<const float2*>(a.pq_r) + ((c0 / REP) * NV + jv) * 32 + lane);
+          bv[0] = x.x; bv[1] = x.y;
+        } else {
+          const float4 x = __ldg(reinterpret_cast<const float4*>(a.pq_r) + ((c0 / REP) * NV + jv) * 32 + lane);
+          bv[0] = x.x; bv[1] = x.y; bv[VW - 2] = x.z; bv[VW - 1] = x.w;
+        }
+#pragma unroll
+        for (int i = 0; i < VW; ++i) {
+          const float df = rm[jv * VW + i] - bv[i];
+          t = fmaf(df, df, t);
+        }
       }
+      const uint32_t v = __float2uint_rn(t * scale);
+      // replica (rep + cofs) mod REP at store rep: the 32 lanes write 32 different banks
+#pragma unroll
+      for (int rep = 0; rep < REP; ++rep) lut[c * 32 + my_m + ((rep + cofs) % REP) * M] = v;
     }
     __syncthreads();
     // C3 + C4: scan and select
     bytes += (unsigned long long)len * M;
-    const uint8_t* cl = a.codes + lb * M;
-    const char* lutb = reinterpret_cast<const char*>(lut);
-    for (int64_t v0 = 0; v0 < len; v0 += SCAN_THREADS) {
-      const int64_t v = v0 + tid;
+    const uint32_t pos0 = (uint32_t)lb;
+    for (int v0 = 0; v0 < len; v0 += SCAN_THREADS) {
+      const int v = v0 + tid;
       const bool ok = v < len;
+      uint32_t w[MW];
+#pragma unroll
+      for (int i = 0; i < MW; ++i) w[i] = nxt[i];
+      if (v + SCAN_THREADS < len) load_code<MW>(cl + (size_t)(uint32_t)(v + SCAN_THREADS) * M, nxt);
       float dist = 0.f;
       if (ok) {
-        uint32_t w[MW];
-        load_code<MW>(cl + v * M, w);
         rotate_bytes<MW>(w, rot);
         uint32_t acc = 0u;
-#pragma unroll
-        for (int s2 = 0; s2 < M; ++s2) {
-          const uint32_t c = (w[s2 >> 2] >> (8 * (s2 & 3))) & 255u;
-          acc += *reinterpret_cast<const uint32_t*>(lutb + c * 128 + (((s2 + lane) & 31) << 2));
-        }
+        rot_gather<0, M>(w, base, acc);
         dist = (float)acc * inv_scale;
       }
-      const bool cand = ok && sel.maybe(dist);
+      const float bound = fminf(sel.thr_val, __uint_as_float(*reinterpret_cast<volatile uint32_t*>(&cta_bound)));
+      const bool cand = ok && !(dist > bound);
       if (__any_sync(kFull, cand)) {
-        const uint64_t key = make_key(dist, (uint32_t)(lb + v));
+        const uint64_t key = make_key(dist, pos0 + (uint32_t)v);
+        const uint64_t thr_before = sel.thr;
         sel.push(cand && sel.wants(key), key);
+        if (sel.thr != thr_before && lane == 0) atomicMin(&cta_bound, __float_as_uint(sel.thr_val));
       }
     }
   }
@@ -451,23 +479,214 @@ __global__ void __launch_bounds__(SCAN_THREADS) ivfpq_scan_rot_kernel(const Scan
   }
 }
 
-template <int NQ, int M>
+// ---------------------------------------------------------------------------
+// The same fixed-point scan, persistent (FS_IVFPQ_SCAN=grp): one CTA of GRP_N groups of 8 warps per
+// SM.  The regrouped codebook (pq_r, 256 d floats) is resident in shared memory, shared by the
+// groups; every group owns one table and walks its own (query, list group) items, handed out by
+// an atomic counter, synchronising with a named barrier: the groups overlap each other's table
+// builds and scans like independent CTAs would, but no table build reads global memory.
+// Shared memory: cb[256 d] | per group: lut[256][32] (merge area aliases it) | r[d] | select batches
+// ---------------------------------------------------------------------------
+constexpr int GRP_N = 3;
+constexpr int GRP_THREADS = SCAN_THREADS * GRP_N;
+
+__device__ __forceinline__ void group_sync(int gid) {
+  asm volatile("bar.sync %0, %1;" ::"r"(gid + 1), "n"(SCAN_THREADS) : "memory");
+}
+
+template <int NQ, int M, int DS>
+__global__ void __launch_bounds__(GRP_THREADS, 1) ivfpq_scan_grp_kernel(const ScanArgs a, unsigned int* __restrict__ work,
+                                                                         int64_t n_items) {
+  extern __shared__ __align__(1024) unsigned char scan_smem[];
+  constexpr int K = 32 * NQ;
+  constexpr int NB = 2;
+  constexpr int MW = M / 4;
+  constexpr int REP = 32 / M;
+  constexpr int VW = DS == 6 ? 2 : 4;
+  constexpr int NV = DS / VW;
+  static_assert(SCAN_WARPS * K * 8 <= 256 * 32 * 4, "merge area must fit the table it aliases");
+  const int d = a.d, dpad = (d + 3) & ~3;
+  const int gid = threadIdx.x / SCAN_THREADS, tid = threadIdx.x % SCAN_THREADS, lane = tid & 31, warp = tid >> 5;
+  float* cb = reinterpret_cast<float*>(scan_smem);  // pq_r, as laid out by pq_regroup_kernel
+  const size_t grp_bytes = (size_t)256 * 32 * 4 + (size_t)dpad * 4 + (size_t)SCAN_WARPS * warp_select_smem_keys<NB>() * 8;
+  unsigned char* gbase = scan_smem + (size_t)256 * d * 4 + gid * grp_bytes;
+  uint32_t* lut = reinterpret_cast<uint32_t*>(gbase);
+  float* r = reinterpret_cast<float*>(lut + 256 * 32);
+  uint64_t* bufs = reinterpret_cast<uint64_t*>(r + dpad);
+  uint64_t* merge = reinterpret_cast<uint64_t*>(lut);  // the table is dead when the queues are merged
+  __shared__ uint32_t grp_bound[GRP_N];
+  __shared__ int grp_item[GRP_N];
+
+  for (int i = threadIdx.x; i < 256 * d / 4; i += GRP_THREADS)
+    reinterpret_cast<float4*>(cb)[i] = __ldg(reinterpret_cast<const float4*>(a.pq_r) + i);
+  __syncthreads();
+
+  WarpSelect<NQ, NB> sel;
+  sel.init(bufs + warp * warp_select_smem_keys<NB>(), lane);
+  unsigned long long bytes = 0;
+  const int rot = lane % M;
+  const int my_m = lane % M, cofs = lane / M;
+  const float my_bmax = a.bmax[my_m];
+  const uint32_t lutb = (uint32_t)__cvta_generic_to_shared(lut);
+  uint32_t base[M];
+#pragma unroll
+  for (int s = 0; s < M; ++s) base[s] = lutb + (((lane + s) & 31) << 2);
+
+  while (true) {
+    group_sync(gid);  // the previous item's merge is done with the table / merge area
+    if (tid == 0) {
+      grp_item[gid] = (int)atomicAdd(work, 1u);
+      grp_bound[gid] = 0x7F800000u;
+    }
+    group_sync(gid);
+    const int64_t item = grp_item[gid];
+    if (item >= n_items) break;
+    const int64_t q = item / a.ngroups;
+    const int g = (int)(item - q * a.ngroups);
+    const int p_begin = g * a.G;
+    const int p_end = (p_begin + a.G) < a.nprobe ? (p_begin + a.G) : a.nprobe;
+    sel.reset();
+
+    for (int p = p_begin; p < p_end; ++p) {
+      const int64_t L = a.probe_ids[q * a.nprobe + p];
+      if (a.out_probed && tid == 0) a.out_probed[q * a.nprobe + p] = (int32_t)L;
+      if (L < 0) continue;
+      const int64_t lb = a.offsets[L], le = a.offsets[L + 1];
+      if (le == lb) continue;  // empty lists are probed and contribute nothing
+      const int len = (int)(le - lb);
+      group_sync(gid);  // previous list's table is no longer read
+      const uint8_t* cl = a.codes + lb * M;
+      uint32_t nxt[MW] = {};
+      if (tid < len) load_code<MW>(cl + (size_t)tid * M, nxt);
+      for (int j = tid; j < d; j += SCAN_THREADS) r[j] = a.xq[q * d + j] - a.coarse[L * d + j];
+      group_sync(gid);
+      // C2: scale from the bound, then the fixed-point table (Eq. 10)
+      float rm[DS];
+      float n = 0.f;
+#pragma unroll
+      for (int j = 0; j < DS; ++j) {
+        rm[j] = r[my_m * DS + j];
+        n = fmaf(rm[j], rm[j], n);
+      }
+      float u = sqrtf(n) + my_bmax;
+      u = u * u * 1.001f;  // >= every entry of T_m as the float code below computes it
+#pragma unroll
+      for (int sft = 16; sft >= 1; sft >>= 1) u = fmaxf(u, __shfl_xor_sync(kFull, u, sft));
+      int ex = 0;
+      if (u > 0.f && u < 3.0e38f) frexpf(u, &ex);  // u < 2^ex
+      int se = 27 - ex;                            // scaled entries < 2^27
+      se = se > 100 ? 100 : (se < -100 ? -100 : se);
+      const float scale = __uint_as_float((uint32_t)(127 + se) << 23);
+      const float inv_scale = __uint_as_float((uint32_t)(127 - se) << 23);
+#pragma unroll 4
+      for (int c0 = warp * REP; c0 < 256; c0 += SCAN_WARPS * REP) {
+        const int c = c0 + cofs;
+        float t = 0.f;
+#pragma unroll
+        for (int jv = 0; jv < NV; ++jv) {
+          float bv[VW];
+          if (VW == 2) {
+            const float2 x = reinterpret_cast<const float2*>(cb)[((c0 / REP) * NV + jv) * 32 + lane];
+            bv[0] = x.x; bv[1] = x.y;
+          } else {
+            const float4 x = reinterpret_cast<const float4*>(cb)[((c0 / REP) * NV + jv) * 32 + lane];
+            bv[0] = x.x; bv[1] = x.y; bv[VW - 2] = x.z; bv[VW - 1] = x.w;
+          }
+#pragma unroll
+          for (int i = 0; i < VW; ++i) {
+            const float df = rm[jv * VW + i] - bv[i];
+            t = fmaf(df, df, t);
+          }
+        }
+        const uint32_t v = __float2uint_rn(t * scale);
+#pragma unroll
+        for (int rep = 0; rep < REP; ++rep) lut[c * 32 + my_m + ((rep + cofs) % REP) * M] = v;
+      }
+      group_sync(gid);
+      // C3 + C4: scan and select
+      if (tid == 0) bytes += (unsigned long long)len * M;
+      const uint32_t pos0 = (uint32_t)lb;
+      for (int v0 = 0; v0 < len; v0 += SCAN_THREADS) {
+        const int v = v0 + tid;
+        const bool ok = v < len;
+        uint32_t w[MW];
+#pragma unroll
+        for (int i = 0; i < MW; ++i) w[i] = nxt[i];
+        if (v + SCAN_THREADS < len) load_code<MW>(cl + (size_t)(uint32_t)(v + SCAN_THREADS) * M, nxt);
+        float dist = 0.f;
+        if (ok) {
+          rotate_bytes<MW>(w, rot);
+          uint32_t acc = 0u;
+          rot_gather<0, M>(w, base, acc);
+          dist = (float)acc * inv_scale;
+        }
+        const float bound = fminf(sel.thr_val, __uint_as_float(*reinterpret_cast<volatile uint32_t*>(grp_bound + gid)));
+        const bool cand = ok && !(dist > bound);
+        if (__any_sync(kFull, cand)) {
+          const uint64_t key = make_key(dist, pos0 + (uint32_t)v);
+          const uint64_t thr_before = sel.thr;
+          sel.push(cand && sel.wants(key), key);
+          if (sel.thr != thr_before && lane == 0) atomicMin(grp_bound + gid, __float_as_uint(sel.thr_val));
+        }
+      }
+    }
+    sel.finish();
+    group_sync(gid);  // every warp is done with the table: the merge area takes its place
+#pragma unroll
+    for (int rr = 0; rr < NQ; ++rr) merge[warp * K + rr * 32 + lane] = sel.W[rr];
+    group_sync(gid);
+    if (warp == 0) {
+      sel.reset();
+      for (int e0 = 0; e0 < SCAN_WARPS * K; e0 += 32) {
+        const uint64_t key = merge[e0 + lane];
+        sel.push(key < sel.thr, key);
+      }
+      sel.finish();
+      uint64_t* W = a.Wg + item * K;
+#pragma unroll
+      for (int rr = 0; rr < NQ; ++rr) W[rr * 32 + lane] = sel.W[rr];
+    }
+  }
+  if (tid == 0 && bytes) atomicAdd(a.scanned, bytes);
+}
+
+template <int NQ, int M, int DS>
+int launch_scan_grp(const ScanArgs& a, int64_t nq, unsigned int* work, cudaStream_t s) {
+  const size_t grp_bytes = (size_t)256 * 32 * 4 + (size_t)((a.d + 3) & ~3) * 4 +
+                           (size_t)SCAN_WARPS * warp_select_smem_keys<2>() * 8;
+  const size_t smem = (size_t)256 * a.d * 4 + GRP_N * grp_bytes;
+  if (smem > 227 * 1024) return set_error(FS_EUNSUPPORTED, "fs_ivfpq_search: shared memory (%zu B) exceeds 227 KB", smem);
+  static size_t attr_smem = 0;
+  if (smem > attr_smem) {
+    FS_CUDA(cudaFuncSetAttribute(ivfpq_scan_grp_kernel<NQ, M, DS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    attr_smem = smem;
+  }
+  const int64_t n_items = nq * a.ngroups;
+  int64_t grid = sm_count();
+  if (grid * GRP_N > n_items) grid = ceil_div(n_items, (int64_t)GRP_N);
+  FS_CUDA(cudaMemsetAsync(work, 0, sizeof(unsigned int), s));
+  ivfpq_scan_grp_kernel<NQ, M, DS><<<(unsigned)grid, GRP_THREADS, smem, s>>>(a, work, n_items);
+  FS_LAUNCHED();
+  return FS_OK;
+}
+
+template <int NQ, int M, int DS>
 int launch_scan_rot(const ScanArgs& a, int64_t nq, cudaStream_t s) {
   constexpr int K = 32 * NQ;
-  const size_t smem = (size_t)(((a.d + 3) & ~3) + ((M * 257 + 3) & ~3) + 256 * 32 + 8) * sizeof(float) +
+  const size_t smem = (size_t)(256 * 32 + ((a.d + 3) & ~3)) * sizeof(float) +
                       (size_t)(SCAN_WARPS * warp_select_smem_keys<2>() + SCAN_WARPS * K) * sizeof(uint64_t);
   if (smem > 227 * 1024) return set_error(FS_EUNSUPPORTED, "fs_ivfpq_search: shared memory (%zu B) exceeds 227 KB", smem);
   static size_t attr_smem = 0;
   if (smem > attr_smem) {
-    FS_CUDA(cudaFuncSetAttribute(ivfpq_scan_rot_kernel<NQ, M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    FS_CUDA(cudaFuncSetAttribute(ivfpq_scan_rot_kernel<NQ, M, DS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const char* e = getenv("FS_IVFPQ_CARVEOUT");
-    FS_CUDA(cudaFuncSetAttribute(ivfpq_scan_rot_kernel<NQ, M>, cudaFuncAttributePreferredSharedMemoryCarveout,
-                                 e ? atoi(e) : 100));
+    FS_CUDA(cudaFuncSetAttribute(ivfpq_scan_rot_kernel<NQ, M, DS>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                                 e ? atoi(e) : 60));
     attr_smem = smem;
   }
   const int64_t grid = nq * a.ngroups;
   if (grid > 0x7fffffffLL) return set_error(FS_EUNSUPPORTED, "fs_ivfpq_search: nq * groups too large");
-  ivfpq_scan_rot_kernel<NQ, M><<<(unsigned)grid, SCAN_THREADS, smem, s>>>(a);
+  ivfpq_scan_rot_kernel<NQ, M, DS><<<(unsigned)grid, SCAN_THREADS, smem, s>>>(a);
   FS_LAUNCHED();
   return FS_OK;
 }
@@ -498,15 +717,20 @@ int launch_scan_m(const ScanArgs& a, int64_t nq, cudaStream_t s) {
 
 template <int NQ>
 int launch_scan(const ScanArgs& a, int64_t nq, cudaStream_t s) {
-  // FS_IVFPQ_SCAN=rot selects the bank-conflict-free fixed-point kernel (A/B runs): correct, but
-  // its second table pass and larger footprint cost more than the conflicts (profiles/r01_ivfpq.md)
-  static int plain = -1;
-  if (plain < 0) {
+  // FS_IVFPQ_SCAN = pair (float tables, one CTA per item) | rot (fixed-point conflict-free tables, one
+  // CTA per item) | grp (the same, persistent groups with the codebook resident): A/B runs
+  static int mode = -1;
+  if (mode < 0) {
     const char* e = getenv("FS_IVFPQ_SCAN");
-    plain = (e && strcmp(e, "rot") == 0) ? 0 : 1;
+    mode = (e && strcmp(e, "rot") == 0) ? 1 : (e && strcmp(e, "grp") == 0) ? 2 : 0;
   }
-  if (!plain && NQ <= 8 && a.M == 16) return launch_scan_rot<NQ, 16>(a, nq, s);
-  if (!plain && NQ <= 8 && a.M == 8) return launch_scan_rot<NQ, 8>(a, nq, s);
+  if constexpr (NQ <= 8) {
+    const bool fx = a.len32 && a.pq_r;
+    if (mode == 2 && fx && a.M == 16 && a.dsub == 6) return launch_scan_grp<NQ, 16, 6>(a, nq, a.work, s);
+    if (mode == 2 && fx && a.M == 8 && a.dsub == 12) return launch_scan_grp<NQ, 8, 12>(a, nq, a.work, s);
+    if (mode == 1 && fx && a.M == 16 && a.dsub == 6) return launch_scan_rot<NQ, 16, 6>(a, nq, s);
+    if (mode == 1 && fx && a.M == 8 && a.dsub == 12) return launch_scan_rot<NQ, 8, 12>(a, nq, s);
+  }
   if (a.M == 16 && a.dsub == 6) return launch_scan_m<NQ, 16, 6>(a, nq, s);
   if (a.M == 8 && a.dsub == 12) return launch_scan_m<NQ, 8, 12>(a, nq, s);
   if (a.M == 16) return launch_scan_m<NQ, 16, 0>(a, nq, s);
@@ -539,13 +763,23 @@ int ivfpq_search_device(fs_ivfpq* ix, const float* xq, int64_t nq, int nprobe, i
   a.xq = xq;
   a.coarse = ix->coarse.as<float>();
   a.pq = ix->pq.as<float>();
+  a.len32 = ix->ntotal() < ((int64_t)1 << 31);
+  a.work = reinterpret_cast<unsigned int*>(w + p.off_work);
   a.pq_t = nullptr;
+  a.pq_r = nullptr;
+  a.bmax = nullptr;
   if ((ix->M == 16 && ix->dsub == 6) || (ix->M == 8 && ix->dsub == 12)) {
     float* pq_t = reinterpret_cast<float*>(w + p.off_pqt);
+    float* pq_r = reinterpret_cast<float*>(w + p.off_pqr);
+    float* bmax = pq_r + (size_t)256 * ix->d;
     const int n = 256 * ix->d;
-    pq_regroup_kernel<<<ceil_div(n, 256), 256, 0, s>>>(a.pq, pq_t, ix->M, ix->dsub, ix->dsub == 6 ? 2 : 4);
+    pq_regroup_kernel<<<ceil_div(n, 256), 256, 0, s>>>(a.pq, pq_t, pq_r, ix->M, ix->dsub, ix->dsub == 6 ? 2 : 4);
+    FS_LAUNCHED();
+    pq_bmax_kernel<<<ix->M, 32, 0, s>>>(a.pq, bmax, ix->dsub);
     FS_LAUNCHED();
     a.pq_t = pq_t;
+    a.pq_r = pq_r;
+    a.bmax = bmax;
   }
   a.probe_ids = cids;
   a.offsets = ix->offsets.as<int64_t>();
