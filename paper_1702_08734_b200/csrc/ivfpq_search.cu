@@ -435,8 +435,8 @@ __global__ void __launch_bounds__(SCAN_THREADS, 3) ivfpq_scan_rot_kernel(const S
     // C3 + C4: scan and select
     bytes += (unsigned long long)len * M;
     const uint32_t pos0 = (uint32_t)lb;
-    for (int v0 = 0; v0 < len; v0 += SCAN_THREADS) {
-      const int v = v0 + tid;
+    for (int v0 = warp * 32; v0 < len; v0 += SCAN_THREADS) {  // a warp stops after its last 32 vectors
+      const int v = v0 + lane;
       const bool ok = v < len;
       uint32_t w[MW];
 #pragma unroll
@@ -547,18 +547,37 @@ __global__ void __launch_bounds__(GRP_THREADS, 1) ivfpq_scan_grp_kernel(const Sc
     const int p_end = (p_begin + a.G) < a.nprobe ? (p_begin + a.G) : a.nprobe;
     sel.reset();
 
+    // The dependent loads of a list (probe id -> list bounds, centroid) are issued one and two
+    // lists ahead and stay in registers: none of their latency is on the path.
+    const float xj = tid < d ? a.xq[q * d + tid] : 0.f;
+    const int64_t* pid = a.probe_ids + q * a.nprobe;
+    int64_t L1 = pid[p_begin];                                // list of the coming iteration
+    int64_t L2 = p_begin + 1 < p_end ? pid[p_begin + 1] : -1;  // and of the one after
+    int64_t lb1 = 0, le1 = 0;
+    float c1 = 0.f;
+    if (L1 >= 0) {
+      lb1 = a.offsets[L1];
+      le1 = a.offsets[L1 + 1];
+      if (tid < d) c1 = a.coarse[L1 * d + tid];
+    }
     for (int p = p_begin; p < p_end; ++p) {
-      const int64_t L = a.probe_ids[q * a.nprobe + p];
+      const int64_t L = L1, lb = lb1, le = le1;
+      const float cj = c1;
+      L1 = L2;
+      if (L1 >= 0) {
+        lb1 = a.offsets[L1];
+        le1 = a.offsets[L1 + 1];
+        if (tid < d) c1 = a.coarse[L1 * d + tid];
+      }
+      L2 = p + 2 < p_end ? pid[p + 2] : -1;
       if (a.out_probed && tid == 0) a.out_probed[q * a.nprobe + p] = (int32_t)L;
-      if (L < 0) continue;
-      const int64_t lb = a.offsets[L], le = a.offsets[L + 1];
-      if (le == lb) continue;  // empty lists are probed and contribute nothing
+      if (L < 0 || le == lb) continue;  // empty lists are probed and contribute nothing
       const int len = (int)(le - lb);
       group_sync(gid);  // previous list's table is no longer read
       const uint8_t* cl = a.codes + lb * M;
       uint32_t nxt[MW] = {};
       if (tid < len) load_code<MW>(cl + (size_t)tid * M, nxt);
-      for (int j = tid; j < d; j += SCAN_THREADS) r[j] = a.xq[q * d + j] - a.coarse[L * d + j];
+      if (tid < d) r[tid] = xj - cj;
       group_sync(gid);
       // C2: scale from the bound, then the fixed-point table (Eq. 10)
       float rm[DS];
@@ -606,8 +625,8 @@ __global__ void __launch_bounds__(GRP_THREADS, 1) ivfpq_scan_grp_kernel(const Sc
       // C3 + C4: scan and select
       if (tid == 0) bytes += (unsigned long long)len * M;
       const uint32_t pos0 = (uint32_t)lb;
-      for (int v0 = 0; v0 < len; v0 += SCAN_THREADS) {
-        const int v = v0 + tid;
+      for (int v0 = warp * 32; v0 < len; v0 += SCAN_THREADS) {  // a warp stops after its last 32 vectors
+        const int v = v0 + lane;
         const bool ok = v < len;
         uint32_t w[MW];
 #pragma unroll
@@ -717,17 +736,21 @@ int launch_scan_m(const ScanArgs& a, int64_t nq, cudaStream_t s) {
 
 template <int NQ>
 int launch_scan(const ScanArgs& a, int64_t nq, cudaStream_t s) {
-  // FS_IVFPQ_SCAN = pair (float tables, one CTA per item) | rot (fixed-point conflict-free tables, one
-  // CTA per item) | grp (the same, persistent groups with the codebook resident): A/B runs
-  static int mode = -1;
-  if (mode < 0) {
+  // Three scan kernels (profiles/r01_ivfpq.md): pair = float tables, one CTA per item; rot = fixed-point
+  // conflict-free tables, one CTA per item; grp = the same in persistent groups with the codebook
+  // resident in shared memory.  Default: grp where it is measured faster (items of >= 32 lists, enough
+  // items to fill the persistent groups), else pair.  FS_IVFPQ_SCAN=pair|rot|grp forces one (A/B runs).
+  static int forced = -1;
+  if (forced < 0) {
     const char* e = getenv("FS_IVFPQ_SCAN");
-    mode = (e && strcmp(e, "rot") == 0) ? 1 : (e && strcmp(e, "grp") == 0) ? 2 : 0;
+    forced = !e ? 0 : strcmp(e, "pair") == 0 ? 3 : strcmp(e, "rot") == 0 ? 1 : strcmp(e, "grp") == 0 ? 2 : 0;
   }
+  int mode = forced == 3 ? 0 : forced;
+  if (forced == 0 && a.G >= 32 && nq * a.ngroups >= (int64_t)3 * GRP_N * sm_count()) mode = 2;
   if constexpr (NQ <= 8) {
     const bool fx = a.len32 && a.pq_r;
-    if (mode == 2 && fx && a.M == 16 && a.dsub == 6) return launch_scan_grp<NQ, 16, 6>(a, nq, a.work, s);
-    if (mode == 2 && fx && a.M == 8 && a.dsub == 12) return launch_scan_grp<NQ, 8, 12>(a, nq, a.work, s);
+    if (mode == 2 && fx && a.d <= SCAN_THREADS && a.M == 16 && a.dsub == 6) return launch_scan_grp<NQ, 16, 6>(a, nq, a.work, s);
+    if (mode == 2 && fx && a.d <= SCAN_THREADS && a.M == 8 && a.dsub == 12) return launch_scan_grp<NQ, 8, 12>(a, nq, a.work, s);
     if (mode == 1 && fx && a.M == 16 && a.dsub == 6) return launch_scan_rot<NQ, 16, 6>(a, nq, s);
     if (mode == 1 && fx && a.M == 8 && a.dsub == 12) return launch_scan_rot<NQ, 8, 12>(a, nq, s);
   }
