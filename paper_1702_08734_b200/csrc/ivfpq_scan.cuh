@@ -49,6 +49,28 @@ __device__ __forceinline__ void rotate_bytes(uint32_t (&w)[MW], int r) {
   for (int i = 0; i < MW; ++i) w[i] = t[i];
 }
 
+// Packed fp32 pairs (sm_100 FADD2 / FFMA2): two lanes of a 64-bit register per instruction
+__device__ __forceinline__ uint64_t f2_pack(float a, float b) {
+  uint64_t r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b));
+  return r;
+}
+__device__ __forceinline__ uint64_t f2_sub(uint64_t a, uint64_t b) {
+  uint64_t r;
+  asm("sub.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+__device__ __forceinline__ uint64_t f2_fma(uint64_t a, uint64_t b, uint64_t c) {
+  uint64_t r;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+  return r;
+}
+__device__ __forceinline__ float f2_hsum(uint64_t v) {
+  float a, b;
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v));
+  return a + b;
+}
+
 // One code = MW words.  Streaming loads (evict-first): the codes pass through L1 once, the
 // codebook that every table build re-reads should stay there.
 template <int MW>

@@ -587,6 +587,9 @@ __global__ void __launch_bounds__(GRP_THREADS, 1) ivfpq_scan_grp_kernel(const Sc
         rm[j] = r[my_m * DS + j];
         n = fmaf(rm[j], rm[j], n);
       }
+      uint64_t rm2[DS / 2];  // the residual sub-vector as packed pairs (FADD2 / FFMA2 below)
+#pragma unroll
+      for (int j = 0; j < DS / 2; ++j) rm2[j] = f2_pack(rm[2 * j], rm[2 * j + 1]);
       float u = sqrtf(n) + my_bmax;
       u = u * u * 1.001f;  // >= every entry of T_m as the float code below computes it
 #pragma unroll
@@ -600,23 +603,23 @@ __global__ void __launch_bounds__(GRP_THREADS, 1) ivfpq_scan_grp_kernel(const Sc
 #pragma unroll 4
       for (int c0 = warp * REP; c0 < 256; c0 += SCAN_WARPS * REP) {
         const int c = c0 + cofs;
-        float t = 0.f;
+        // even and odd dimensions accumulate in the two halves of one packed register
+        uint64_t acc2 = 0ull;
 #pragma unroll
         for (int jv = 0; jv < NV; ++jv) {
-          float bv[VW];
           if (VW == 2) {
-            const float2 x = reinterpret_cast<const float2*>(cb)[((c0 / REP) * NV + jv) * 32 + lane];
-            bv[0] = x.x; bv[1] = x.y;
+            const uint64_t b2 = reinterpret_cast<const uint64_t*>(cb)[((c0 / REP) * NV + jv) * 32 + lane];
+            const uint64_t d2 = f2_sub(rm2[jv], b2);
+            acc2 = f2_fma(d2, d2, acc2);
           } else {
-            const float4 x = reinterpret_cast<const float4*>(cb)[((c0 / REP) * NV + jv) * 32 + lane];
-            bv[0] = x.x; bv[1] = x.y; bv[VW - 2] = x.z; bv[VW - 1] = x.w;
-          }
-#pragma unroll
-          for (int i = 0; i < VW; ++i) {
-            const float df = rm[jv * VW + i] - bv[i];
-            t = fmaf(df, df, t);
+            const ulonglong2 b4 = reinterpret_cast<const ulonglong2*>(cb)[((c0 / REP) * NV + jv) * 32 + lane];
+            const uint64_t d2a = f2_sub(rm2[(2 * jv) % (DS / 2)], b4.x);
+            acc2 = f2_fma(d2a, d2a, acc2);
+            const uint64_t d2b = f2_sub(rm2[(2 * jv + 1) % (DS / 2)], b4.y);
+            acc2 = f2_fma(d2b, d2b, acc2);
           }
         }
+        const float t = f2_hsum(acc2);
         const uint32_t v = __float2uint_rn(t * scale);
 #pragma unroll
         for (int rep = 0; rep < REP; ++rep) lut[c * 32 + my_m + ((rep + cofs) % REP) * M] = v;
