@@ -159,8 +159,9 @@ __device__ __noinline__ void sort_block(uint64_t* base, int n) {
 // staging area.  Counter of (bin d, lane l) lives in 32-bit word
 // (d >> 1) * 32 + l, half (d & 1): a lane only ever touches its own words (no
 // races, no atomics) and the 32 lanes of an access hit 32 different banks.
-// RB = digit width: 6 bits (4 KB of counters) for the large queue classes, 5 bits
-// (2 KB) for the small ones, where shared memory per warp decides the occupancy.
+// RB = digit width: 5 bits (2 KB of counters) wherever shared memory per warp decides the
+// occupancy -- also for k = 1024, where 9 resident warps per SM instead of 8 outweigh the extra
+// counting passes (0.907 -> 0.839 ms at cfg2, 0.362 -> 0.306 ms on the 2^27 row); 6 bits for k = 512.
 template <int RB>
 constexpr int sel_scratch_bytes() { return (1 << RB) * 32 * 2; }
 
@@ -281,7 +282,13 @@ template <> struct TSelCfg<2> { static constexpr int LCAP = 32, RB = 5, WARPS = 
 template <> struct TSelCfg<4> { static constexpr int LCAP = 36, RB = 5, WARPS = 1; };
 template <> struct TSelCfg<8> { static constexpr int LCAP = 48, RB = 5, WARPS = 1; };
 template <> struct TSelCfg<16> { static constexpr int LCAP = 60, RB = 6, WARPS = 1; };
-template <> struct TSelCfg<32> { static constexpr int LCAP = 72, RB = 6, WARPS = 1; };
+#ifndef FS_K32_LCAP
+#define FS_K32_LCAP 72
+#endif
+#ifndef FS_K32_RB
+#define FS_K32_RB 5
+#endif
+template <> struct TSelCfg<32> { static constexpr int LCAP = FS_K32_LCAP, RB = FS_K32_RB, WARPS = 1; };
 
 // How many of the S sample elements the sampled bound should let through so that at
 // least k of the len elements pass with ~3 sigma confidence: the count c of sample
