@@ -102,6 +102,8 @@ __device__ __forceinline__ void bulk_g2s_a(uint32_t dst, const void* src, uint32
 #endif
 constexpr int kSeg = FS_KSEG;    // floats per ring segment (2 KB)
 constexpr int kStages = FS_KSTAGES;   // ring depth per warp
+static_assert(kSeg >= 512 && kSeg % 512 == 0, "the sampled bound reads the first 1024 elements as two ring segments");
+static_assert(kStages >= 2, "the sample spans two segments");
 constexpr int kSample = 1024;
 
 struct ItemDesc {
