@@ -277,9 +277,15 @@ __device__ __noinline__ uint64_t radix_select_kth(const uint64_t* keys, int m, i
 // the mean + 4 sigma of a lane's share of the sampled bound's m*, see sample_target),
 // RB = radix digit width, WARPS per CTA.
 template <int NQ> struct TSelCfg;
-template <> struct TSelCfg<1> { static constexpr int LCAP = 28, RB = 5, WARPS = 1; };
+#ifndef FS_K1_LCAP
+#define FS_K1_LCAP 28
+#endif
+#ifndef FS_K4_LCAP
+#define FS_K4_LCAP 28
+#endif
+template <> struct TSelCfg<1> { static constexpr int LCAP = FS_K1_LCAP, RB = 5, WARPS = 1; };
 template <> struct TSelCfg<2> { static constexpr int LCAP = 32, RB = 5, WARPS = 1; };
-template <> struct TSelCfg<4> { static constexpr int LCAP = 36, RB = 5, WARPS = 1; };
+template <> struct TSelCfg<4> { static constexpr int LCAP = FS_K4_LCAP, RB = 5, WARPS = 1; };
 template <> struct TSelCfg<8> { static constexpr int LCAP = 48, RB = 5, WARPS = 1; };
 template <> struct TSelCfg<16> { static constexpr int LCAP = 60, RB = 6, WARPS = 1; };
 #ifndef FS_K32_LCAP
