@@ -132,5 +132,10 @@ def test_cfg4_shaped_index():
         sub = np.unique(rng.integers(0, nq, 24))
         xs = xq[torch.from_numpy(sub).cuda()].cpu().numpy()
         sd, si, _ = check_search(ix, coarse, pq, offs, codes, lids, xs, nprobe, k)
-        assert np.array_equal(si, gi[torch.from_numpy(sub).cuda()].cpu().numpy())  # batch == subset run
+        # batch run vs subset run: the dispatch may pick different scan kernels for the two (float
+        # tables / fixed-point tables, DESIGN 5.3), so near-ties may swap; everything else is equal
+        bi_s = gi[torch.from_numpy(sub).cuda()].cpu().numpy()
+        bd_s = gd[torch.from_numpy(sub).cuda()].cpu().numpy()
+        assert np.allclose(bd_s, sd, rtol=1e-3, atol=0)
+        assert (bi_s == si).mean() >= 0.98
     ix.close()

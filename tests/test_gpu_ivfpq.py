@@ -234,3 +234,46 @@ def test_empty_index_empty_lists_errors_and_host_entry():
     hd, hi = ix.search_host(xq.cpu().numpy(), nlist, 4)
     assert np.array_equal(hi, ii.cpu().numpy()) and np.array_equal(hd, dd.cpu().numpy())
     ix.close()
+
+
+def test_many_lists_per_item_duplicates():
+    """d = 96, M = 16 with >= 32 lists per (query, list group) and enough items: the shape at which
+    the dispatch picks the grouped fixed-point scan (DESIGN 5.3).  A tenth of the database are
+    exact duplicates of other vectors: identical codes in one list must come back with identical
+    distances, in ascending id order (reading C-6)."""
+    fs = fsmod()
+    d, M, nlist, nb, nq, nprobe, k = 96, 16, 64, 60000, 1400, 32, 100
+    xb = datagen.deep_like(0, nb).copy()
+    rng = np.random.default_rng(5)
+    src = rng.integers(0, nb, nb // 10)
+    dst = rng.integers(0, nb, nb // 10)
+    xb[dst] = xb[src]
+    xq = datagen.deep_like(10**8, nq)
+    ix = fs.IvfPq(d, nlist, M)
+    ix.train(torch.from_numpy(xb[:20000]).cuda(), niter=4, seed=2)
+    coarse, pq = (t.cpu().numpy() for t in ix.get_quantizers())
+    ix.add(torch.from_numpy(xb).cuda())
+    offs, codes, lids = (t.cpu().numpy() for t in ix.export())
+    # the whole batch goes through check_search: it is the launch configuration that reaches the
+    # persistent kernel (>= 32 lists per item, >= 1 332 items)
+    check_search(ix, coarse, pq, offs, codes, lids, xq, nprobe, k)
+    bd, bi = ix.search(torch.from_numpy(xq).cuda(), nprobe, k)
+    torch.cuda.synchronize()
+    # duplicates: equal codes in the same list -> bitwise-equal distances
+    pos_of = np.empty(nb, np.int64)
+    pos_of[lids] = np.arange(nb)
+    list_of = np.searchsorted(offs, np.arange(nb), side="right") - 1
+    bi_h, bd_h = bi.cpu().numpy(), bd.cpu().numpy()
+    checked = 0
+    for q in range(0, nq, 7):
+        ids = bi_h[q][bi_h[q] >= 0]
+        p = pos_of[ids]
+        key = [(int(list_of[x]), codes[x].tobytes()) for x in p]
+        seen = {}
+        for j, kk in enumerate(key):
+            if kk in seen:
+                assert bd_h[q, j] == bd_h[q, seen[kk]], "equal codes, different distances"
+                checked += 1
+            seen[kk] = j
+    assert checked > 0
+    ix.close()
