@@ -52,7 +52,7 @@ __device__ __forceinline__ void lookup_all(const uint32_t* cw, uint32_t Tb, floa
 
 // Shared memory: T[M][256] | r[d] | per-warp batches | merge area [SCAN_WARPS][K]
 // MT = M when M is 8 or 16 (code loaded with one 8 / 16-byte load, lookups unrolled), else 0;
-// DS = d / M when it is 6 or 12 and MT != 0 (table build unrolled, 8 / 16-byte codebook loads), else 0.
+// DS = d / M when it is 6, 8, 12 or 16 and MT != 0 (table build unrolled, 8 / 16-byte codebook loads), else 0.
 template <int NQ, int MT, int DS>
 __global__ void __launch_bounds__(SCAN_THREADS) ivfpq_scan_kernel(const ScanArgs a) {
   extern __shared__ __align__(1024) unsigned char scan_smem[];
@@ -758,8 +758,10 @@ int launch_scan(const ScanArgs& a, int64_t nq, cudaStream_t s) {
     if (mode == 1 && fx && a.M == 16 && a.dsub == 6) return launch_scan_rot<NQ, 16, 6>(a, nq, s);
     if (mode == 1 && fx && a.M == 8 && a.dsub == 12) return launch_scan_rot<NQ, 8, 12>(a, nq, s);
   }
-  if (a.M == 16 && a.dsub == 6) return launch_scan_m<NQ, 16, 6>(a, nq, s);
-  if (a.M == 8 && a.dsub == 12) return launch_scan_m<NQ, 8, 12>(a, nq, s);
+  if (a.pq_t && a.M == 16 && a.dsub == 6) return launch_scan_m<NQ, 16, 6>(a, nq, s);
+  if (a.pq_t && a.M == 8 && a.dsub == 12) return launch_scan_m<NQ, 8, 12>(a, nq, s);
+  if (a.pq_t && a.M == 16 && a.dsub == 8) return launch_scan_m<NQ, 16, 8>(a, nq, s);   // d = 128
+  if (a.pq_t && a.M == 8 && a.dsub == 16) return launch_scan_m<NQ, 8, 16>(a, nq, s);   // d = 128
   if (a.M == 16) return launch_scan_m<NQ, 16, 0>(a, nq, s);
   if (a.M == 8) return launch_scan_m<NQ, 8, 0>(a, nq, s);
   return launch_scan_m<NQ, 0, 0>(a, nq, s);
@@ -795,7 +797,7 @@ int ivfpq_search_device(fs_ivfpq* ix, const float* xq, int64_t nq, int nprobe, i
   a.pq_t = nullptr;
   a.pq_r = nullptr;
   a.bmax = nullptr;
-  if ((ix->M == 16 && ix->dsub == 6) || (ix->M == 8 && ix->dsub == 12)) {
+  if ((ix->M == 16 && (ix->dsub == 6 || ix->dsub == 8)) || (ix->M == 8 && (ix->dsub == 12 || ix->dsub == 16))) {
     float* pq_t = reinterpret_cast<float*>(w + p.off_pqt);
     float* pq_r = reinterpret_cast<float*>(w + p.off_pqr);
     float* bmax = pq_r + (size_t)256 * ix->d;

@@ -277,3 +277,21 @@ def test_many_lists_per_item_duplicates():
             seen[kk] = j
     assert checked > 0
     ix.close()
+
+
+@pytest.mark.parametrize("M", [8, 16])
+def test_d128_shapes(M):
+    """d = 128 (SIFT-like integer-valued data): dsub = 16 / 8, the other shapes with an unrolled
+    table build."""
+    fs = fsmod()
+    d, nlist, nb, nq = 128, 32, 12000, 40
+    xb = datagen.sift_like(0, nb)
+    xq = datagen.sift_like(10**7, nq)
+    ix = fs.IvfPq(d, nlist, M)
+    ix.train(torch.from_numpy(xb[:6000]).cuda(), niter=4, seed=3)
+    coarse, pq = (t.cpu().numpy() for t in ix.get_quantizers())
+    ix.add(torch.from_numpy(xb).cuda())
+    offs, codes, lids = check_add(ix, coarse, pq, xb)
+    for nprobe, k in ((4, 10), (nlist, 100)):
+        check_search(ix, coarse, pq, offs, codes, lids, xq, nprobe, k)
+    ix.close()
