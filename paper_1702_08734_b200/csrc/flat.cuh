@@ -35,8 +35,10 @@ struct FlatTcPlan {
 };
 bool flat_tc_supported(int d);  // d % 32 == 0, 32 <= d <= 128, not disabled by FS_FLAT_ENGINE=ffma
 FlatTcPlan flat_tc_plan(int64_t nq, int64_t nb, int d, int k);
+// dout != NULL: distance-matrix mode -- no selection, dout[q * dld + j] = ||y_j||^2 - 2 <x_q, y_j>
+// (dld % 4 == 0, dout 16-byte aligned); k, out_dist and out_ids are ignored, the workspace is that of k = 1.
 int flat_knn_tc_device(const float* xq, int64_t nq, const float* xb, int64_t nb, int d, int k, float* out_dist,
-                       int64_t* out_ids, void* ws, cudaStream_t s);
+                       int64_t* out_ids, void* ws, cudaStream_t s, float* dout = nullptr, int64_t dld = 0);
 
 // B4: S partial queues per query -> k results (+||x||^2 if xnorm != NULL).
 int launch_flat_finish(const uint64_t* Wg, int64_t nq, int S, int k, const float* xnorm,

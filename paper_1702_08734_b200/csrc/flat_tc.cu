@@ -75,6 +75,8 @@ struct TcArgs {
   unsigned int* hclaim;        // [nq][HB_LEVELS] slots handed out per level
   uint64_t* cbuf;              // [gridDim.x][EPI_GROUPS][BM][cap]: winners so far, then new candidates
   const unsigned int* lo_flag; // != 0: lo planes are not all zero (3xTF32)
+  float* dout;                 // != NULL: no selection, d'(q, j) = ||y_j||^2 - 2 <x_q, y_j> is written to
+  int64_t dld;                 //          dout[q * dld + j] (dld % 4 == 0); the launch passes k = 1
 };
 
 // ---------------------------------------------------------------------------
@@ -422,6 +424,21 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
             v[j] = __float_as_uint(dp);
             rej[j >> 5] = __funnelshift_l(__float_as_uint(thr_val - dp), rej[j >> 5], 1);
           }
+          if (a.dout != nullptr) {  // distance-matrix mode: the block goes to global memory as it is
+            if (valid) {
+              float* o = a.dout + q * a.dld + cbase;
+              if (climit >= BW) {
+#pragma unroll
+                for (int j = 0; j < BW; j += 4)
+                  *reinterpret_cast<uint4*>(o + j) = make_uint4(v[j], v[j + 1], v[j + 2], v[j + 3]);
+              } else {
+#pragma unroll
+                for (int j = 0; j < BW; ++j)
+                  if (j < climit) o[j] = __uint_as_float(v[j]);
+              }
+            }
+            continue;
+          }
           uint32_t mk[2];
 #pragma unroll
           for (int h = 0; h < 2; ++h) {
@@ -472,6 +489,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
           sm100::mbar_arrive(yempty + ys);
         }
       }
+      if (a.dout != nullptr) continue;  // nothing was selected
       flush_rows(cnt >= k, true);  // establishes the split's k-th distance (published below)
       __syncwarp();
       // the row's partial queue for B4 (unordered, sentinel padded), and this split's k-th
@@ -623,7 +641,8 @@ FlatTcPlan flat_tc_plan(int64_t nq, int64_t nb, int d, int k) {
 }
 
 int flat_knn_tc_device(const float* xq, int64_t nq, const float* xb, int64_t nb, int d, int k, float* out_dist,
-                       int64_t* out_ids, void* ws, cudaStream_t s) {
+                       int64_t* out_ids, void* ws, cudaStream_t s, float* dout, int64_t dld) {
+  if (dout != nullptr) k = 1;  // distance-matrix mode: the plan of the cheapest queue class
   const FlatTcPlan p = flat_tc_plan(nq, nb, d, k);
   if (p.nstage < 2) return set_error(FS_EUNSUPPORTED, "flat tensor-core engine: d = %d leaves no room for the stage ring", d);
   char* w = static_cast<char*>(ws);
@@ -671,6 +690,8 @@ int flat_knn_tc_device(const float* xq, int64_t nq, const float* xb, int64_t nb,
   a.hclaim = reinterpret_cast<unsigned int*>(w + p.off_hclaim);
   a.cbuf = reinterpret_cast<uint64_t*>(w + p.off_cbuf);
   a.lo_flag = flag;
+  a.dout = dout;
+  a.dld = dld;
   static size_t attr_smem = 0;
   if (p.smem > attr_smem) {
     FS_CUDA(cudaFuncSetAttribute(flat_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem));
@@ -694,6 +715,7 @@ int flat_knn_tc_device(const float* xq, int64_t nq, const float* xb, int64_t nb,
     FS_CUDA(cudaLaunchKernelEx(&cfg, flat_tc_kernel, ma_hi, ma_lo, mb_hi, mb_lo, a));
     FS_LAUNCHED();
   }
+  if (dout != nullptr) return FS_OK;
   return launch_flat_finish(a.Wg, nq, p.S * EPI_GROUPS, k, xnorm, out_dist, out_ids, s);
 }
 

@@ -26,6 +26,11 @@
 
 namespace fs {
 
+// kselect.cu
+size_t kselect_ws_bytes(int64_t n_rows, int64_t n, int k);
+int kselect_device(const float* rows, int64_t n_rows, int64_t n, int64_t ld, int k, float* out_val,
+                   int32_t* out_idx, void* ws, cudaStream_t s);
+
 namespace {
 
 constexpr int SCAN_WARPS = 8;
@@ -279,10 +284,35 @@ __global__ void pq_bmax_kernel(const float* __restrict__ pq, float* __restrict__
   if (lane == 0) bmax[m] = sqrtf(mx);
 }
 
+// C1 for a coarse quantizer of modest size and nprobe >= 16: the fused engine's selection runs
+// almost entirely on its unbounded first tiles there (profiles/r01_ivfpq.md: 0.95 / 1.2 / 2.7 ms at
+// nlist = 8 192, 1.9 / 2.8 / 10.8 ms at 65 536 for nprobe 16 / 64 / 256, against 0.3 / 0.7 ms for
+// k = 1).  The paper's own two-step form is cheaper: the tensor-core engine writes the
+// distance matrix (no selection), fs_kselect's kernels take nprobe per row.  FS_IVFPQ_C1=fused|matrix
+// forces one (A/B runs).
+bool c1_matrix(int64_t nq, int64_t nlist, int nprobe, int d) {
+  static int forced = -1;
+  if (forced < 0) {
+    const char* e = getenv("FS_IVFPQ_C1");
+    forced = !e ? 0 : strcmp(e, "fused") == 0 ? 1 : strcmp(e, "matrix") == 0 ? 2 : 0;
+  }
+  if (!flat_tc_supported(d) || nq < 1 || nprobe > nlist || nlist >= ((int64_t)1 << 31)) return false;
+  if (forced == 1) return false;
+  if (forced == 2) return true;
+  if (nprobe < 16 || nq < 256) return false;
+  return nlist <= 16384 || (nprobe >= 64 && nlist <= 131072) || nprobe >= 128;
+}
+
+__global__ void widen_ids_kernel(const int32_t* __restrict__ in, int64_t* __restrict__ out, int64_t n) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) out[i] = in[i];
+}
+
 struct SearchPlan {
   int G, ngroups, K;
   FlatPlan coarse;
-  size_t off_cdist, off_cids, off_W, off_work, off_pqt, off_pqr, bytes;
+  size_t off_cdist, off_cids, off_W, off_work, off_pqt, off_pqr, off_D, off_cval, off_cidx, off_ksws, bytes;
+  int64_t c1_chunk, c1_ld;  // C1 through a distance matrix: queries per pass (0 = fused engine), row stride
 };
 
 SearchPlan search_plan(const fs_ivfpq* ix, int64_t nq, int nprobe, int k) {
@@ -297,6 +327,16 @@ SearchPlan search_plan(const fs_ivfpq* ix, int64_t nq, int nprobe, int k) {
   p.ngroups = (int)ceil_div(nprobe, p.G);
   p.coarse = flat_plan(nq, ix->nlist, ix->d, nprobe);
   size_t o = align_up(p.coarse.bytes, 256);
+  p.c1_chunk = 0;
+  p.c1_ld = 0;
+  if (c1_matrix(nq, ix->nlist, nprobe, ix->d)) {
+    p.c1_ld = (ix->nlist + 3) & ~(int64_t)3;
+    int64_t c = ((int64_t)1 << 30) / (p.c1_ld * 4);  // <= 1 GB of distances per pass
+    if (c < 256) c = 256;
+    p.c1_chunk = c < nq ? c : nq;
+    const size_t fb = flat_plan(p.c1_chunk, ix->nlist, ix->d, 1).bytes;
+    if (fb > o) o = align_up(fb, 256);
+  }
   p.off_cdist = o;
   o += align_up((size_t)nq * nprobe * sizeof(float), 256);
   p.off_cids = o;
@@ -307,6 +347,17 @@ SearchPlan search_plan(const fs_ivfpq* ix, int64_t nq, int nprobe, int k) {
   o += align_up((size_t)256 * ix->d * sizeof(float), 256);
   p.off_pqr = o;
   o += align_up((size_t)256 * ix->d * sizeof(float), 256) + 256;  // + bmax[M]
+  p.off_D = p.off_cval = p.off_cidx = p.off_ksws = o;
+  if (p.c1_chunk > 0) {
+    p.off_D = o;
+    o += align_up((size_t)p.c1_chunk * p.c1_ld * sizeof(float), 256);
+    p.off_cval = o;
+    o += align_up((size_t)p.c1_chunk * nprobe * sizeof(float), 256);
+    p.off_cidx = o;
+    o += align_up((size_t)p.c1_chunk * nprobe * sizeof(int32_t), 256);
+    p.off_ksws = o;
+    o += align_up(kselect_ws_bytes(p.c1_chunk, ix->nlist, nprobe), 256);
+  }
   p.off_W = o;
   const int qpi = scan2_supported(ix->d, ix->M, k) ? scan2_queues_per_item() : 1;
   o += align_up((size_t)nq * p.ngroups * qpi * p.K * sizeof(uint64_t), 256);
@@ -783,9 +834,25 @@ int ivfpq_search_device(fs_ivfpq* ix, const float* xq, int64_t nq, int nprobe, i
   uint64_t* Wg = reinterpret_cast<uint64_t*>(w + p.off_W);
   int rc;
   // C1
-  rc = flat_knn_device(xq, nq, ix->coarse.as<float>(), ix->nlist, ix->d, nprobe,
-                       ix->cnorm.as<float>(), cdist, cids, w, s);
-  if (rc != FS_OK) return rc;
+  if (p.c1_chunk > 0) {
+    float* D = reinterpret_cast<float*>(w + p.off_D);
+    float* cval = reinterpret_cast<float*>(w + p.off_cval);
+    int32_t* cidx = reinterpret_cast<int32_t*>(w + p.off_cidx);
+    for (int64_t q0 = 0; q0 < nq; q0 += p.c1_chunk) {
+      const int64_t n = nq - q0 < p.c1_chunk ? nq - q0 : p.c1_chunk;
+      rc = flat_knn_tc_device(xq + q0 * ix->d, n, ix->coarse.as<float>(), ix->nlist, ix->d, 1, nullptr, nullptr, w, s,
+                              D, p.c1_ld);
+      if (rc != FS_OK) return rc;
+      rc = kselect_device(D, n, ix->nlist, p.c1_ld, nprobe, cval, cidx, w + p.off_ksws, s);
+      if (rc != FS_OK) return rc;
+      widen_ids_kernel<<<(unsigned)ceil_div(n * nprobe, 256), 256, 0, s>>>(cidx, cids + q0 * nprobe, n * nprobe);
+      FS_LAUNCHED();
+    }
+  } else {
+    rc = flat_knn_device(xq, nq, ix->coarse.as<float>(), ix->nlist, ix->d, nprobe,
+                         ix->cnorm.as<float>(), cdist, cids, w, s);
+    if (rc != FS_OK) return rc;
+  }
   FS_CUDA(cudaMemsetAsync(ix->scanned.p, 0, sizeof(unsigned long long), s));
   // C2-C4
   ScanArgs a;
