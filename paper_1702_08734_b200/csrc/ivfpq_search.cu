@@ -17,6 +17,7 @@
 //   C5 pass-2 + ids      the groups' partial lists are selected again to k; int64
 //                        ids are fetched for the winners only
 #include <cstdlib>
+#include <algorithm>
 #include <cstring>
 
 #include "flat.cuh"
@@ -300,7 +301,10 @@ bool c1_matrix(int64_t nq, int64_t nlist, int nprobe, int d) {
   if (forced == 1) return false;
   if (forced == 2) return true;
   if (nprobe < 16 || nq < 256) return false;
-  return nlist <= 16384 || (nprobe >= 64 && nlist <= 131072) || nprobe >= 128;
+  // measured (nq = 10^4, d = 96; search of a tiny index, ms, fused / matrix): nlist 8 192: nprobe 16
+  // 1.40 / 0.81, 256 9.07 / 6.83; nlist 65 536: 16 2.04 / 2.48, 64 3.49 / 3.11, 256 13.2 / 5.2;
+  // nlist 262 144: 128 8.7 / 12.0, 256 22.4 / 14.0
+  return nlist <= 16384 || (nprobe >= 64 && nlist <= 131072) || nprobe >= 256;
 }
 
 __global__ void widen_ids_kernel(const int32_t* __restrict__ in, int64_t* __restrict__ out, int64_t n) {
@@ -334,7 +338,10 @@ SearchPlan search_plan(const fs_ivfpq* ix, int64_t nq, int nprobe, int k) {
     int64_t c = ((int64_t)1 << 30) / (p.c1_ld * 4);  // <= 1 GB of distances per pass
     if (c < 256) c = 256;
     p.c1_chunk = c < nq ? c : nq;
-    const size_t fb = flat_plan(p.c1_chunk, ix->nlist, ix->d, 1).bytes;
+    // two pass sizes occur (full passes and the last one): the workspaces take the larger plan
+    const int64_t last = nq % p.c1_chunk;
+    size_t fb = flat_plan(p.c1_chunk, ix->nlist, ix->d, 1).bytes;
+    if (last > 0) fb = std::max(fb, flat_plan(last, ix->nlist, ix->d, 1).bytes);
     if (fb > o) o = align_up(fb, 256);
   }
   p.off_cdist = o;
@@ -356,7 +363,10 @@ SearchPlan search_plan(const fs_ivfpq* ix, int64_t nq, int nprobe, int k) {
     p.off_cidx = o;
     o += align_up((size_t)p.c1_chunk * nprobe * sizeof(int32_t), 256);
     p.off_ksws = o;
-    o += align_up(kselect_ws_bytes(p.c1_chunk, ix->nlist, nprobe), 256);
+    const int64_t last = nq % p.c1_chunk;
+    size_t kb = kselect_ws_bytes(p.c1_chunk, ix->nlist, nprobe);
+    if (last > 0) kb = std::max(kb, kselect_ws_bytes(last, ix->nlist, nprobe));
+    o += align_up(kb, 256);
   }
   p.off_W = o;
   const int qpi = scan2_supported(ix->d, ix->M, k) ? scan2_queues_per_item() : 1;
