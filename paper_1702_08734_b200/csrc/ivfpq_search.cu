@@ -335,8 +335,13 @@ SearchPlan search_plan(const fs_ivfpq* ix, int64_t nq, int nprobe, int k) {
   p.c1_ld = 0;
   if (c1_matrix(nq, ix->nlist, nprobe, ix->d)) {
     p.c1_ld = (ix->nlist + 3) & ~(int64_t)3;
-    int64_t c = ((int64_t)1 << 30) / (p.c1_ld * 4);  // <= 1 GB of distances per pass
-    if (c < 256) c = 256;
+    static int64_t budget = 0;  // bytes of distances per pass: 1 GB; FS_IVFPQ_C1_BYTES overrides (tests)
+    if (budget == 0) {
+      const char* e = getenv("FS_IVFPQ_C1_BYTES");
+      budget = e && atoll(e) > 0 ? atoll(e) : ((int64_t)1 << 30);
+    }
+    int64_t c = budget / (p.c1_ld * 4);
+    if (c < 128) c = 128;
     p.c1_chunk = c < nq ? c : nq;
     // two pass sizes occur (full passes and the last one): the workspaces take the larger plan
     const int64_t last = nq % p.c1_chunk;

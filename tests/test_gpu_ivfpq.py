@@ -295,3 +295,21 @@ def test_d128_shapes(M):
     for nprobe, k in ((4, 10), (nlist, 100)):
         check_search(ix, coarse, pq, offs, codes, lids, xq, nprobe, k)
     ix.close()
+
+
+def test_c1_large_nlist():
+    """A coarse quantizer of 32 768 centroids with nprobe = 64: C1 goes through the distance matrix
+    (DESIGN 5.3); tests/test_gpu_ivfpq_variants.py runs it again in passes of 512 queries, whose last
+    pass (188 queries) takes the long-row k-selection plan."""
+    fs = fsmod()
+    d, M, nlist, nb, nq, nprobe, k = 96, 16, 32768, 50000, 700, 64, 10
+    coarse = datagen.deep_like(5 * 10**7, nlist)
+    rng = np.random.default_rng(11)
+    pq = (0.05 * rng.standard_normal((M, 256, d // M))).astype(np.float32)
+    xb = datagen.deep_like(0, nb)
+    xq = datagen.deep_like(10**8, nq)
+    ix = make_index(d, nlist, M, coarse, pq)
+    ix.add(torch.from_numpy(xb).cuda())
+    offs, codes, lids = (t.cpu().numpy() for t in ix.export())
+    check_search(ix, coarse, pq, offs, codes, lids, xq, nprobe, k)
+    ix.close()
