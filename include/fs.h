@@ -77,7 +77,10 @@ FS_API void fs_reset_launch_count(void);
 FS_API int fs_kselect(const float* rows, int64_t n_rows, int64_t n, int64_t ld, int k, float* out_val,
                int32_t* out_idx, void* ws, size_t ws_bytes, fs_stream stream);
 FS_API size_t fs_kselect_ws_bytes(int64_t n_rows, int64_t n, int k);
-/* Same with HOST buffers (copies in and out, synchronises). */
+/* Same with HOST buffers (pinned or pageable): rows are copied in, selected and copied out in up to
+ * 8 slices on three internal streams (copy-in of a slice overlaps the selection of the previous one and
+ * the copy-out of the one before); returns after everything has landed.  Device staging is a grow-only
+ * allocation owned by the library (kept for the next call, one call at a time per process). */
 FS_API int fs_kselect_host(const float* rows_host, int64_t n_rows, int64_t n, int64_t ld, int k,
                     float* out_val_host, int32_t* out_idx_host);
 

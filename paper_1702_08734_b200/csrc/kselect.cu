@@ -18,6 +18,8 @@
 // ahead across item boundaries (the next row is already arriving while the current
 // one is being selected).  "Lane j reads a_{32i+j}" becomes: lane j reads
 // elements 4j..4j+3 of each 128-element group with one 128-bit shared-memory load.
+#include <mutex>
+
 #include "common.cuh"
 #include "select.cuh"
 #include "tselect.cuh"
@@ -766,6 +768,35 @@ int validate(const void* rows, int64_t n_rows, int64_t n, int64_t ld, int k, con
 
 }  // namespace
 
+// Device staging of the host entry point: one grow-only allocation, three streams, events per slice.
+struct HostStage {
+  void* p = nullptr;
+  size_t bytes = 0;
+  cudaStream_t s_in = nullptr, s_run = nullptr, s_out = nullptr;
+  cudaEvent_t ev_in[8] = {}, ev_run[8] = {};
+  int ensure(size_t need) {
+    if (!s_in) {
+      if (cudaStreamCreateWithFlags(&s_in, cudaStreamNonBlocking) != cudaSuccess ||
+          cudaStreamCreateWithFlags(&s_run, cudaStreamNonBlocking) != cudaSuccess ||
+          cudaStreamCreateWithFlags(&s_out, cudaStreamNonBlocking) != cudaSuccess)
+        return set_error(FS_ECUDA, "fs_kselect_host: cudaStreamCreate failed");
+      for (int i = 0; i < 8; ++i)
+        if (cudaEventCreateWithFlags(&ev_in[i], cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&ev_run[i], cudaEventDisableTiming) != cudaSuccess)
+          return set_error(FS_ECUDA, "fs_kselect_host: cudaEventCreate failed");
+    }
+    if (need > bytes) {
+      if (p) cudaFree(p);
+      p = nullptr;
+      bytes = 0;
+      const cudaError_t e = cudaMalloc(&p, need);
+      if (e != cudaSuccess) return set_error(FS_ECUDA, "fs_kselect_host: cudaMalloc(%zu) failed: %s", need, cudaGetErrorString(e));
+      bytes = need;
+    }
+    return FS_OK;
+  }
+};
+
 // Selection over device rows; also used by the flat and IVFPQ drivers.
 size_t kselect_ws_bytes(int64_t n_rows, int64_t n, int k) { return make_plan(n_rows, n, k).bytes; }
 
@@ -850,33 +881,54 @@ int fs_kselect_host(const float* rows_host, int64_t n_rows, int64_t n, int64_t l
   int rc = fs::validate(rows_host, n_rows, n, ld, k, out_val_host, out_idx_host);
   if (rc != FS_OK) return rc;
   if (n_rows == 0) return FS_OK;
-  float* d_rows = nullptr;
-  float* d_val = nullptr;
-  int32_t* d_idx = nullptr;
+  // Rows go through in up to 8 slices on three streams: slice c + 1 is copied in while slice c is
+  // selected and slice c - 1 is copied out (PCIe is full duplex).  Device staging comes from a
+  // grow-only arena that lives as long as the library (no cudaMalloc / cudaFree per call).
+  static std::mutex mu;
+  std::lock_guard<std::mutex> lock(mu);
+  static fs::HostStage st;
+  const int64_t n_slices = n_rows < 8 ? n_rows : 8;
+  const int64_t per = (n_rows + n_slices - 1) / n_slices;
   const size_t in_b = (size_t)n_rows * ld * sizeof(float), out_n = (size_t)n_rows * k;
-  cudaStream_t s = nullptr;
-  rc = FS_OK;
-  auto fail = [&](cudaError_t e, const char* what) {
-    rc = fs::set_error(FS_ECUDA, "%s failed: %s", what, cudaGetErrorString(e));
+  size_t ws_b = 0;
+  for (int64_t r0 = 0; r0 < n_rows; r0 += per) {
+    const size_t b = fs::kselect_ws_bytes(n_rows - r0 < per ? n_rows - r0 : per, n, k);
+    ws_b = b > ws_b ? b : ws_b;
+  }
+  const size_t o_rows = 0, o_val = fs::align_up(in_b, 256), o_idx = o_val + fs::align_up(out_n * sizeof(float), 256),
+               o_ws = o_idx + fs::align_up(out_n * sizeof(int32_t), 256), total = o_ws + fs::align_up(ws_b, 256);
+  if ((rc = st.ensure(total)) != FS_OK) return rc;
+  char* base = static_cast<char*>(st.p);
+  float* d_rows = reinterpret_cast<float*>(base + o_rows);
+  float* d_val = reinterpret_cast<float*>(base + o_val);
+  int32_t* d_idx = reinterpret_cast<int32_t*>(base + o_idx);
+  cudaError_t e = cudaSuccess;
+  auto ck = [&](cudaError_t err, const char* what) {
+    if (err != cudaSuccess && rc == FS_OK) rc = fs::set_error(FS_ECUDA, "%s failed: %s", what, cudaGetErrorString(err));
+    return err == cudaSuccess;
   };
-  cudaError_t e;
-  if ((e = cudaMalloc(&d_rows, in_b ? in_b : 16)) != cudaSuccess) fail(e, "cudaMalloc");
-  if (rc == FS_OK && (e = cudaMalloc(&d_val, out_n * sizeof(float))) != cudaSuccess) fail(e, "cudaMalloc");
-  if (rc == FS_OK && (e = cudaMalloc(&d_idx, out_n * sizeof(int32_t))) != cudaSuccess) fail(e, "cudaMalloc");
-  if (rc == FS_OK && in_b &&
-      (e = cudaMemcpyAsync(d_rows, rows_host, in_b, cudaMemcpyHostToDevice, s)) != cudaSuccess)
-    fail(e, "cudaMemcpyAsync H2D");
-  if (rc == FS_OK) rc = fs_kselect(d_rows, n_rows, n, ld, k, d_val, d_idx, nullptr, 0, s);
-  if (rc == FS_OK && (e = cudaMemcpyAsync(out_val_host, d_val, out_n * sizeof(float),
-                                          cudaMemcpyDeviceToHost, s)) != cudaSuccess)
-    fail(e, "cudaMemcpyAsync D2H");
-  if (rc == FS_OK && (e = cudaMemcpyAsync(out_idx_host, d_idx, out_n * sizeof(int32_t),
-                                          cudaMemcpyDeviceToHost, s)) != cudaSuccess)
-    fail(e, "cudaMemcpyAsync D2H");
-  if ((e = cudaStreamSynchronize(s)) != cudaSuccess && rc == FS_OK) fail(e, "cudaStreamSynchronize");
-  cudaFree(d_rows);
-  cudaFree(d_val);
-  cudaFree(d_idx);
+  int slice = 0;
+  for (int64_t r0 = 0; r0 < n_rows && rc == FS_OK; r0 += per, ++slice) {
+    const int64_t nr = n_rows - r0 < per ? n_rows - r0 : per;
+    if (!ck(cudaMemcpyAsync(d_rows + r0 * ld, rows_host + r0 * ld, (size_t)nr * ld * sizeof(float),
+                            cudaMemcpyHostToDevice, st.s_in), "cudaMemcpyAsync H2D")) break;
+    if (!ck(cudaEventRecord(st.ev_in[slice], st.s_in), "cudaEventRecord")) break;
+    if (!ck(cudaStreamWaitEvent(st.s_run, st.ev_in[slice], 0), "cudaStreamWaitEvent")) break;
+    rc = fs::kselect_device(d_rows + r0 * ld, nr, n, ld, k, d_val + r0 * k, d_idx + r0 * k, base + o_ws, st.s_run);
+    if (rc != FS_OK) break;
+    if (!ck(cudaEventRecord(st.ev_run[slice], st.s_run), "cudaEventRecord")) break;
+    if (!ck(cudaStreamWaitEvent(st.s_out, st.ev_run[slice], 0), "cudaStreamWaitEvent")) break;
+    if (!ck(cudaMemcpyAsync(out_val_host + r0 * k, d_val + r0 * k, (size_t)nr * k * sizeof(float),
+                            cudaMemcpyDeviceToHost, st.s_out), "cudaMemcpyAsync D2H")) break;
+    if (!ck(cudaMemcpyAsync(out_idx_host + r0 * k, d_idx + r0 * k, (size_t)nr * k * sizeof(int32_t),
+                            cudaMemcpyDeviceToHost, st.s_out), "cudaMemcpyAsync D2H")) break;
+  }
+  e = cudaStreamSynchronize(st.s_in);
+  ck(e, "cudaStreamSynchronize");
+  e = cudaStreamSynchronize(st.s_run);
+  ck(e, "cudaStreamSynchronize");
+  e = cudaStreamSynchronize(st.s_out);
+  ck(e, "cudaStreamSynchronize");
   return rc;
 }
 
