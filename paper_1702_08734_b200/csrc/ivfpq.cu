@@ -519,7 +519,7 @@ int fs_ivfpq_destroy(fs_ivfpq* ix) {
   if (!ix) return FS_OK;
   cudaDeviceSynchronize();
   fs::DevBuf* bufs[] = {&ix->coarse, &ix->cnorm, &ix->pq, &ix->offsets, &ix->codes, &ix->ids,
-                        &ix->st_list, &ix->st_codes, &ix->st_ids, &ix->scanned};
+                        &ix->st_list, &ix->st_codes, &ix->st_ids, &ix->scanned, &ix->term1};
   for (fs::DevBuf* b : bufs) b->release();
   delete ix;
   return FS_OK;
@@ -536,6 +536,7 @@ int fs_ivfpq_set_quantizers(fs_ivfpq* ix, const float* coarse, const float* pq, 
   int rc = fs::launch_row_norms(ix->coarse.as<float>(), ix->nlist, ix->d, ix->cnorm.as<float>(), s);
   if (rc != FS_OK) return rc;
   ix->have_quantizers = true;
+  ix->term1_valid = false;
   return FS_OK;
 }
 

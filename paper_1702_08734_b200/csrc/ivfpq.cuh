@@ -31,6 +31,11 @@ struct fs_ivfpq {
   fs::DevBuf coarse;  // [nlist][d] fp32
   fs::DevBuf cnorm;   // [nlist] fp32: ||c||^2 (B1 of the coarse search, precomputed)
   fs::DevBuf pq;      // [M][256][dsub] fp32
+  // Eq. 11 term 1, ||B[m][c]||^2 + 2 <c_L^m, B[m][c]> for every list, in the lane
+  // order of the fixed-point table build (ivfpq_search.cu); built lazily by the first search that
+  // uses it, dropped when the quantizers change.
+  fs::DevBuf term1;   // [nlist][M * 256] fp32
+  bool term1_valid = false;
 
   // Finalised inverted file, CSR over list number (codes and
   // ids in separate arrays, each list contiguous, append order kept).

@@ -16,6 +16,7 @@ struct ScanArgs {
   const float* pq_t;         // pq regrouped for vector loads (ivfpq_search.cu), or NULL
   const float* pq_r;         // pq regrouped for the rotated fixed-point kernel, or NULL
   const float* bmax;         // [M] max_c ||B[m][c]||, or NULL
+  const float* term1;        // [nlist][M * 256] Eq. 11 term 1 in lane order, or NULL
   const int64_t* probe_ids;  // [nq][nprobe], ascending coarse distance
   const int64_t* offsets;    // [nlist+1]
   const uint8_t* codes;      // [ntotal][M]

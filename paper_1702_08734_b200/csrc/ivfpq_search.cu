@@ -307,6 +307,31 @@ bool c1_matrix(int64_t nq, int64_t nlist, int nprobe, int d) {
   return nlist <= 16384 || (nprobe >= 64 && nlist <= 131072) || nprobe >= 256;
 }
 
+int scan_forced_mode() {  // 0 none, 1 rot, 2 grp, 3 pair, 4 pre
+  static int forced = -1;
+  if (forced < 0) {
+    const char* e = getenv("FS_IVFPQ_SCAN");
+    forced = !e ? 0 : strcmp(e, "pair") == 0 ? 3 : strcmp(e, "rot") == 0 ? 1 : strcmp(e, "grp") == 0 ? 2 : strcmp(e, "pre") == 0 ? 4 : 0;
+  }
+  return forced;
+}
+bool scan_forced_pre() { return scan_forced_mode() == 4; }
+// (M = 8: half the lookups per vector, the float kernel stays ahead: 7.7 against 9.7 ms, cfg5 shape)
+bool scan_auto_grouped(int M, int G, int64_t n_items) {
+  return scan_forced_mode() == 0 && M == 16 && G >= 32 && n_items >= (int64_t)9 * sm_count();  // 3 rounds of 3 groups per SM
+}
+
+// The decomposed table build needs M = 16 and nlist * 16 KB of device memory (<= 4 GB here); it is
+// the default wherever the grouped fixed-point scan is (launch_scan), FS_IVFPQ_SCAN=pre forces it.
+bool want_term1(const fs_ivfpq* ix) {
+  static int on = -1;
+  if (on < 0) {
+    const char* e = getenv("FS_IVFPQ_SCAN");
+    on = !e ? 1 : strcmp(e, "pre") == 0 ? 1 : 0;
+  }
+  return on && ix->M == 16 && ix->d <= SCAN_THREADS && (size_t)ix->nlist * 16 * 256 * sizeof(float) <= ((size_t)4 << 30);
+}
+
 __global__ void widen_ids_kernel(const int32_t* __restrict__ in, int64_t* __restrict__ out, int64_t n) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) out[i] = in[i];
@@ -738,6 +763,233 @@ __global__ void __launch_bounds__(GRP_THREADS, 1) ivfpq_scan_grp_kernel(const Sc
   if (tid == 0 && bytes) atomicAdd(a.scanned, bytes);
 }
 
+// ---------------------------------------------------------------------------
+// The grouped fixed-point scan with the paper's table decomposition (Eq. 11, P:L300-311;
+// FS_IVFPQ_SCAN=pre):  T_m[c] = ||x^m - c_L^m - B[m][c]||^2
+//     = (||B[m][c]||^2 + 2 <c_L^m, B[m][c]>)      term 1: per list, precomputed (ivfpq_term1_kernel)
+//     + ||x^m - c_L^m||^2                          term 2: per (query, list, m), constant over c
+//     + (-2 <x^m, B[m][c]>)                        term 3: per query, built once per work item
+// so the table of a (query, list) pair costs one load, two adds and the conversion per entry
+// instead of 2 dsub flops, and no codebook is needed in shared memory (any dsub).  Entries are
+// clamped at 0 before the fixed-point conversion (the three terms cancel to rounding).
+// Shared memory per group: lut[256][32] (merge area aliases it) | t3[M * 256] | r[d] | select batches
+// ---------------------------------------------------------------------------
+template <int M>
+__global__ void __launch_bounds__(256) ivfpq_term1_kernel(const float* __restrict__ coarse, const float* __restrict__ pq,
+                                                          float* __restrict__ term1, int d, int dsub) {
+  constexpr int REP = 32 / M;
+  const int64_t L = blockIdx.x;
+  const float* cL = coarse + L * d;
+  for (int e = threadIdx.x; e < M * 256; e += 256) {
+    const int st = e >> 5, lane = e & 31;
+    const int m = lane % M, c = st * REP + lane / M;
+    const float* b = pq + ((int64_t)m * 256 + c) * dsub;
+    float bn = 0.f, cb = 0.f;
+    for (int j = 0; j < dsub; ++j) {
+      bn = fmaf(b[j], b[j], bn);
+      cb = fmaf(cL[m * dsub + j], b[j], cb);
+    }
+    term1[L * (M * 256) + e] = fmaf(2.f, cb, bn);
+  }
+}
+
+#ifndef FS_PRE_N
+#define FS_PRE_N 3
+#endif
+constexpr int PRE_N = FS_PRE_N;  // groups per CTA (a fourth fits -- no resident codebook -- but measures the same)
+constexpr int PRE_THREADS = SCAN_THREADS * PRE_N;
+
+template <int NQ, int M>
+__global__ void __launch_bounds__(PRE_THREADS, 1) ivfpq_scan_pre_kernel(const ScanArgs a, unsigned int* __restrict__ work,
+                                                                         int64_t n_items) {
+  extern __shared__ __align__(1024) unsigned char scan_smem[];
+  constexpr int K = 32 * NQ;
+  constexpr int NB = 2;
+  constexpr int MW = M / 4;
+  constexpr int REP = 32 / M;
+  constexpr int NE = M * 256 / SCAN_THREADS;  // table entries per thread
+  static_assert(SCAN_WARPS * K * 8 <= 256 * 32 * 4, "merge area must fit the table it aliases");
+  const int d = a.d, dsub = a.dsub, dpad = (d + 3) & ~3;
+  const int gid = threadIdx.x / SCAN_THREADS, tid = threadIdx.x % SCAN_THREADS, lane = tid & 31, warp = tid >> 5;
+  const size_t grp_bytes = (size_t)256 * 32 * 4 + (size_t)M * 256 * 4 + (size_t)dpad * 4 +
+                           (size_t)SCAN_WARPS * warp_select_smem_keys<NB>() * 8;
+  unsigned char* gbase = scan_smem + gid * grp_bytes;
+  uint32_t* lut = reinterpret_cast<uint32_t*>(gbase);
+  float* t3 = reinterpret_cast<float*>(lut + 256 * 32);
+  float* r = t3 + M * 256;
+  uint64_t* bufs = reinterpret_cast<uint64_t*>(r + dpad);
+  uint64_t* merge = reinterpret_cast<uint64_t*>(lut);  // the table is dead when the queues are merged
+  __shared__ uint32_t grp_bound[PRE_N];
+  __shared__ int grp_item[PRE_N];
+
+  WarpSelect<NQ, NB> sel;
+  sel.init(bufs + warp * warp_select_smem_keys<NB>(), lane);
+  unsigned long long bytes = 0;
+  const int rot = lane % M;
+  const int my_m = lane % M, cofs = lane / M;
+  const float my_bmax = a.bmax[my_m];
+  const uint32_t lutb = (uint32_t)__cvta_generic_to_shared(lut);
+  uint32_t base[M];
+#pragma unroll
+  for (int s = 0; s < M; ++s) base[s] = lutb + (((lane + s) & 31) << 2);
+
+  while (true) {
+    group_sync(gid);  // the previous item's merge is done with the table / merge area
+    if (tid == 0) {
+      grp_item[gid] = (int)atomicAdd(work, 1u);
+      grp_bound[gid] = 0x7F800000u;
+    }
+    group_sync(gid);
+    const int64_t item = grp_item[gid];
+    if (item >= n_items) break;
+    const int64_t q = item / a.ngroups;
+    const int g = (int)(item - q * a.ngroups);
+    const int p_begin = g * a.G;
+    const int p_end = (p_begin + a.G) < a.nprobe ? (p_begin + a.G) : a.nprobe;
+    sel.reset();
+    // term 3 of this query, in the lane order of the build: entry e = step * 32 + lane
+    for (int e = tid; e < M * 256; e += SCAN_THREADS) {
+      const int st = e >> 5, ln = e & 31;
+      const int m = ln % M, c = st * REP + ln / M;
+      const float* b = a.pq + ((int64_t)m * 256 + c) * dsub;
+      const float* xm = a.xq + q * d + m * dsub;
+      float acc = 0.f;
+      for (int j = 0; j < dsub; ++j) acc = fmaf(__ldg(xm + j), __ldg(b + j), acc);
+      t3[e] = -2.f * acc;
+    }
+
+    // The dependent loads of a list (probe id -> list bounds, centroid) are issued one and two
+    // lists ahead and stay in registers: none of their latency is on the path.
+    const float xj = tid < d ? a.xq[q * d + tid] : 0.f;
+    const int64_t* pid = a.probe_ids + q * a.nprobe;
+    int64_t L1 = pid[p_begin];
+    int64_t L2 = p_begin + 1 < p_end ? pid[p_begin + 1] : -1;
+    int64_t lb1 = 0, le1 = 0;
+    float c1 = 0.f;
+    if (L1 >= 0) {
+      lb1 = a.offsets[L1];
+      le1 = a.offsets[L1 + 1];
+      if (tid < d) c1 = a.coarse[L1 * d + tid];
+    }
+    for (int p = p_begin; p < p_end; ++p) {
+      const int64_t L = L1, lb = lb1, le = le1;
+      const float cj = c1;
+      L1 = L2;
+      if (L1 >= 0) {
+        lb1 = a.offsets[L1];
+        le1 = a.offsets[L1 + 1];
+        if (tid < d) c1 = a.coarse[L1 * d + tid];
+      }
+      L2 = p + 2 < p_end ? pid[p + 2] : -1;
+      if (a.out_probed && tid == 0) a.out_probed[q * a.nprobe + p] = (int32_t)L;
+      if (L < 0 || le == lb) continue;  // empty lists are probed and contribute nothing
+      const int len = (int)(le - lb);
+      // term 1 of this list: this thread's NE entries, requested before anything waits
+      float t1[NE];
+      const float* t1g = a.term1 + L * (M * 256) + warp * 32 + lane;
+#pragma unroll
+      for (int i = 0; i < NE; ++i) t1[i] = __ldg(t1g + i * SCAN_THREADS);
+      group_sync(gid);  // previous list's table is no longer read (and t3 is complete)
+      const uint8_t* cl = a.codes + lb * M;
+      uint32_t nxt[MW] = {};
+      if (tid < len) load_code<MW>(cl + (size_t)tid * M, nxt);
+      if (tid < d) r[tid] = xj - cj;
+      group_sync(gid);
+      // term 2 of this lane's sub-quantizer, and the scale from the bound
+      float n = 0.f;
+      for (int j = 0; j < dsub; ++j) {
+        const float v = r[my_m * dsub + j];
+        n = fmaf(v, v, n);
+      }
+      float u = sqrtf(n) + my_bmax;
+      u = u * u * 1.001f;
+#pragma unroll
+      for (int sft = 16; sft >= 1; sft >>= 1) u = fmaxf(u, __shfl_xor_sync(kFull, u, sft));
+      int ex = 0;
+      if (u > 0.f && u < 3.0e38f) frexpf(u, &ex);  // u < 2^ex
+      int se = 27 - ex;                            // scaled entries < 2^27
+      se = se > 100 ? 100 : (se < -100 ? -100 : se);
+      const float scale = __uint_as_float((uint32_t)(127 + se) << 23);
+      const float inv_scale = __uint_as_float((uint32_t)(127 - se) << 23);
+      const float cap = u;  // the bound also clamps from above: rounding cannot push an entry past it
+#pragma unroll
+      for (int i = 0; i < NE; ++i) {
+        const int st = warp + i * SCAN_WARPS;  // entry e = st * 32 + lane
+        const int c = st * REP + cofs;
+        float t = (t1[i] + t3[st * 32 + lane]) + n;
+        t = fminf(fmaxf(t, 0.f), cap);
+        const uint32_t v = __float2uint_rn(t * scale);
+#pragma unroll
+        for (int rep = 0; rep < REP; ++rep) lut[c * 32 + my_m + ((rep + cofs) % REP) * M] = v;
+      }
+      group_sync(gid);
+      // C3 + C4: scan and select
+      if (tid == 0) bytes += (unsigned long long)len * M;
+      const uint32_t pos0 = (uint32_t)lb;
+      for (int v0 = warp * 32; v0 < len; v0 += SCAN_THREADS) {
+        const int v = v0 + lane;
+        const bool ok = v < len;
+        uint32_t w[MW];
+#pragma unroll
+        for (int i = 0; i < MW; ++i) w[i] = nxt[i];
+        if (v + SCAN_THREADS < len) load_code<MW>(cl + (size_t)(uint32_t)(v + SCAN_THREADS) * M, nxt);
+        float dist = 0.f;
+        if (ok) {
+          rotate_bytes<MW>(w, rot);
+          uint32_t acc = 0u;
+          rot_gather<0, M>(w, base, acc);
+          dist = (float)acc * inv_scale;
+        }
+        const float bound = fminf(sel.thr_val, __uint_as_float(*reinterpret_cast<volatile uint32_t*>(grp_bound + gid)));
+        const bool cand = ok && !(dist > bound);
+        if (__any_sync(kFull, cand)) {
+          const uint64_t key = make_key(dist, pos0 + (uint32_t)v);
+          const uint64_t thr_before = sel.thr;
+          sel.push(cand && sel.wants(key), key);
+          if (sel.thr != thr_before && lane == 0) atomicMin(grp_bound + gid, __float_as_uint(sel.thr_val));
+        }
+      }
+    }
+    sel.finish();
+    group_sync(gid);  // every warp is done with the table: the merge area takes its place
+#pragma unroll
+    for (int rr = 0; rr < NQ; ++rr) merge[warp * K + rr * 32 + lane] = sel.W[rr];
+    group_sync(gid);
+    if (warp == 0) {
+      sel.reset();
+      for (int e0 = 0; e0 < SCAN_WARPS * K; e0 += 32) {
+        const uint64_t key = merge[e0 + lane];
+        sel.push(key < sel.thr, key);
+      }
+      sel.finish();
+      uint64_t* W = a.Wg + item * K;
+#pragma unroll
+      for (int rr = 0; rr < NQ; ++rr) W[rr * 32 + lane] = sel.W[rr];
+    }
+  }
+  if (tid == 0 && bytes) atomicAdd(a.scanned, bytes);
+}
+
+template <int NQ, int M>
+int launch_scan_pre(const ScanArgs& a, int64_t nq, unsigned int* work, cudaStream_t s) {
+  const size_t grp_bytes = (size_t)256 * 32 * 4 + (size_t)M * 256 * 4 + (size_t)((a.d + 3) & ~3) * 4 +
+                           (size_t)SCAN_WARPS * warp_select_smem_keys<2>() * 8;
+  const size_t smem = PRE_N * grp_bytes;
+  if (smem > 227 * 1024) return set_error(FS_EUNSUPPORTED, "fs_ivfpq_search: shared memory (%zu B) exceeds 227 KB", smem);
+  static size_t attr_smem = 0;
+  if (smem > attr_smem) {
+    FS_CUDA(cudaFuncSetAttribute(ivfpq_scan_pre_kernel<NQ, M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    attr_smem = smem;
+  }
+  const int64_t n_items = nq * a.ngroups;
+  int64_t grid = sm_count();
+  if (grid * PRE_N > n_items) grid = ceil_div(n_items, (int64_t)PRE_N);
+  FS_CUDA(cudaMemsetAsync(work, 0, sizeof(unsigned int), s));
+  ivfpq_scan_pre_kernel<NQ, M><<<(unsigned)grid, PRE_THREADS, smem, s>>>(a, work, n_items);
+  FS_LAUNCHED();
+  return FS_OK;
+}
+
 template <int NQ, int M, int DS>
 int launch_scan_grp(const ScanArgs& a, int64_t nq, unsigned int* work, cudaStream_t s) {
   const size_t grp_bytes = (size_t)256 * 32 * 4 + (size_t)((a.d + 3) & ~3) * 4 +
@@ -805,19 +1057,17 @@ int launch_scan_m(const ScanArgs& a, int64_t nq, cudaStream_t s) {
 
 template <int NQ>
 int launch_scan(const ScanArgs& a, int64_t nq, cudaStream_t s) {
-  // Three scan kernels (profiles/r01_ivfpq.md): pair = float tables, one CTA per item; rot = fixed-point
+  // Scan kernels (profiles/r01_ivfpq.md): pair = float tables, one CTA per item; rot = fixed-point
   // conflict-free tables, one CTA per item; grp = the same in persistent groups with the codebook
-  // resident in shared memory.  Default: grp where it is measured faster (items of >= 32 lists, enough
-  // items to fill the persistent groups), else pair.  FS_IVFPQ_SCAN=pair|rot|grp forces one (A/B runs).
-  static int forced = -1;
-  if (forced < 0) {
-    const char* e = getenv("FS_IVFPQ_SCAN");
-    forced = !e ? 0 : strcmp(e, "pair") == 0 ? 3 : strcmp(e, "rot") == 0 ? 1 : strcmp(e, "grp") == 0 ? 2 : 0;
-  }
+  // resident in shared memory; pre = grp with the table built from the Eq. 11 terms.  Default: pre
+  // (else grp) where the grouped kernels are measured faster (M = 16, items of >= 32 lists, enough
+  // items to fill the persistent groups), else pair.  FS_IVFPQ_SCAN=pair|rot|grp|pre forces one (A/B runs).
+  const int forced = scan_forced_mode();
   int mode = forced == 3 ? 0 : forced;
-  // (M = 8: half the lookups per vector, the float kernel stays ahead: 7.7 against 9.7 ms, cfg5 shape)
-  if (forced == 0 && a.M == 16 && a.G >= 32 && nq * a.ngroups >= (int64_t)3 * GRP_N * sm_count()) mode = 2;
+  if (forced == 0 && scan_auto_grouped(a.M, a.G, nq * a.ngroups)) mode = a.term1 ? 4 : 2;
   if constexpr (NQ <= 8) {
+    if (mode == 4 && a.len32 && a.term1 && a.bmax && a.d <= SCAN_THREADS && a.M == 16)
+      return launch_scan_pre<NQ, 16>(a, nq, a.work, s);
     const bool fx = a.len32 && a.pq_r;
     if (mode == 2 && fx && a.d <= SCAN_THREADS && a.M == 16 && a.dsub == 6) return launch_scan_grp<NQ, 16, 6>(a, nq, a.work, s);
     if (mode == 2 && fx && a.d <= SCAN_THREADS && a.M == 8 && a.dsub == 12) return launch_scan_grp<NQ, 8, 12>(a, nq, a.work, s);
@@ -882,15 +1132,30 @@ int ivfpq_search_device(fs_ivfpq* ix, const float* xq, int64_t nq, int nprobe, i
   if ((ix->M == 16 && (ix->dsub == 6 || ix->dsub == 8)) || (ix->M == 8 && (ix->dsub == 12 || ix->dsub == 16))) {
     float* pq_t = reinterpret_cast<float*>(w + p.off_pqt);
     float* pq_r = reinterpret_cast<float*>(w + p.off_pqr);
-    float* bmax = pq_r + (size_t)256 * ix->d;
     const int n = 256 * ix->d;
     pq_regroup_kernel<<<ceil_div(n, 256), 256, 0, s>>>(a.pq, pq_t, pq_r, ix->M, ix->dsub, ix->dsub == 6 ? 2 : 4);
     FS_LAUNCHED();
-    pq_bmax_kernel<<<ix->M, 32, 0, s>>>(a.pq, bmax, ix->dsub);
-    FS_LAUNCHED();
     a.pq_t = pq_t;
     a.pq_r = pq_r;
+  }
+  if (ix->M == 16 || ix->M == 8) {
+    float* bmax = reinterpret_cast<float*>(w + p.off_pqr) + (size_t)256 * ix->d;
+    pq_bmax_kernel<<<ix->M, 32, 0, s>>>(a.pq, bmax, ix->dsub);
+    FS_LAUNCHED();
     a.bmax = bmax;
+  }
+  // Eq. 11 term 1 for every list (16 KB per list at M = 16): built by the first search that wants it
+  a.term1 = nullptr;
+  if (want_term1(ix) && (scan_forced_pre() || scan_auto_grouped(ix->M, p.G, nq * p.ngroups))) {
+    if (!ix->term1_valid) {
+      const size_t tb = (size_t)ix->nlist * ix->M * 256 * sizeof(float);
+      if ((rc = ix->term1.ensure(tb, 0, s)) != FS_OK) return rc;
+      ivfpq_term1_kernel<16><<<(unsigned)ix->nlist, 256, 0, s>>>(ix->coarse.as<float>(), a.pq, ix->term1.as<float>(),
+                                                                ix->d, ix->dsub);
+      FS_LAUNCHED();
+      ix->term1_valid = true;
+    }
+    a.term1 = ix->term1.as<float>();
   }
   a.probe_ids = cids;
   a.offsets = ix->offsets.as<int64_t>();

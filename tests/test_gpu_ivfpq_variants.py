@@ -13,7 +13,7 @@ pytestmark = pytest.mark.gpu
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-@pytest.mark.parametrize("variant", ["pair", "rot", "grp", "persistent", "c1-fused", "c1-matrix-multipass", "c1-matrix-long-rows"])
+@pytest.mark.parametrize("variant", ["pair", "rot", "grp", "pre", "persistent", "c1-fused", "c1-matrix-multipass", "c1-matrix-long-rows"])
 def test_scan_variant(variant):
     if variant == "c1-fused":          # C1 on the fused engine whatever the shape
         env = dict(os.environ, FS_IVFPQ_C1="fused")
