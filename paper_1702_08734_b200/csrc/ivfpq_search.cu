@@ -329,7 +329,8 @@ bool want_term1(const fs_ivfpq* ix) {
     const char* e = getenv("FS_IVFPQ_SCAN");
     on = !e ? 1 : strcmp(e, "pre") == 0 ? 1 : 0;
   }
-  return on && ix->M == 16 && ix->d <= SCAN_THREADS && (size_t)ix->nlist * 16 * 256 * sizeof(float) <= ((size_t)4 << 30);
+  return on && (ix->M == 16 || (ix->M == 8 && scan_forced_pre())) && ix->d <= SCAN_THREADS &&
+         (size_t)ix->nlist * ix->M * 256 * sizeof(float) <= ((size_t)4 << 30);
 }
 
 __global__ void widen_ids_kernel(const int32_t* __restrict__ in, int64_t* __restrict__ out, int64_t n) {
@@ -1068,6 +1069,8 @@ int launch_scan(const ScanArgs& a, int64_t nq, cudaStream_t s) {
   if constexpr (NQ <= 8) {
     if (mode == 4 && a.len32 && a.term1 && a.bmax && a.d <= SCAN_THREADS && a.M == 16)
       return launch_scan_pre<NQ, 16>(a, nq, a.work, s);
+    if (mode == 4 && a.len32 && a.term1 && a.bmax && a.d <= SCAN_THREADS && a.M == 8)
+      return launch_scan_pre<NQ, 8>(a, nq, a.work, s);
     const bool fx = a.len32 && a.pq_r;
     if (mode == 2 && fx && a.d <= SCAN_THREADS && a.M == 16 && a.dsub == 6) return launch_scan_grp<NQ, 16, 6>(a, nq, a.work, s);
     if (mode == 2 && fx && a.d <= SCAN_THREADS && a.M == 8 && a.dsub == 12) return launch_scan_grp<NQ, 8, 12>(a, nq, a.work, s);
@@ -1150,8 +1153,12 @@ int ivfpq_search_device(fs_ivfpq* ix, const float* xq, int64_t nq, int nprobe, i
     if (!ix->term1_valid) {
       const size_t tb = (size_t)ix->nlist * ix->M * 256 * sizeof(float);
       if ((rc = ix->term1.ensure(tb, 0, s)) != FS_OK) return rc;
-      ivfpq_term1_kernel<16><<<(unsigned)ix->nlist, 256, 0, s>>>(ix->coarse.as<float>(), a.pq, ix->term1.as<float>(),
-                                                                ix->d, ix->dsub);
+      if (ix->M == 16)
+        ivfpq_term1_kernel<16><<<(unsigned)ix->nlist, 256, 0, s>>>(ix->coarse.as<float>(), a.pq, ix->term1.as<float>(),
+                                                                  ix->d, ix->dsub);
+      else
+        ivfpq_term1_kernel<8><<<(unsigned)ix->nlist, 256, 0, s>>>(ix->coarse.as<float>(), a.pq, ix->term1.as<float>(),
+                                                                 ix->d, ix->dsub);
       FS_LAUNCHED();
       ix->term1_valid = true;
     }
