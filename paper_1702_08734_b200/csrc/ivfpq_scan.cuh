@@ -50,6 +50,26 @@ __device__ __forceinline__ void rotate_bytes(uint32_t (&w)[MW], int r) {
   for (int i = 0; i < MW; ++i) w[i] = t[i];
 }
 
+// out byte i = in byte (i ^ r) of the MW-word little-endian value w (r < 4 MW, per-lane constant):
+// the fixed-point kernels let lane l add sub-quantizer (s ^ l) mod M at step s (any order gives the
+// same integer sum), so that step s reads bank l ^ s -- 32 different banks -- and the address is one
+// XOR away from a per-lane constant.
+template <int MW>
+__device__ __forceinline__ void xor_permute_bytes(uint32_t (&w)[MW], int r) {
+  const uint32_t sel = 0x3210u ^ (0x1111u * (uint32_t)(r & 3));  // nibble i -> i ^ (r & 3)
+#pragma unroll
+  for (int i = 0; i < MW; ++i) w[i] = __byte_perm(w[i], 0u, sel);
+#pragma unroll
+  for (int bit = 1; bit < MW; bit <<= 1) {
+    const bool on = ((r >> 2) & bit) != 0;
+    uint32_t t[MW];
+#pragma unroll
+    for (int i = 0; i < MW; ++i) t[i] = on ? w[i ^ bit] : w[i];
+#pragma unroll
+    for (int i = 0; i < MW; ++i) w[i] = t[i];
+  }
+}
+
 // Packed fp32 pairs (sm_100 FADD2 / FFMA2): two lanes of a 64-bit register per instruction
 __device__ __forceinline__ uint64_t f2_pack(float a, float b) {
   uint64_t r;

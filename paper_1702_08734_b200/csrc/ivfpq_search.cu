@@ -321,15 +321,11 @@ bool scan_auto_grouped(int M, int G, int64_t n_items) {
   return scan_forced_mode() == 0 && M == 16 && G >= 32 && n_items >= (int64_t)9 * sm_count();  // 3 rounds of 3 groups per SM
 }
 
-// The decomposed table build needs M = 16 and nlist * 16 KB of device memory (<= 4 GB here); it is
-// the default wherever the grouped fixed-point scan is (launch_scan), FS_IVFPQ_SCAN=pre forces it.
+// The decomposed table build (FS_IVFPQ_SCAN=pre) needs M = 8 / 16 and nlist * M * 1 KB of device memory
+// (<= 4 GB here).  Measured level with the direct build once both scans use the XOR order (9.26 against
+// 8.89 ms at nprobe 64): kept as a forced variant, not the default.
 bool want_term1(const fs_ivfpq* ix) {
-  static int on = -1;
-  if (on < 0) {
-    const char* e = getenv("FS_IVFPQ_SCAN");
-    on = !e ? 1 : strcmp(e, "pre") == 0 ? 1 : 0;
-  }
-  return on && (ix->M == 16 || (ix->M == 8 && scan_forced_pre())) && ix->d <= SCAN_THREADS &&
+  return scan_forced_pre() && (ix->M == 16 || ix->M == 8) && ix->d <= SCAN_THREADS &&
          (size_t)ix->nlist * ix->M * 256 * sizeof(float) <= ((size_t)4 << 30);
 }
 
@@ -430,6 +426,18 @@ __device__ __forceinline__ void rot_gather(const uint32_t* w, const uint32_t* ba
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(base[s] + c * 128u));
     acc += v;
     rot_gather<s + 1, M>(w, base, acc);
+  }
+}
+
+// acc += lut[byte s of w][bank lane ^ s] for s = s0 .. M-1; A = table + 4 * lane (table 128-byte aligned)
+template <int s, int M>
+__device__ __forceinline__ void xor_gather(const uint32_t* w, uint32_t A, uint32_t& acc) {
+  if constexpr (s < M) {
+    const uint32_t c = __byte_perm(w[s >> 2], 0u, 0x4440u + (s & 3));  // byte s, zero-extended
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"((A ^ (4u * s)) + c * 128u));
+    acc += v;
+    xor_gather<s + 1, M>(w, A, acc);
   }
 }
 
@@ -620,9 +628,7 @@ __global__ void __launch_bounds__(GRP_THREADS, 1) ivfpq_scan_grp_kernel(const Sc
   const int my_m = lane % M, cofs = lane / M;
   const float my_bmax = a.bmax[my_m];
   const uint32_t lutb = (uint32_t)__cvta_generic_to_shared(lut);
-  uint32_t base[M];
-#pragma unroll
-  for (int s = 0; s < M; ++s) base[s] = lutb + (((lane + s) & 31) << 2);
+  const uint32_t lane_base = lutb + ((uint32_t)lane << 2);  // step s reads bank lane ^ s
 
   while (true) {
     group_sync(gid);  // the previous item's merge is done with the table / merge area
@@ -729,9 +735,9 @@ __global__ void __launch_bounds__(GRP_THREADS, 1) ivfpq_scan_grp_kernel(const Sc
         if (v + SCAN_THREADS < len) load_code<MW>(cl + (size_t)(uint32_t)(v + SCAN_THREADS) * M, nxt);
         float dist = 0.f;
         if (ok) {
-          rotate_bytes<MW>(w, rot);
+          xor_permute_bytes<MW>(w, rot);
           uint32_t acc = 0u;
-          rot_gather<0, M>(w, base, acc);
+          xor_gather<0, M>(w, lane_base, acc);
           dist = (float)acc * inv_scale;
         }
         const float bound = fminf(sel.thr_val, __uint_as_float(*reinterpret_cast<volatile uint32_t*>(grp_bound + gid)));
@@ -830,9 +836,6 @@ __global__ void __launch_bounds__(PRE_THREADS, 1) ivfpq_scan_pre_kernel(const Sc
   const int my_m = lane % M, cofs = lane / M;
   const float my_bmax = a.bmax[my_m];
   const uint32_t lutb = (uint32_t)__cvta_generic_to_shared(lut);
-  uint32_t base[M];
-#pragma unroll
-  for (int s = 0; s < M; ++s) base[s] = lutb + (((lane + s) & 31) << 2);
 
   while (true) {
     group_sync(gid);  // the previous item's merge is done with the table / merge area
@@ -925,6 +928,7 @@ __global__ void __launch_bounds__(PRE_THREADS, 1) ivfpq_scan_pre_kernel(const Sc
       }
       group_sync(gid);
       // C3 + C4: scan and select
+      const uint32_t lane_base = lutb + ((uint32_t)lane << 2);  // step s reads bank lane ^ s
       if (tid == 0) bytes += (unsigned long long)len * M;
       const uint32_t pos0 = (uint32_t)lb;
       for (int v0 = warp * 32; v0 < len; v0 += SCAN_THREADS) {
@@ -936,9 +940,9 @@ __global__ void __launch_bounds__(PRE_THREADS, 1) ivfpq_scan_pre_kernel(const Sc
         if (v + SCAN_THREADS < len) load_code<MW>(cl + (size_t)(uint32_t)(v + SCAN_THREADS) * M, nxt);
         float dist = 0.f;
         if (ok) {
-          rotate_bytes<MW>(w, rot);
+          xor_permute_bytes<MW>(w, rot);
           uint32_t acc = 0u;
-          rot_gather<0, M>(w, base, acc);
+          xor_gather<0, M>(w, lane_base, acc);
           dist = (float)acc * inv_scale;
         }
         const float bound = fminf(sel.thr_val, __uint_as_float(*reinterpret_cast<volatile uint32_t*>(grp_bound + gid)));
@@ -1060,12 +1064,12 @@ template <int NQ>
 int launch_scan(const ScanArgs& a, int64_t nq, cudaStream_t s) {
   // Scan kernels (profiles/r01_ivfpq.md): pair = float tables, one CTA per item; rot = fixed-point
   // conflict-free tables, one CTA per item; grp = the same in persistent groups with the codebook
-  // resident in shared memory; pre = grp with the table built from the Eq. 11 terms.  Default: pre
-  // (else grp) where the grouped kernels are measured faster (M = 16, items of >= 32 lists, enough
-  // items to fill the persistent groups), else pair.  FS_IVFPQ_SCAN=pair|rot|grp|pre forces one (A/B runs).
+  // resident in shared memory; pre = grp with the table built from the Eq. 11 terms.  Default: grp
+  // where it is measured faster (M = 16, items of >= 32 lists, enough items to fill the persistent
+  // groups), else pair.  FS_IVFPQ_SCAN=pair|rot|grp|pre forces one (A/B runs).
   const int forced = scan_forced_mode();
   int mode = forced == 3 ? 0 : forced;
-  if (forced == 0 && scan_auto_grouped(a.M, a.G, nq * a.ngroups)) mode = a.term1 ? 4 : 2;
+  if (forced == 0 && scan_auto_grouped(a.M, a.G, nq * a.ngroups)) mode = 2;
   if constexpr (NQ <= 8) {
     if (mode == 4 && a.len32 && a.term1 && a.bmax && a.d <= SCAN_THREADS && a.M == 16)
       return launch_scan_pre<NQ, 16>(a, nq, a.work, s);
@@ -1149,7 +1153,7 @@ int ivfpq_search_device(fs_ivfpq* ix, const float* xq, int64_t nq, int nprobe, i
   }
   // Eq. 11 term 1 for every list (16 KB per list at M = 16): built by the first search that wants it
   a.term1 = nullptr;
-  if (want_term1(ix) && (scan_forced_pre() || scan_auto_grouped(ix->M, p.G, nq * p.ngroups))) {
+  if (want_term1(ix)) {
     if (!ix->term1_valid) {
       const size_t tb = (size_t)ix->nlist * ix->M * 256 * sizeof(float);
       if ((rc = ix->term1.ensure(tb, 0, s)) != FS_OK) return rc;
