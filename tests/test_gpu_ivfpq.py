@@ -313,3 +313,27 @@ def test_c1_large_nlist():
     offs, codes, lids = (t.cpu().numpy() for t in ix.export())
     check_search(ix, coarse, pq, offs, codes, lids, xq, nprobe, k)
     ix.close()
+
+
+@pytest.mark.parametrize("d,M,nlist,nq,nprobe,k", [
+    (96, 16, 16, 300, 16, 5),      # nprobe = nlist = 16: the k-selection of C1 takes every column
+    (96, 16, 17, 257, 17, 100),    # nlist not a multiple of 4: padded row stride of the distance matrix
+    (96, 8, 33, 400, 33, 1),
+    (64, 16, 40, 1000, 40, 10),
+    (128, 16, 20, 260, 16, 7),
+    (96, 16, 64, 3000, 48, 100),   # >= 32 lists per item and enough items: grouped fixed-point scan
+])
+def test_c1_matrix_and_scan_edge_shapes(d, M, nlist, nq, nprobe, k):
+    """nq >= 256 and nprobe >= 16 on small coarse quantizers: C1 through the distance matrix, with the
+    scan kernel the dispatch picks for the shape (DESIGN 5.3)."""
+    rng = np.random.default_rng(nlist * 1000 + nq)
+    coarse = rng.standard_normal((nlist, d)).astype(np.float32)
+    pq = (0.2 * rng.standard_normal((M, 256, d // M))).astype(np.float32)
+    nb = 5000
+    xb = (coarse[rng.integers(0, nlist, nb)] + 0.3 * rng.standard_normal((nb, d))).astype(np.float32)
+    xq = (coarse[rng.integers(0, nlist, nq)] + 0.3 * rng.standard_normal((nq, d))).astype(np.float32)
+    ix = make_index(d, nlist, M, coarse, pq)
+    ix.add(torch.from_numpy(xb).cuda())
+    offs, codes, lids = (t.cpu().numpy() for t in ix.export())
+    check_search(ix, coarse, pq, offs, codes, lids, xq, nprobe, k)
+    ix.close()
