@@ -55,6 +55,14 @@ constexpr int TMA_WARP = EPI_GROUPS * 4, MMA_WARP = EPI_GROUPS * 4 + 1;
 constexpr int EPI_RB = 4;                     // radix digit width of the epilogue selection (1 KB of counters per warp)
 constexpr int STAGE_KEYS = 256;               // row buffers up to this size are selected in shared memory
 constexpr int SCRATCH_BYTES = EPI_GROUPS * 4 * ((1 << EPI_RB) * 64 + STAGE_KEYS * 8);  // 8 warps x (1 KB + 2 KB)
+#ifndef FS_TC_EAGER
+#define FS_TC_EAGER 48
+#endif
+#ifndef FS_TC_EAGER_Q
+#define FS_TC_EAGER_Q 3
+#endif
+constexpr int EAGER_EXTRA = FS_TC_EAGER;       // idle-time restore of rows holding >= k + max(this, k * FS_TC_EAGER_Q / 4) keys
+                                              // (sweep in profiles/r01_flat.md)
 constexpr int HB_LEVELS = 3;                  // hierarchical bound: levels 1..3 (2, 4, 8 queues)
 constexpr int HB_SLOTS = 2 + 4 + 8;
 constexpr int SMEM_LIMIT = 227 * 1024;
@@ -385,6 +393,11 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
         const uint32_t as = tile_count & 1u;
         const int64_t col0 = b_begin + (int64_t)t * BN;
         const int ncols = (int)(b_end - col0 < BN ? b_end - col0 : BN);
+        // The accumulator is not ready (the other epilogue group or the peer CTA holds the pipeline
+        // back): restore the rows that already hold more than k keys now instead of spinning -- it
+        // tightens their bounds early and takes restore work off the path of later tiles.
+        if (k > 1 && a.dout == nullptr && !__all_sync(kFull, sm100::mbar_test(tfull + as, (tile_count >> 1) & 1u)))
+          flush_rows(cnt >= k + (EAGER_EXTRA > (k * FS_TC_EAGER_Q >> 2) ? EAGER_EXTRA : (k * FS_TC_EAGER_Q >> 2)), false);
         sm100::mbar_wait(tfull + as, (tile_count >> 1) & 1u);
         sm100::tc_fence_after();
         const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + as * BN;
