@@ -55,6 +55,9 @@ constexpr int TMA_WARP = EPI_GROUPS * 4, MMA_WARP = EPI_GROUPS * 4 + 1;
 constexpr int EPI_RB = 4;                     // radix digit width of the epilogue selection (1 KB of counters per warp)
 constexpr int STAGE_KEYS = 256;               // row buffers up to this size are selected in shared memory
 constexpr int SCRATCH_BYTES = EPI_GROUPS * 4 * ((1 << EPI_RB) * 64 + STAGE_KEYS * 8);  // 8 warps x (1 KB + 2 KB)
+#ifndef FS_TC_REFRESH
+#define FS_TC_REFRESH 8  // tiles between two looks at the published bounds (power of two)
+#endif
 #ifndef FS_TC_EAGER
 #define FS_TC_EAGER 48
 #endif
@@ -319,7 +322,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
         }
       }
       if (gb > 0xFF800000u) gb = 0xFF800000u;  // no bound yet: +inf
-      const uint64_t thr0 = valid ? (((uint64_t)gb << 32) | 0xFFFFFFFFull) : 0ull;
+      uint64_t thr0 = valid ? (((uint64_t)gb << 32) | 0xFFFFFFFFull) : 0ull;
       uint64_t thr_key = thr0;
       float thr_val = valid ? ord_f32((uint32_t)(thr0 >> 32)) : __uint_as_float(0xFF800000u);
       int cnt = 0;  // keys in this row's buffer: the winners so far, then new candidates
@@ -385,12 +388,26 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
             thr_key = kth < thr0 ? kth : thr0;
             thr_val = key_val(thr_key);
             cnt = k;
+            // this queue's k-th distance bounds the query's: splits running now may use it at once
+            if (kth < thr0) atomicMin(a.gbound + q, (unsigned int)(kth >> 32));
           }
         }
       };
 
       for (int t = 0; t < ntiles; ++t, ++tile_count) {
         const uint32_t as = tile_count & 1u;
+        if (k > 1 && (t & (FS_TC_REFRESH - 1)) == (FS_TC_REFRESH - 1) && valid) {
+          // adopt what the other splits of this query have published since the item began
+          const uint32_t g2 = *reinterpret_cast<volatile unsigned int*>(a.gbound + q);
+          const uint64_t t2 = ((uint64_t)g2 << 32) | 0xFFFFFFFFull;
+          if (t2 < thr0) {
+            thr0 = t2;
+            if (t2 < thr_key) {
+              thr_key = t2;
+              thr_val = ord_f32(g2);
+            }
+          }
+        }
         const int64_t col0 = b_begin + (int64_t)t * BN;
         const int ncols = (int)(b_end - col0 < BN ? b_end - col0 : BN);
         // The accumulator is not ready (the other epilogue group or the peer CTA holds the pipeline
