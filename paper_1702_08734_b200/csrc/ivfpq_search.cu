@@ -301,10 +301,10 @@ bool c1_matrix(int64_t nq, int64_t nlist, int nprobe, int d) {
   if (forced == 1) return false;
   if (forced == 2) return true;
   if (nprobe < 16 || nq < 256) return false;
-  // measured (nq = 10^4, d = 96; search of a tiny index, ms, fused / matrix): nlist 8 192: nprobe 16
-  // 1.40 / 0.81, 256 9.07 / 6.83; nlist 65 536: 16 2.04 / 2.48, 64 3.49 / 3.11, 256 13.2 / 5.2;
-  // nlist 262 144: 128 8.7 / 12.0, 256 22.4 / 14.0
-  return nlist <= 16384 || (nprobe >= 64 && nlist <= 131072) || nprobe >= 256;
+  // measured (nq = 10^4, d = 96; search of a tiny index, ms, fused / matrix): nlist 8 192: nprobe 64
+  // 2.79 / 1.95, 256 8.25 / 6.30; nlist 65 536: 16 1.71 / 2.41, 64 2.85 / 2.97, 256 9.24 / 4.93;
+  // nlist 262 144: 64 4.98 / 11.1, 256 14.4 / 13.6
+  return nlist <= 16384 || (nprobe >= 128 && nlist <= 131072) || nprobe >= 256;
 }
 
 int scan_forced_mode() {  // 0 none, 1 rot, 2 grp, 3 pair, 4 pre
