@@ -49,6 +49,49 @@ def test_handworked_example():
     assert r2["probed"][0].tolist() == [0, 1] and r2["coarse64"][0].tolist() == [0.0, 20000.0]
 
 
+def test_handworked_margins():
+    """Pins the best/second-best margins of oracle.ivfpq_encode (the outputs the GPU parity
+    tests use to excuse near-ties) to values worked by hand in ivfpq_handworked.txt."""
+    g = load("ivfpq_handworked.txt")
+    coarse, pq = toy_quantizers()
+    y = g["y"].astype(np.float32).reshape(-1, 2)
+    lst, codes, cm, km = oracle.ivfpq_encode(coarse, pq, y, margins=True)
+    assert cm[0] == g["coarse_margin_y0_num"][0] / g["coarse_margin_y0_den"][0]
+    assert cm[2] == g["coarse_margin_y2_num"][0] / g["coarse_margin_y2_den"][0]
+    assert km[0].tolist() == g["code_margin_y0"].tolist()
+    assert km[2].tolist() == g["code_margin_y2"].tolist()      # exact codeword tie -> margin 0
+    # y1 = (101.4, 99.6) is not exact in fp32: residual ~(1.4, -0.4); sub-quantizer 0: best codeword 1
+    # at 0.4^2, second codeword 2 at 0.6^2 -> (0.36 - 0.16) / 0.36; sub-quantizer 1: 0.4^2 vs 0.6^2 too
+    assert np.allclose(km[1], [(0.36 - 0.16) / 0.36] * 2, rtol=0, atol=2e-5)
+    assert abs(cm[1] - (20202.12 - 2.12) / 20202.12) < 1e-9
+    e = g["extra"].astype(np.float32).reshape(-1, 2)
+    el, _, ecm, ekm = oracle.ivfpq_encode(coarse, pq, e, margins=True)
+    assert el.tolist() == g["extra_lists"].tolist()            # equidistant -> lower centroid
+    assert ecm.tolist() == g["extra_coarse_margin"].tolist()   # equidistant -> 0, on a centroid -> 1
+
+
+def test_margins_against_sorted_distances():
+    """Margins are (second - best) / second of the sorted distance lists (numpy, independent of
+    the oracle's running best/second update), in [0, 1], and 0 exactly where two candidates tie."""
+    rng = np.random.default_rng(11)
+    nlist, d, M, n = 7, 8, 4, 300
+    coarse = rng.integers(-3, 4, size=(nlist, d)).astype(np.float32)   # small integers: exact ties occur
+    pq = rng.integers(-2, 3, size=(M, 256, d // M)).astype(np.float32)
+    y = rng.integers(-4, 5, size=(n, d)).astype(np.float32)
+    lst, codes, cm, km = oracle.ivfpq_encode(coarse, pq, y, margins=True)
+    dc = ((y[:, None, :].astype(np.float64) - coarse[None]) ** 2).sum(-1)
+    s = np.sort(dc, axis=1)
+    want = (s[:, 1] - s[:, 0]) / np.maximum(s[:, 1], 1e-300)
+    assert np.array_equal(cm, want) and (cm == 0).any() and np.all((cm >= 0) & (cm <= 1))
+    assert np.array_equal(lst, dc.argmin(1))
+    r = (y.astype(np.float64) - coarse[lst]).reshape(n, M, d // M)
+    ds = ((r[:, :, None, :] - pq[None].astype(np.float64)) ** 2).sum(-1)   # [n, M, 256]
+    s = np.sort(ds, axis=2)
+    want = (s[:, :, 1] - s[:, :, 0]) / np.maximum(s[:, :, 1], 1e-300)
+    assert np.array_equal(km, want) and np.all((km >= 0) & (km <= 1))
+    assert np.array_equal(codes, ds.argmin(2))
+
+
 def test_lut_identity_eq10_and_eq11():
     """Reconstruction distance (Eq. 7) == sum of table look-ups (Eq. 10) ==
     term1 + term2 - 2 term3 (Eq. 11), to 1e-12 relative."""
