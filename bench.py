@@ -2,7 +2,7 @@
 """bench.py -- measures the hot path of arXiv 1702.08734 on B200 through the C ABI.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
-                    [--skip-also] [--ivfpq-nb NB]
+                    [--skip-also] [--skip-cfg5] [--no-cpu] [--ivfpq-nb NB]
 
 Headline (BASELINE.json configs[1], "k-select GB/s as % HBM peak"): one STEP is
 fs_kselect over the whole cfg2 batch -- 10 000 rows x 16 384 fp32 ~U[0,1) (1 % of
@@ -12,10 +12,12 @@ k = 1024.  value = algorithmic bytes (4 B per input eleme
 in HBM; e2e = the same step through fs_kselect_host from pinned HOST buffers, copies
 inside the timed region.  Inputs (1.19 GB per rank) are larger than the 126 MB L2.
 
-"also" (same JSON line): fs_flat_l2_knn on cfg3 (nb = 10^6, nq = 10^4, d = 128, SIFT-like
-integers, k = 1, 10, 100; rows B1-B4) in queries/s, and fs_ivfpq_search on a REDUCED
-cfg4-shaped index (rows C1-C5; the full 10^8-vector build does not fit a default run;
-see profiles/ for the full-size runs) in queries/s and code-scan GB/s.
+"also" (same JSON line; compact copies under roofline.also and cpu_baseline.also):
+fs_flat_l2_knn on cfg3 (nb = 10^6, nq = 10^4, d = 128, SIFT-like integers and real-valued
+data, k = 1, 10, 100; rows B1-B4) in queries/s and tensor-pipe fraction, and fs_ivfpq_search
+on cfg4 (10^8 vectors, nlist 65 536, M = 16) and cfg5 (10^9 vectors, nlist 262 144, M = 8) at
+their stated size (rows C1-C5, D1-D3 for the build) in queries/s, whole-search and
+scan-stage GB/s on code bytes; each with the oracle timed on a seeded query subset.
 
 With N > 1 (torchrun) every rank runs the same step on its own rows (the path
 partitions by row/query: no data-path collective): weak scaling, time = max
@@ -58,8 +60,9 @@ def peaks():
             j = json.load(f)
         return dict(hbm=float(j["hbm_gbs"]), bf16=float(j["bf16_tflops"]),
                     bf16_sustained=float(j.get("bf16_tflops_sustained", j["bf16_tflops"])),
-                    source="measured (MEASURED_PEAKS.json)")
-    return dict(hbm=6650.0, bf16=1590.0, bf16_sustained=1400.0, source="fallback (B200_PROFILING.md)")
+                    sm_max_mhz=float(j.get("sm_max_mhz", 1965.0)), source="measured (MEASURED_PEAKS.json)")
+    return dict(hbm=6650.0, bf16=1590.0, bf16_sustained=1400.0, sm_max_mhz=1965.0,
+                source="fallback (B200_PROFILING.md)")
 
 
 # ----------------------------------------------------------------------------
@@ -207,7 +210,10 @@ def timed(fn, reps, warm=1):
     return ts[0], ts[len(ts) // 2]
 
 
-def also_flat(fs, gt, pk):
+def also_flat(fs, gt, pk, cpu=True):
+    """fs_flat_l2_knn on cfg3; per k: the call as a user makes it (database norm / operand pre-pass
+    inside) and the tensor-pipe fraction; plus the oracle on a seeded query subset (cpu_baseline)."""
+    import numpy as np
     import torch
     nb, nq, d = 1_000_000, 10_000, 128
     tf32_peak = pk["bf16"] / 2.0  # dense TF32 = half the measured BF16 rate (B200_PROFILING.md nominal ratio)
@@ -223,30 +229,64 @@ def also_flat(fs, gt, pk):
         best, med = timed(lambda: fs.flat_l2_knn(xq, xb, k, out_dist=od, out_ids=oi, ws=ws), 3)
         tf = 2.0 * nb * nq * d / med / 1e9
         return {"ms": med, "queries_per_s": nq / med * 1e3, "tflops": tf, "issued_tflops": passes * tf,
-                "tensor_frac": passes * tf / tf32_peak}
+                "tensor_frac": passes * tf / tf32_peak}, od, oi
 
     xb = gt.sift_like(0, nb)
     xq = gt.sift_like(nb, nq)
+    res = {}
     for k in (1, 10, 100):
-        out["k%d" % k] = run(xq, xb, k, 1)
-    del xb, xq
+        out["k%d" % k], od, oi = run(xq, xb, k, 1)
+        res[k] = (od, oi)
+    if cpu:
+        import datagen
+        import oracle
+        sub = datagen.unique_sample_ids(64, nq, stream=36)
+        xs = xq[torch.from_numpy(sub).cuda()].cpu().numpy()
+        xb_h = xb.cpu().numpy()
+        oracle.flat_l2_knn(xs[:2], xb_h[:1000], 1)
+        t0 = time.perf_counter()
+        o = {k: oracle.flat_l2_knn(xs, xb_h, k) for k in (1, 10, 100)}
+        dt = time.perf_counter() - t0
+        st = torch.from_numpy(sub).cuda()
+        exact = all(np.array_equal(res[k][1][st].cpu().numpy(), o[k][1]) and
+                    np.array_equal(res[k][0][st].cpu().numpy(), o[k][0]) for k in (1, 10, 100))
+        out["cpu_baseline"] = {"value": 3 * len(sub) / dt, "unit": "queries/s", "cores": oracle.num_threads(),
+                               "kind": "oracle", "seconds": dt,
+                               "sample": "oracle.flat_l2_knn (direct-difference double + full sort) on a seeded %d-query "
+                                         "subset of cfg3 at k in {1,10,100}" % len(sub),
+                               "gpu_matches_oracle_bit_for_bit": bool(exact)}
+        del xb_h
+    del xb, xq, res
     torch.cuda.empty_cache()
     xb = gt.gaussian_vectors(0, nb, d)
     xq = gt.gaussian_vectors(nb, nq, d)
-    out["real_valued"] = {"workload": "same shape, i.i.d. ~N(0,1) fp32 (3xTF32 path)", "k10": run(xq, xb, 10, 3)}
+    out["real_valued"] = {"workload": "same shape, i.i.d. ~N(0,1) fp32 (3xTF32 path)"}
+    for k in (1, 10, 100):
+        out["real_valued"]["k%d" % k] = run(xq, xb, k, 3)[0]
     del xb, xq
     return out
 
 
-def also_ivfpq(fs, gt, pk, nb, cfg5=False):
+def also_ivfpq(fs, gt, pk, cfg, nb=None, cpu=True):
+    """fs_ivfpq_search on BASELINE.json configs[3] (cfg 4) / configs[4] (cfg 5): build the index, time
+    every (nprobe, k), report the whole search and the scan stage (C2-C4: tables + list scan + pass-1
+    selection, events inside the library) on code bytes, and time the oracle on the seeded query
+    subset over the GPU-built lists those queries probed (cpu_baseline, with the parity it shows)."""
+    import math
+    import numpy as np
     import torch
-    d, M, nq, k = 96, (8 if cfg5 else 16), 10_000, 100
-    per_list = 3815 if cfg5 else 1526
-    nlist = max(64, min(262_144 if cfg5 else 65_536, int(2 ** round(__import__("math").log2(max(nb // per_list, 64))))))
-    ntrain = min(nb, max(256, min(4_194_304 if cfg5 else 1_000_000, 16 * nlist)))
+    import datagen
+    c = dict(datagen.IVFPQ_CONFIGS[cfg])
+    full = nb is None or nb >= c["nb"]
+    if not full:  # reduced run (profiling aid): same shape, fewer vectors, nlist scaled
+        per_list = c["nb"] // c["nlist"]
+        c["nlist"] = max(64, min(c["nlist"], int(2 ** round(math.log2(max(nb // per_list, 64))))))
+        c["ntrain"] = min(nb, max(256, min(c["ntrain"], 16 * c["nlist"])))
+        c["nb"] = nb
+    nb, d, nlist, M, nq = c["nb"], c["d"], c["nlist"], c["M"], c["nq"]
     t0 = time.perf_counter()
     ix = fs.IvfPq(d, nlist, M)
-    ix.train(gt.deep_like(0, ntrain), niter=10, seed=0)
+    ix.train(gt.deep_like(0, c["ntrain"]), niter=10, seed=0)
     torch.cuda.synchronize()
     t_train = time.perf_counter() - t0
     t0 = time.perf_counter()
@@ -257,22 +297,68 @@ def also_ivfpq(fs, gt, pk, nb, cfg5=False):
     ix.search(xq[:8], 1, 1)  # finalise the lists
     torch.cuda.synchronize()
     t_add = time.perf_counter() - t0
-    out = {"workload": "cfg%d%s: nb=%d deep-like d=96, nlist=%d, M=%d, nq=1e4"
-                       % (5 if cfg5 else 4, "" if nb >= (10**9 if cfg5 else 10**8) else "-shaped, REDUCED", nb, nlist, M),
+    out = {"workload": "cfg%d%s: nb=%d deep-like d=96, nlist=%d, M=%d, nq=%d"
+                       % (cfg, "" if full else "-shaped, REDUCED", nb, nlist, M, nq),
            "train_s": t_train, "add_s": t_add, "add_vectors_per_s": nb / t_add}
-    od = torch.empty((nq, k), dtype=torch.float32, device="cuda")
-    oi = torch.empty((nq, k), dtype=torch.int64, device="cuda")
-    for nprobe, k in (((32, 1), (32, 100), (128, 1), (128, 100)) if cfg5 else ((16, 100), (64, 100), (256, 100))):
+    smem_lookups_peak = 148 * 32 * pk["sm_max_mhz"] * 1e6
+    sub = datagen.unique_sample_ids(min(c["check_queries"], nq), nq, stream=10 * cfg + 6)
+    st = torch.from_numpy(sub).cuda()
+    runs = []
+    for nprobe, k in c["searches"]:
         if nprobe > nlist:
             continue
         ws = torch.empty(ix.search_ws_bytes(nq, nprobe, k), dtype=torch.uint8, device="cuda")
         od = torch.empty((nq, k), dtype=torch.float32, device="cuda")
         oi = torch.empty((nq, k), dtype=torch.int64, device="cuda")
         best, med = timed(lambda: ix.search(xq, nprobe, k, out_dist=od, out_ids=oi, ws=ws), 3)
+        stage = []
+        for _ in range(3):  # stage times from the events the library records (read after the call ended)
+            ix.search(xq, nprobe, k, out_dist=od, out_ids=oi, ws=ws)
+            torch.cuda.synchronize()
+            stage.append(ix.last_stage_ms)
+        stage = sorted(stage, key=lambda t: t[1])[1]  # median by scan time
         codes = ix.last_scanned_codes
-        out[("nprobe%d_k%d" % (nprobe, k)) if cfg5 else ("nprobe%d" % nprobe)] = {"ms": med, "queries_per_s": nq / med * 1e3, "code_bytes": codes,
-                                    "code_GBps_whole_search": codes / med / 1e6,
-                                    "frac_hbm_whole_search": codes / med / 1e6 / pk["hbm"]}
+        key = "nprobe%d_k%d" % (nprobe, k)
+        out[key] = {"ms": med, "queries_per_s": nq / med * 1e3, "code_bytes": codes,
+                    "code_GBps_whole_search": codes / med / 1e6,
+                    "frac_hbm_whole_search": codes / med / 1e6 / pk["hbm"],
+                    "stage_ms": {"coarse_C1": stage[0], "scan_C2_C4": stage[1], "merge_C5": stage[2]},
+                    "scan_stage_GBps": codes / stage[1] / 1e6,
+                    "scan_stage_frac_hbm": codes / stage[1] / 1e6 / pk["hbm"],
+                    "scan_stage_lookups_per_s": codes / stage[1] * 1e3,
+                    "scan_stage_frac_smem_lookup_rate": codes / stage[1] * 1e3 / smem_lookups_peak}
+        if cpu:
+            gd, gi, gp = ix.search(xq, nprobe, k, want_probed=True)
+            runs.append((nprobe, k, key, gd[st].cpu().numpy(), gi[st].cpu().numpy(), gp[st].cpu().numpy()))
+        del ws, od, oi
+    if cpu and runs:
+        import oracle
+        coarse, pq = (t.cpu().numpy() for t in ix.get_quantizers())
+        xs = xq[st].cpu().numpy()
+        lists = np.unique(np.concatenate([r[5].reshape(-1) for r in runs]))
+        so, sc, si = ix.export_lists(lists)
+        offs = np.zeros(nlist + 1, np.int64)
+        lens = np.zeros(nlist, np.int64)
+        lens[lists] = np.diff(so)
+        np.cumsum(lens, out=offs[1:])
+        codes_h, ids_h = sc.cpu().numpy(), si.cpu().numpy()
+        del sc, si
+        oracle.ivfpq_search(coarse, pq, offs, codes_h, ids_h, xs[:1], 1, 1)  # load the library
+        for nprobe, k, key, gd, gi, gp in runs:
+            t0 = time.perf_counter()
+            o = oracle.ivfpq_search(coarse, pq, offs, codes_h, ids_h, xs, nprobe, k, probed_in=gp)
+            dt = time.perf_counter() - t0
+            fin = np.isfinite(o["dist64"]) & (gi >= 0)
+            rel = np.abs(gd[fin] - o["dist64"][fin]) / np.maximum(o["dist64"][fin], 1e-30)
+            out[key]["cpu_baseline"] = {
+                "value": len(sub) / dt, "unit": "queries/s", "cores": oracle.num_threads(), "kind": "oracle",
+                "seconds": dt,
+                "sample": "oracle.ivfpq_search (Alg. 4 by explicit reconstruction in double, full sort) on the seeded "
+                          "%d-query subset over the GPU-built lists those queries probed; coarse step given" % len(sub),
+                "gpu_vs_oracle": {"ids_equal_frac": float((gi == o["ids"]).mean()),
+                                  "queries_identical_frac": float((gi == o["ids"]).all(1).mean()),
+                                  "max_rel_dist_err": float(rel.max()) if rel.size else 0.0,
+                                  "within_1e-3": bool(rel.size == 0 or rel.max() <= 1e-3)}}
     ix.close()
     return out
 
@@ -298,8 +384,10 @@ def run_ours(args):
     pk = peaks()
 
     if args.case in ("flat", "ivfpq", "ivfpq5"):  # profiling aid: only that "also" leg
-        out = also_flat(fs, gt, pk) if args.case == "flat" else also_ivfpq(fs, gt, pk, args.ivfpq_nb,
-                                                                         cfg5=args.case == "ivfpq5")
+        if args.case == "flat":
+            out = also_flat(fs, gt, pk, cpu=not args.no_cpu)
+        else:
+            out = also_ivfpq(fs, gt, pk, 5 if args.case == "ivfpq5" else 4, args.ivfpq_nb, cpu=not args.no_cpu)
         print(json.dumps({"case": args.case, **out}))
         return
 
@@ -429,14 +517,43 @@ def run_ours(args):
         if not args.skip_also:
             torch.cuda.empty_cache()
             also = {}
-            try:
-                also["flat_l2_knn"] = also_flat(fs, gt, pk)
-                torch.cuda.empty_cache()
-                also["ivfpq_search"] = also_ivfpq(fs, gt, pk, args.ivfpq_nb)
-            except Exception as e:  # the headline stands on its own
-                also["error"] = repr(e)
+            for name, fn in (("flat_l2_knn", lambda: also_flat(fs, gt, pk, cpu=not args.no_cpu)),
+                             ("ivfpq_search_cfg4", lambda: also_ivfpq(fs, gt, pk, 4, args.ivfpq_nb, cpu=not args.no_cpu)),
+                             ("ivfpq_search_cfg5", lambda: also_ivfpq(fs, gt, pk, 5, None, cpu=not args.no_cpu))):
+                if name == "ivfpq_search_cfg5" and args.skip_cfg5:
+                    continue
+                try:
+                    torch.cuda.empty_cache()
+                    also[name] = fn()
+                except Exception as e:  # the headline stands on its own
+                    also[name] = {"error": repr(e)}
             line["also"] = also
+            # the other two paths' rooflines and CPU baselines, inside the keys the driver keeps
+            rl = {}
+            fl = also.get("flat_l2_knn", {})
+            for kk in ("k1", "k10", "k100"):
+                if kk in fl:
+                    rl["flat_cfg3_" + kk] = {"bound": "tensor", "achieved": fl[kk]["issued_tflops"], "peak": fl["tf32_peak_tflops"],
+                                             "unit": "TFLOP/s", "frac": fl[kk]["tensor_frac"], "ms": fl[kk]["ms"],
+                                             "queries_per_s": fl[kk]["queries_per_s"]}
+            for name in ("ivfpq_search_cfg4", "ivfpq_search_cfg5"):
+                for kk, v in also.get(name, {}).items():
+                    if isinstance(v, dict) and "scan_stage_GBps" in v:
+                        rl[name[13:] + "_" + kk] = {"bound": "hbm", "achieved": v["scan_stage_GBps"], "peak": pk["hbm"],
+                                                   "unit": "GB/s", "frac": v["scan_stage_frac_hbm"],
+                                                   "whole_search_frac": v["frac_hbm_whole_search"], "ms": v["ms"],
+                                                   "queries_per_s": v["queries_per_s"]}
+            roofline["also"] = rl
         line["cpu_baseline"] = cpu_baseline()
+        if not args.skip_also:
+            cb = {}
+            if "cpu_baseline" in line["also"].get("flat_l2_knn", {}):
+                cb["flat_cfg3"] = line["also"]["flat_l2_knn"]["cpu_baseline"]
+            for name in ("ivfpq_search_cfg4", "ivfpq_search_cfg5"):
+                for kk, v in line["also"].get(name, {}).items():
+                    if isinstance(v, dict) and "cpu_baseline" in v:
+                        cb[name[13:] + "_" + kk] = v["cpu_baseline"]
+            line["cpu_baseline"]["also"] = cb
     if rank == 0:
         print(json.dumps(line))
     if world > 1:
@@ -451,7 +568,10 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--skip-also", action="store_true")
-    ap.add_argument("--ivfpq-nb", type=int, default=10_000_000)
+    ap.add_argument("--ivfpq-nb", type=int, default=None,
+                    help="cfg4 leg with fewer vectors (profiling aid; default: BASELINE.json's 10^8)")
+    ap.add_argument("--skip-cfg5", action="store_true", help="leave out the 10^9-vector leg (about 5 min of index build)")
+    ap.add_argument("--no-cpu", action="store_true", help="leave out the oracle timings of the flat / IVFPQ legs")
     ap.add_argument("--case", default="", help="comma list of k1,k32,k128,k1024,bigrow_k1024 (time only these calls), or flat / ivfpq (only that leg)")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -139,15 +139,22 @@ def sift_like(i0: int, n: int, d: int = 128, seed: int = 0, cfg: int = 3,
 # cfg4/5: deep-feature-like: 4096-component mixture, skewed weights, unit norm
 # --------------------------------------------------------------------------
 def deep_like(i0: int, n: int, d: int = 96, seed: int = 0, cfg: int = 4,
-              ncomp: int = 4096) -> np.ndarray:
+              ncomp: int = 4096, ids=None) -> np.ndarray:
     """c = floor(ncomp * u^1.5) (u*sqrt(u) in double), x = mu_c + 0.35 g, then
     L2-normalised: squared norm accumulated in double in dimension order, one
-    double sqrt, one double divide per element, rounded to fp32."""
+    double sqrt, one double divide per element, rounded to fp32.
+    With ``ids`` (int array) the vectors with exactly those indices are generated
+    (i0 and n are ignored): any vector of a 10^9-vector set can be regenerated."""
+    if ids is not None:
+        ids = np.asarray(ids, dtype=np.int64)
+        n = len(ids)
     out = np.empty((n, d), np.float32)
     step = max(1, (1 << 20) // d)
     for s in range(0, n, step):
         e = min(n, s + step)
         i, j = _grid(i0 + s, e - s, d)
+        if ids is not None:
+            i = ids[s:e].astype(U64)[:, None]
         u = uniform(seed, 10 * cfg + 3, i, U64(0)).astype(np.float64)
         comp = np.minimum(np.floor(np.float64(ncomp) * (u * np.sqrt(u))), ncomp - 1).astype(U64)
         mu = normal(seed, 10 * cfg + 2, comp, j)
@@ -177,3 +184,31 @@ def gather(fn, ids: np.ndarray, **kw) -> np.ndarray:
             out = np.empty((len(ids), v.shape[1]), np.float32)
         out[t] = v[0]
     return out
+
+
+# --------------------------------------------------------------------------
+# Shapes of BASELINE.json configs[3] / configs[4] (cfg4 / cfg5): sizes only, shared by
+# tests/ and bench.py so that both build the same index.  ntrain for cfg5 is not fixed by
+# BASELINE.json (SURVEY 8d proposes 16 per centroid).  check_queries = the size of the
+# seeded oracle query subset, add_check = how many seeded ids the add path is re-encoded for.
+# --------------------------------------------------------------------------
+IVFPQ_CONFIGS = {
+    4: dict(nb=100_000_000, d=96, nlist=65_536, M=16, ntrain=1_000_000, nq=10_000,
+            searches=((16, 100), (64, 100), (256, 100)), check_queries=500, add_check=10_000),
+    5: dict(nb=1_000_000_000, d=96, nlist=262_144, M=8, ntrain=4_194_304, nq=10_000,
+            searches=((32, 1), (32, 100), (128, 1), (128, 100)), check_queries=200, add_check=10_000),
+}
+
+
+def unique_sample_ids(count: int, modulo: int, seed: int = 0, stream: int = 46) -> np.ndarray:
+    """`count` distinct ids in [0, modulo), ascending: the first distinct values of the
+    seeded sequence h(seed, stream, s, 0) % modulo (streams 10*cfg + 6 / + 7 of the header)."""
+    assert count <= modulo
+    got = np.empty(0, np.int64)
+    s0 = 0
+    while len(got) < count:
+        s = np.arange(s0, s0 + 2 * count, dtype=U64)
+        got = np.unique(np.concatenate([got, (h(seed, stream, s, U64(0)) % U64(modulo)).astype(np.int64)]))
+        s0 += 2 * count
+    rng_order = np.argsort(h(seed, stream + 1000, got.astype(U64), U64(0)), kind="stable")
+    return np.sort(got[rng_order[:count]])

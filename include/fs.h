@@ -151,6 +151,11 @@ FS_API int64_t fs_ivfpq_ntotal(const fs_ivfpq* index);
 /* Total code bytes the probed lists of the last fs_ivfpq_search held
  * (sum over (query, list) pairs of len * M): the scan's algorithmic bytes. */
 FS_API int64_t fs_ivfpq_last_scanned_codes(const fs_ivfpq* index);
+/* Device time of the three stages of the last fs_ivfpq_search on its stream (CUDA events the
+ * search records): ms[0] = C1 coarse top-nprobe, ms[1] = C2-C4 (tables, list scan, pass-1
+ * selection: the stage the scan roofline is quoted on), ms[2] = C5 merge + ids.  HOST float
+ * [3]; waits for that search to finish. */
+FS_API int fs_ivfpq_last_stage_ms(const fs_ivfpq* index, float* ms);
 /* Read-only device views of one list, valid until the next add/destroy. */
 FS_API int fs_ivfpq_list(const fs_ivfpq* index, int list_no, const uint8_t** codes, const int64_t** ids,
                   int64_t* len);
@@ -159,6 +164,13 @@ FS_API int fs_ivfpq_list(const fs_ivfpq* index, int list_no, const uint8_t** cod
  * the three may be NULL. */
 FS_API int fs_ivfpq_export(const fs_ivfpq* index, int64_t* offsets, uint8_t* codes, int64_t* ids,
                     fs_stream stream);
+/* The same for a subset of the lists (what a checker of a 10^9-vector index copies out: only the
+ * lists some queries probed).  list_nos: HOST int32 [n_lists], each in [0, nlist).  offsets_host:
+ * HOST int64 [n_lists + 1], always written: list j occupies [offsets_host[j], offsets_host[j+1])
+ * of the outputs.  codes (uint8 [total][M]) and ids (int64 [total]) are DEVICE buffers of
+ * total = offsets_host[n_lists] entries, or NULL (call once with NULL to size them). */
+FS_API int fs_ivfpq_export_lists(const fs_ivfpq* index, const int32_t* list_nos, int64_t n_lists,
+                          int64_t* offsets_host, uint8_t* codes, int64_t* ids, fs_stream stream);
 
 #ifdef __cplusplus
 }

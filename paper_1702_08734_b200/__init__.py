@@ -239,6 +239,13 @@ class IvfPq:
     def last_scanned_codes(self) -> int:
         return int(lib().fs_ivfpq_last_scanned_codes(self._h))
 
+    @property
+    def last_stage_ms(self):
+        """fs_ivfpq_last_stage_ms: (C1, C2-C4, C5) device milliseconds of the last search."""
+        ms = (ctypes.c_float * 3)()
+        _check(lib().fs_ivfpq_last_stage_ms(self._h, ms))
+        return tuple(float(v) for v in ms)
+
     def search_ws_bytes(self, nq: int, nprobe: int, k: int) -> int:
         return int(lib().fs_ivfpq_search_ws_bytes(self._h, _i64(nq), _int(nprobe), _int(k)))
 
@@ -277,3 +284,18 @@ class IvfPq:
         ids = torch.empty(nt, dtype=torch.int64, device=dev)
         _check(lib().fs_ivfpq_export(self._h, _ptr(offsets), _ptr(codes), _ptr(ids), _stream()))
         return offsets, codes, ids
+
+    def export_lists(self, list_nos):
+        """fs_ivfpq_export_lists: the given lists back to back.  list_nos: int sequence / numpy array.
+        Returns (offsets numpy int64 [n+1] (host), codes uint8 [total,M] (device), ids int64 [total] (device))."""
+        import numpy as np
+        ln = np.ascontiguousarray(list_nos, dtype=np.int32)
+        offs = np.empty(len(ln) + 1, np.int64)
+        lp, op = _vp(ln.ctypes.data), _vp(offs.ctypes.data)
+        _check(lib().fs_ivfpq_export_lists(self._h, lp, _i64(len(ln)), op, _vp(0), _vp(0), _stream()))
+        dev = torch.device("cuda", torch.cuda.current_device())
+        total = int(offs[-1])
+        codes = torch.empty((total, self.M), dtype=torch.uint8, device=dev)
+        ids = torch.empty(total, dtype=torch.int64, device=dev)
+        _check(lib().fs_ivfpq_export_lists(self._h, lp, _i64(len(ln)), op, _ptr(codes), _ptr(ids), _stream()))
+        return offs, codes, ids

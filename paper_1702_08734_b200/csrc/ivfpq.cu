@@ -511,6 +511,11 @@ int fs_ivfpq_create(fs_ivfpq** out, int d, int nlist, int M) {
     return rc;
   }
   cudaMemset(ix->scanned.p, 0, sizeof(unsigned long long));
+  for (cudaEvent_t& e : ix->ev)
+    if (cudaEventCreate(&e) != cudaSuccess) {
+      fs_ivfpq_destroy(ix);
+      return fs::set_error(FS_ECUDA, "fs_ivfpq_create: cudaEventCreate failed");
+    }
   *out = ix;
   return FS_OK;
 }
@@ -521,6 +526,8 @@ int fs_ivfpq_destroy(fs_ivfpq* ix) {
   fs::DevBuf* bufs[] = {&ix->coarse, &ix->cnorm, &ix->pq, &ix->offsets, &ix->codes, &ix->ids,
                         &ix->st_list, &ix->st_codes, &ix->st_ids, &ix->scanned, &ix->term1};
   for (fs::DevBuf* b : bufs) b->release();
+  for (cudaEvent_t e : ix->ev)
+    if (e) cudaEventDestroy(e);
   delete ix;
   return FS_OK;
 }
@@ -570,6 +577,14 @@ int64_t fs_ivfpq_last_scanned_codes(const fs_ivfpq* ix) {
   return (int64_t)v;
 }
 
+int fs_ivfpq_last_stage_ms(const fs_ivfpq* ix, float* ms) {
+  if (!ix || !ms) return fs::set_error(FS_EINVAL, "fs_ivfpq_last_stage_ms: NULL pointer");
+  if (!ix->ev_valid) return fs::set_error(FS_ESTATE, "fs_ivfpq_last_stage_ms: no search has run");
+  FS_CUDA(cudaEventSynchronize(ix->ev[3]));
+  for (int i = 0; i < 3; ++i) FS_CUDA(cudaEventElapsedTime(ms + i, ix->ev[i], ix->ev[i + 1]));
+  return FS_OK;
+}
+
 int fs_ivfpq_list(const fs_ivfpq* cix, int list_no, const uint8_t** codes, const int64_t** ids,
                   int64_t* len) {
   fs_ivfpq* ix = const_cast<fs_ivfpq*>(cix);
@@ -598,6 +613,42 @@ int fs_ivfpq_export(const fs_ivfpq* cix, int64_t* offsets, uint8_t* codes, int64
     FS_CUDA(cudaMemcpyAsync(codes, ix->codes.p, (size_t)ix->n_csr * ix->M, cudaMemcpyDeviceToDevice, s));
   if (ids && ix->n_csr > 0)
     FS_CUDA(cudaMemcpyAsync(ids, ix->ids.p, (size_t)ix->n_csr * sizeof(int64_t), cudaMemcpyDeviceToDevice, s));
+  return FS_OK;
+}
+
+int fs_ivfpq_export_lists(const fs_ivfpq* cix, const int32_t* list_nos, int64_t n_lists, int64_t* offsets_host,
+                          uint8_t* codes, int64_t* ids, fs_stream stream) {
+  fs_ivfpq* ix = const_cast<fs_ivfpq*>(cix);
+  if (!ix) return fs::set_error(FS_EINVAL, "fs_ivfpq_export_lists: NULL index");
+  if (n_lists < 0 || !offsets_host || (n_lists > 0 && !list_nos))
+    return fs::set_error(FS_EINVAL, "fs_ivfpq_export_lists: bad arguments");
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  int rc = fs::ivfpq_finalise(ix, s);
+  if (rc != FS_OK) return rc;
+  int64_t total = 0;
+  for (int64_t j = 0; j < n_lists; ++j) {
+    const int L = list_nos[j];
+    if (L < 0 || L >= ix->nlist) return fs::set_error(FS_EINVAL, "fs_ivfpq_export_lists: list %d out of range", L);
+    offsets_host[j] = total;
+    total += ix->offsets_host[L + 1] - ix->offsets_host[L];
+  }
+  offsets_host[n_lists] = total;
+  if (!codes && !ids) return FS_OK;
+  // one copy per run of consecutive list numbers (their CSR ranges are adjacent)
+  for (int64_t j = 0; j < n_lists;) {
+    int64_t e = j + 1;
+    while (e < n_lists && list_nos[e] == list_nos[e - 1] + 1) ++e;
+    const int64_t src = ix->offsets_host[list_nos[j]], len = offsets_host[e] - offsets_host[j];
+    if (len > 0) {
+      if (codes)
+        FS_CUDA(cudaMemcpyAsync(codes + offsets_host[j] * ix->M, ix->codes.as<uint8_t>() + src * ix->M,
+                                (size_t)len * ix->M, cudaMemcpyDeviceToDevice, s));
+      if (ids)
+        FS_CUDA(cudaMemcpyAsync(ids + offsets_host[j], ix->ids.as<int64_t>() + src, (size_t)len * sizeof(int64_t),
+                                cudaMemcpyDeviceToDevice, s));
+    }
+    j = e;
+  }
   return FS_OK;
 }
 

@@ -53,6 +53,9 @@ struct fs_ivfpq {
 
   // Code bytes scanned by the last search (device counter, read lazily).
   fs::DevBuf scanned;  // unsigned long long [1]
+  // Stage boundaries of the last search on its stream: start, after C1, after C2-C4, end.
+  cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+  bool ev_valid = false;
 
   int64_t ntotal() const { return n_csr + n_staged; }
 };

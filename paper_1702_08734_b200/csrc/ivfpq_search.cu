@@ -1105,6 +1105,8 @@ int ivfpq_search_device(fs_ivfpq* ix, const float* xq, int64_t nq, int nprobe, i
   int64_t* cids = reinterpret_cast<int64_t*>(w + p.off_cids);
   uint64_t* Wg = reinterpret_cast<uint64_t*>(w + p.off_W);
   int rc;
+  ix->ev_valid = false;
+  FS_CUDA(cudaEventRecord(ix->ev[0], s));
   // C1
   if (p.c1_chunk > 0) {
     float* D = reinterpret_cast<float*>(w + p.off_D);
@@ -1125,6 +1127,7 @@ int ivfpq_search_device(fs_ivfpq* ix, const float* xq, int64_t nq, int nprobe, i
                          ix->cnorm.as<float>(), cdist, cids, w, s);
     if (rc != FS_OK) return rc;
   }
+  FS_CUDA(cudaEventRecord(ix->ev[1], s));
   FS_CUDA(cudaMemsetAsync(ix->scanned.p, 0, sizeof(unsigned long long), s));
   // C2-C4
   ScanArgs a;
@@ -1195,6 +1198,7 @@ int ivfpq_search_device(fs_ivfpq* ix, const float* xq, int64_t nq, int nprobe, i
     default: rc = launch_scan<32>(a, nq, s); break;
   }
   if (rc != FS_OK) return rc;
+  FS_CUDA(cudaEventRecord(ix->ev[2], s));
   // C5
   rc = launch_flat_finish(Wg, nq, p.ngroups * qpi, k, nullptr, out_dist, out_ids, s);
   if (rc != FS_OK) return rc;
@@ -1202,6 +1206,8 @@ int ivfpq_search_device(fs_ivfpq* ix, const float* xq, int64_t nq, int nprobe, i
   ivfpq_resolve_kernel<<<(unsigned)ceil_div(nq, 4), 128, smem, s>>>(out_dist, out_ids,
                                                                     ix->ids.as<int64_t>(), nq, k);
   FS_LAUNCHED();
+  FS_CUDA(cudaEventRecord(ix->ev[3], s));
+  ix->ev_valid = true;
   return FS_OK;
 }
 

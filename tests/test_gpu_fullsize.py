@@ -7,10 +7,14 @@ The oracle cannot run the whole workloads in seconds, so (SURVEY 8c / the tier r
         elements <= the k-th value (found with numpy's partition), which is the whole answer.
   cfg3  nb = 10^6, nq = 10^4, d = 128 integer data through fs_flat_l2_knn as in bench.py; a
         seeded sample of queries is compared bit for bit with the oracle.
-  cfg4  the 10^8-vector index does not fit a test run; a cfg4-shaped index of 2 * 10^6
-        vectors (same generator, same d / M / k / nprobe, nlist scaled) is built and searched
-        with nq = 2 000; a seeded query subset is checked by the oracle over the GPU-built
-        lists and a seeded sample of the add path is re-encoded by the oracle.
+  cfg4  nb = 10^8, nlist = 65 536, M = 16 and cfg5 nb = 10^9, nlist = 262 144, M = 8 are built in
+        full (datagen.IVFPQ_CONFIGS) and checked as SURVEY C-12 says: (i) structure of the
+        GPU-built inverted file (sum of lengths, every id exactly once, append order),
+        (ii) the add path on >= 10 000 seeded ids regenerated on the CPU and re-encoded by the
+        oracle, (iii) the whole 10^4-query batch is searched at every (nprobe, k) of
+        BASELINE.json and the rows of a seeded 500 / 200-query subset of THAT output meet the
+        oracle run over the GPU-built lists those queries probed (copied out with
+        fs_ivfpq_export_lists).  A 2 * 10^6-vector index of the cfg4 shape stays as a quick case.
 Inputs come from datagen's torch twin on the device (bit-identical to the numpy generator,
 tests/test_datagen.py).
 """
@@ -139,3 +143,100 @@ def test_cfg4_shaped_index():
         assert np.allclose(bd_s, sd, rtol=1e-3, atol=0)
         assert (bi_s == si).mean() >= 0.98
     ix.close()
+
+
+def _full_config(cfg):
+    """SURVEY C-12 (i)-(iii) on BASELINE.json configs[3] / configs[4] at their stated size."""
+    from datagen import gen_torch as gt
+    from test_gpu_ivfpq import verify_search
+    fs = fsmod()
+    c = datagen.IVFPQ_CONFIGS[cfg]
+    nb, d, nlist, M, nq = c["nb"], c["d"], c["nlist"], c["M"], c["nq"]
+    ix = fs.IvfPq(d, nlist, M)
+    ix.train(gt.deep_like(0, c["ntrain"]), niter=10, seed=0)
+    chunk = 1 << 22
+    for b in range(0, nb, chunk):
+        ix.add(gt.deep_like(b, min(chunk, nb - b)))
+    assert ix.ntotal == nb
+    coarse, pq = (t.cpu().numpy() for t in ix.get_quantizers())
+    assert np.isfinite(coarse).all() and np.isfinite(pq).all()
+    offs_d, codes_d, lids_d = ix.export()
+    torch.cuda.synchronize()
+
+    # (i) structure, on the device copy of the inverted file
+    offs = offs_d.cpu().numpy()
+    assert offs[0] == 0 and offs[-1] == nb and np.all(np.diff(offs) >= 0)
+    assert lids_d.numel() == nb and int(lids_d.sum().item()) == nb * (nb - 1) // 2
+    x = lids_d.clone()
+    while x.numel() > 1:                        # xor of all ids = xor of 0..nb-1
+        if x.numel() & 1:
+            x = torch.cat([x, x.new_zeros(1)])
+        h = x.numel() // 2
+        x = x[:h] ^ x[h:]
+    want_xor = [nb - 1, 1, nb, 0][(nb - 1) % 4]  # xor of 0..m for m = nb - 1
+    assert int(x.item()) == want_xor
+    del x
+    pos = torch.empty(nb, dtype=torch.int64, device="cuda")
+    pos[lids_d] = torch.arange(nb, dtype=torch.int64, device="cuda")
+    step = 1 << 26
+    for a in range(0, nb, step):                # every id is stored, and nb slots in all: exactly once
+        e = min(nb, a + step)
+        assert torch.equal(lids_d[pos[a:e]], torch.arange(a, e, dtype=torch.int64, device="cuda"))
+    asc = lids_d[1:] > lids_d[:-1]              # append order = ascending id inside every list
+    inner = offs_d[1:-1]
+    inner = inner[(inner > 0) & (inner < nb)]
+    asc[inner - 1] = True
+    assert bool(asc.all())
+    del asc
+    for L in datagen.unique_sample_ids(64, nlist, stream=10 * cfg + 5).tolist():   # sort-unique on sampled lists
+        seg = lids_d[offs[L]:offs[L + 1]]
+        assert torch.unique(seg).numel() == seg.numel()
+
+    # (ii) sampled add path: regenerate seeded ids on the CPU, oracle steps 1-3 of Add
+    sid = datagen.unique_sample_ids(c["add_check"], nb, stream=10 * cfg + 7)
+    ys = datagen.deep_like(0, 0, ids=sid)
+    for t in range(3):                          # device generator == numpy generator at these ids
+        assert np.array_equal(ys[t], gt.deep_like(int(sid[t]), 1).cpu().numpy()[0])
+    olist, ocodes, cm, km = oracle.ivfpq_encode(coarse, pq, ys, margins=True)
+    p = pos[torch.from_numpy(sid).cuda()]
+    glist = (torch.searchsorted(offs_d, p, right=True) - 1).cpu().numpy()
+    gcodes = codes_d[p].cpu().numpy()
+    assert not ((glist != olist) & (cm >= 1e-5)).any(), "coarse assignment differs beyond near-ties"
+    same = glist == olist
+    assert not ((gcodes != ocodes) & (km >= 1e-5) & same[:, None]).any(), "codes differ beyond near-ties"
+    assert same.mean() > 0.999 and (gcodes == ocodes)[same].mean() > 0.999
+    del pos, offs_d, codes_d, lids_d
+    torch.cuda.empty_cache()
+
+    # (iii) full batch at every (nprobe, k); the seeded subset of that output meets the oracle
+    xq = gt.deep_like(nb, nq)
+    sub = datagen.unique_sample_ids(c["check_queries"], nq, stream=10 * cfg + 6)
+    xs = xq[torch.from_numpy(sub).cuda()].cpu().numpy()
+    assert np.array_equal(xs[:2], datagen.deep_like(0, 0, ids=nb + sub[:2]))
+    runs = []
+    for nprobe, k in c["searches"]:
+        gd, gi, gp = ix.search(xq, nprobe, k, want_probed=True)
+        torch.cuda.synchronize()
+        st = torch.from_numpy(sub).cuda()
+        runs.append((nprobe, k, gd[st].cpu().numpy(), gi[st].cpu().numpy(), gp[st].cpu().numpy()))
+        i_all = gi.cpu().numpy()
+        assert i_all.max() < nb and np.all(np.diff(gd.cpu().numpy(), axis=1) >= 0)
+    lists = np.unique(np.concatenate([r[4].reshape(-1) for r in runs]))
+    so, sc, si = ix.export_lists(lists)
+    offs_sub = np.zeros(nlist + 1, np.int64)    # CSR over all lists, the ones never probed empty
+    lens = np.zeros(nlist, np.int64)
+    lens[lists] = np.diff(so)
+    np.cumsum(lens, out=offs_sub[1:])
+    codes_sub, lids_sub = sc.cpu().numpy(), si.cpu().numpy()
+    del sc, si
+    for nprobe, k, gd, gi, gp in runs:
+        verify_search(coarse, pq, offs_sub, codes_sub, lids_sub, xs, nprobe, k, gd, gi, gp)
+    ix.close()
+
+
+def test_cfg4_full():
+    _full_config(4)
+
+
+def test_cfg5_full():
+    _full_config(5)

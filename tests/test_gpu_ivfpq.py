@@ -66,16 +66,19 @@ def check_add(ix, coarse, pq, xb, ids=None):
     return offs, codes, lids
 
 
-def check_search(ix, coarse, pq, offs, codes, lids, xq, nprobe, k):
-    gd, gi, gp = ix.search(torch.from_numpy(xq).cuda(), nprobe, k, want_probed=True)
-    torch.cuda.synchronize()
-    gd, gi, gp = gd.cpu().numpy(), gi.cpu().numpy(), gp.cpu().numpy()
+def verify_search(coarse, pq, offs, codes, lids, xq, nprobe, k, gd, gi, gp):
+    """The acceptance predicates of the header on GPU outputs (gd, gi, gp) for the queries xq.
+
+    (offs, codes, lids) is the GPU-built inverted file in CSR form on the host; for the big
+    configs it is the sub-index of the lists these queries probe (every other list empty).
+    Look-ups go through one sort of lids, so 10^8-entry files are fine."""
     nq = xq.shape[0]
     # (1) probed lists vs the oracle's own coarse step (Eq. 5)
     o1 = oracle.ivfpq_search(coarse, pq, offs, codes, lids, xq, nprobe, k)
     xn = (xq.astype(np.float64) ** 2).sum(1)
     cn = (coarse.astype(np.float64) ** 2).sum(1)
     for q in range(nq):
+        assert len(set(gp[q].tolist())) == nprobe, "probed lists repeat"
         if np.array_equal(gp[q], o1["probed"][q]):
             continue
         kth = o1["coarse64"][q, -1]
@@ -84,8 +87,8 @@ def check_search(ix, coarse, pq, offs, codes, lids, xq, nprobe, k):
             assert abs(dL - kth) <= 1e-4 * (xn[q] + cn[L]), "probed list %d of query %d is no near-tie" % (L, q)
     # (2) steps 2-3 over the lists the GPU probed
     o = oracle.ivfpq_search(coarse, pq, offs, codes, lids, xq, nprobe, k, probed_in=gp)
-    list_of = np.searchsorted(offs, np.arange(len(lids)), side="right") - 1
-    pos_of = {int(i): p for p, i in enumerate(lids)}
+    order = np.argsort(lids, kind="stable")
+    sorted_ids = lids[order]
     n_exact = 0
     for q in range(nq):
         valid = gi[q] >= 0
@@ -96,9 +99,13 @@ def check_search(ix, coarse, pq, offs, codes, lids, xq, nprobe, k):
             continue
         ids = gi[q, :nv]
         assert len(set(ids.tolist())) == nv, "duplicate ids"
-        pos = np.array([pos_of[int(i)] for i in ids])
-        assert np.isin(list_of[pos], gp[q]).all(), "id outside the probed lists"
-        adc = oracle.adc_reconstruct(coarse, pq, np.repeat(xq[q:q + 1], nv, 0), list_of[pos], codes[pos])
+        at = np.searchsorted(sorted_ids, ids)
+        assert np.all(at < len(sorted_ids)) and np.array_equal(sorted_ids[np.minimum(at, len(sorted_ids) - 1)], ids), \
+            "id not stored in the (probed part of the) inverted file"
+        pos = order[at]
+        list_of = np.searchsorted(offs, pos, side="right") - 1
+        assert np.isin(list_of, gp[q]).all(), "id outside the probed lists"
+        adc = oracle.adc_reconstruct(coarse, pq, np.repeat(xq[q:q + 1], nv, 0), list_of, codes[pos])
         assert np.all(np.abs(gd[q, :nv] - adc) <= RTOL * adc + 1e-30), "ADC distance off"
         kth = o["dist64"][q, nv - 1]
         assert np.all(adc <= (1 + RTOL) * kth + 1e-30), "returned id is not in the top-k within tolerance"
@@ -107,6 +114,14 @@ def check_search(ix, coarse, pq, offs, codes, lids, xq, nprobe, k):
         assert np.all(np.diff(ids)[dd == 0] > 0), "exact ties not in ascending id order"
         n_exact += int(np.array_equal(ids, o["ids"][q, :nv]))
     assert n_exact >= 0.9 * nq, "only %d of %d queries match the oracle id for id" % (n_exact, nq)
+    return n_exact
+
+
+def check_search(ix, coarse, pq, offs, codes, lids, xq, nprobe, k):
+    gd, gi, gp = ix.search(torch.from_numpy(xq).cuda(), nprobe, k, want_probed=True)
+    torch.cuda.synchronize()
+    gd, gi, gp = gd.cpu().numpy(), gi.cpu().numpy(), gp.cpu().numpy()
+    verify_search(coarse, pq, offs, codes, lids, xq, nprobe, k, gd, gi, gp)
     return gd, gi, gp
 
 
