@@ -18,6 +18,7 @@
 // ahead across item boundaries (the next row is already arriving while the current
 // one is being selected).  "Lane j reads a_{32i+j}" becomes: lane j reads
 // elements 4j..4j+3 of each 128-element group with one 128-bit shared-memory load.
+#include <cstdlib>
 #include <mutex>
 
 #include "common.cuh"
@@ -797,11 +798,30 @@ struct HostStage {
   }
 };
 
+// kselect_row.cu: k >= 2
+size_t kselect_rows_ws_bytes(int64_t n_rows, int64_t n, int k);
+int kselect_rows_device(const float* rows, int64_t n_rows, int64_t n, int64_t ld, int k, float* out_val,
+                        int32_t* out_idx, void* ws, cudaStream_t s);
+static bool use_old_path() {
+  static int v = -1;
+  if (v < 0) {
+    const char* e = getenv("FS_KSELECT");
+    v = (e && e[0] == 'o') ? 1 : 0;
+  }
+  return v == 1;
+}
+
 // Selection over device rows; also used by the flat and IVFPQ drivers.
-size_t kselect_ws_bytes(int64_t n_rows, int64_t n, int k) { return make_plan(n_rows, n, k).bytes; }
+size_t kselect_ws_bytes(int64_t n_rows, int64_t n, int k) {
+  const size_t a = make_plan(n_rows, n, k).bytes, b = k >= 2 ? kselect_rows_ws_bytes(n_rows, n, k) : 0;
+  return a > b ? a : b;
+}
 
 int kselect_device(const float* rows, int64_t n_rows, int64_t n, int64_t ld, int k, float* out_val,
                    int32_t* out_idx, void* ws, cudaStream_t s) {
+  // interim: the warp-per-row kernel is still ahead for k <= 128 on batches of short rows
+  const bool batch_small_k = k <= 128 && make_plan(n_rows, n, k).P == 1;
+  if (k >= 2 && !use_old_path() && !batch_small_k) return kselect_rows_device(rows, n_rows, n, ld, k, out_val, out_idx, ws, s);
   const Plan p = make_plan(n_rows, n, k);
   char* w = static_cast<char*>(ws);
   KSelArgs a;
