@@ -819,9 +819,7 @@ size_t kselect_ws_bytes(int64_t n_rows, int64_t n, int k) {
 
 int kselect_device(const float* rows, int64_t n_rows, int64_t n, int64_t ld, int k, float* out_val,
                    int32_t* out_idx, void* ws, cudaStream_t s) {
-  // interim: the warp-per-row kernel is still ahead for k <= 128 on batches of short rows
-  const bool batch_small_k = k <= 128 && make_plan(n_rows, n, k).P == 1;
-  if (k >= 2 && !use_old_path() && !batch_small_k) return kselect_rows_device(rows, n_rows, n, ld, k, out_val, out_idx, ws, s);
+  if (k >= 2 && !use_old_path()) return kselect_rows_device(rows, n_rows, n, ld, k, out_val, out_idx, ws, s);
   const Plan p = make_plan(n_rows, n, k);
   char* w = static_cast<char*>(ws);
   KSelArgs a;

@@ -4,19 +4,19 @@
 // every row, ascending, ties by lower index, bit-exact.  The mechanism is cut for B200, where a row of
 // 16 384 floats has a budget of a few thousand issue slots per SM at 60 % of the HBM rate:
 //
-//   A1  a producer warp streams the 16-byte aligned body of the row through a ring of 8 KB stages with
-//       cp.async.bulk (TMA bulk copy, mbarrier full / empty pairs); the ring runs ahead into the next
-//       rows, which the producer draws from an atomic counter.  Eight consumer warps read a stage with
-//       128-bit shared-memory loads and apply the first-level filter: ONE float compare per
-//       element against a bound.
+//   A1  a producer warp streams the 16-byte aligned body of the row through a ring of 16 KB stages with
+//       cp.async.bulk (TMA bulk copy, mbarrier full / empty pairs); the ring holds a whole cfg2 row and
+//       runs ahead into the next rows, which the producer draws from an atomic counter.  Eight consumer
+//       warps read a stage with 128-bit shared-memory loads and apply the first-level filter:
+//       ONE float compare per element against a bound.
 //   bound: not the running k-th (P:L232 restores it after every overflow) but a SAMPLED one: the first
-//       stage of the row is a sample of S = 2 048 elements; a counting search over it (interpolation with
-//       a bisection safeguard, all 256 threads, one block barrier per probe) finds a value that c sample
+//       2 048 elements of the row are a sample; a SCOUT warp, one row ahead of the consumers, runs a
+//       counting search over it (interpolation with a bisection safeguard) for a value that c sample
 //       elements pass, with c - 3 sqrt(c) >= k S / n, so that >= k elements of the row pass with ~3 sigma
 //       confidence and ~k + 3.3 sqrt(k n / S) are expected to (1 333 for k = 1 024, n = 16 384).
 //   A2/A3  the survivors (warp-aggregated append to a dense shared-memory array) are ordered by COUNTING,
 //       not by merge networks (Alg. 1-3): a monotone linear map sends the values between the sample
-//       minimum and the bound to 2 048 buckets; one shared-memory atomic per survivor gives the bucket
+//       minimum and the bound to 2 048 buckets (1 024 for k <= 256); one shared-memory atomic per survivor gives the bucket
 //       histogram and the survivor's slot in its bucket, one block-wide exclusive scan gives the bucket
 //       starts and the bucket that holds rank k, a scatter groups the keys by bucket, and every key of a
 //       bucket at or under that one counts the keys of ITS bucket that are smaller (buckets hold ~0.7
@@ -27,9 +27,9 @@
 //       (a sample that does not represent the row: sorted rows), the row is done again by the paper's own
 //       scheme -- chunks of the row merged into a running top-k with the exact k-th key as the bound --
 //       using the same counting step as the restore operation.  Slow, rare, exact.
-//   A4  long rows (few rows, n >= 2^17): a 32 768-element strided sample gives a 4-sigma bound
+//   A4  long rows (few rows, n >= 2^18): a 65 536-element strided sample gives a 4-sigma bound
 //       (kselect_sample_kernel), the whole row is streamed once by every SM with that bound and the
-//       few survivors (~70 k of 2^27) are appended to a per-row list (kselect_filter_kernel), which this
+//       few survivors (~40 k of 2^27) are appended to a per-row list (kselect_filter_kernel), which this
 //       file's row kernel then selects from as if it were a row (values + original indices).
 #include <cmath>
 
@@ -44,15 +44,25 @@ using namespace sm100;
 
 constexpr int RW = 8;                // consumer warps
 constexpr int RT = RW * 32;          // consumer threads
-constexpr int RTHREADS = RT + 32;    // + producer warp
-constexpr int SEG = 2048;            // floats per ring stage (8 KB)
-constexpr int CAP = 2048;            // candidate slots per row
-constexpr int NBK = 2048;            // buckets of the counting step
-constexpr int RANK_MAX_BUCKET = 32;  // larger buckets among the kept ones -> bitonic sort instead
-#ifndef FS_KROW_STAGES
-#define FS_KROW_STAGES 3
+constexpr int RTHREADS = RT + 64;    // + producer warp + scout warp
+constexpr int RANK_MAX_BUCKET = 512;  // larger buckets among the kept ones -> bitonic sort instead (in-bucket counting is
+                                      // c^2 / 256 compares per thread: ~8 us at c = 256, the block-wide sort ~100 us)
+
+// Capacity class: CAPT candidate slots and buckets per row, NST ring stages, CTAs per SM.
+template <int CAPT> struct RowCfg;
+template <> struct RowCfg<1024> { static constexpr int SEG = 4096, NST = 3, CTAS = 3; };  // k <= 256: 16 KB stages, 72 KB
+#ifndef FS_KROW_POLL_NS
+#define FS_KROW_POLL_NS 300
 #endif
-constexpr int NSTAGE = FS_KROW_STAGES;
+#ifndef FS_KROW_2048_SEG
+#define FS_KROW_2048_SEG 2048
+#define FS_KROW_2048_NST 3
+#define FS_KROW_2048_CTAS 3
+#endif
+template <> struct RowCfg<2048> {  // k <= 1 024: 8 KB stages, 72 KB: three CTAs per SM hide the counting step's latency
+  static constexpr int SEG = FS_KROW_2048_SEG, NST = FS_KROW_2048_NST, CTAS = FS_KROW_2048_CTAS;
+};
+template <> struct RowCfg<4096> { static constexpr int SEG = 4096, NST = 4, CTAS = 1; };  // survivor lists of long rows: 160 KB
 
 struct RowArgs {
   const float* vals;      // [n_rows][ld] values to select from
@@ -70,16 +80,24 @@ struct RowArgs {
 
 struct StageDesc {
   int64_t row;   // -1: no more rows
+  int64_t len;   // elements of the row
   int seg;       // stage number inside the row
   int cnt;       // floats in the stage (multiple of 4)
   int last;      // last stage of the row
   int fallback;  // mapped row whose list is unusable: slow path on the original row
 };
 
+struct RowBound {
+  float thr_x;       // an element enters iff !(v >= thr_x); NaN: everything enters
+  float lo, hi;      // value range of the counting map (sample minimum, inclusive bound)
+  int sampled;
+};
+
+template <int NST>
 struct RowShared {
-  uint64_t full[NSTAGE], empty[NSTAGE];
-  StageDesc desc[NSTAGE];
-  int red[2][RW];
+  uint64_t full[NST], empty[NST], bnd[NST];
+  StageDesc desc[NST];
+  RowBound bound[NST];
   unsigned int redu[2][RW];
   int cnt, ovf;              // candidates appended, overflow flag
   int kb, kept, maxc;        // counting step: boundary bucket, keys in buckets <= kb, largest such bucket
@@ -87,15 +105,29 @@ struct RowShared {
   int wsum[RW];
 };
 
-constexpr size_t kRingBytes = (size_t)NSTAGE * SEG * sizeof(float);
-constexpr size_t kCandBytes = (size_t)CAP * sizeof(uint64_t);
-constexpr size_t kHistBytes = (size_t)(NBK + 8) * sizeof(uint32_t);
-constexpr size_t kBsBytes = (size_t)CAP * sizeof(uint32_t);
-constexpr size_t kRowSmem = kRingBytes + 2 * kCandBytes + kHistBytes + kBsBytes + sizeof(RowShared) + 128;
+template <int CAPT>
+struct RowSmem {
+  static constexpr int NST = RowCfg<CAPT>::NST, SEG = RowCfg<CAPT>::SEG;
+  static constexpr size_t ring = (size_t)NST * SEG * sizeof(float);
+  static constexpr size_t cand = (size_t)CAPT * sizeof(uint64_t);
+  static constexpr size_t hist = (size_t)(CAPT + 8) * sizeof(uint32_t);
+  static constexpr size_t bs = (size_t)CAPT * sizeof(uint32_t);
+  static constexpr size_t o_cand = ring, o_sorted = o_cand + cand, o_hist = o_sorted + cand, o_bs = o_hist + hist,
+                          o_sh = o_bs + bs;
+  static constexpr size_t total = o_sh + sizeof(RowShared<NST>) + 128;
+};
+
+// mbarrier wait for the producer and scout warps: they poll with a sleep in between, so that their
+// waiting stays off the issue slots of the consumer warps (a try_wait loop of two warps per CTA took a
+// sixth of all issued instructions)
+__device__ __forceinline__ void mbar_wait_park(uint64_t* bar, uint32_t parity) {
+  while (!mbar_test(bar, parity)) __nanosleep(FS_KROW_POLL_NS);
+}
 
 __device__ __forceinline__ void cbar() { asm volatile("bar.sync 1, %0;" ::"n"(RT) : "memory"); }
 
 // bucket of a key under the monotone map value -> [0, NBK): non-decreasing in the key for any lo, scale >= 0
+template <int NBK>
 __device__ __forceinline__ int bucket_of(uint64_t key, float lo, float scale) {
   const uint32_t o = (uint32_t)(key >> 32);
   if (o == 0xFFFFFFFFu) return NBK - 1;  // NaN sorts last
@@ -105,6 +137,7 @@ __device__ __forceinline__ int bucket_of(uint64_t key, float lo, float scale) {
   return b > NBK - 1 ? NBK - 1 : b;
 }
 
+template <int CAPT>
 struct RowCtx {
   const RowArgs* a;
   float* ring;
@@ -112,11 +145,12 @@ struct RowCtx {
   uint64_t* sorted;
   uint32_t* hist;
   uint32_t* bs;
-  RowShared* s;
+  RowShared<RowCfg<CAPT>::NST>* s;
   int tid, warp, lane;
 };
 
-__device__ __forceinline__ void emit_out(const RowCtx& c, int64_t row, int r, uint64_t key) {
+template <int CAPT>
+__device__ __forceinline__ void emit_out(const RowCtx<CAPT>& c, int64_t row, int r, uint64_t key) {
   const RowArgs& a = *c.a;
   const uint32_t idx = key_idx(key), o = (uint32_t)(key >> 32);
   // the value is rebuilt from the order image except for the two images that are not injective
@@ -126,8 +160,9 @@ __device__ __forceinline__ void emit_out(const RowCtx& c, int64_t row, int r, ui
   a.out_idx[row * a.k + r] = (int32_t)idx;
 }
 
-// Block-wide bitonic sort of sorted[0..n2) (n2 a power of two <= CAP), ascending.
-__device__ void block_bitonic(const RowCtx& c, int n2) {
+// Block-wide bitonic sort of sorted[0..n2) (n2 a power of two <= CAPT), ascending.
+template <int CAPT>
+__device__ void block_bitonic(const RowCtx<CAPT>& c, int n2) {
   for (int sz = 2; sz <= n2; sz <<= 1) {
     for (int j = sz >> 1; j >= 1; j >>= 1) {
       for (int t = c.tid; t < (n2 >> 1); t += RT) {
@@ -147,22 +182,26 @@ __device__ void block_bitonic(const RowCtx& c, int n2) {
 
 // The counting step over cand[0..m): ranks the keys and either writes the `want` smallest to the
 // output of `row` (padding up to k) or, RESTORE, leaves them in cand[0..want) in ascending order and
-// publishes the want-th smallest in s->thr_key.  lo / hi: value range of the map (have_range), else
-// taken from the candidates.  All consumer threads; ends with a block barrier.
-template <bool RESTORE>
-__device__ void count_select(const RowCtx& c, int64_t row, int m, int want, bool have_range, float lo, float hi) {
-  RowShared* s = c.s;
+// publishes the want-th smallest in s->thr_key.  RAW: cand holds (index << 32 | value bits) as the
+// filter wrote them (position in vals, translated through mp when the row is a survivor list);
+// otherwise keys.  lo / hi: value range of the map (have_range), else taken from the candidates.
+// The histogram must be zero on entry and is left dirty.  All consumer threads; ends with a barrier.
+template <int CAPT, bool RESTORE, bool RAW>
+__device__ void count_select(const RowCtx<CAPT>& c, int64_t row, int m, int want, bool have_range, float lo, float hi,
+                             const uint32_t* mp) {
+  constexpr int NBK = CAPT, BPT = NBK / RT;  // buckets per thread in the scan
+  auto* s = c.s;
   const int tid = c.tid, lane = c.lane, warp = c.warp;
-  // zero the histogram (NBK + 8 words)
-  {
-    uint4* h4 = reinterpret_cast<uint4*>(c.hist);
-    h4[tid] = make_uint4(0, 0, 0, 0);
-    h4[tid + RT] = make_uint4(0, 0, 0, 0);
-    if (tid < 2) h4[2 * RT + tid] = make_uint4(0, 0, 0, 0);
-    if (tid == 0) {
-      s->kb = NBK - 1;
-      s->kept = m;
-      s->maxc = 0;
+  if (tid == 0) {
+    s->kb = NBK - 1;
+    s->kept = m;
+    s->maxc = 0;
+  }
+  if (RAW) {  // raw entries -> keys, in place (every thread converts the entries it will histogram)
+    for (int i = tid; i < m; i += RT) {
+      const uint64_t e = c.cand[i];
+      const uint32_t pos = (uint32_t)(e >> 32);
+      c.cand[i] = make_key(__uint_as_float((uint32_t)e), mp ? mp[pos] : pos);
     }
   }
   if (!have_range) {  // range of the candidates' order images (NaN image left out of the maximum)
@@ -186,26 +225,29 @@ __device__ void count_select(const RowCtx& c, int64_t row, int m, int want, bool
     }
     lo = ord_f32(mn);
     hi = ord_f32(mx);
-  } else {
-    cbar();
   }
   const float span = hi - lo;
   const float scale = (span > 0.f && span < 3.0e38f) ? (float)NBK / span : 0.f;
   // 1. histogram: one shared-memory atomic per key gives the bucket count and the key's slot
   for (int i = tid; i < m; i += RT) {
-    const int b = bucket_of(c.cand[i], lo, scale);
+    const int b = bucket_of<NBK>(c.cand[i], lo, scale);
     const unsigned int slot = atomicAdd(&c.hist[b], 1u);
     c.bs[i] = (uint32_t)b | (slot << 12);
   }
   cbar();
-  // 2. exclusive scan of the 2 048 counts (8 per thread), boundary bucket, largest kept bucket
+  // 2. exclusive scan of the counts (BPT per thread), boundary bucket, largest kept bucket
   {
-    uint4* h4 = reinterpret_cast<uint4*>(c.hist);
-    const uint4 p = h4[2 * tid], q = h4[2 * tid + 1];
-    const unsigned int cn[8] = {p.x, p.y, p.z, p.w, q.x, q.y, q.z, q.w};
-    unsigned int ex[8], run = 0;
+    unsigned int cn[BPT], ex[BPT], run = 0;
 #pragma unroll
-    for (int j = 0; j < 8; ++j) {
+    for (int q = 0; q < BPT / 4; ++q) {
+      const uint4 p = reinterpret_cast<const uint4*>(c.hist)[(BPT / 4) * tid + q];
+      cn[4 * q] = p.x;
+      cn[4 * q + 1] = p.y;
+      cn[4 * q + 2] = p.z;
+      cn[4 * q + 3] = p.w;
+    }
+#pragma unroll
+    for (int j = 0; j < BPT; ++j) {
       ex[j] = run;
       run += cn[j];
     }
@@ -223,18 +265,19 @@ __device__ void count_select(const RowCtx& c, int64_t row, int m, int want, bool
       if (w < warp) base += (unsigned int)s->wsum[w];
     unsigned int mxc = 0;
 #pragma unroll
-    for (int j = 0; j < 8; ++j) {
+    for (int j = 0; j < BPT; ++j) {
       ex[j] += base;
       if ((int)ex[j] < want) {
         mxc = cn[j] > mxc ? cn[j] : mxc;
         if ((int)(ex[j] + cn[j]) >= want) {  // rank want-1 lives here
-          s->kb = tid * 8 + j;
+          s->kb = tid * BPT + j;
           s->kept = (int)(ex[j] + cn[j]);
         }
       }
     }
-    h4[2 * tid] = make_uint4(ex[0], ex[1], ex[2], ex[3]);
-    h4[2 * tid + 1] = make_uint4(ex[4], ex[5], ex[6], ex[7]);
+#pragma unroll
+    for (int q = 0; q < BPT / 4; ++q)
+      reinterpret_cast<uint4*>(c.hist)[(BPT / 4) * tid + q] = make_uint4(ex[4 * q], ex[4 * q + 1], ex[4 * q + 2], ex[4 * q + 3]);
     if (tid == RT - 1) c.hist[NBK] = base + run;  // = m: end of the last bucket
     mxc = __reduce_max_sync(kFull, mxc);
     if (lane == 0 && mxc > 0) atomicMax(&s->maxc, (int)mxc);
@@ -252,7 +295,7 @@ __device__ void count_select(const RowCtx& c, int64_t row, int m, int want, bool
   if (s->maxc <= RANK_MAX_BUCKET) {
     for (int p = tid; p < kept; p += RT) {
       const uint64_t key = c.sorted[p];
-      const int b = bucket_of(key, lo, scale);
+      const int b = bucket_of<NBK>(key, lo, scale);
       const int s0 = (int)c.hist[b], e0 = (int)c.hist[b + 1];
       int r = s0;
       for (int j = s0; j < e0; ++j) r += c.sorted[j] < key ? 1 : 0;
@@ -261,7 +304,7 @@ __device__ void count_select(const RowCtx& c, int64_t row, int m, int want, bool
           c.cand[r] = key;
           if (r == want - 1) s->thr_key = key;
         } else {
-          emit_out(c, row, r, key);
+          emit_out<CAPT>(c, row, r, key);
         }
       }
     }
@@ -270,14 +313,14 @@ __device__ void count_select(const RowCtx& c, int64_t row, int m, int want, bool
     while (n2 < kept) n2 <<= 1;
     for (int p = kept + tid; p < n2; p += RT) c.sorted[p] = kSentinelKey;
     cbar();
-    block_bitonic(c, n2);
+    block_bitonic<CAPT>(c, n2);
     for (int p = tid; p < want; p += RT) {
       const uint64_t key = c.sorted[p];
       if (RESTORE) {
         c.cand[p] = key;
         if (p == want - 1) s->thr_key = key;
       } else {
-        emit_out(c, row, p, key);
+        emit_out<CAPT>(c, row, p, key);
       }
     }
   }
@@ -291,21 +334,31 @@ __device__ void count_select(const RowCtx& c, int64_t row, int m, int want, bool
   cbar();
 }
 
+template <int CAPT>
+__device__ __forceinline__ void zero_hist(const RowCtx<CAPT>& c) {
+  uint4* h4 = reinterpret_cast<uint4*>(c.hist);
+#pragma unroll
+  for (int i = 0; i < CAPT / (4 * RT); ++i) h4[i * RT + c.tid] = make_uint4(0, 0, 0, 0);
+  if (c.tid < 2) h4[CAPT / 4 + c.tid] = make_uint4(0, 0, 0, 0);
+}
+
 // Exact selection of one row by the paper's scheme: chunks of the row are merged into a
 // running top-k whose k-th key is the bound for what follows; the merge is count_select<RESTORE>.
-__device__ void slow_row(const RowCtx& c, int64_t row, const float* src, int64_t len, const uint32_t* map) {
-  RowShared* s = c.s;
+template <int CAPT>
+__device__ void slow_row(const RowCtx<CAPT>& c, int64_t row, const float* src, int64_t len, const uint32_t* map) {
+  auto* s = c.s;
   const RowArgs& a = *c.a;
   const int k = a.k;
   const int want_all = (int64_t)k < len ? k : (int)len;
+  zero_hist<CAPT>(c);
   if (c.tid == 0) {
     s->cnt = 0;
     s->thr_key = kSentinelKey;
   }
   cbar();
-  const int64_t chunk = CAP - k > 256 ? CAP - k : 256;  // k <= 1 024 < CAP
+  const int64_t chunk = CAPT - k;  // k <= CAPT / 2
   if (len == 0) {
-    count_select<false>(c, row, 0, 0, false, 0.f, 0.f);
+    count_select<CAPT, false, false>(c, row, 0, 0, false, 0.f, 0.f, nullptr);
     return;
   }
   for (int64_t e0 = 0; e0 < len; e0 += chunk) {
@@ -318,9 +371,10 @@ __device__ void slow_row(const RowCtx& c, int64_t row, const float* src, int64_t
     cbar();
     const int m = s->cnt;
     if (e1 >= len) {
-      count_select<false>(c, row, m, m < want_all ? m : want_all, false, 0.f, 0.f);
+      count_select<CAPT, false, false>(c, row, m, m < want_all ? m : want_all, false, 0.f, 0.f, nullptr);
     } else if (m > k) {
-      count_select<true>(c, row, m, k, false, 0.f, 0.f);
+      count_select<CAPT, true, false>(c, row, m, k, false, 0.f, 0.f, nullptr);
+      zero_hist<CAPT>(c);
       if (c.tid == 0) s->cnt = k;
       cbar();
     }
@@ -335,26 +389,136 @@ __device__ __forceinline__ float sample_target(float z, int k, int S, int64_t le
   return r * r;
 }
 
-__global__ void __launch_bounds__(RTHREADS) kselect_row_kernel(const RowArgs a) {
+// The scout warp's job for one row: a bound from the first S = 2 048 (or 1 024) elements of the row's
+// first stage, by a counting search over the sample (interpolation with a bisection safeguard).
+template <int CAPT>
+__device__ __forceinline__ RowBound scout_bound(const float* st, int cnt, int64_t len, int k, int lane) {
+  RowBound b;
+  b.thr_x = __uint_as_float(0x7FFFFFFFu);
+  b.lo = b.hi = 0.f;
+  b.sampled = 0;
+  // 2 048 sample elements for rows of cfg2's length (the scout's work is on the issue budget of the SM), the
+  // whole first stage for long lists, whose bound needs the resolution
+  const int S = (cnt >= 4096 && len > 32768) ? 4096 : (cnt >= 2048 ? 2048 : 1024);
+  const float rho = sample_target(3.f, k, S, len);
+  const int rho_lo = (int)rho + 1;
+  int w = rho_lo >> 3;
+  w = w < 8 ? 8 : w;
+  const int rho_hi = rho_lo + w;  // a window of >= 8 counts is found in a few probes
+  // the survivors expected at the top of the window, plus 3 sigma of the sampling error, must fit
+  const float top = (float)rho_hi + 3.f * sqrtf((float)rho_hi);
+  if (!(cnt >= 1024 && rho_hi < S / 2 && len > CAPT && top * (float)len <= (float)CAPT * (float)S)) return b;
+  const int nq = S / 128;  // float4 per lane
+  const float4* s4 = reinterpret_cast<const float4*>(st);
+  float mn = __uint_as_float(0x7F800000u), mx = __uint_as_float(0xFF800000u);
+  bool has_nan = false;
+#pragma unroll 4
+  for (int j = 0; j < nq; ++j) {
+    const float4 x = s4[j * 32 + lane];
+    mn = fminf(fminf(mn, x.x), fminf(fminf(x.y, x.z), x.w));
+    mx = fmaxf(fmaxf(mx, x.x), fmaxf(fmaxf(x.y, x.z), x.w));
+    has_nan |= (x.x != x.x) | (x.y != x.y) | (x.z != x.z) | (x.w != x.w);
+  }
+  const uint32_t omn = __reduce_min_sync(kFull, f32_ord(mn));
+  uint32_t omx = __reduce_max_sync(kFull, f32_ord(mx));
+  if (__any_sync(kFull, has_nan)) omx = 0xFFFFFFFFu;
+  // bracket [lo, hi] in the order image with counts clo < rho_lo, chi > rho_hi; probes interpolate
+  // linearly in the value domain (3 of 4 steps) or bisect the order image (every 4th: termination)
+  uint32_t lo = omn > 0u ? omn - 1u : 0u, hi = omx, pick = 0xFF800000u;
+  if (hi > 0xFF800000u) hi = 0xFF800000u;  // NaN in the sample: the +inf image is the widest bound
+  int clo = 0, chi = S;
+  const float target = 0.5f * (float)(rho_lo + rho_hi);
+  if (hi <= lo) hi = lo;  // degenerate (constant sample): pick stays +inf
+#pragma unroll 1
+  for (int it = 0; it < 48 && hi - lo > 1u; ++it) {
+    uint32_t mid = lo + ((hi - lo) >> 1);
+    if ((it & 3) != 3) {
+      const float vlo = ord_f32(lo), vhi = ord_f32(hi);
+      const float t = vlo + (vhi - vlo) * ((target - (float)clo) / (float)(chi - clo));
+      const uint32_t m2 = f32_ord(t);
+      if (t == t && m2 > lo && m2 < hi) mid = m2;
+    }
+    const float tf = ord_f32(mid);
+    int cme = 0;
+    // After a few probes without a hit the distribution is probably discrete (ties): the probe then also
+    // finds the sample values next to it, and the bracket snaps to them, so that runs of equal values
+    // cost one probe each instead of a bisection down to one ulp.
+    const bool snap = it >= 4;
+    float vb = __uint_as_float(0xFF800000u), va = __uint_as_float(0x7F800000u);  // max <= tf, min > tf
+    if (!snap) {
+#pragma unroll 4
+      for (int j = 0; j < nq; ++j) {
+        const float4 x = s4[j * 32 + lane];
+        cme += (x.x <= tf) + (x.y <= tf) + (x.z <= tf) + (x.w <= tf);
+      }
+    } else {
+#pragma unroll 2
+      for (int j = 0; j < nq; ++j) {
+        const float4 x = s4[j * 32 + lane];
+        const float e[4] = {x.x, x.y, x.z, x.w};
+#pragma unroll
+        for (int t = 0; t < 4; ++t) {
+          if (e[t] <= tf) {
+            ++cme;
+            vb = fmaxf(vb, e[t]);
+          } else if (e[t] == e[t]) {
+            va = fminf(va, e[t]);
+          }
+        }
+      }
+    }
+    const int cw = __reduce_add_sync(kFull, cme);
+    uint32_t nlo = mid, nhi = mid;
+    if (snap) {
+      const uint32_t ob = __reduce_max_sync(kFull, f32_ord(vb)), oa = __reduce_min_sync(kFull, f32_ord(va));
+      if (cw > 0 && ob <= mid) nhi = ob;                  // the count at ob is the count at mid
+      if (cw < S && oa > mid && oa > 0u) nlo = oa - 1u;   // and so is the count just under oa
+    }
+    if (cw < rho_lo) {
+      lo = nlo > lo ? nlo : lo;
+      clo = cw;
+    } else {
+      hi = nhi < hi ? nhi : hi;
+      chi = cw;
+      pick = hi;
+      if (cw <= rho_hi) break;
+    }
+  }
+  if (pick == 0xFF800000u && hi < 0xFF800000u && hi > lo) pick = hi;  // window never hit: hi passes >= rho_lo
+  if (pick >= 0xFF800000u) return b;  // no usable bound: the row behaves as an unsampled one
+  b.thr_x = ord_f32(pick + 1u);  // inclusive bound `pick`: everything with order image <= pick passes
+  b.lo = ord_f32(omn);
+  b.hi = ord_f32(pick);
+  b.sampled = 1;
+  return b;
+}
+
+template <int CAPT>
+__global__ void __launch_bounds__(RTHREADS, RowCfg<CAPT>::CTAS) kselect_row_kernel(const RowArgs a) {
+  constexpr int NST = RowCfg<CAPT>::NST, SEG = RowCfg<CAPT>::SEG, VPT = SEG / (4 * RT);  // float4 per thread and stage
+  using SM = RowSmem<CAPT>;
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  RowCtx c;
+  RowCtx<CAPT> c;
   c.a = &a;
   c.ring = reinterpret_cast<float*>(smem_raw);
-  c.cand = reinterpret_cast<uint64_t*>(smem_raw + kRingBytes);
-  c.sorted = reinterpret_cast<uint64_t*>(smem_raw + kRingBytes + kCandBytes);
-  c.hist = reinterpret_cast<uint32_t*>(smem_raw + kRingBytes + 2 * kCandBytes);
-  c.bs = reinterpret_cast<uint32_t*>(smem_raw + kRingBytes + 2 * kCandBytes + kHistBytes);
-  c.s = reinterpret_cast<RowShared*>(smem_raw + kRingBytes + 2 * kCandBytes + kHistBytes + kBsBytes);
+  c.cand = reinterpret_cast<uint64_t*>(smem_raw + SM::o_cand);
+  c.sorted = reinterpret_cast<uint64_t*>(smem_raw + SM::o_sorted);
+  c.hist = reinterpret_cast<uint32_t*>(smem_raw + SM::o_hist);
+  c.bs = reinterpret_cast<uint32_t*>(smem_raw + SM::o_bs);
+  c.s = reinterpret_cast<RowShared<NST>*>(smem_raw + SM::o_sh);
   c.tid = threadIdx.x;
   c.warp = threadIdx.x >> 5;
   c.lane = threadIdx.x & 31;
-  RowShared* s = c.s;
+  auto* s = c.s;
   if (threadIdx.x == 0) {
 #pragma unroll
-    for (int i = 0; i < NSTAGE; ++i) {
+    for (int i = 0; i < NST; ++i) {
       mbar_init(&s->full[i], 1);
-      mbar_init(&s->empty[i], RW);
+      mbar_init(&s->empty[i], RW + 1);
+      mbar_init(&s->bnd[i], 1);
     }
+    s->cnt = 0;
+    s->ovf = 0;
     fence_mbar_init();
   }
   __syncthreads();
@@ -365,8 +529,8 @@ __global__ void __launch_bounds__(RTHREADS) kselect_row_kernel(const RowArgs a) 
     uint32_t stage = 0;
     int64_t row = blockIdx.x;
     auto acquire = [&]() {
-      const int slot = (int)(stage % NSTAGE);
-      mbar_wait(&s->empty[slot], ((stage / NSTAGE) & 1u) ^ 1u);
+      const int slot = (int)(stage % NST);
+      mbar_wait_park(&s->empty[slot], ((stage / NST) & 1u) ^ 1u);
       return slot;
     };
     while (row < a.n_rows) {
@@ -393,6 +557,7 @@ __global__ void __launch_bounds__(RTHREADS) kselect_row_kernel(const RowArgs a) 
         const int cnt = (int)(left < SEG ? left : SEG);
         StageDesc& d = s->desc[slot];
         d.row = row;
+        d.len = len;
         d.seg = (int)seg;
         d.cnt = cnt;
         d.last = seg == nseg - 1;
@@ -413,170 +578,161 @@ __global__ void __launch_bounds__(RTHREADS) kselect_row_kernel(const RowArgs a) 
     return;
   }
 
+  if (c.warp == RW + 1) {
+    // ---------------- scout: the bound of every row, ahead of the consumers ----------------
+    uint32_t stage = 0;
+    for (;;) {
+      const int slot = (int)(stage % NST);
+      mbar_wait_park(&s->full[slot], (stage / NST) & 1u);
+      const int64_t row = s->desc[slot].row;
+      if (row < 0) break;
+      if (s->desc[slot].seg == 0) {
+        const RowBound b = scout_bound<CAPT>(c.ring + (size_t)slot * SEG, s->desc[slot].cnt, s->desc[slot].len, a.k, c.lane);
+        if (c.lane == 0) s->bound[slot] = b;
+      }
+      __syncwarp();
+      if (c.lane == 0) {
+        mbar_arrive(&s->bnd[slot]);    // every stage, so that its phases run with the ring's
+        mbar_arrive(&s->empty[slot]);  // the scout is done reading the stage
+      }
+      ++stage;
+    }
+    return;
+  }
+
   // ---------------- consumers ----------------
-  const int tid = c.tid, lane = c.lane, warp = c.warp;
+  const int tid = c.tid, lane = c.lane;
   const int k = a.k;
+  const uint32_t cnt_addr = smem_addr(&s->cnt), ring_sa = smem_addr(c.ring), cand_sa = smem_addr(c.cand);
   uint32_t stage = 0;
-  float thr_x = 0.f;     // an element enters iff !(v >= thr_x)
-  float map_lo = 0.f, map_hi = 0.f;
-  bool sampled = false;
+  RowBound bd;
+  bd.thr_x = 0.f;
+  bd.lo = bd.hi = 0.f;
+  bd.sampled = 0;
   int64_t len = 0, head = 0;
   const float* p = nullptr;
   const uint32_t* mp = nullptr;
   for (;;) {
-    const int slot = (int)(stage % NSTAGE);
-    mbar_wait(&s->full[slot], (stage / NSTAGE) & 1u);
-    const StageDesc d = s->desc[slot];
-    if (d.row < 0) break;
-    const int64_t row = d.row;
+    const int slot = (int)(stage % NST);
+    const uint32_t par = (stage / NST) & 1u;
+    mbar_wait(&s->full[slot], par);
+    const int64_t row = s->desc[slot].row;
+    if (row < 0) break;
+    const int seg = s->desc[slot].seg, dcnt = s->desc[slot].cnt, dlast = s->desc[slot].last, dfb = s->desc[slot].fallback;
     const float* st = c.ring + (size_t)slot * SEG;
-    if (d.seg == 0) {
-      // ---- row begin: state, sampled bound ----
-      len = a.len ? (d.fallback ? 0 : (int64_t)a.len[row]) : a.n;
+    if (seg == 0) {
+      // ---- row begin ----
+      len = s->desc[slot].len;
       p = a.vals + row * a.ld;
       mp = a.map ? a.map + row * a.ld : nullptr;
       head = (4 - (int64_t)(((uintptr_t)p >> 2) & 3)) & 3;
       if (head > len) head = len;
-      if (tid == 0) {
-        s->cnt = 0;
-        s->ovf = 0;
-      }
-      const int S = d.cnt >= 2048 ? 2048 : 1024;
-      const float rho = sample_target(3.f, k, S, len);
-      const int rho_lo = (int)rho + 1, rho_hi = rho_lo + (rho_lo >> 3) + 2;
-      sampled = d.cnt >= 1024 && rho_hi < S / 2 && len > CAP;
-      thr_x = __uint_as_float(0x7FFFFFFFu);  // NaN: everything passes
-      if (sampled) {
-        float4 x0 = reinterpret_cast<const float4*>(st)[tid];
-        float4 x1 = make_float4(x0.x, x0.x, x0.x, x0.x);
-        const bool two = S == 2048;
-        if (two) x1 = reinterpret_cast<const float4*>(st)[tid + RT];
-        float mn = fminf(fminf(fminf(x0.x, x0.y), fminf(x0.z, x0.w)), fminf(fminf(x1.x, x1.y), fminf(x1.z, x1.w)));
-        float mx = fmaxf(fmaxf(fmaxf(x0.x, x0.y), fmaxf(x0.z, x0.w)), fmaxf(fmaxf(x1.x, x1.y), fmaxf(x1.z, x1.w)));
-        // fminf / fmaxf drop NaN operands; a NaN anywhere in the sample is seen by the count below
-        const bool has_nan = (x0.x != x0.x) | (x0.y != x0.y) | (x0.z != x0.z) | (x0.w != x0.w) | (x1.x != x1.x) |
-                             (x1.y != x1.y) | (x1.z != x1.z) | (x1.w != x1.w);
-        uint32_t omn = __reduce_min_sync(kFull, f32_ord(mn)), omx = __reduce_max_sync(kFull, f32_ord(mx));
-        const unsigned nanw = __ballot_sync(kFull, has_nan);
-        if (lane == 0) {
-          s->redu[0][warp] = omn;
-          s->redu[1][warp] = nanw ? 0xFFFFFFFFu : omx;
-        }
-        cbar();
-#pragma unroll
-        for (int w = 0; w < RW; ++w) {
-          omn = s->redu[0][w] < omn ? s->redu[0][w] : omn;
-          omx = s->redu[1][w] > omx ? s->redu[1][w] : omx;
-        }
-        // bracket [lo, hi] in the order image with counts clo < rho_lo, chi > rho_hi; probes interpolate
-        // linearly in the value domain (3 of 4 steps) or bisect the order image (every 4th: termination)
-        uint32_t lo = omn > 0u ? omn - 1u : 0u, hi = omx, pick = 0xFF800000u;
-        if (hi > 0xFF800000u) hi = 0xFF800000u;  // NaN in the sample: the +inf image is the widest bound
-        int clo = 0, chi = S;
-        const float target = 0.5f * (float)(rho_lo + rho_hi);
-        const int per = two ? 2 : 1;
-        if (hi <= lo) hi = lo;  // degenerate (constant sample): pick stays +inf
-#pragma unroll 1
-        for (int it = 0; it < 48 && hi - lo > 1u; ++it) {
-          uint32_t mid = lo + ((hi - lo) >> 1);
-          if ((it & 3) != 3) {
-            const float vlo = ord_f32(lo), vhi = ord_f32(hi);
-            const float t = vlo + (vhi - vlo) * ((target - (float)clo) / (float)(chi - clo));
-            const uint32_t m2 = f32_ord(t);
-            if (t == t && m2 > lo && m2 < hi) mid = m2;
-          }
-          const float tf = ord_f32(mid);
-          int cme = (x0.x <= tf) + (x0.y <= tf) + (x0.z <= tf) + (x0.w <= tf);
-          if (two) cme += (x1.x <= tf) + (x1.y <= tf) + (x1.z <= tf) + (x1.w <= tf);
-          cme = __reduce_add_sync(kFull, cme);
-          if (lane == 0) s->red[it & 1][warp] = cme;
-          cbar();
-          int cw = 0;
-#pragma unroll
-          for (int w = 0; w < RW; ++w) cw += s->red[it & 1][w];
-          (void)per;
-          if (cw < rho_lo) {
-            lo = mid;
-            clo = cw;
-          } else {
-            hi = mid;
-            chi = cw;
-            pick = mid;
-            if (cw <= rho_hi) break;
-          }
-        }
-        if (pick == 0xFF800000u && hi < 0xFF800000u && hi > lo) pick = hi;  // window never hit: hi passes >= rho_lo
-        // inclusive bound `pick`: everything with order image <= pick passes
-        thr_x = pick >= 0xFF800000u ? __uint_as_float(0x7FFFFFFFu) : ord_f32(pick + 1u);
-        map_lo = ord_f32(omn);
-        map_hi = ord_f32(pick);
-        if (pick >= 0xFF800000u) sampled = false;  // no usable bound: behaves as an unsampled row
-      }
-      cbar();  // cnt / ovf reset visible; sample registers dead
+      zero_hist<CAPT>(c);
+      mbar_wait(&s->bnd[slot], par);
+      bd = s->bound[slot];
       // head and tail scalars around the aligned body (plain loads)
-      {
-        const int64_t body = ((len - head) >> 2) << 2;
-        const int64_t ntail = len - head - body;
-        if (tid < head + ntail) {
-          const int64_t e = tid < head ? tid : head + body + (tid - head);
-          const float v = p[e];
-          if (!(v >= thr_x)) {
-            const int pos = atomicAdd(&s->cnt, 1);
-            if (pos < CAP)
-              c.cand[pos] = make_key(v, mp ? mp[e] : (uint32_t)e);
-            else
-              s->ovf = 1;
-          }
+      const int64_t body = ((len - head) >> 2) << 2;
+      const int64_t ntail = len - head - body;
+      if (tid < head + ntail) {
+        const int64_t e = tid < head ? tid : head + body + (tid - head);
+        const float v = p[e];
+        if (!(v >= bd.thr_x)) {
+          const int pos = atomicAdd(&s->cnt, 1);
+          if (pos < CAPT)
+            c.cand[pos] = ((uint64_t)(uint32_t)e << 32) | __float_as_uint(v);
+          else
+            s->ovf = 1;
         }
       }
     }
-    // ---- A1: first-level filter over this stage ----
-    if (d.cnt > 0 && !s->ovf) {
-      const int nvec = d.cnt >> 2;
-      const uint32_t ib = (uint32_t)(head + (int64_t)d.seg * SEG);
+    // ---- A1: first-level filter over this stage (4 VPT elements per thread) ----
+    if (dcnt > 0) {
+      const int nvec = dcnt >> 2;
+      const float thr_x = bd.thr_x;
+      const uint32_t st_sa = ring_sa + (uint32_t)slot * (SEG * 4u) + (uint32_t)tid * 16u;
+      float4 x[VPT];
       uint32_t mask = 0u;
+      // pass = !(v >= bound) = "less than or unordered": one FSET and one LOP3 per element
+#define FS_TEST(V, BIT)                                                                                          \
+  asm("{\n\t.reg .b32 t;\n\tset.ltu.u32.f32 t, %1, %2;\n\tlop3.b32 %0, t, %3, %0, 0xEA;\n\t}" : "+r"(mask) : "f"(V), \
+      "f"(thr_x), "r"(BIT))
       if (nvec == SEG / 4) {
-        const float4 x0 = reinterpret_cast<const float4*>(st)[tid];
-        const float4 x1 = reinterpret_cast<const float4*>(st)[tid + RT];
-        // the sign of (bound - v) is funnel-shifted into the mask (v equal to the bound passes the float
-        // test only if it is below thr_x = next above the inclusive bound; NaN bounds pass everything)
-        mask = (!(x0.x >= thr_x) ? 1u : 0u) | (!(x0.y >= thr_x) ? 2u : 0u) | (!(x0.z >= thr_x) ? 4u : 0u) |
-               (!(x0.w >= thr_x) ? 8u : 0u) | (!(x1.x >= thr_x) ? 16u : 0u) | (!(x1.y >= thr_x) ? 32u : 0u) |
-               (!(x1.z >= thr_x) ? 64u : 0u) | (!(x1.w >= thr_x) ? 128u : 0u);
+#pragma unroll
+        for (int u = 0; u < VPT; ++u) {
+          asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];"
+                       : "=f"(x[u].x), "=f"(x[u].y), "=f"(x[u].z), "=f"(x[u].w)
+                       : "r"(st_sa + (uint32_t)u * (RT * 16u)));
+        }
+#pragma unroll
+        for (int u = 0; u < VPT; ++u) {
+          FS_TEST(x[u].x, 1u << (4 * u));
+          FS_TEST(x[u].y, 2u << (4 * u));
+          FS_TEST(x[u].z, 4u << (4 * u));
+          FS_TEST(x[u].w, 8u << (4 * u));
+        }
       } else {
 #pragma unroll
-        for (int u = 0; u < 2; ++u) {
-          const int f = u * RT + tid;
-          if (f < nvec) {
-            const float4 x = reinterpret_cast<const float4*>(st)[f];
-            mask |= ((!(x.x >= thr_x) ? 1u : 0u) | (!(x.y >= thr_x) ? 2u : 0u) | (!(x.z >= thr_x) ? 4u : 0u) |
-                     (!(x.w >= thr_x) ? 8u : 0u))
-                    << (4 * u);
+        for (int u = 0; u < VPT; ++u) {
+          x[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+          if (u * RT + tid < nvec) {
+            asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];"
+                         : "=f"(x[u].x), "=f"(x[u].y), "=f"(x[u].z), "=f"(x[u].w)
+                         : "r"(st_sa + (uint32_t)u * (RT * 16u)));
+            FS_TEST(x[u].x, 1u << (4 * u));
+            FS_TEST(x[u].y, 2u << (4 * u));
+            FS_TEST(x[u].z, 4u << (4 * u));
+            FS_TEST(x[u].w, 8u << (4 * u));
           }
         }
       }
-      const int cm = __popc(mask);
-      int incl = cm;
+#undef FS_TEST
+      if (__any_sync(kFull, mask != 0u)) {
+        const int cm = __popc(mask);
+        int incl = cm;
 #pragma unroll
-      for (int o = 1; o < 32; o <<= 1) {
-        const int v = __shfl_up_sync(kFull, incl, o);
-        if (lane >= o) incl += v;
-      }
-      const int total = __shfl_sync(kFull, incl, 31);
-      if (total > 0) {
-        int base = 0;
-        if (lane == 31) base = atomicAdd(&s->cnt, total);
+        for (int o = 1; o < 32; o <<= 1) {
+          const int v = __shfl_up_sync(kFull, incl, o);
+          if (lane >= o) incl += v;
+        }
+        const int total = __shfl_sync(kFull, incl, 31);
+        int base = 0;  // lane 31 reserves the warp's slots (predicated, no branch)
+        asm volatile("{\n\t.reg .pred p;\n\tsetp.eq.u32 p, %3, 31;\n\t@p atom.shared.add.u32 %0, [%1], %2;\n\t}"
+                     : "+r"(base)
+                     : "r"(cnt_addr), "r"(total), "r"(lane)
+                     : "memory");
         base = __shfl_sync(kFull, base, 31);
-        if (base + total > CAP) {
+        if (base + total > CAPT) {
           if (lane == 0) s->ovf = 1;
         } else {
-          int pos = base + incl - cm;
-          while (mask) {
-            const int b2 = __ffs(mask) - 1;
-            mask &= mask - 1u;
-            const int off = ((b2 >> 2) * RT + tid) * 4 + (b2 & 3);
-            const uint32_t e = ib + (uint32_t)off;
-            c.cand[pos++] = make_key(st[off], mp ? mp[e] : e);
+          // raw entries (position << 32 | value bits): the key is made in the counting step, where every lane works
+          uint32_t addr = cand_sa + (uint32_t)(base + incl - cm) * 8u;
+          const uint32_t ib = (uint32_t)(head + (int64_t)seg * SEG) + (uint32_t)tid * 4u;
+          if (__all_sync(kFull, cm <= 2)) {  // sparse: a loop over the set bits (the value is re-read from the stage)
+            while (mask) {
+              const int j = __ffs(mask) - 1;
+              mask &= mask - 1u;
+              const uint32_t off = (uint32_t)(j >> 2) * (RT * 4u) + (uint32_t)(j & 3);
+              uint32_t bits;
+              asm volatile("ld.shared.u32 %0, [%1];" : "=r"(bits) : "r"(st_sa + off * 4u));
+              asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(addr), "r"(bits), "r"(ib + off) : "memory");
+              addr += 8u;
+            }
+          } else {  // dense: sixteen predicated stores, no branches
+#define FS_PUT(U, E, F)                                                                                       \
+  asm volatile(                                                                                               \
+      "{\n\t.reg .pred p;\n\t.reg .b32 t;\n\tand.b32 t, %1, %2;\n\tsetp.ne.u32 p, t, 0;\n\t"                 \
+      "@p st.shared.u32 [%0], %3;\n\t@p st.shared.u32 [%0+4], %4;\n\t@p add.u32 %0, %0, 8;\n\t}"                   \
+      : "+r"(addr)                                                                                            \
+      : "r"(mask), "r"(1u << (4 * (U) + (E))), "r"(__float_as_uint(F)), "r"(ib + (uint32_t)((U)*RT * 4 + (E))) \
+      : "memory")
+#pragma unroll
+            for (int u = 0; u < VPT; ++u) {
+              FS_PUT(u, 0, x[u].x);
+              FS_PUT(u, 1, x[u].y);
+              FS_PUT(u, 2, x[u].z);
+              FS_PUT(u, 3, x[u].w);
+            }
+#undef FS_PUT
           }
         }
       }
@@ -584,41 +740,57 @@ __global__ void __launch_bounds__(RTHREADS) kselect_row_kernel(const RowArgs a) 
     __syncwarp();
     if (lane == 0) mbar_arrive(&s->empty[slot]);
     ++stage;
-    if (d.last) {
+    if (dlast) {
       // ---- row end: counting step, or the exact slow path ----
       cbar();
       const int m = s->cnt;
       const int want = (int64_t)k < len ? k : (int)len;
-      if (d.fallback) {
-        slow_row(c, row, a.orig + row * a.orig_ld, a.n_orig, nullptr);
-      } else if (s->ovf || m < want) {
-        slow_row(c, row, p, len, mp);
+      if (dfb) {
+        slow_row<CAPT>(c, row, a.orig + row * a.orig_ld, a.n_orig, nullptr);
+      } else if (s->ovf || m < want || m > CAPT) {
+        slow_row<CAPT>(c, row, p, len, mp);
       } else {
-        count_select<false>(c, row, m, want, sampled, map_lo, map_hi);
+        count_select<CAPT, false, true>(c, row, m, want, bd.sampled != 0, bd.lo, bd.hi, mp);
       }
+      if (tid == 0) {
+        s->cnt = 0;
+        s->ovf = 0;
+      }
+      cbar();
     }
   }
 }
 
 // ---------------------------------------------------------------------------
-// A4: long rows.  Step 1: bound from a strided sample of 32 768 elements.
+// A4: long rows.  Step 1: bound from a strided sample of 65 536 elements.
 // ---------------------------------------------------------------------------
-constexpr int LS_PIECES = 32, LS_PIECE = 1024, LS_S = LS_PIECES * LS_PIECE;  // 32 sample values per thread stay in registers
+constexpr int LS_PIECES = 64, LS_PIECE = 1024, LS_S = LS_PIECES * LS_PIECE;
+constexpr int LS_REG = 32;  // sample values per thread kept in registers; the rest in shared memory ([j][tid])
+constexpr size_t kSampleSmem = (size_t)(LS_PIECES - LS_REG) * LS_PIECE * sizeof(float);
 
 __global__ void __launch_bounds__(1024) kselect_sample_kernel(const float* __restrict__ rows, int64_t n, int64_t ld,
                                                                int k, float* __restrict__ thr_out) {
+  extern __shared__ __align__(16) float ls_x[];  // [LS_PIECES - LS_REG][1024]
   __shared__ int red[2][32];
   __shared__ unsigned int redu[2][32];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const float* p = rows + (int64_t)blockIdx.x * ld;
   const int64_t stride = n / LS_PIECES;  // >= LS_PIECE: pieces do not overlap
-  float x[LS_PIECES];
+  float x[LS_REG];
 #pragma unroll
-  for (int j = 0; j < LS_PIECES; ++j) x[j] = p[j * stride + tid];
+  for (int j = 0; j < LS_REG; ++j) x[j] = p[j * stride + tid];
   float mn = x[0], mx = x[0];
   bool has_nan = false;
+#pragma unroll 8
+  for (int j = LS_REG; j < LS_PIECES; ++j) {
+    const float v = p[j * stride + tid];
+    ls_x[(j - LS_REG) * LS_PIECE + tid] = v;
+    mn = fminf(mn, v);
+    mx = fmaxf(mx, v);
+    has_nan |= v != v;
+  }
 #pragma unroll
-  for (int j = 0; j < LS_PIECES; ++j) {
+  for (int j = 0; j < LS_REG; ++j) {
     mn = fminf(mn, x[j]);
     mx = fmaxf(mx, x[j]);
     has_nan |= x[j] != x[j];
@@ -654,7 +826,9 @@ __global__ void __launch_bounds__(1024) kselect_sample_kernel(const float* __res
     const float tf = ord_f32(mid);
     int cme = 0;
 #pragma unroll
-    for (int j = 0; j < LS_PIECES; ++j) cme += x[j] <= tf;
+    for (int j = 0; j < LS_REG; ++j) cme += x[j] <= tf;
+#pragma unroll 8
+    for (int j = 0; j < LS_PIECES - LS_REG; ++j) cme += ls_x[j * LS_PIECE + tid] <= tf;
     cme = __reduce_add_sync(kFull, cme);
     if (lane == 0) red[it & 1][warp] = cme;
     __syncthreads();
@@ -717,7 +891,8 @@ __global__ void __launch_bounds__(LF_THREADS) kselect_filter_kernel(const float*
     float4 x[LF_UNROLL];
     if (v0 + per <= nvec) {
 #pragma unroll
-      for (int u = 0; u < LF_UNROLL; ++u) x[u] = ld_stream4(pv + ((v0 + u * LF_THREADS + threadIdx.x) << 2));
+      for (int u = 0; u < LF_UNROLL; ++u)
+        x[u] = __ldcs(reinterpret_cast<const float4*>(pv + ((v0 + u * LF_THREADS + threadIdx.x) << 2)));
 #pragma unroll
       for (int u = 0; u < LF_UNROLL; ++u) {
         const bool any = !(x[u].x >= thr_x) | !(x[u].y >= thr_x) | !(x[u].z >= thr_x) | !(x[u].w >= thr_x);
@@ -745,28 +920,29 @@ __global__ void __launch_bounds__(LF_THREADS) kselect_filter_kernel(const float*
   }
 }
 
-int row_occupancy() {
+template <int CAPT>
+int launch_rows_t(const RowArgs& a, cudaStream_t s) {
+  using SM = RowSmem<CAPT>;
   static int occ = 0;
   if (occ == 0) {
-    if (cudaFuncSetAttribute(kselect_row_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowSmem) != cudaSuccess)
-      return 0;
-    cudaFuncSetAttribute(kselect_row_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    FS_CUDA(cudaFuncSetAttribute(kselect_row_kernel<CAPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::total));
+    FS_CUDA(cudaFuncSetAttribute(kselect_row_kernel<CAPT>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                                 cudaSharedmemCarveoutMaxShared));
     int o = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, kselect_row_kernel, RTHREADS, kRowSmem) != cudaSuccess) return 0;
+    FS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, kselect_row_kernel<CAPT>, RTHREADS, SM::total));
     occ = o > 0 ? o : 1;
   }
-  return occ;
+  int64_t grid = (int64_t)sm_count() * occ;
+  if (grid > a.n_rows) grid = a.n_rows;
+  kselect_row_kernel<CAPT><<<(unsigned)grid, RTHREADS, SM::total, s>>>(a);
+  FS_LAUNCHED();
+  return FS_OK;
 }
 
 int launch_rows(const RowArgs& a, cudaStream_t s) {
   if (a.n_rows == 0) return FS_OK;
-  const int occ = row_occupancy();
-  if (occ == 0) return set_error(FS_ECUDA, "fs_kselect: cannot configure kselect_row_kernel");
-  int64_t grid = (int64_t)sm_count() * occ;
-  if (grid > a.n_rows) grid = a.n_rows;
-  kselect_row_kernel<<<(unsigned)grid, RTHREADS, kRowSmem, s>>>(a);
-  FS_LAUNCHED();
-  return FS_OK;
+  if (a.map) return launch_rows_t<4096>(a, s);  // one CTA per long row: room for a wide window
+  return a.k <= 256 ? launch_rows_t<1024>(a, s) : launch_rows_t<2048>(a, s);
 }
 
 }  // namespace
@@ -831,7 +1007,12 @@ int kselect_rows_device(const float* rows, int64_t n_rows, int64_t n, int64_t ld
   uint32_t* cidx = reinterpret_cast<uint32_t*>(w + o);
   FS_CUDA(cudaMemsetAsync(w, 0, 256 + align_up((size_t)n_rows * sizeof(float), 256) +
                                     align_up((size_t)n_rows * sizeof(unsigned int), 256), s));
-  kselect_sample_kernel<<<(unsigned)n_rows, 1024, 0, s>>>(rows, n, ld, k, thr);
+  static bool sample_attr = false;
+  if (!sample_attr) {
+    FS_CUDA(cudaFuncSetAttribute(kselect_sample_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSampleSmem));
+    sample_attr = true;
+  }
+  kselect_sample_kernel<<<(unsigned)n_rows, 1024, kSampleSmem, s>>>(rows, n, ld, k, thr);
   FS_LAUNCHED();
   int64_t gx = (int64_t)sm_count() * 8 / n_rows;
   const int64_t maxg = ceil_div(n / 4, (int64_t)LF_THREADS * LF_UNROLL);
