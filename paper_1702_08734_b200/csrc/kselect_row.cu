@@ -342,6 +342,43 @@ __device__ __forceinline__ void zero_hist(const RowCtx<CAPT>& c) {
   if (c.tid < 2) h4[CAPT / 4 + c.tid] = make_uint4(0, 0, 0, 0);
 }
 
+// Second look at a row whose sampled bound let the wrong number of elements through (m_seen of them,
+// counted exactly): the bound is moved along the line through (lo, 0) and (hi, m_seen) to where
+// ~1.3 want elements are expected, and the row (still in L2) is filtered again with plain loads into
+// raw entries.  Returns the new inclusive bound; s->cnt holds the number that passed (entries beyond
+// CAPT are not stored).  The caller decides between the counting step and the exact slow path.
+template <int CAPT>
+__device__ float refilter_row(const RowCtx<CAPT>& c, const float* src, int64_t len, float lo, float hi, int m_seen,
+                              int want) {
+  auto* s = c.s;
+  float f = 1.3f * (float)want / (float)(m_seen > 0 ? m_seen : 1);
+  f = f > 16.f ? 16.f : f;
+  const float nb = lo + (hi - lo) * f;
+  const float thr_x = ord_f32(f32_ord(nb) + 1u);  // inclusive bound nb
+  if (c.tid == 0) s->cnt = 0;
+  cbar();
+  const unsigned lt = (1u << c.lane) - 1u;
+  const int64_t n32 = (len + 31) & ~(int64_t)31;
+  for (int64_t e0 = (int64_t)c.warp * 32; e0 < n32; e0 += RT) {
+    const int64_t e = e0 + c.lane;
+    float v = 0.f;
+    bool pass = false;
+    if (e < len) {
+      v = src[e];
+      pass = !(v >= thr_x);
+    }
+    const unsigned b = __ballot_sync(kFull, pass);
+    if (b == 0u) continue;
+    int base = 0;
+    if (c.lane == 0) base = atomicAdd(&s->cnt, __popc(b));
+    base = __shfl_sync(kFull, base, 0);
+    const int pos = base + __popc(b & lt);
+    if (pass && pos < CAPT) c.cand[pos] = ((uint64_t)(uint32_t)e << 32) | __float_as_uint(v);
+  }
+  cbar();
+  return nb;
+}
+
 // Exact selection of one row by the paper's scheme: chunks of the row are merged into a
 // running top-k whose k-th key is the bound for what follows; the merge is count_select<RESTORE>.
 template <int CAPT>
@@ -748,7 +785,19 @@ __global__ void __launch_bounds__(RTHREADS, RowCfg<CAPT>::CTAS) kselect_row_kern
       if (dfb) {
         slow_row<CAPT>(c, row, a.orig + row * a.orig_ld, a.n_orig, nullptr);
       } else if (s->ovf || m < want || m > CAPT) {
-        slow_row<CAPT>(c, row, p, len, mp);
+        // the sample did not represent the row (sorted rows, runs): one more filter pass with the bound
+        // rescaled by what this pass counted, then the exact scheme if that fails too
+        bool done = false;
+        if (bd.sampled && bd.hi > bd.lo) {
+          const float nb = refilter_row<CAPT>(c, p, len, bd.lo, bd.hi, m, want);
+          const int m2 = s->cnt;
+          if (m2 >= want && m2 <= CAPT) {
+            count_select<CAPT, false, true>(c, row, m2, want, false, 0.f, 0.f, mp);
+            done = true;
+          }
+          (void)nb;
+        }
+        if (!done) slow_row<CAPT>(c, row, p, len, mp);
       } else {
         count_select<CAPT, false, true>(c, row, m, want, bd.sampled != 0, bd.lo, bd.hi, mp);
       }

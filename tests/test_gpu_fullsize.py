@@ -76,6 +76,30 @@ def test_cfg2_long_row():
     assert np.array_equal(val[0].cpu().numpy().view(np.uint32), ev[0].view(np.uint32))
 
 
+@pytest.mark.parametrize("kind", ["ascending", "descending", "constant"])
+def test_cfg2_long_row_structured(kind):
+    """The 2^27-element row when it is sorted or constant: the answer is known in closed form."""
+    fs = fsmod()
+    n, k = 1 << 27, 1024
+    if kind == "constant":
+        row = torch.full((1, n), 0.25, dtype=torch.float32, device="cuda")
+        want_idx = np.arange(k)
+        want_val = np.full(k, 0.25, np.float32)
+    else:
+        asc = torch.arange(n, dtype=torch.float32, device="cuda")  # exact up to 2^24, then runs of equal values
+        row = (asc if kind == "ascending" else asc.flip(0))[None, :].contiguous()
+        host = row[0].cpu().numpy()
+        if kind == "ascending":
+            want_idx = np.arange(k)
+        else:  # the k smallest values sit at the end; equal values (runs above 2^24 only) keep index order
+            want_idx = np.arange(n - 1, n - 1 - k, -1)
+        want_val = host[want_idx]
+    val, idx = fs.kselect(row, k)
+    torch.cuda.synchronize()
+    assert np.array_equal(idx[0].cpu().numpy(), want_idx.astype(np.int32))
+    assert np.array_equal(val[0].cpu().numpy().view(np.uint32), want_val.view(np.uint32))
+
+
 @pytest.mark.parametrize("k", [1, 10, 100])
 def test_cfg3_full_sampled_queries(k):
     from datagen import gen_torch as gt

@@ -98,6 +98,33 @@ def test_long_row_is_split(k):
     assert_exact(rows, k)
 
 
+@pytest.mark.parametrize("k", [2, 100, 1024])
+def test_long_rows_monotone_constant_and_ties(k):
+    """A4 on rows a first-elements sample would misjudge: ascending, descending, constant, few distinct
+    values.  The long-row bound comes from a strided sample; results stay bit-exact either way."""
+    n = 1 << 20
+    asc = np.arange(n, dtype=np.float32)
+    rows = np.stack([asc, asc[::-1].copy(), np.full(n, 1.5, np.float32), (np.arange(n) % 5).astype(np.float32)])
+    assert_exact(rows, k)
+
+
+@pytest.mark.parametrize("k", [2, 32, 300, 1024])
+def test_batch_rows_that_mislead_the_sample(k):
+    """Rows of cfg2's length whose first 2 048 elements do not represent them (sorted both ways, runs,
+    a few distinct values, a block of small values at the end): the sampled bound lets too few or too
+    many through and the kernel must take its second filter pass or the exact slow path."""
+    n = 16384
+    rng = np.random.default_rng(k)
+    asc = np.sort(rng.random(n, dtype=np.float32))
+    late = rng.random(n, dtype=np.float32) + 1.0
+    late[-3000:] -= 1.0
+    runs = np.repeat(rng.random(n // 64, dtype=np.float32), 64)
+    few = rng.integers(0, 3, n).astype(np.float32)
+    rows = np.stack([asc, asc[::-1].copy(), late, late[::-1].copy(), runs, few, np.zeros(n, np.float32)])
+    rows = np.concatenate([rows, datagen.kselect_rows(0, 500, n, duplicates=False)[:, :n]])  # enough rows to fill the GPU
+    assert_exact(rows, k)
+
+
 def test_host_entry_point_and_errors():
     import paper_1702_08734_b200 as fs
     rows = datagen.kselect_rows(7, 5, 3000)
