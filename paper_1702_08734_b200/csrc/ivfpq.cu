@@ -64,17 +64,21 @@ __global__ void __launch_bounds__(ENC_WARPS * 32)
     pq_encode_kernel(const float* __restrict__ y, int64_t n, int d, int M, int dsub,
                      const float* __restrict__ coarse, const int64_t* __restrict__ assign,
                      const float* __restrict__ pq, uint8_t* __restrict__ codes_out,
-                     uint32_t* __restrict__ list_out) {
+                     uint32_t* __restrict__ list_out, float* __restrict__ s1_out) {
   extern __shared__ __align__(16) float enc_smem[];
   const int dsp = dsub | 1;                    // odd stride: conflict-free codeword reads
   float* cb = enc_smem;                        // [256][dsp]
   float* res = cb + 256 * dsp;                 // [TV][dsub]
-  uint8_t* cd = reinterpret_cast<uint8_t*>(res + ENC_TV * dsub);  // [TV][M]
+  float* cen = res + ENC_TV * dsub;            // [TV][dsub] the centroid's sub-vector (for term 1)
+  float* s1a = cen + ENC_TV * dsub;            // [TV] term 1 accumulated over the sub-quantizers
+  uint8_t* cd = reinterpret_cast<uint8_t*>(s1a + ENC_TV);  // [TV][M]
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int64_t ntiles = (n + ENC_TV - 1) / ENC_TV;
   for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
     const int64_t v0 = tile * ENC_TV;
     const int nv = (int)((n - v0) < ENC_TV ? (n - v0) : ENC_TV);
+    __syncthreads();
+    if (tid < ENC_TV) s1a[tid] = 0.f;
     for (int m = 0; m < M; ++m) {
       __syncthreads();
       for (int e = tid; e < 256 * dsub; e += ENC_WARPS * 32) {
@@ -83,12 +87,14 @@ __global__ void __launch_bounds__(ENC_WARPS * 32)
       }
       for (int e = tid; e < ENC_TV * dsub; e += ENC_WARPS * 32) {
         const int v = e / dsub, j = e - v * dsub;
-        float r = 0.f;
+        float r = 0.f, cj = 0.f;
         if (v < nv) {
           const int64_t L = assign[v0 + v];
-          r = y[(v0 + v) * d + m * dsub + j] - coarse[L * d + m * dsub + j];
+          cj = coarse[L * d + m * dsub + j];
+          r = y[(v0 + v) * d + m * dsub + j] - cj;
         }
         res[e] = r;
+        cen[e] = cj;
       }
       __syncthreads();
       // warp w: vectors w*4 .. w*4+3
@@ -119,21 +125,34 @@ __global__ void __launch_bounds__(ENC_WARPS * 32)
         for (int c = 0; c < 8; ++c) best = umin64(best, make_key(acc[v][c], (uint32_t)(c * 32 + lane)));
 #pragma unroll
         for (int s = 16; s >= 1; s >>= 1) best = umin64(best, shfl_xor64(best, s));
-        if (lane == 0) cd[(warp * ENC_VPW + v) * M + m] = (uint8_t)key_idx(best);
+        const int cbest = (int)key_idx(best);
+        if (lane == 0) cd[(warp * ENC_VPW + v) * M + m] = (uint8_t)cbest;
+        // Eq. 11 term 1 of this sub-quantizer: ||B||^2 + 2 <c, B> = sum_j B_j (B_j + 2 c_j), in dimension
+        // order by one lane (fixed order: the same vector always gets the same bits)
+        if (lane == 0) {
+          const float* bw = cb + cbest * dsp;
+          const float* cw = cen + (warp * ENC_VPW + v) * dsub;
+          float t = 0.f;
+          for (int j = 0; j < dsub; ++j) t = fmaf(bw[j], bw[j] + 2.f * cw[j], t);
+          s1a[warp * ENC_VPW + v] += t;
+        }
       }
     }
     __syncthreads();
     for (int e = tid; e < nv * M; e += ENC_WARPS * 32) codes_out[v0 * M + e] = cd[e];
-    if (tid < nv) list_out[v0 + tid] = (uint32_t)assign[v0 + tid];
+    if (tid < nv) {
+      list_out[v0 + tid] = (uint32_t)assign[v0 + tid];
+      s1_out[v0 + tid] = s1a[tid];
+    }
   }
 }
 }  // namespace
 
 int launch_pq_encode(const fs_ivfpq* ix, const float* y, int64_t n, const int64_t* assign,
-                     uint8_t* codes_out, uint32_t* list_out, cudaStream_t s) {
+                     uint8_t* codes_out, uint32_t* list_out, float* s1_out, cudaStream_t s) {
   if (n == 0) return FS_OK;
   const int dsub = ix->dsub, dsp = dsub | 1;
-  const size_t smem = (size_t)(256 * dsp + ENC_TV * dsub) * sizeof(float) + (size_t)ENC_TV * ix->M;
+  const size_t smem = (size_t)(256 * dsp + 2 * ENC_TV * dsub + ENC_TV) * sizeof(float) + (size_t)ENC_TV * ix->M;
   static size_t attr_smem = 0;
   if (smem > attr_smem) {
     FS_CUDA(cudaFuncSetAttribute(pq_encode_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -144,7 +163,7 @@ int launch_pq_encode(const fs_ivfpq* ix, const float* y, int64_t n, const int64_
   const int64_t maxg = (int64_t)sm_count() * 8;
   pq_encode_kernel<<<(unsigned)(ntiles < maxg ? ntiles : maxg), ENC_WARPS * 32, smem, s>>>(
       y, n, ix->d, ix->M, dsub, ix->coarse.as<float>(), assign, ix->pq.as<float>(), codes_out,
-      list_out);
+      list_out, s1_out);
   FS_LAUNCHED();
   return FS_OK;
 }
@@ -267,29 +286,64 @@ __global__ void csr_offsets_kernel(const uint32_t* __restrict__ keys, int64_t n,
     for (int64_t l = k1 + 1; l <= nlist; ++l) offsets[l] = n;
 }
 
-__global__ void csr_gather_kernel(const uint32_t* __restrict__ perm, int64_t n, int64_t n_old,
-                                  int M, const uint8_t* __restrict__ old_codes,
-                                  const int64_t* __restrict__ old_ids,
-                                  const uint8_t* __restrict__ st_codes,
-                                  const int64_t* __restrict__ st_ids,
-                                  uint8_t* __restrict__ codes, int64_t* __restrict__ ids) {
+// Moves every vector to its CSR position p.  perm[p] = arrival index (old CSR entries first, then the
+// staged ones); keys[p] = list number of position p.  With `permute` the code bytes are stored in the lane
+// order of the fixed-point scan: byte i of the vector at position v of its list holds sub-quantizer
+// i ^ (v mod M) (M = 8 / 16); old entries are moved from the order of their old position to the new one.
+__global__ void csr_gather_kernel(const uint32_t* __restrict__ perm, const uint32_t* __restrict__ keys, int64_t n,
+                                  int64_t n_old, int M, bool permute, const int64_t* __restrict__ old_offsets,
+                                  const int64_t* __restrict__ new_offsets, const uint8_t* __restrict__ old_codes,
+                                  const int64_t* __restrict__ old_ids, const float* __restrict__ old_s1,
+                                  const uint8_t* __restrict__ st_codes, const int64_t* __restrict__ st_ids,
+                                  const float* __restrict__ st_s1, uint8_t* __restrict__ codes,
+                                  int64_t* __restrict__ ids, float* __restrict__ s1) {
   const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= n) return;
   const int64_t a = perm[p];
   const uint8_t* src;
+  int r = 0;
+  if (permute) {
+    const int64_t L = keys[p];
+    r = (int)((p - new_offsets[L]) & (M - 1));
+    if (a < n_old) r ^= (int)((a - old_offsets[L]) & (M - 1));
+  }
   if (a < n_old) {
     src = old_codes + a * M;
     ids[p] = old_ids[a];
+    s1[p] = old_s1[a];
   } else {
     src = st_codes + (a - n_old) * M;
     ids[p] = st_ids[a - n_old];
+    s1[p] = st_s1[a - n_old];
   }
   uint8_t* dst = codes + p * M;
-  if ((M & 3) == 0) {
+  if (permute) {
+    uint32_t w[4];
+    for (int i = 0; i < M / 4; ++i) w[i] = reinterpret_cast<const uint32_t*>(src)[i];
+    const uint32_t sel = 0x3210u ^ (0x1111u * (uint32_t)(r & 3));  // byte i <- byte i ^ (r & 3) of the same word
+    for (int i = 0; i < M / 4; ++i) reinterpret_cast<uint32_t*>(dst)[i] = __byte_perm(w[i ^ (r >> 2)], 0u, sel);
+  } else if ((M & 3) == 0) {
     for (int w = 0; w < M / 4; ++w)
       reinterpret_cast<uint32_t*>(dst)[w] = reinterpret_cast<const uint32_t*>(src)[w];
   } else {
     for (int b = 0; b < M; ++b) dst[b] = src[b];
+  }
+}
+
+// Plain order of the stored codes of whole lists: block j copies list list_nos[j] (or list j) from the CSR
+// arrays to dst + dst_offsets[j] * M, undoing the permutation of csr_gather_kernel.
+__global__ void csr_unpermute_kernel(const uint8_t* __restrict__ codes, const int64_t* __restrict__ offsets,
+                                     const int32_t* __restrict__ list_nos, const int64_t* __restrict__ dst_offsets,
+                                     int M, uint8_t* __restrict__ dst) {
+  const int64_t L = list_nos ? list_nos[blockIdx.x] : blockIdx.x;
+  const int64_t b = offsets[L], len = offsets[L + 1] - b;
+  uint8_t* out = dst + (dst_offsets ? dst_offsets[blockIdx.x] : b) * M;
+  for (int64_t v = threadIdx.x; v < len; v += blockDim.x) {
+    const int r = (int)(v & (M - 1));
+    const uint32_t sel = 0x3210u ^ (0x1111u * (uint32_t)(r & 3));
+    uint32_t w[4];
+    for (int i = 0; i < M / 4; ++i) w[i] = reinterpret_cast<const uint32_t*>(codes + (b + v) * M)[i];
+    for (int i = 0; i < M / 4; ++i) reinterpret_cast<uint32_t*>(out + v * M)[i] = __byte_perm(w[i ^ (r >> 2)], 0u, sel);
   }
 }
 
@@ -305,7 +359,7 @@ int ivfpq_finalise(fs_ivfpq* ix, cudaStream_t s) {
   const int nlist = ix->nlist, M = ix->M;
   int rc;
   if (n >= (1LL << 32)) return set_error(FS_EUNSUPPORTED, "fs_ivfpq: more than 2^32-1 vectors");
-  DevBuf noffsets, ncodes, nids;
+  DevBuf noffsets, ncodes, nids, ns1;
   if ((rc = noffsets.ensure((size_t)(nlist + 1) * sizeof(int64_t), 0, s)) != FS_OK) return rc;
   if (n == 0) {
     FS_CUDA(cudaMemsetAsync(noffsets.p, 0, (size_t)(nlist + 1) * sizeof(int64_t), s));
@@ -338,6 +392,7 @@ int ivfpq_finalise(fs_ivfpq* ix, cudaStream_t s) {
       noffsets.release();
       ncodes.release();
       nids.release();
+      ns1.release();
     };
     // keys in arrival order: old CSR entries (already grouped), then the staged ones
     if (ix->n_csr > 0) {
@@ -375,16 +430,17 @@ int ivfpq_finalise(fs_ivfpq* ix, cudaStream_t s) {
       return set_error(FS_ECUDA, "fs_ivfpq finalise: sort launch failed");
     }
     if ((rc = ncodes.ensure((size_t)n * M, 0, s)) != FS_OK ||
-        (rc = nids.ensure((size_t)n * sizeof(int64_t), 0, s)) != FS_OK) {
+        (rc = nids.ensure((size_t)n * sizeof(int64_t), 0, s)) != FS_OK ||
+        (rc = ns1.ensure((size_t)n * sizeof(float), 0, s)) != FS_OK) {
       cleanup();
       return rc;
     }
     csr_offsets_kernel<<<(unsigned)ceil_div(n, 256), 256, 0, s>>>(kin, n, nlist,
                                                                   noffsets.as<int64_t>());
     csr_gather_kernel<<<(unsigned)ceil_div(n, 256), 256, 0, s>>>(
-        vin, n, ix->n_csr, M, ix->codes.as<uint8_t>(), ix->ids.as<int64_t>(),
-        ix->st_codes.as<uint8_t>(), ix->st_ids.as<int64_t>(), ncodes.as<uint8_t>(),
-        nids.as<int64_t>());
+        vin, kin, n, ix->n_csr, M, ix->permuted(), ix->offsets.as<int64_t>(), noffsets.as<int64_t>(),
+        ix->codes.as<uint8_t>(), ix->ids.as<int64_t>(), ix->s1.as<float>(), ix->st_codes.as<uint8_t>(),
+        ix->st_ids.as<int64_t>(), ix->st_s1.as<float>(), ncodes.as<uint8_t>(), nids.as<int64_t>(), ns1.as<float>());
     launch_counter() += 2;
     cudaError_t e = cudaStreamSynchronize(s);
     if (e == cudaSuccess) e = cudaGetLastError();
@@ -393,20 +449,24 @@ int ivfpq_finalise(fs_ivfpq* ix, cudaStream_t s) {
       noffsets.release();
       ncodes.release();
       nids.release();
+      ns1.release();
       return set_error(FS_ECUDA, "fs_ivfpq finalise failed: %s", cudaGetErrorString(e));
     }
   }
   ix->offsets.release();
   ix->codes.release();
   ix->ids.release();
+  ix->s1.release();
   ix->offsets = noffsets;
   ix->codes = ncodes;
   ix->ids = nids;
+  ix->s1 = ns1;
   ix->n_csr = n;
   ix->n_staged = 0;
   ix->st_list.release();
   ix->st_codes.release();
   ix->st_ids.release();
+  ix->st_s1.release();
   ix->offsets_host.resize(nlist + 1);
   FS_CUDA(cudaMemcpyAsync(ix->offsets_host.data(), ix->offsets.p, (size_t)(nlist + 1) * sizeof(int64_t),
                           cudaMemcpyDeviceToHost, s));
@@ -454,7 +514,8 @@ static int ivfpq_add_device(fs_ivfpq* ix, const float* xb, int64_t n, const int6
     return set_error(FS_EUNSUPPORTED, "fs_ivfpq_add: more than 2^32-1 vectors");
   if ((rc = ix->st_list.ensure((size_t)(base + n) * sizeof(uint32_t), (size_t)base * sizeof(uint32_t), s)) != FS_OK ||
       (rc = ix->st_codes.ensure((size_t)(base + n) * M, (size_t)base * M, s)) != FS_OK ||
-      (rc = ix->st_ids.ensure((size_t)(base + n) * sizeof(int64_t), (size_t)base * sizeof(int64_t), s)) != FS_OK)
+      (rc = ix->st_ids.ensure((size_t)(base + n) * sizeof(int64_t), (size_t)base * sizeof(int64_t), s)) != FS_OK ||
+      (rc = ix->st_s1.ensure((size_t)(base + n) * sizeof(float), (size_t)base * sizeof(float), s)) != FS_OK)
     return rc;
   DevBuf assign;
   if ((rc = assign.ensure((size_t)n * sizeof(int64_t), 0, s)) != FS_OK) return rc;
@@ -462,7 +523,7 @@ static int ivfpq_add_device(fs_ivfpq* ix, const float* xb, int64_t n, const int6
                       assign.as<int64_t>(), s);
   if (rc == FS_OK)
     rc = launch_pq_encode(ix, xb, n, assign.as<int64_t>(), ix->st_codes.as<uint8_t>() + base * M,
-                          ix->st_list.as<uint32_t>() + base, s);
+                          ix->st_list.as<uint32_t>() + base, ix->st_s1.as<float>() + base, s);
   if (rc == FS_OK) {
     if (ids) {
       cudaMemcpyAsync(ix->st_ids.as<int64_t>() + base, ids, (size_t)n * sizeof(int64_t),
@@ -524,7 +585,7 @@ int fs_ivfpq_destroy(fs_ivfpq* ix) {
   if (!ix) return FS_OK;
   cudaDeviceSynchronize();
   fs::DevBuf* bufs[] = {&ix->coarse, &ix->cnorm, &ix->pq, &ix->offsets, &ix->codes, &ix->ids,
-                        &ix->st_list, &ix->st_codes, &ix->st_ids, &ix->scanned, &ix->term1};
+                        &ix->st_list, &ix->st_codes, &ix->st_ids, &ix->scanned, &ix->s1, &ix->st_s1};
   for (fs::DevBuf* b : bufs) b->release();
   for (cudaEvent_t e : ix->ev)
     if (e) cudaEventDestroy(e);
@@ -543,7 +604,6 @@ int fs_ivfpq_set_quantizers(fs_ivfpq* ix, const float* coarse, const float* pq, 
   int rc = fs::launch_row_norms(ix->coarse.as<float>(), ix->nlist, ix->d, ix->cnorm.as<float>(), s);
   if (rc != FS_OK) return rc;
   ix->have_quantizers = true;
-  ix->term1_valid = false;
   return FS_OK;
 }
 
@@ -609,8 +669,15 @@ int fs_ivfpq_export(const fs_ivfpq* cix, int64_t* offsets, uint8_t* codes, int64
   if (offsets)
     FS_CUDA(cudaMemcpyAsync(offsets, ix->offsets.p, (size_t)(ix->nlist + 1) * sizeof(int64_t),
                             cudaMemcpyDeviceToDevice, s));
-  if (codes && ix->n_csr > 0)
-    FS_CUDA(cudaMemcpyAsync(codes, ix->codes.p, (size_t)ix->n_csr * ix->M, cudaMemcpyDeviceToDevice, s));
+  if (codes && ix->n_csr > 0) {
+    if (ix->permuted()) {
+      fs::csr_unpermute_kernel<<<(unsigned)ix->nlist, 128, 0, s>>>(ix->codes.as<uint8_t>(), ix->offsets.as<int64_t>(),
+                                                                 nullptr, nullptr, ix->M, codes);
+      FS_LAUNCHED();
+    } else {
+      FS_CUDA(cudaMemcpyAsync(codes, ix->codes.p, (size_t)ix->n_csr * ix->M, cudaMemcpyDeviceToDevice, s));
+    }
+  }
   if (ids && ix->n_csr > 0)
     FS_CUDA(cudaMemcpyAsync(ids, ix->ids.p, (size_t)ix->n_csr * sizeof(int64_t), cudaMemcpyDeviceToDevice, s));
   return FS_OK;
@@ -634,6 +701,22 @@ int fs_ivfpq_export_lists(const fs_ivfpq* cix, const int32_t* list_nos, int64_t 
   }
   offsets_host[n_lists] = total;
   if (!codes && !ids) return FS_OK;
+  if (codes && ix->permuted() && total > 0) {
+    // the lists' codes in plain byte order: one block per list, list numbers and output offsets uploaded
+    int32_t* d_ln = nullptr;
+    int64_t* d_off = nullptr;
+    FS_CUDA(cudaMallocAsync(&d_ln, (size_t)n_lists * sizeof(int32_t), s));
+    FS_CUDA(cudaMallocAsync(&d_off, (size_t)(n_lists + 1) * sizeof(int64_t), s));
+    FS_CUDA(cudaMemcpyAsync(d_ln, list_nos, (size_t)n_lists * sizeof(int32_t), cudaMemcpyHostToDevice, s));
+    FS_CUDA(cudaMemcpyAsync(d_off, offsets_host, (size_t)(n_lists + 1) * sizeof(int64_t), cudaMemcpyHostToDevice, s));
+    fs::csr_unpermute_kernel<<<(unsigned)n_lists, 128, 0, s>>>(ix->codes.as<uint8_t>(), ix->offsets.as<int64_t>(), d_ln,
+                                                              d_off, ix->M, codes);
+    FS_LAUNCHED();
+    FS_CUDA(cudaFreeAsync(d_ln, s));
+    FS_CUDA(cudaFreeAsync(d_off, s));
+    FS_CUDA(cudaStreamSynchronize(s));  // list_nos / offsets_host are the caller's: copied before returning
+    codes = nullptr;
+  }
   // one copy per run of consecutive list numbers (their CSR ranges are adjacent)
   for (int64_t j = 0; j < n_lists;) {
     int64_t e = j + 1;

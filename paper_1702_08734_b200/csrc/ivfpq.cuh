@@ -31,18 +31,14 @@ struct fs_ivfpq {
   fs::DevBuf coarse;  // [nlist][d] fp32
   fs::DevBuf cnorm;   // [nlist] fp32: ||c||^2 (B1 of the coarse search, precomputed)
   fs::DevBuf pq;      // [M][256][dsub] fp32
-  // Eq. 11 term 1, ||B[m][c]||^2 + 2 <c_L^m, B[m][c]> for every list, in the lane
-  // order of the fixed-point table build (ivfpq_search.cu); built lazily by the first search that
-  // uses it, dropped when the quantizers change.
-  fs::DevBuf term1;   // [nlist][M * 256] fp32
-  bool term1_valid = false;
-
   // Finalised inverted file, CSR over list number (codes and
   // ids in separate arrays, each list contiguous, append order kept).
   int64_t n_csr = 0;
   fs::DevBuf offsets;  // int64 [nlist+1]
-  fs::DevBuf codes;    // uint8 [n_csr][M]
+  fs::DevBuf codes;    // uint8 [n_csr][M]; M = 8 / 16: byte i of the vector at position p of its list holds
+                       // sub-quantizer i ^ (p mod M) (the lane order of the conflict-free scan, see permuted())
   fs::DevBuf ids;      // int64 [n_csr]
+  fs::DevBuf s1;       // float [n_csr]: Eq. 11 term 1 of the stored vector, ||q2||^2 + 2 <q1, q2>
   std::vector<int64_t> offsets_host;
 
   // Vectors added since the last finalise, in arrival order.
@@ -50,6 +46,7 @@ struct fs_ivfpq {
   fs::DevBuf st_list;   // uint32 [n_staged]
   fs::DevBuf st_codes;  // uint8 [n_staged][M]
   fs::DevBuf st_ids;    // int64 [n_staged]
+  fs::DevBuf st_s1;     // float [n_staged]
 
   // Code bytes scanned by the last search (device counter, read lazily).
   fs::DevBuf scanned;  // unsigned long long [1]
@@ -58,6 +55,9 @@ struct fs_ivfpq {
   bool ev_valid = false;
 
   int64_t ntotal() const { return n_csr + n_staged; }
+  // CSR codes stored pre-permuted for the fixed-point scan (the per-vector byte permutation is done once,
+  // when the lists are built, instead of once per scanned vector); export undoes it.
+  bool permuted() const { return M == 8 || M == 16; }
 };
 
 namespace fs {
@@ -67,7 +67,7 @@ int ivfpq_finalise(fs_ivfpq* ix, cudaStream_t s);
 
 // D2: residual PQ encoding of n vectors with known coarse assignment.
 int launch_pq_encode(const fs_ivfpq* ix, const float* y, int64_t n, const int64_t* assign,
-                     uint8_t* codes_out, uint32_t* list_out, cudaStream_t s);
+                     uint8_t* codes_out, uint32_t* list_out, float* s1_out, cudaStream_t s);
 
 // Generic Lloyd k-means on device data x [n][d] -> cent [K][d] (ivfpq_train.cu).
 int kmeans_device(const float* x, int64_t n, int d, int K, int niter, uint64_t seed, float* cent,

@@ -147,6 +147,5 @@ extern "C" int fs_ivfpq_train(fs_ivfpq* ix, const float* x, int64_t n, int niter
   sub.release();
   if (rc != FS_OK) return rc;
   ix->have_quantizers = true;
-  ix->term1_valid = false;
   return FS_OK;
 }
