@@ -298,6 +298,26 @@ __device__ __forceinline__ void xor_gather(const uint32_t* w, uint32_t A, uint32
   }
 }
 
+// The same for two vectors at once (independent chains).  As[s] = A ^ 4 s is kept in registers; the
+// address is one IMAD and the sum one IMAD too (FMA pipe), so that the ALU pipe -- the busiest one of
+// this kernel, 67 % in the first version -- only extracts the byte.
+template <int s, int M>
+__device__ __forceinline__ void xor_gather2(const uint32_t* w0, const uint32_t* w1, const uint32_t (&As)[M], uint32_t& acc0,
+                                            uint32_t& acc1) {
+  if constexpr (s < M) {
+    const uint32_t c0 = __byte_perm(w0[s >> 2], 0u, 0x4440u + (s & 3));
+    const uint32_t c1 = __byte_perm(w1[s >> 2], 0u, 0x4440u + (s & 3));
+    uint32_t a0, a1, v0, v1;
+    asm("mad.lo.u32 %0, %1, 128, %2;" : "=r"(a0) : "r"(c0), "r"(As[s]));
+    asm("mad.lo.u32 %0, %1, 128, %2;" : "=r"(a1) : "r"(c1), "r"(As[s]));
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v0) : "r"(a0));
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v1) : "r"(a1));
+    asm("mad.lo.u32 %0, %1, 1, %0;" : "+r"(acc0) : "r"(v0));
+    asm("mad.lo.u32 %0, %1, 1, %0;" : "+r"(acc1) : "r"(v1));
+    xor_gather2<s + 1, M>(w0, w1, As, acc0, acc1);
+  }
+}
+
 // The scan of M = 8 / 16 indexes.  Persistent CTAs of 8 warps draw (query, list group) items from a
 // counter; per item the query's table is copied from Tq into the replicated shared-memory layout (16
 // loads and 16 x REP stores per thread), then the warps stream the group's lists: one 8 / 16-byte code
@@ -306,13 +326,16 @@ __device__ __forceinline__ void xor_gather(const uint32_t* w, uint32_t A, uint32
 #ifndef FS_QS_CTAS
 #define FS_QS_CTAS 4
 #endif
-constexpr int QS_CTAS = FS_QS_CTAS;  // CTAs per SM: 4 x (32 KB + 4.5 KB) of shared memory, 32 warps, 64 registers
+constexpr int QS_CTAS = FS_QS_CTAS;  // CTAs per SM (K <= 128): 4 x 8 warps, 64 registers
 
 template <int NQ>
 constexpr int qs_ctas() { return NQ <= 4 ? QS_CTAS : (NQ <= 8 ? 2 : 1); }  // the register queue grows with K = 32 NQ
+constexpr int QS_MAXG = 128;  // lists per work item (their bounds, term 2 and pass prefix sit in shared memory)
+
 template <int NQ>
-constexpr size_t qs_lut_bytes() {  // table, later the merge area of SCAN_WARPS queues
-  return (size_t)SCAN_WARPS * 32 * NQ * 8 > (size_t)256 * 32 * 4 ? (size_t)SCAN_WARPS * 32 * NQ * 8 : (size_t)256 * 32 * 4;
+constexpr size_t qs_smem_bytes(int d) {
+  return (size_t)256 * 32 * 4 + (size_t)SCAN_WARPS * warp_select_smem_keys<2>() * 8 + (size_t)2 * SCAN_WARPS * 32 * NQ * 8 +
+         (size_t)QS_MAXG * 16 + 0 * (size_t)d;
 }
 
 template <int NQ, int M>
@@ -324,35 +347,52 @@ __global__ void __launch_bounds__(SCAN_THREADS, qs_ctas<NQ>())
   constexpr int NB = 2;
   constexpr int MW = M / 4;
   constexpr int REP = 32 / M;
+  // Shared memory: lut[256][32] | select batches | merge areas [2][SCAN_WARPS][K] (warp 0 merges one item's
+  // queues while the warps park the next item's in the other) | per list: begin, length, term 2, first pass
   uint32_t* lut = reinterpret_cast<uint32_t*>(scan_smem);
-  uint64_t* bufs = reinterpret_cast<uint64_t*>(scan_smem + qs_lut_bytes<NQ>());
-  float* xs = reinterpret_cast<float*>(bufs + SCAN_WARPS * warp_select_smem_keys<NB>());  // the query, d floats
-  uint64_t* merge = reinterpret_cast<uint64_t*>(lut);  // the table is dead when the queues are merged
+  uint64_t* bufs = reinterpret_cast<uint64_t*>(lut + 256 * 32);
+  uint64_t* merge = bufs + SCAN_WARPS * warp_select_smem_keys<NB>();
+  uint32_t* l_begin = reinterpret_cast<uint32_t*>(merge + 2 * SCAN_WARPS * K);  // CSR position of the list's first vector
+  int* l_len = reinterpret_cast<int*>(l_begin + QS_MAXG);
+  float* l_t2 = reinterpret_cast<float*>(l_len + QS_MAXG);
+  int* l_pass = reinterpret_cast<int*>(l_t2 + QS_MAXG);  // passes of 64 vectors before this list
   __shared__ uint32_t cta_bound;
-  __shared__ int cta_item;
+  __shared__ int cta_item, cta_pass, cta_npass;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   WarpSelect<NQ, NB> sel;
   sel.init(bufs + warp * warp_select_smem_keys<NB>(), lane);
   unsigned long long bytes = 0;
   const int my_m = lane % M, cofs = lane / M;
   const uint32_t lane_base = (uint32_t)__cvta_generic_to_shared(lut) + ((uint32_t)lane << 2);  // step s reads bank lane ^ s
+  uint32_t As[M];
+#pragma unroll
+  for (int i = 0; i < M; ++i) As[i] = lane_base ^ (4u * i);
+  const int d = a.d;
+  int64_t prev_item = -1;  // warp 0: the item whose queues wait in the merge area
+  int round = 0;           // items this CTA has scanned: parity picks the merge area
 
   while (true) {
-    __syncthreads();  // the previous item's merge is done with the table / merge area
+    __syncthreads();  // A: every warp has scanned its share of the previous item and parked its queue
     if (tid == 0) {
       cta_item = (int)atomicAdd(work, 1u);
       cta_bound = 0x7F800000u;
+      cta_pass = 0;
     }
     __syncthreads();
     const int64_t item = cta_item;
-    if (item >= n_items) break;
-    const int64_t q = item / a.ngroups;
-    const int g = (int)(item - q * a.ngroups);
-    const int p_begin = g * a.G;
-    const int p_end = (p_begin + a.G) < a.nprobe ? (p_begin + a.G) : a.nprobe;
-    sel.reset();
-    // C2: the query's table into the replicated, bank-aligned layout
-    {
+    const bool live = item < n_items;
+    int nl = 0;
+    int64_t q = 0;
+    int p_begin = 0;
+    QMeta mt = {};
+    if (live) {
+      q = item / a.ngroups;
+      const int g = (int)(item - q * a.ngroups);
+      p_begin = g * a.G;
+      const int p_end = (p_begin + a.G) < a.nprobe ? (p_begin + a.G) : a.nprobe;
+      nl = p_end - p_begin;
+      mt = meta[q];
+      // C2: the query's table into the replicated, bank-aligned layout
       const uint32_t* tq = Tq + q * (256 * M);
 #pragma unroll 4
       for (int i = warp; i < 256 / REP; i += SCAN_WARPS) {
@@ -361,114 +401,126 @@ __global__ void __launch_bounds__(SCAN_THREADS, qs_ctas<NQ>())
 #pragma unroll
         for (int rep = 0; rep < REP; ++rep) lut[c * 32 + my_m + ((rep + cofs) % REP) * M] = v;
       }
+      // the lists of the item: bounds and term 2, ||x - c_L||^2 in the direct form (C1's value went through
+      // the Eq. 2 expansion, whose cancellation error is absolute, ~1e-7 (||x||^2 + ||c||^2), and would be the
+      // largest one in the distance of a close vector); one warp per list, fixed summation order
+      const float* xq = a.xq + q * d;
+      for (int j = warp; j < nl; j += SCAN_WARPS) {
+        const int64_t L = a.probe_ids[q * a.nprobe + p_begin + j];
+        int64_t lb = 0, le = 0;
+        float t2 = 0.f;
+        if (L >= 0) {
+          lb = a.offsets[L];
+          le = a.offsets[L + 1];
+          for (int i = lane; i < d; i += 32) {
+            const float df = xq[i] - a.coarse[L * d + i];
+            t2 = fmaf(df, df, t2);
+          }
+        }
+#pragma unroll
+        for (int sft = 16; sft >= 1; sft >>= 1) t2 += __shfl_xor_sync(kFull, t2, sft);
+        if (lane == 0) {
+          l_begin[j] = (uint32_t)lb;
+          l_len[j] = (int)(le - lb);
+          l_t2[j] = t2;
+          if (a.out_probed) a.out_probed[q * a.nprobe + p_begin + j] = (int32_t)L;
+        }
+      }
     }
-    const QMeta mt = meta[q];
-    for (int j = tid; j < a.d; j += SCAN_THREADS) xs[j] = a.xq[q * a.d + j];
-    __syncthreads();
-    // C3 + C4.  The dependent loads of a list (probe id -> list bounds, centroid) are issued one list
-    // ahead and stay in registers.  Term 2, ||x - c_L||^2, is recomputed here in the direct form (every
-    // warp the same sum in the same order): C1's value went through the Eq. 2 expansion, whose
-    // cancellation error is absolute, ~1e-7 (||x||^2 + ||c||^2), and would be the largest one in the
-    // distance of a close vector.
-    const int64_t* pid = a.probe_ids + q * a.nprobe;
-    constexpr int CPL = 4;  // centroid values per lane (d <= 128)
-    const int d = a.d;
-    int64_t L1 = pid[p_begin];
-    int64_t lb1 = 0, le1 = 0;
-    float c1[CPL];
+    __syncthreads();  // B: table and list records are in place
+    if (warp == 0) {
+      if (live) {  // exclusive prefix of the lists' pass counts (nl <= QS_MAXG = 4 x 32)
+        int run = 0;
+        unsigned long long by = 0;
+        for (int j0 = 0; j0 < nl; j0 += 32) {
+          const int j = j0 + lane;
+          const int n = j < nl ? (l_len[j] + 63) >> 6 : 0;
+          if (j < nl) by += (unsigned long long)l_len[j] * M;
+          int incl = n;
 #pragma unroll
-    for (int i = 0; i < CPL; ++i) c1[i] = 0.f;
-    if (L1 >= 0) {
-      lb1 = a.offsets[L1];
-      le1 = a.offsets[L1 + 1];
+          for (int o = 1; o < 32; o <<= 1) {
+            const int v = __shfl_up_sync(kFull, incl, o);
+            if (lane >= o) incl += v;
+          }
+          if (j < nl) l_pass[j] = run + incl - n;
+          run += __shfl_sync(kFull, incl, 31);
+        }
 #pragma unroll
-      for (int i = 0; i < CPL; ++i)
-        if (i * 32 + lane < d) c1[i] = a.coarse[L1 * d + i * 32 + lane];
+        for (int sft = 16; sft >= 1; sft >>= 1) by += __shfl_xor_sync(kFull, by, sft);
+        if (lane == 0) {
+          cta_npass = run;
+          bytes += by;
+        }
+      }
     }
-    for (int p = p_begin; p < p_end; ++p) {
-      const int64_t L = L1, lb = lb1, le = le1;
-      float t2 = 0.f;
-#pragma unroll
-      for (int i = 0; i < CPL; ++i)
-        if (i * 32 + lane < d) {
-          const float df = xs[i * 32 + lane] - c1[i];
-          t2 = fmaf(df, df, t2);
-        }
-      if (d > CPL * 32 && L >= 0)  // long vectors: the rest of the centroid straight from memory
-        for (int j = CPL * 32 + lane; j < d; j += 32) {
-          const float df = xs[j] - a.coarse[L * d + j];
-          t2 = fmaf(df, df, t2);
-        }
-#pragma unroll
-      for (int sft = 16; sft >= 1; sft >>= 1) t2 += __shfl_xor_sync(kFull, t2, sft);
-      const float bias = t2;  // term 2
-      if (p + 1 < p_end) {
-        L1 = pid[p + 1];
-        if (L1 >= 0) {
-          lb1 = a.offsets[L1];
-          le1 = a.offsets[L1 + 1];
-#pragma unroll
-          for (int i = 0; i < CPL; ++i)
-            if (i * 32 + lane < d) c1[i] = a.coarse[L1 * d + i * 32 + lane];
-        }
+    __syncthreads();  // C: pass prefix
+    if (warp == 0 && prev_item >= 0) {
+      // C4, second half: the previous item's eight queues -> one (the other warps are already scanning)
+      WarpSelect<NQ, NB> ms;
+      ms.init(bufs, lane);  // warp 0's own batch area is idle between its items
+      for (int e0 = 0; e0 < SCAN_WARPS * K; e0 += 32) {
+        const uint64_t key = merge[((round - 1) & 1) * (SCAN_WARPS * K) + e0 + lane];
+        ms.push(key < ms.thr, key);
       }
-      if (a.out_probed && tid == 0) a.out_probed[q * a.nprobe + p] = (int32_t)L;
-      if (L < 0 || le == lb) continue;  // empty lists are probed and contribute nothing
-      const int len = (int)(le - lb);
-      const uint8_t* cl = a.codes + lb * M;
-      const float* sl = a.s1 + lb;
-      if (tid == 0) bytes += (unsigned long long)len * M;
-      const uint32_t pos0 = (uint32_t)lb;
-      uint32_t nxt[MW] = {};
-      float s1n = 0.f;
-      if (warp * 32 + lane < len) {
-        load_code<MW>(cl + (size_t)(warp * 32 + lane) * M, nxt);
-        s1n = __ldcs(sl + warp * 32 + lane);
-      }
-      for (int v0 = warp * 32; v0 < len; v0 += SCAN_THREADS) {  // a warp stops after its last 32 vectors
-        const int v = v0 + lane;
-        const bool ok = v < len;
-        uint32_t w[MW];
+      ms.finish();
+      uint64_t* W = a.Wg + prev_item * K;
 #pragma unroll
-        for (int i = 0; i < MW; ++i) w[i] = nxt[i];
-        const float s1v = s1n;
-        if (v + SCAN_THREADS < len) {
-          load_code<MW>(cl + (size_t)(uint32_t)(v + SCAN_THREADS) * M, nxt);
-          s1n = __ldcs(sl + v + SCAN_THREADS);
-        }
-        float dist = 0.f;
-        if (ok) {
-          uint32_t acc = 0u;
-          xor_gather<0, M>(w, lane_base, acc);
-          // term 3 = (acc - isum) / scale, an exact integer step for integer-valued data
-          dist = fmaf((float)(int32_t)(acc - mt.isum), mt.inv_scale, bias + s1v);
-        }
-        const float bound = fminf(sel.thr_val, __uint_as_float(*reinterpret_cast<volatile uint32_t*>(&cta_bound)));
-        const bool cand = ok && !(dist > bound);
-        if (__any_sync(kFull, cand)) {
-          const uint64_t key = make_key(dist, pos0 + (uint32_t)v);
-          const uint64_t thr_before = sel.thr;
-          sel.push(cand && sel.wants(key), key);
-          if (sel.thr != thr_before && lane == 0) atomicMin(&cta_bound, __float_as_uint(sel.thr_val));
-        }
+      for (int rr = 0; rr < NQ; ++rr) W[rr * 32 + lane] = ms.W[rr];
+      __syncwarp();
+    }
+    if (!live) break;
+    prev_item = item;
+    sel.reset();
+    // C3 + C4.  Warps draw passes of 64 consecutive vectors (two per lane: two independent look-up chains)
+    // from a counter, so that the lists of the item are shared evenly whatever their lengths; the list of
+    // a pass is found by walking the prefix array forward (passes are handed out in increasing order).
+    const int npass = cta_npass;
+    int lj = 0;  // cursor: list of the last pass this warp took
+    int t = 0;
+    if (lane == 0) t = atomicAdd(&cta_pass, 1);
+    t = __shfl_sync(kFull, t, 0);
+    while (t < npass) {
+      while (lj + 1 < nl && l_pass[lj + 1] <= t) ++lj;
+      const int len = l_len[lj];
+      const uint32_t pos0 = l_begin[lj];
+      const float bias = l_t2[lj];
+      const int v = ((t - l_pass[lj]) << 6) + lane;
+      const uint8_t* cv = a.codes + ((size_t)pos0 + (uint32_t)v) * M;
+      uint32_t w0[MW] = {}, w1[MW] = {};
+      float s10 = 0.f, s11 = 0.f;
+      if (v < len) {
+        load_code<MW>(cv, w0);
+        s10 = __ldcs(a.s1 + pos0 + v);
       }
+      if (v + 32 < len) {
+        load_code<MW>(cv + 32 * M, w1);
+        s11 = __ldcs(a.s1 + pos0 + v + 32);
+      }
+      int tn = 0;  // the next pass is drawn while the loads are in flight
+      if (lane == 0) tn = atomicAdd(&cta_pass, 1);
+      tn = __shfl_sync(kFull, tn, 0);
+      uint32_t acc0 = 0u, acc1 = 0u;
+      xor_gather2<0, M>(w0, w1, As, acc0, acc1);
+      // term 3 = (acc - isum) / scale, an exact integer step for integer-valued data
+      const float d0 = fmaf((float)(int32_t)(acc0 - mt.isum), mt.inv_scale, bias + s10);
+      const float d1 = fmaf((float)(int32_t)(acc1 - mt.isum), mt.inv_scale, bias + s11);
+      const float bound = fminf(sel.thr_val, __uint_as_float(*reinterpret_cast<volatile uint32_t*>(&cta_bound)));
+      const bool c0 = v < len && !(d0 > bound), c1 = v + 32 < len && !(d1 > bound);
+      if (__any_sync(kFull, c0 || c1)) {
+        const uint64_t thr_before = sel.thr;
+        const uint64_t k0 = make_key(d0, pos0 + (uint32_t)v);
+        sel.push(c0 && sel.wants(k0), k0);
+        const uint64_t k1 = make_key(d1, pos0 + (uint32_t)v + 32u);
+        sel.push(c1 && sel.wants(k1), k1);
+        if (sel.thr != thr_before && lane == 0) atomicMin(&cta_bound, __float_as_uint(sel.thr_val));
+      }
+      t = tn;
     }
     sel.finish();
-    __syncthreads();  // every warp is done with the table: the merge area takes its place
+    // park the queue; the next round's barrier A orders it before warp 0's merge
 #pragma unroll
-    for (int rr = 0; rr < NQ; ++rr) merge[warp * K + rr * 32 + lane] = sel.W[rr];
-    __syncthreads();
-    if (warp == 0) {
-      sel.reset();
-      for (int e0 = 0; e0 < SCAN_WARPS * K; e0 += 32) {
-        const uint64_t key = merge[e0 + lane];
-        sel.push(key < sel.thr, key);
-      }
-      sel.finish();
-      uint64_t* W = a.Wg + item * K;
-#pragma unroll
-      for (int rr = 0; rr < NQ; ++rr) W[rr * 32 + lane] = sel.W[rr];
-    }
+    for (int rr = 0; rr < NQ; ++rr) merge[(round & 1) * (SCAN_WARPS * K) + warp * K + rr * 32 + lane] = sel.W[rr];
+    ++round;
   }
   if (tid == 0 && bytes) atomicAdd(a.scanned, bytes);
 }
@@ -524,6 +576,7 @@ SearchPlan search_plan(const fs_ivfpq* ix, int64_t nq, int nprobe, int k) {
   if (ng > nprobe) ng = nprobe;
   if (ng < 1) ng = 1;
   p.G = (int)ceil_div(nprobe, ng);
+  if (p.qscan && p.G > QS_MAXG) p.G = QS_MAXG;
   p.ngroups = (int)ceil_div(nprobe, p.G);
   p.coarse = flat_plan(nq, ix->nlist, ix->d, nprobe);
   size_t o = align_up(p.coarse.bytes, 256);
@@ -596,8 +649,7 @@ int launch_scan_pair(const ScanArgs& a, int64_t nq, cudaStream_t s) {
 template <int NQ, int M>
 int launch_scan_q(const ScanArgs& a, int64_t nq, const uint32_t* Tq, const QMeta* meta, unsigned int* work,
                   cudaStream_t s) {
-  const size_t smem = qs_lut_bytes<NQ>() + (size_t)SCAN_WARPS * warp_select_smem_keys<2>() * sizeof(uint64_t) +
-                      (size_t)((a.d + 3) & ~3) * sizeof(float);
+  const size_t smem = qs_smem_bytes<NQ>(a.d);
   FS_CUDA(cudaFuncSetAttribute(ivfpq_scan_q_kernel<NQ, M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   FS_CUDA(cudaFuncSetAttribute(ivfpq_scan_q_kernel<NQ, M>, cudaFuncAttributePreferredSharedMemoryCarveout,
                                cudaSharedmemCarveoutMaxShared));
