@@ -298,23 +298,23 @@ __device__ __forceinline__ void xor_gather(const uint32_t* w, uint32_t A, uint32
   }
 }
 
-// The same for two vectors at once (independent chains).  As[s] = A ^ 4 s is kept in registers; the
+// The same for VPL vectors at once (independent chains).  As[s] = A ^ 4 s is kept in registers; the
 // address is one IMAD and the sum one IMAD too (FMA pipe), so that the ALU pipe -- the busiest one of
 // this kernel, 67 % in the first version -- only extracts the byte.
-template <int s, int M>
-__device__ __forceinline__ void xor_gather2(const uint32_t* w0, const uint32_t* w1, const uint32_t (&As)[M], uint32_t& acc0,
-                                            uint32_t& acc1) {
+template <int s, int M, int VPL>
+__device__ __forceinline__ void xor_gather_n(const uint32_t (&w)[VPL][M / 4], const uint32_t (&As)[M], uint32_t (&acc)[VPL]) {
   if constexpr (s < M) {
-    const uint32_t c0 = __byte_perm(w0[s >> 2], 0u, 0x4440u + (s & 3));
-    const uint32_t c1 = __byte_perm(w1[s >> 2], 0u, 0x4440u + (s & 3));
-    uint32_t a0, a1, v0, v1;
-    asm("mad.lo.u32 %0, %1, 128, %2;" : "=r"(a0) : "r"(c0), "r"(As[s]));
-    asm("mad.lo.u32 %0, %1, 128, %2;" : "=r"(a1) : "r"(c1), "r"(As[s]));
-    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v0) : "r"(a0));
-    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v1) : "r"(a1));
-    asm("mad.lo.u32 %0, %1, 1, %0;" : "+r"(acc0) : "r"(v0));
-    asm("mad.lo.u32 %0, %1, 1, %0;" : "+r"(acc1) : "r"(v1));
-    xor_gather2<s + 1, M>(w0, w1, As, acc0, acc1);
+    uint32_t ad[VPL], v[VPL];
+#pragma unroll
+    for (int u = 0; u < VPL; ++u) {
+      const uint32_t c = __byte_perm(w[u][s >> 2], 0u, 0x4440u + (s & 3));  // byte s, zero-extended
+      asm("mad.lo.u32 %0, %1, 128, %2;" : "=r"(ad[u]) : "r"(c), "r"(As[s]));
+    }
+#pragma unroll
+    for (int u = 0; u < VPL; ++u) asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v[u]) : "r"(ad[u]));
+#pragma unroll
+    for (int u = 0; u < VPL; ++u) asm("mad.lo.u32 %0, %1, 1, %0;" : "+r"(acc[u]) : "r"(v[u]));
+    xor_gather_n<s + 1, M, VPL>(w, As, acc);
   }
 }
 
@@ -347,6 +347,8 @@ __global__ void __launch_bounds__(SCAN_THREADS, qs_ctas<NQ>())
   constexpr int NB = 2;
   constexpr int MW = M / 4;
   constexpr int REP = 32 / M;
+  constexpr int VPL = M == 8 ? 4 : 2;  // vectors per lane and pass
+  constexpr int PV = 32 * VPL;         // vectors per pass
   // Shared memory: lut[256][32] | select batches | merge areas [2][SCAN_WARPS][K] (warp 0 merges one item's
   // queues while the warps park the next item's in the other) | per list: begin, length, term 2, first pass
   uint32_t* lut = reinterpret_cast<uint32_t*>(scan_smem);
@@ -355,8 +357,9 @@ __global__ void __launch_bounds__(SCAN_THREADS, qs_ctas<NQ>())
   uint32_t* l_begin = reinterpret_cast<uint32_t*>(merge + 2 * SCAN_WARPS * K);  // CSR position of the list's first vector
   int* l_len = reinterpret_cast<int*>(l_begin + QS_MAXG);
   float* l_t2 = reinterpret_cast<float*>(l_len + QS_MAXG);
-  int* l_pass = reinterpret_cast<int*>(l_t2 + QS_MAXG);  // passes of 64 vectors before this list
+  int* l_pass = reinterpret_cast<int*>(l_t2 + QS_MAXG);  // passes (of PV vectors) before this list
   __shared__ uint32_t cta_bound;
+  __shared__ float cta_sub[SCAN_WARPS];  // each warp's ceil(k / 8)-th smallest distance
   __shared__ int cta_item, cta_pass, cta_npass;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   WarpSelect<NQ, NB> sel;
@@ -378,6 +381,7 @@ __global__ void __launch_bounds__(SCAN_THREADS, qs_ctas<NQ>())
       cta_bound = 0x7F800000u;
       cta_pass = 0;
     }
+    if (tid < SCAN_WARPS) cta_sub[tid] = __uint_as_float(0x7F800000u);
     __syncthreads();
     const int64_t item = cta_item;
     const bool live = item < n_items;
@@ -434,7 +438,7 @@ __global__ void __launch_bounds__(SCAN_THREADS, qs_ctas<NQ>())
         unsigned long long by = 0;
         for (int j0 = 0; j0 < nl; j0 += 32) {
           const int j = j0 + lane;
-          const int n = j < nl ? (l_len[j] + 63) >> 6 : 0;
+          const int n = j < nl ? (l_len[j] + PV - 1) / PV : 0;
           if (j < nl) by += (unsigned long long)l_len[j] * M;
           int incl = n;
 #pragma unroll
@@ -471,48 +475,86 @@ __global__ void __launch_bounds__(SCAN_THREADS, qs_ctas<NQ>())
     if (!live) break;
     prev_item = item;
     sel.reset();
-    // C3 + C4.  Warps draw passes of 64 consecutive vectors (two per lane: two independent look-up chains)
-    // from a counter, so that the lists of the item are shared evenly whatever their lengths; the list of
-    // a pass is found by walking the prefix array forward (passes are handed out in increasing order).
+    sel.set_k(a.k, SCAN_WARPS);
+    // C3 + C4.  Warps draw passes of PV = 32 VPL consecutive vectors (VPL per lane: independent look-up
+    // chains, and the loop, cursor and selection overhead is paid once for all of them) from a counter, so
+    // that the lists of the item are shared evenly whatever their lengths; the list of a pass is found by
+    // walking the prefix array forward (passes are handed out in increasing order).
     const int npass = cta_npass;
-    int lj = 0;  // cursor: list of the last pass this warp took
-    int t = 0;
-    if (lane == 0) t = atomicAdd(&cta_pass, 1);
-    t = __shfl_sync(kFull, t, 0);
+    const uint32_t pass_sa = (uint32_t)__cvta_generic_to_shared(&cta_pass);
+    auto draw = [&]() {
+      int t = 0;  // lane 0 draws (predicated, no branch)
+      asm volatile("{\n\t.reg .pred p;\n\tsetp.eq.u32 p, %2, 0;\n\t@p atom.shared.add.u32 %0, [%1], 1;\n\t}"
+                   : "+r"(t)
+                   : "r"(pass_sa), "r"(lane)
+                   : "memory");
+      return __shfl_sync(kFull, t, 0);
+    };
+    int lj = 0;                                      // cursor: list of the last pass this warp took
+    int nxt_start = nl > 1 ? l_pass[1] : 0x7fffffff;  // first pass of the list after it
+    int t = draw();
     while (t < npass) {
-      while (lj + 1 < nl && l_pass[lj + 1] <= t) ++lj;
+      while (t >= nxt_start) {
+        ++lj;
+        nxt_start = lj + 1 < nl ? l_pass[lj + 1] : 0x7fffffff;
+      }
       const int len = l_len[lj];
       const uint32_t pos0 = l_begin[lj];
       const float bias = l_t2[lj];
-      const int v = ((t - l_pass[lj]) << 6) + lane;
+      const int v = (t - l_pass[lj]) * PV + lane;
       const uint8_t* cv = a.codes + ((size_t)pos0 + (uint32_t)v) * M;
-      uint32_t w0[MW] = {}, w1[MW] = {};
-      float s10 = 0.f, s11 = 0.f;
-      if (v < len) {
-        load_code<MW>(cv, w0);
-        s10 = __ldcs(a.s1 + pos0 + v);
+      const float* sv = a.s1 + pos0 + v;
+      uint32_t w[VPL][MW];
+      float s1v[VPL];
+      if (v + PV - 32 < len) {  // full pass
+#pragma unroll
+        for (int u = 0; u < VPL; ++u) {
+          load_code<MW>(cv + u * 32 * M, w[u]);
+          s1v[u] = __ldcs(sv + u * 32);
+        }
+      } else {
+#pragma unroll
+        for (int u = 0; u < VPL; ++u) {
+#pragma unroll
+          for (int i = 0; i < MW; ++i) w[u][i] = 0u;
+          s1v[u] = 0.f;
+          if (v + u * 32 < len) {
+            load_code<MW>(cv + u * 32 * M, w[u]);
+            s1v[u] = __ldcs(sv + u * 32);
+          }
+        }
       }
-      if (v + 32 < len) {
-        load_code<MW>(cv + 32 * M, w1);
-        s11 = __ldcs(a.s1 + pos0 + v + 32);
-      }
-      int tn = 0;  // the next pass is drawn while the loads are in flight
-      if (lane == 0) tn = atomicAdd(&cta_pass, 1);
-      tn = __shfl_sync(kFull, tn, 0);
-      uint32_t acc0 = 0u, acc1 = 0u;
-      xor_gather2<0, M>(w0, w1, As, acc0, acc1);
-      // term 3 = (acc - isum) / scale, an exact integer step for integer-valued data
-      const float d0 = fmaf((float)(int32_t)(acc0 - mt.isum), mt.inv_scale, bias + s10);
-      const float d1 = fmaf((float)(int32_t)(acc1 - mt.isum), mt.inv_scale, bias + s11);
+      const int tn = draw();  // the next pass is drawn while the loads are in flight
+      uint32_t acc[VPL];
+#pragma unroll
+      for (int u = 0; u < VPL; ++u) acc[u] = 0u;
+      xor_gather_n<0, M, VPL>(w, As, acc);
       const float bound = fminf(sel.thr_val, __uint_as_float(*reinterpret_cast<volatile uint32_t*>(&cta_bound)));
-      const bool c0 = v < len && !(d0 > bound), c1 = v + 32 < len && !(d1 > bound);
-      if (__any_sync(kFull, c0 || c1)) {
+      float dist[VPL];
+      bool any = false;
+#pragma unroll
+      for (int u = 0; u < VPL; ++u) {
+        // term 3 = (acc - isum) / scale, an exact integer step for integer-valued data
+        dist[u] = fmaf((float)(int32_t)(acc[u] - mt.isum), mt.inv_scale, bias + s1v[u]);
+        if (!(v + u * 32 < len)) dist[u] = __uint_as_float(0x7F800000u);  // past the end: never a candidate
+        any |= !(dist[u] > bound) && v + u * 32 < len;
+      }
+      if (__any_sync(kFull, any)) {
         const uint64_t thr_before = sel.thr;
-        const uint64_t k0 = make_key(d0, pos0 + (uint32_t)v);
-        sel.push(c0 && sel.wants(k0), k0);
-        const uint64_t k1 = make_key(d1, pos0 + (uint32_t)v + 32u);
-        sel.push(c1 && sel.wants(k1), k1);
-        if (sel.thr != thr_before && lane == 0) atomicMin(&cta_bound, __float_as_uint(sel.thr_val));
+#pragma unroll
+        for (int u = 0; u < VPL; ++u) {
+          const uint64_t key = make_key(dist[u], pos0 + (uint32_t)(v + u * 32));
+          sel.push(v + u * 32 < len && !(dist[u] > bound) && sel.wants(key), key);
+        }
+        if (sel.thr != thr_before && lane == 0) {
+          // two bounds of the item's k-th distance: this warp's own k-th, and the largest of the eight
+          // warps' ceil(k / 8)-th distances (their queues cover disjoint passes of the same stream)
+          cta_sub[warp] = sel.sub_val;
+          float mx = sel.sub_val;
+#pragma unroll
+          for (int w8 = 0; w8 < SCAN_WARPS; ++w8) mx = fmaxf(mx, *reinterpret_cast<volatile float*>(&cta_sub[w8]));
+          atomicMin(&cta_bound, __float_as_uint(fminf(mx, sel.thr_val)));
+        }
       }
       t = tn;
     }

@@ -193,22 +193,35 @@ struct WarpSelect {
   static constexpr int C = 32 * NB;
 
   uint64_t W[NQ];    // lane-stride, ascending; kSentinelKey marks empty slots
-  uint64_t thr;      // W[K-1], broadcast: a key must be < thr to matter
+  uint64_t thr;      // W[kq] (default the tail W[K-1]), broadcast: a key must be < thr to matter
   float thr_val;     // float image of thr for the one-instruction pre-filter
+  float sub_val;     // float image of W[ks] (set_k): lets several warps that share a stream bound each other
   uint64_t* buf;     // this warp's shared-memory batch
   int cnt;           // keys in the batch (warp-uniform)
   int lane;
+  int kq, ks;        // sorted positions (0-based) whose keys are published as thr / sub_val
 
   __device__ __forceinline__ void init(uint64_t* smem_buf, int lane_) {
     buf = smem_buf;
     lane = lane_;
+    kq = K - 1;
+    ks = K - 1;
     reset();
+  }
+  // Select exactly k <= K: the bound becomes the k-th smallest key instead of the K-th (fewer
+  // candidates pass), and sub_val follows the ceil(k / parts)-th smallest: if each of `parts` queues
+  // over disjoint parts of a stream holds that many keys <= x, their union holds k keys <= x, so
+  // max over the queues of sub_val bounds the union's k-th smallest.
+  __device__ __forceinline__ void set_k(int k, int parts) {
+    kq = k - 1;
+    ks = (k + parts - 1) / parts - 1;
   }
   __device__ __forceinline__ void reset() {
 #pragma unroll
     for (int r = 0; r < NQ; ++r) W[r] = kSentinelKey;
     thr = kSentinelKey;
     thr_val = __uint_as_float(0x7FFFFFFFu);  // NaN: "!(v > thr_val)" passes everything
+    sub_val = __uint_as_float(0x7F800000u);
     cnt = 0;
   }
   // Cheap necessary condition for "key(v, idx) < thr" (exact test: wants()).
@@ -225,6 +238,11 @@ struct WarpSelect {
   }
   __device__ __forceinline__ void flush() {
     thr = warp_flush<NQ, NB>(W, 1, buf, cnt);
+    if (kq != K - 1) {  // (W went through memory for the call: the indexed reads are plain loads)
+      thr = __shfl_sync(kFull, W[kq >> 5], kq & 31);
+      const uint64_t sk = __shfl_sync(kFull, W[ks >> 5], ks & 31);
+      sub_val = sk == kSentinelKey ? __uint_as_float(0x7F800000u) : key_val(sk);
+    }
     thr_val = key_val(thr);
     cnt = 0;
   }
