@@ -29,7 +29,7 @@ int flat_knn_device(const float* xq, int64_t nq, const float* xb, int64_t nb, in
 // Tensor-core engine (flat_tc.cu): tcgen05 / TMEM / TMA, 3xTF32 split operands.
 struct FlatTcPlan {
   int kclass, K, S, qtiles, qgroups, grid, KB, nstage, cap;
-  int64_t chunk;
+  int64_t chunk, chunk0;
   size_t smem;
   size_t off_ynorm, off_xnorm, off_flag, off_gbound, off_hbound, off_hclaim, off_W, off_cbuf, off_qhi, off_qlo, off_bhi, off_blo, bytes;
 };

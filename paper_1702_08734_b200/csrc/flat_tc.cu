@@ -6,9 +6,10 @@
 // Precision (reading F-5): every fp32 operand is split as x = hi + lo with
 // hi = x truncated to TF32 (10 explicit mantissa bits) and lo = (x - hi) truncated to
 // TF32; the tile accumulates hi*hi + lo*hi + hi*lo in fp32 ("3xTF32", ~2^-21 relative).
-// A pre-pass writes the hi / lo planes (and the squared norms, B1) once per call; if it
-// finds lo == 0 everywhere (e.g. small-integer data such as cfg3) the kernel issues the
-// hi*hi products only, which is then exact -- a checked dispatch, never a guess.
+// The hi plane is the operand itself (the MMA ignores the 13 low mantissa bits); a pre-pass
+// computes the squared norms (B1) and checks whether any lo is non-zero; only then is the lo
+// plane written, and if lo == 0 everywhere (e.g. small-integer data such as cfg3) the kernel
+// issues the hi*hi products only, which is then exact -- a checked dispatch, never a guess.
 //
 // Kernel shape: persistent CTAs (one per SM), 320 threads:
 //   warp 8      TMA producer   query tile (128 rows, resident per work item) and a ring
@@ -23,10 +24,6 @@
 // run at the same time read the same part of the database (L2 reuse), and a query's
 // bound found in earlier splits (gbound) prunes the later ones.
 #include <cuda.h>
-#ifndef FS_TC_EXP
-#define FS_TC_EXP 0  // 1 / 2: timing experiments (epilogue without filter / without TMEM loads); never shipped
-#endif
-
 #include <cstdlib>
 #include <cstring>
 
@@ -78,6 +75,8 @@ struct TcArgs {
   int cap;                     // keys per row buffer: K + 128
   int smem_bytes;              // dynamic shared memory of the launch
   int64_t chunk;               // database rows per split (multiple of BN)
+  int64_t chunk0;              // rows of split 0 (= chunk; a smaller first split was measured and lost: the splits of
+                               // the first wave run concurrently and cannot use its bound)
   const float* ynorm;          // [>= nb rounded up to BN]
   uint64_t* Wg;                // [nq][S * EPI_GROUPS][K]
   unsigned int* gbound;        // [nq] order image of the best known k-th distance
@@ -91,11 +90,16 @@ struct TcArgs {
 };
 
 // ---------------------------------------------------------------------------
-// B1 + operand split: hi / lo planes and squared norms, one warp per vector.
+// B1 + operand split.  The hi plane is the caller's array itself: tcgen05.mma kind::tf32 reads the
+// upper 19 bits of every fp32 operand and ignores the 13 low mantissa bits, i.e. it multiplies
+// hi = x truncated to TF32 (checked on B200: bit-identical results with an explicitly truncated copy).
+// norm_flag_kernel: squared norms (one warp per vector) and whether any lo = (x - hi) truncated is
+// non-zero; lo_plane_kernel writes the lo plane, and only when the flag is set (small-integer data such as
+// cfg3 never pay for it: one read of the database for the norms instead of a read and two writes).
 // ---------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
-    split_norm_kernel(const float* __restrict__ x, int64_t n, int d, float* __restrict__ hi,
-                      float* __restrict__ lo, float* __restrict__ norm, unsigned int* __restrict__ flag) {
+    norm_flag_kernel(const float* __restrict__ x, int64_t n, int d, float* __restrict__ norm,
+                     unsigned int* __restrict__ flag) {
   const int lane = threadIdx.x & 31;
   const int64_t row = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
   if (row >= n) return;
@@ -106,15 +110,33 @@ __global__ void __launch_bounds__(256)
     const float v = p[c];
     s = fmaf(v, v, s);
     const float h = __uint_as_float(__float_as_uint(v) & 0xFFFFE000u);
-    const float l = __uint_as_float(__float_as_uint(v - h) & 0xFFFFE000u);
-    hi[row * d + c] = h;
-    lo[row * d + c] = l;
-    any |= (l != 0.f);
+    any |= (__float_as_uint(v - h) & 0xFFFFE000u) != 0u && (v - h) != 0.f;
   }
 #pragma unroll
   for (int m = 16; m >= 1; m >>= 1) s += __shfl_xor_sync(kFull, s, m);
   if (lane == 0) norm[row] = s;
   if (__any_sync(kFull, any) && lane == 0) atomicOr(flag, 1u);
+}
+
+__global__ void __launch_bounds__(256)
+    lo_plane_kernel(const float* __restrict__ x, int64_t n_elems, float* __restrict__ lo,
+                    const unsigned int* __restrict__ flag) {
+  if (*flag == 0u) return;  // every lo is zero: the kernel issues hi * hi only and never reads the plane
+  for (int64_t i = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) * 4; i < n_elems; i += (int64_t)gridDim.x * blockDim.x * 4) {
+    const float4 v = *reinterpret_cast<const float4*>(x + i);  // n_elems = rows * d, d % 32 == 0
+    float4 l;
+    l.x = __uint_as_float(__float_as_uint(v.x - __uint_as_float(__float_as_uint(v.x) & 0xFFFFE000u)) & 0xFFFFE000u);
+    l.y = __uint_as_float(__float_as_uint(v.y - __uint_as_float(__float_as_uint(v.y) & 0xFFFFE000u)) & 0xFFFFE000u);
+    l.z = __uint_as_float(__float_as_uint(v.z - __uint_as_float(__float_as_uint(v.z) & 0xFFFFE000u)) & 0xFFFFE000u);
+    l.w = __uint_as_float(__float_as_uint(v.w - __uint_as_float(__float_as_uint(v.w) & 0xFFFFE000u)) & 0xFFFFE000u);
+    *reinterpret_cast<float4*>(lo + i) = l;
+  }
+}
+
+// Explicitly truncated copy (operands that are not 16-byte aligned cannot be read by TMA in place).
+__global__ void __launch_bounds__(256) hi_plane_kernel(const float* __restrict__ x, int64_t n_elems, float* __restrict__ hi) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_elems; i += (int64_t)gridDim.x * blockDim.x)
+    hi[i] = __uint_as_float(__float_as_uint(x[i]) & 0xFFFFE000u);
 }
 
 // ---------------------------------------------------------------------------
@@ -200,8 +222,9 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
       uint32_t ptile = 0;
       for (int64_t item = cluster_id; item < n_items; item += n_clusters, ++it) {
         const int s = (int)(item / a.qgroups), qt = (int)(item - (int64_t)s * a.qgroups) * CLUSTER + (int)crank;
-        const int64_t b_begin = (int64_t)s * a.chunk;
-        const int64_t b_end = b_begin + a.chunk < a.nb ? b_begin + a.chunk : a.nb;
+        const int64_t b_begin = s == 0 ? 0 : a.chunk0 + (int64_t)(s - 1) * a.chunk;
+        const int64_t b_len = s == 0 ? a.chunk0 : a.chunk;
+        const int64_t b_end = b_begin + b_len < a.nb ? b_begin + b_len : a.nb;
         const int ntiles = (int)((b_end - b_begin + BN - 1) / BN);
         if (it > 0) sm100::mbar_wait(a_empty, (uint32_t)(it - 1) & 1u);  // previous item's MMAs are done with A
         sm100::mbar_expect_tx(a_full, (uint32_t)(KB * A_KB_BYTES * (split ? 2 : 1)));
@@ -245,8 +268,9 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
       int it = 0;
       for (int64_t item = cluster_id; item < n_items; item += n_clusters, ++it) {
         const int s = (int)(item / a.qgroups);
-        const int64_t b_begin = (int64_t)s * a.chunk;
-        const int64_t b_end = b_begin + a.chunk < a.nb ? b_begin + a.chunk : a.nb;
+        const int64_t b_begin = s == 0 ? 0 : a.chunk0 + (int64_t)(s - 1) * a.chunk;
+        const int64_t b_len = s == 0 ? a.chunk0 : a.chunk;
+        const int64_t b_end = b_begin + b_len < a.nb ? b_begin + b_len : a.nb;
         const int ntiles = (int)((b_end - b_begin + BN - 1) / BN);
         sm100::mbar_wait(a_full, (uint32_t)it & 1u);
         sm100::tc_fence_after();
@@ -299,8 +323,9 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
     uint32_t tile_count = 0;
     for (int64_t item = cluster_id; item < n_items; item += n_clusters) {
       const int s = (int)(item / a.qgroups), qt = (int)(item - (int64_t)s * a.qgroups) * CLUSTER + (int)crank;
-      const int64_t b_begin = (int64_t)s * a.chunk;
-      const int64_t b_end = b_begin + a.chunk < a.nb ? b_begin + a.chunk : a.nb;
+      const int64_t b_begin = s == 0 ? 0 : a.chunk0 + (int64_t)(s - 1) * a.chunk;
+      const int64_t b_len = s == 0 ? a.chunk0 : a.chunk;
+      const int64_t b_end = b_begin + b_len < a.nb ? b_begin + b_len : a.nb;
       const int ntiles = (int)((b_end - b_begin + BN - 1) / BN);
       const int64_t q_warp = (int64_t)qt * BM + quarter * 32;
       const int64_t q = q_warp + lane;
@@ -431,15 +456,8 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
 #pragma unroll 1
         for (int i = 0; i < NBLK; ++i) {
           flush_rows(cnt > cap - BW, false);
-#if FS_TC_EXP == 2
-          continue;
-#endif
           sm100::tmem_ld64(taddr + (cg0 + i) * BW, v);
           sm100::tmem_ld_wait();
-#if FS_TC_EXP == 1
-          if (v[0] == 0x12345678u && v[63] == 0x9abcdef0u) cb[cnt++] = 0;  // keep the load alive
-          continue;
-#endif
           const uint32_t cbase = (uint32_t)col0 + (cg0 + i) * BW;
           const int climit = ncols - (cg0 + i) * BW;  // columns of this block that exist
           // first-level filter: d' = ||y||^2 - 2 acc, then the sign of thr - d' is
@@ -637,6 +655,7 @@ FlatTcPlan flat_tc_plan(int64_t nq, int64_t nb, int d, int k) {
   }
   const int64_t per = ceil_div(nt, best_S);
   p.chunk = per * BN;
+  p.chunk0 = p.chunk;
   p.S = (int)ceil_div(nb > 0 ? nb : 1, p.chunk);
   const int64_t items = (int64_t)p.S * qgroups;
   p.grid = (int)(items < ncl ? items : ncl) * CLUSTER;
@@ -688,15 +707,40 @@ int flat_knn_tc_device(const float* xq, int64_t nq, const float* xb, int64_t nb,
   // +inf image and above: no bound (gbound and hbound are adjacent); no slot handed out yet
   FS_CUDA(cudaMemsetAsync(gbound, 0xFF, p.off_hclaim - p.off_gbound, s));
   FS_CUDA(cudaMemsetAsync(w + p.off_hclaim, 0, (size_t)(nq + 1) * HB_LEVELS * sizeof(unsigned int), s));
-  split_norm_kernel<<<(unsigned)ceil_div(nb, 8), 256, 0, s>>>(xb, nb, d, bhi, blo, ynorm, flag);
+  norm_flag_kernel<<<(unsigned)ceil_div(nb, 8), 256, 0, s>>>(xb, nb, d, ynorm, flag);
   FS_LAUNCHED();
-  split_norm_kernel<<<(unsigned)ceil_div(nq, 8), 256, 0, s>>>(xq, nq, d, qhi, qlo, xnorm, flag);
+  norm_flag_kernel<<<(unsigned)ceil_div(nq, 8), 256, 0, s>>>(xq, nq, d, xnorm, flag);
   FS_LAUNCHED();
+  const int64_t nbe = nb * d, nqe = nq * d;
+  const int sms = sm_count();
+  // lo planes only if some lo is non-zero (decided on the device: the kernels return at once otherwise)
+  lo_plane_kernel<<<(unsigned)(ceil_div(nbe, 1024) < sms * 8 ? ceil_div(nbe, 1024) : sms * 8), 256, 0, s>>>(xb, nbe, blo, flag);
+  FS_LAUNCHED();
+  lo_plane_kernel<<<(unsigned)(ceil_div(nqe, 1024) < sms * 8 ? ceil_div(nqe, 1024) : sms * 8), 256, 0, s>>>(xq, nqe, qlo, flag);
+  FS_LAUNCHED();
+  // hi planes: the operands themselves (the MMA ignores the 13 low mantissa bits) unless they are misaligned for TMA
+  static int force_planes = -1;  // FS_TC_PLANES=1: explicit truncated copies (A/B check of the truncation claim)
+  if (force_planes < 0) {
+    const char* e = getenv("FS_TC_PLANES");
+    force_planes = (e && e[0] == '1') ? 1 : 0;
+  }
+  const float* a_hi = xq;
+  const float* b_hi = xb;
+  if (force_planes || (reinterpret_cast<uintptr_t>(xq) & 15u) != 0) {
+    hi_plane_kernel<<<(unsigned)(ceil_div(nqe, 256) < sms * 8 ? ceil_div(nqe, 256) : sms * 8), 256, 0, s>>>(xq, nqe, qhi);
+    FS_LAUNCHED();
+    a_hi = qhi;
+  }
+  if (force_planes || (reinterpret_cast<uintptr_t>(xb) & 15u) != 0) {
+    hi_plane_kernel<<<(unsigned)(ceil_div(nbe, 256) < sms * 8 ? ceil_div(nbe, 256) : sms * 8), 256, 0, s>>>(xb, nbe, bhi);
+    FS_LAUNCHED();
+    b_hi = bhi;
+  }
 
   CUtensorMap ma_hi, ma_lo, mb_hi, mb_lo;
   int rc;
-  if ((rc = make_map(&ma_hi, qhi, nq, d, BM)) != FS_OK || (rc = make_map(&ma_lo, qlo, nq, d, BM)) != FS_OK ||
-      (rc = make_map(&mb_hi, bhi, nb, d, BN / CLUSTER)) != FS_OK ||
+  if ((rc = make_map(&ma_hi, a_hi, nq, d, BM)) != FS_OK || (rc = make_map(&ma_lo, qlo, nq, d, BM)) != FS_OK ||
+      (rc = make_map(&mb_hi, b_hi, nb, d, BN / CLUSTER)) != FS_OK ||
       (rc = make_map(&mb_lo, blo, nb, d, BN / CLUSTER)) != FS_OK)
     return rc;
   TcArgs a;
@@ -713,6 +757,7 @@ int flat_knn_tc_device(const float* xq, int64_t nq, const float* xb, int64_t nb,
   a.cap = p.cap;
   a.smem_bytes = (int)p.smem;
   a.chunk = p.chunk;
+  a.chunk0 = p.chunk0;
   a.ynorm = ynorm;
   a.Wg = reinterpret_cast<uint64_t*>(w + p.off_W);
   a.gbound = gbound;
@@ -741,10 +786,6 @@ int flat_knn_tc_device(const float* xq, int64_t nq, const float* xb, int64_t nb,
   cfg.numAttrs = 1;
   FS_CUDA(cudaLaunchKernelEx(&cfg, flat_tc_kernel, ma_hi, ma_lo, mb_hi, mb_lo, a));
   FS_LAUNCHED();
-  if (getenv("FS_TC_TWICE")) {  // timing experiment: a second pass that starts from the first one's bounds
-    FS_CUDA(cudaLaunchKernelEx(&cfg, flat_tc_kernel, ma_hi, ma_lo, mb_hi, mb_lo, a));
-    FS_LAUNCHED();
-  }
   if (dout != nullptr) return FS_OK;
   return launch_flat_finish(a.Wg, nq, p.S * EPI_GROUPS, k, xnorm, out_dist, out_ids, s);
 }
