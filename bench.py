@@ -363,6 +363,69 @@ def also_ivfpq(fs, gt, pk, cfg, nb=None, cpu=True):
     return out
 
 
+def run_shard(args):
+    """--mode shard: the database of cfg3 cut into N contiguous id shards, one per rank; every
+    rank answers all 10^4 queries over its shard, one all-gather of the [nq][k] lists, then fs_merge_topk.
+    Strong scaling (total work fixed): value = queries/s of the whole job, time = max over ranks."""
+    import torch
+    import torch.distributed as dist
+
+    import paper_1702_08734_b200 as fs
+    from paper_1702_08734_b200 import multirank as mr
+    from datagen import gen_torch as gt
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    fs.lib()
+    nb, nq, d, k = 1_000_000, 10_000, 128, 10
+    first, n = mr.shard_range(rank, world, nb)
+    xb = gt.sift_like(first, n)
+    xq = gt.sift_like(nb, nq)
+    ws = torch.empty(fs.flat_l2_knn_ws_bytes(nq, n, d, k), dtype=torch.uint8, device="cuda")
+    od = torch.empty((nq, k), dtype=torch.float32, device="cuda")
+    oi = torch.empty((nq, k), dtype=torch.int64, device="cuda")
+
+    def step():
+        return mr.sharded_search(lambda: fs.flat_l2_knn(xq, xb, k, out_dist=od, out_ids=oi, ws=ws), fs.merge_topk, first)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    sampler = ClockSampler(local)
+    barrier()
+    fs.reset_launch_count()
+    sampler.start()
+    t0, t1 = event_pair()
+    t0.record()
+    for _ in range(args.steps):
+        step()
+    t1.record()
+    barrier()
+    sampler.stop()
+    ms = mr.max_over_ranks(t0.elapsed_time(t1), "cuda") / args.steps
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": nq / ms * 1e3, "unit": "queries/s", "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "scaling": "strong",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic (seeded, datagen/)", "mode": "shard",
+            "config": {"workload": "cfg3 flat L2 k-NN, nb=1e6 cut into %d id shards, nq=1e4, d=128, k=%d: local "
+                                   "search + one all-gather of nq*k (dist, id) + fs_merge_topk" % (world, k),
+                       "parallelism": "database shards, one NCCL all-gather per step", "l2": "database larger than L2"},
+            "clocks": sampler.summary(), "gpu_launches": int(fs.launch_count()),
+            "exchange_bytes_per_rank_per_step": nq * k * 12}))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
 def run_ours(args):
     import numpy as np
     import torch
@@ -568,6 +631,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--skip-also", action="store_true")
+    ap.add_argument("--mode", default="replica", choices=["replica", "shard"],
+                    help="N > 1: replica = rows split over ranks (weak scaling, the headline); shard = cfg3 database "
+                         "cut into id shards, all-gather + merge (strong scaling)")
     ap.add_argument("--ivfpq-nb", type=int, default=None,
                     help="cfg4 leg with fewer vectors (profiling aid; default: BASELINE.json's 10^8)")
     ap.add_argument("--skip-cfg5", action="store_true", help="leave out the 10^9-vector leg (about 5 min of index build)")
@@ -576,6 +642,8 @@ def main():
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.mode == "shard":
+        run_shard(args)
     else:
         run_ours(args)
 

@@ -104,6 +104,21 @@ FS_API int fs_flat_l2_knn_host(const float* xq_host, int64_t nq, const float* xb
                         int k, float* out_dist_host, int64_t* out_ids_host);
 
 /* --------------------------------------------------------------------------
+ * Merge of partial results (database sharding, 5.4 P:L355-363: every shard answers the full query
+ * set, "an additional round of k-selection is still required" to join the partial results).
+ *   dist device fp32 [nq][G][k], ids device int64 [nq][G][k]: the G lists of every query (from
+ *   fs_flat_l2_knn / fs_ivfpq_search on G shards, ids already global); entries with id < 0 are padding.
+ *   out_dist [nq][k], out_ids [nq][k]: the k smallest (distance, id) pairs, ascending, ties by lower id,
+ *   padded with (+INF, -1).  Distances are taken as they are (no arithmetic; negative values clamp at 0).
+ *   Entries of equal distance always come out in ascending id order; which of several entries tied at the
+ *   k-th place are kept is decided by (list number, place in the list), which is the id order when every
+ *   list is sorted by (distance, id) and list g holds ids below those of list g + 1 -- contiguous id shards.
+ * ------------------------------------------------------------------------ */
+FS_API int fs_merge_topk(const float* dist, const int64_t* ids, int64_t nq, int G, int k, float* out_dist,
+                  int64_t* out_ids, void* ws, size_t ws_bytes, fs_stream stream);
+FS_API size_t fs_merge_topk_ws_bytes(int64_t nq, int G, int k);
+
+/* --------------------------------------------------------------------------
  * IVFADC index with 8-bit residual product quantizer (Eq. 3-7, P:L59-90;
  * layout 5.2-5.3, Alg. 4).
  *   d % M == 0, 1 <= M <= 64, nlist >= 1, 256 codewords per

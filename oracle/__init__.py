@@ -204,3 +204,23 @@ def successive_mink_count(a: np.ndarray, k: int) -> int:
     """Appendix Eq. (13), P:L575-577 -- elements in the min-k of their prefix."""
     a = _f32(a)
     return int(lib().orc_successive_mink_count(_p(a), _i64(a.shape[0]), _i64(k)))
+
+
+def merge_topk(dist: np.ndarray, ids: np.ndarray, k: int):
+    """join of G partial k-NN lists per query by one more k-selection: the k smallest
+    (distance, id) pairs of the union, ascending, ties by lower id; ids < 0 are padding.
+    dist [nq, G, kk] (any float), ids [nq, G, kk] -> (dist [nq, k] same dtype, ids int64 [nq, k])."""
+    dist = np.asarray(dist)
+    ids = np.asarray(ids, dtype=np.int64)
+    nq = dist.shape[0]
+    d2 = dist.reshape(nq, -1)
+    i2 = ids.reshape(nq, -1)
+    od = np.full((nq, k), np.inf, dist.dtype)
+    oi = np.full((nq, k), -1, np.int64)
+    for q in range(nq):
+        keep = i2[q] >= 0
+        dq, iq = d2[q][keep], i2[q][keep]
+        order = np.lexsort((iq, dq))[:k]      # by distance, then id
+        od[q, :len(order)] = dq[order]
+        oi[q, :len(order)] = iq[order]
+    return od, oi

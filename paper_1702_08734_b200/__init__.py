@@ -53,7 +53,8 @@ def lib():
         L.fs_flat_engine.restype = ctypes.c_char_p
         L.fs_launch_count.restype = _i64
         L.fs_reset_launch_count.restype = None
-        for name in ("fs_kselect_ws_bytes", "fs_flat_l2_knn_ws_bytes", "fs_ivfpq_search_ws_bytes"):
+        for name in ("fs_kselect_ws_bytes", "fs_flat_l2_knn_ws_bytes", "fs_ivfpq_search_ws_bytes",
+                     "fs_merge_topk_ws_bytes"):
             if hasattr(L, name):
                 getattr(L, name).restype = _sz
         for name in ("fs_ivfpq_ntotal", "fs_ivfpq_last_scanned_codes"):
@@ -184,6 +185,23 @@ def flat_l2_knn_host(xq, xb, k: int, out_dist=None, out_ids=None):
     _check(lib().fs_flat_l2_knn_host(_vp(qp), _i64(nq), _vp(bp), _i64(xb.shape[0]), _int(d), _int(k),
                                      _vp(dp), _vp(ip)))
     return dist, ids
+
+
+def merge_topk(dist: torch.Tensor, ids: torch.Tensor, out_dist=None, out_ids=None):
+    """fs_merge_topk: dist fp32 [nq, G, k] and ids int64 [nq, G, k] (G partial lists per query, ids < 0 =
+    padding) -> the k smallest (distance, id) pairs per query, ascending, ties by lower id."""
+    _dev(dist, torch.float32, "dist")
+    _dev(ids, torch.int64, "ids")
+    nq, G, k = dist.shape
+    if tuple(ids.shape) != (nq, G, k):
+        raise ValueError("ids must have the shape of dist")
+    if out_dist is None:
+        out_dist = torch.empty((nq, k), dtype=torch.float32, device=dist.device)
+    if out_ids is None:
+        out_ids = torch.empty((nq, k), dtype=torch.int64, device=dist.device)
+    _check(lib().fs_merge_topk(_ptr(dist), _ptr(ids), _i64(nq), _int(G), _int(k), _ptr(out_dist), _ptr(out_ids),
+                               _vp(0), _sz(0), _stream()))
+    return out_dist, out_ids
 
 
 # ---------------------------------------------------------------------------

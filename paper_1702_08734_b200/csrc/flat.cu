@@ -298,6 +298,83 @@ static int launch_finish_t(const uint64_t* Wg, int64_t nq, int S, int k, const f
   return FS_OK;
 }
 
+// ---------------------------------------------------------------------------
+// Positions -> ids after a selection on (distance, position) keys (IVFPQ C5, shard merge).
+// ---------------------------------------------------------------------------
+// C5 second half: positions -> ids; entries with bitwise-equal distance are put
+// in ascending id order (positions order them by list and append order, which is
+// ascending id only inside a list filled in ascending id order).  One warp per query.
+__global__ void __launch_bounds__(128)
+    resolve_ids_kernel(float* __restrict__ dist, int64_t* __restrict__ ids_io,
+                       const int64_t* __restrict__ ids_all, int64_t table_stride, int64_t nq, int k) {
+  extern __shared__ __align__(16) unsigned char res_smem[];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int64_t q = (int64_t)blockIdx.x * 4 + warp;
+  if (q >= nq) return;
+  const int64_t* ids = ids_all + q * table_stride;  // per-query table (shard merge) or one table (stride 0)
+  int64_t* sid = reinterpret_cast<int64_t*>(res_smem) + (size_t)warp * k;
+  float* sd = reinterpret_cast<float*>(reinterpret_cast<int64_t*>(res_smem) + (size_t)4 * k) +
+              (size_t)warp * k;
+  for (int i = lane; i < k; i += 32) {
+    const int64_t pos = ids_io[q * k + i];
+    sid[i] = pos < 0 ? -1 : ids[pos];
+    sd[i] = dist[q * k + i];
+  }
+  __syncwarp();
+  for (int i = lane; i < k; i += 32) {
+    const float di = sd[i];
+    const int64_t id = sid[i];
+    int rank = i;
+    if (id >= 0) {
+      int s = i, e = i;
+      while (s > 0 && sd[s - 1] == di && sid[s - 1] >= 0) --s;
+      while (e + 1 < k && sd[e + 1] == di && sid[e + 1] >= 0) ++e;
+      if (e > s) {
+        rank = s;
+        for (int j = s; j <= e; ++j) rank += (sid[j] < id) || (sid[j] == id && j < i);
+      }
+    }
+    ids_io[q * k + rank] = id;
+  }
+}
+
+int launch_resolve_ids(float* dist, int64_t* ids_io, const int64_t* table, int64_t nq, int k, cudaStream_t s,
+                       int64_t table_stride) {
+  if (nq == 0) return FS_OK;
+  const size_t smem = (size_t)4 * k * (sizeof(int64_t) + sizeof(float));
+  resolve_ids_kernel<<<(unsigned)ceil_div(nq, 4), 128, smem, s>>>(dist, ids_io, table, table_stride, nq, k);
+  FS_LAUNCHED();
+  return FS_OK;
+}
+
+// ---------------------------------------------------------------------------
+// Merge of G partial results per query (database shards: "an additional round of
+// k-selection is still required"): (distance, id) pairs -> keys (distance image, position in the
+// query's G * k candidates), padded to the queue class.
+// ---------------------------------------------------------------------------
+__global__ void merge_pack_kernel(const float* __restrict__ dist, const int64_t* __restrict__ ids, int64_t nq, int G, int k,
+                                  int K, uint64_t* __restrict__ Wg) {
+  const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;  // over [nq][G][K]
+  if (e >= nq * G * K) return;
+  const int i = (int)(e % K);
+  const int64_t qg = e / K;  // q * G + g
+  uint64_t key = kSentinelKey;
+  if (i < k) {
+    const int64_t src = qg * k + i;
+    const int g = (int)(qg % G);
+    if (ids[src] >= 0) key = make_key(dist[src], (uint32_t)(g * k + i));
+  }
+  Wg[e] = key;
+}
+
+int launch_merge_pack(const float* dist, const int64_t* ids, int64_t nq, int G, int k, int K, uint64_t* Wg, cudaStream_t s) {
+  const int64_t n = nq * G * K;
+  if (n == 0) return FS_OK;
+  merge_pack_kernel<<<(unsigned)ceil_div(n, 256), 256, 0, s>>>(dist, ids, nq, G, k, K, Wg);
+  FS_LAUNCHED();
+  return FS_OK;
+}
+
 int launch_flat_finish(const uint64_t* Wg, int64_t nq, int S, int k, const float* xnorm,
                        float* out_dist, int64_t* out_ids, cudaStream_t s) {
   if (nq == 0) return FS_OK;
@@ -437,6 +514,31 @@ int fs_flat_l2_knn(const float* xq, int64_t nq, const float* xb, int64_t nb, int
   rc = t.acquire(ws, ws_bytes, fs::flat_plan(nq, nb, d, k).bytes, s);
   if (rc != FS_OK) return rc;
   return fs::flat_knn_device(xq, nq, xb, nb, d, k, nullptr, out_dist, out_ids, t.ptr, s);
+}
+
+size_t fs_merge_topk_ws_bytes(int64_t nq, int G, int k) {
+  if (nq < 0 || G < 1 || k < 1 || k > FS_MAX_K) return 0;
+  return fs::align_up((size_t)nq * G * (32 << fs::k_class(k)) * sizeof(uint64_t), 256);
+}
+
+int fs_merge_topk(const float* dist, const int64_t* ids, int64_t nq, int G, int k, float* out_dist,
+                  int64_t* out_ids, void* ws, size_t ws_bytes, fs_stream stream) {
+  if (nq < 0 || G < 1) return fs::set_error(FS_EINVAL, "fs_merge_topk: need nq >= 0, G >= 1");
+  if (k < 1) return fs::set_error(FS_EINVAL, "fs_merge_topk: k must be >= 1");
+  if (k > FS_MAX_K) return fs::set_error(FS_EUNSUPPORTED, "fs_merge_topk: k = %d > %d", k, FS_MAX_K);
+  if ((int64_t)G * k >= (1LL << 31)) return fs::set_error(FS_EUNSUPPORTED, "fs_merge_topk: G * k too large");
+  if (nq > 0 && (!dist || !ids || !out_dist || !out_ids)) return fs::set_error(FS_EINVAL, "fs_merge_topk: NULL pointer");
+  if (nq == 0) return FS_OK;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  fs::TempWs t;
+  int rc = t.acquire(ws, ws_bytes, fs_merge_topk_ws_bytes(nq, G, k), s);
+  if (rc != FS_OK) return rc;
+  uint64_t* Wg = static_cast<uint64_t*>(t.ptr);
+  const int K = 32 << fs::k_class(k);
+  if ((rc = fs::launch_merge_pack(dist, ids, nq, G, k, K, Wg, s)) != FS_OK) return rc;
+  if ((rc = fs::launch_flat_finish(Wg, nq, G, k, nullptr, out_dist, out_ids, s)) != FS_OK) return rc;
+  // positions in the query's G * k candidates -> ids; equal distances in ascending id order
+  return fs::launch_resolve_ids(out_dist, out_ids, ids, nq, k, s, (int64_t)G * k);
 }
 
 int fs_flat_l2_knn_host(const float* xq_host, int64_t nq, const float* xb_host, int64_t nb, int d,

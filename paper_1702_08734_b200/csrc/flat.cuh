@@ -44,4 +44,11 @@ int flat_knn_tc_device(const float* xq, int64_t nq, const float* xb, int64_t nb,
 int launch_flat_finish(const uint64_t* Wg, int64_t nq, int S, int k, const float* xnorm,
                        float* out_dist, int64_t* out_ids, cudaStream_t s);
 
+// Positions -> ids: ids_io[q][i] holds a position into table (or < 0); it becomes table[position], and
+// entries of a query with bitwise-equal distance are put in ascending id order.
+int launch_resolve_ids(float* dist, int64_t* ids_io, const int64_t* table, int64_t nq, int k, cudaStream_t s,
+                       int64_t table_stride = 0);
+// keys of the G partial lists of every query for launch_flat_finish: Wg [nq][G][K]
+int launch_merge_pack(const float* dist, const int64_t* ids, int64_t nq, int G, int k, int K, uint64_t* Wg, cudaStream_t s);
+
 }  // namespace fs

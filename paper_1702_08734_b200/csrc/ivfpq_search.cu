@@ -158,42 +158,6 @@ __global__ void __launch_bounds__(SCAN_THREADS) ivfpq_scan_kernel(const ScanArgs
   }
 }
 
-// C5 second half: positions -> ids; entries with bitwise-equal distance are put
-// in ascending id order (positions order them by list and append order, which is
-// ascending id only inside a list filled in ascending id order).  One warp per query.
-__global__ void __launch_bounds__(128)
-    ivfpq_resolve_kernel(float* __restrict__ dist, int64_t* __restrict__ ids_io,
-                         const int64_t* __restrict__ ids, int64_t nq, int k) {
-  extern __shared__ __align__(16) unsigned char res_smem[];
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int64_t q = (int64_t)blockIdx.x * 4 + warp;
-  if (q >= nq) return;
-  int64_t* sid = reinterpret_cast<int64_t*>(res_smem) + (size_t)warp * k;
-  float* sd = reinterpret_cast<float*>(reinterpret_cast<int64_t*>(res_smem) + (size_t)4 * k) +
-              (size_t)warp * k;
-  for (int i = lane; i < k; i += 32) {
-    const int64_t pos = ids_io[q * k + i];
-    sid[i] = pos < 0 ? -1 : ids[pos];
-    sd[i] = dist[q * k + i];
-  }
-  __syncwarp();
-  for (int i = lane; i < k; i += 32) {
-    const float di = sd[i];
-    const int64_t id = sid[i];
-    int rank = i;
-    if (id >= 0) {
-      int s = i, e = i;
-      while (s > 0 && sd[s - 1] == di && sid[s - 1] >= 0) --s;
-      while (e + 1 < k && sd[e + 1] == di && sid[e + 1] >= 0) ++e;
-      if (e > s) {
-        rank = s;
-        for (int j = s; j <= e; ++j) rank += (sid[j] < id) || (sid[j] == id && j < i);
-      }
-    }
-    ids_io[q * k + rank] = id;
-  }
-}
-
 __global__ void pq_bmax_kernel(const float* __restrict__ pq, float* __restrict__ bmax, int dsub) {
   const int m = blockIdx.x, lane = threadIdx.x;  // one warp per sub-quantizer
   float mx = 0.f;
@@ -806,10 +770,7 @@ int ivfpq_search_device(fs_ivfpq* ix, const float* xq, int64_t nq, int nprobe, i
   // C5
   rc = launch_flat_finish(Wg, nq, p.ngroups, k, nullptr, out_dist, out_ids, s);
   if (rc != FS_OK) return rc;
-  const size_t smem = (size_t)4 * k * (sizeof(int64_t) + sizeof(float));
-  ivfpq_resolve_kernel<<<(unsigned)ceil_div(nq, 4), 128, smem, s>>>(out_dist, out_ids,
-                                                                    ix->ids.as<int64_t>(), nq, k);
-  FS_LAUNCHED();
+  if ((rc = launch_resolve_ids(out_dist, out_ids, ix->ids.as<int64_t>(), nq, k, s)) != FS_OK) return rc;
   FS_CUDA(cudaEventRecord(ix->ev[3], s));
   ix->ev_valid = true;
   return FS_OK;
