@@ -139,6 +139,16 @@ FS_API int fs_ivfpq_get_quantizers(const fs_ivfpq* index, float* coarse, float* 
 FS_API int fs_ivfpq_train(fs_ivfpq* index, const float* x, int64_t n, int niter, uint64_t seed,
                    fs_stream stream);
 
+/* Lloyd's k-means on n device vectors x [n][d] (section 6.2: the assignment step is the exact
+ * search with k = 1).  centroids: device fp32 [K][d], in / out: with init != 0 they start as the evenly
+ * strided input points x[floor(c n / K)], else as given.  niter iterations of (assign to the nearest centroid,
+ * ties to the lower one; replace every centroid by the mean of its points -- summed in ascending point order
+ * in double precision, so the result is deterministic; an empty cluster c at iteration it is re-seeded from
+ * point mix(mix(seed + 0x9E3779B97F4A7C15 (it + 1)) + c) mod n, mix = the splitmix64 finaliser).
+ * assign: device int64 [n] or NULL: the assignment the last update was computed from.  n >= K, n < 2^32. */
+FS_API int fs_kmeans(const float* x, int64_t n, int d, int K, int niter, uint64_t seed, int init,
+              float* centroids, int64_t* assign, fs_stream stream);
+
 /* Add (D1-D3): coarse assignment q1(y) = argmin_c ||y - c||^2 by the flat
  * kernel with k = 1, residual PQ encoding (Eq. 3; byte
  * m = sub-quantizer m), append of (code, id) to list q1(y).

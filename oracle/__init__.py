@@ -206,6 +206,21 @@ def successive_mink_count(a: np.ndarray, k: int) -> int:
     return int(lib().orc_successive_mink_count(_p(a), _i64(a.shape[0]), _i64(k)))
 
 
+def kmeans_step(x: np.ndarray, centroids: np.ndarray, seed: int = 0, it: int = 0, margins: bool = False):
+    """one Lloyd iteration: assignment to the nearest centroid (double, ties to the lower
+    centroid), means in double; an empty cluster takes the hashed point of fs_kmeans's stated rule.
+    Returns (centroids fp32 [K, d], assignment int64 [n]) (+ best/second-best margins [n])."""
+    x, centroids = _f32(x), _f32(centroids)
+    n, d = x.shape
+    K = centroids.shape[0]
+    out = np.empty((K, d), np.float32)
+    assign = np.empty(n, np.int64)
+    mg = np.empty(n, np.float64) if margins else None
+    lib().orc_kmeans_step(_p(x), _i64(n), _i64(d), _p(centroids), _i64(K), ctypes.c_uint64(seed), _i64(it),
+                          _p(out), _p(assign), _p(mg))
+    return (out, assign, mg) if margins else (out, assign)
+
+
 def merge_topk(dist: np.ndarray, ids: np.ndarray, k: int):
     """join of G partial k-NN lists per query by one more k-selection: the k smallest
     (distance, id) pairs of the union, ascending, ties by lower id; ids < 0 are padding.

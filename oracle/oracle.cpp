@@ -26,6 +26,9 @@
 //                                 look-ups; exists so that a test can pin
 //                                 "reconstruction distance == LUT sum".
 //   orc_adc_eq11       P:L302     Eq. (11): term1 + term2 - 2*term3.
+//   orc_kmeans_step    P:L392-398 one Lloyd iteration: nearest-centroid assignment
+//                                 (double, direct form), cluster means; the library's
+//                                 stated empty-cluster rule restated (fs.h, fs_kmeans).
 //
 // Readings of the paper where it is silent:
 //   ties -> lower index / lower id / lower centroid number; -0 == +0; NaN sorts
@@ -361,6 +364,58 @@ int64_t orc_successive_mink_count(const float* a, int64_t n, int64_t k) {
     }
   }
   return count;
+}
+
+// ---------------------------------------------------------------------------
+// One Lloyd iteration of k-means (section 6.2: "k-means ... the assignment
+// is a k = 1 exact search").  The paper fixes nothing else; the library's stated rules
+// (include/fs.h, fs_kmeans) are restated here: assignment = nearest centroid by the direct
+// squared distance in double, ties to the lower centroid; new centroid = mean of its points
+// (double, rounded to fp32 once); an EMPTY cluster c at iteration `iter` takes the point
+// mix(mix(seed + 0x9E3779B97F4A7C15 (iter + 1)) + c) mod n, mix = the splitmix64 finaliser.
+// margin (may be NULL): (d_second - d_best) / d_second of every point's assignment.
+// ---------------------------------------------------------------------------
+static inline uint64_t orc_mix64(uint64_t z) {
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+  return z ^ (z >> 31);
+}
+
+void orc_kmeans_step(const float* x, int64_t n, int64_t d, const float* cent_in, int64_t K, uint64_t seed,
+                     int64_t iter, float* cent_out, int64_t* assign_out, double* margin_out) {
+#pragma omp parallel for schedule(dynamic, 64)
+  for (int64_t i = 0; i < n; ++i) {
+    double best = std::numeric_limits<double>::infinity(), second = best;
+    int64_t bc = -1;
+    for (int64_t c = 0; c < K; ++c) {
+      const double dist = l2_direct(x + i * d, cent_in + c * d, d);
+      if (dist < best) {
+        second = best;
+        best = dist;
+        bc = c;
+      } else if (dist < second) {
+        second = dist;
+      }
+    }
+    assign_out[i] = bc;
+    if (margin_out) margin_out[i] = (second - best) / std::max(second, 1e-300);
+  }
+  std::vector<double> sum((size_t)K * d, 0.0);
+  std::vector<int64_t> cnt((size_t)K, 0);
+  for (int64_t i = 0; i < n; ++i) {  // ascending point order
+    const int64_t c = assign_out[i];
+    ++cnt[c];
+    for (int64_t j = 0; j < d; ++j) sum[c * d + j] += (double)x[i * d + j];
+  }
+  for (int64_t c = 0; c < K; ++c) {
+    if (cnt[c] > 0) {
+      for (int64_t j = 0; j < d; ++j) cent_out[c * d + j] = (float)(sum[c * d + j] / (double)cnt[c]);
+    } else {
+      const uint64_t src =
+          orc_mix64(orc_mix64(seed + 0x9E3779B97F4A7C15ull * (uint64_t)(iter + 1)) + (uint64_t)c) % (uint64_t)n;
+      for (int64_t j = 0; j < d; ++j) cent_out[c * d + j] = x[src * d + j];
+    }
+  }
 }
 
 }  // extern "C"

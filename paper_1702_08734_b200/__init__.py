@@ -187,6 +187,21 @@ def flat_l2_knn_host(xq, xb, k: int, out_dist=None, out_ids=None):
     return dist, ids
 
 
+def kmeans(x: torch.Tensor, K: int, niter: int, seed: int = 0, centroids: torch.Tensor | None = None,
+           want_assign: bool = False):
+    """fs_kmeans: Lloyd's k-means on CUDA fp32 x [n, d].  centroids given: start from them (they are not
+    modified; a copy is returned), else from evenly strided input points.  Returns centroids [K, d]
+    (and the int64 assignment of the last iteration with want_assign)."""
+    _dev(x, torch.float32, "x")
+    n, d = x.shape
+    init = centroids is None
+    cent = torch.empty((K, d), dtype=torch.float32, device=x.device) if init else _dev(centroids, torch.float32, "centroids").clone()
+    assign = torch.empty(n, dtype=torch.int64, device=x.device) if want_assign else None
+    _check(lib().fs_kmeans(_ptr(x), _i64(n), _int(d), _int(K), _int(niter), ctypes.c_uint64(seed), _int(1 if init else 0),
+                           _ptr(cent), _ptr(assign), _stream()))
+    return (cent, assign) if want_assign else cent
+
+
 def merge_topk(dist: torch.Tensor, ids: torch.Tensor, out_dist=None, out_ids=None):
     """fs_merge_topk: dist fp32 [nq, G, k] and ids int64 [nq, G, k] (G partial lists per query, ids < 0 =
     padding) -> the k smallest (distance, id) pairs per query, ascending, ties by lower id."""

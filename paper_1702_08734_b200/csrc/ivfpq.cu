@@ -353,6 +353,51 @@ __global__ void iota_ids_kernel(int64_t* ids, int64_t n, int64_t start) {
 }
 }  // namespace
 
+// Stable LSD radix sort of n 32-bit keys (values < 2^nbits) with their arrival indices as the values.
+// keysA holds the input keys (overwritten); tmp must hold 3 * nb4 + hist bytes more (laid out as the
+// caller of stable_sort_ws says).  On return *keys_sorted / *order point into the buffers.
+size_t stable_sort_ws(int64_t n) {
+  const size_t nb4 = align_up((size_t)n * sizeof(uint32_t), 256);
+  int64_t grid = ceil_div(n, (int64_t)RS_WARPS * 32 * 64);
+  const int64_t maxg = (int64_t)sm_count() * 4;
+  if (grid > maxg) grid = maxg;
+  if (grid < 1) grid = 1;
+  return 4 * nb4 + align_up((size_t)256 * grid * RS_WARPS * sizeof(uint32_t), 256);
+}
+
+int stable_sort_by_key(char* t, int64_t n, int nbits, const uint32_t** keys_sorted, const uint32_t** order,
+                       cudaStream_t s) {
+  const size_t nb4 = align_up((size_t)n * sizeof(uint32_t), 256);
+  const int passes = nbits <= 0 ? 1 : (nbits + 7) / 8;
+  int64_t grid = ceil_div(n, (int64_t)RS_WARPS * 32 * 64);
+  const int64_t maxg = (int64_t)sm_count() * 4;
+  if (grid > maxg) grid = maxg;
+  if (grid < 1) grid = 1;
+  const int nwt = (int)grid * RS_WARPS;
+  const int64_t per_warp = ceil_div(ceil_div(n, nwt), 32) * 32;
+  uint32_t* kA = reinterpret_cast<uint32_t*>(t);
+  uint32_t* vA = reinterpret_cast<uint32_t*>(t + nb4);
+  uint32_t* kB = reinterpret_cast<uint32_t*>(t + 2 * nb4);
+  uint32_t* vB = reinterpret_cast<uint32_t*>(t + 3 * nb4);
+  uint32_t* hist = reinterpret_cast<uint32_t*>(t + 4 * nb4);
+  const uint32_t* vin = nullptr;
+  uint32_t *kin = kA, *kout = kB, *vout = vB, *vother = vA;
+  for (int pass = 0; pass < passes; ++pass) {
+    const int shift = 8 * pass;
+    rs_hist_kernel<<<(unsigned)grid, RS_WARPS * 32, 0, s>>>(kin, n, shift, per_warp, hist, nwt);
+    rs_scan_kernel<<<1, 1024, 0, s>>>(hist, (int64_t)256 * nwt);
+    rs_scatter_kernel<<<(unsigned)grid, RS_WARPS * 32, 0, s>>>(kin, vin, kout, vout, n, shift, per_warp, hist, nwt);
+    launch_counter() += 3;
+    vin = vout;
+    uint32_t* tk = kin; kin = kout; kout = tk;
+    uint32_t* tv = vout; vout = vother; vother = tv;
+  }
+  if (cudaGetLastError() != cudaSuccess) return set_error(FS_ECUDA, "stable sort: launch failed");
+  *keys_sorted = kin;
+  *order = vin;
+  return FS_OK;
+}
+
 int ivfpq_finalise(fs_ivfpq* ix, cudaStream_t s) {
   if (ix->n_staged == 0 && !ix->offsets_host.empty()) return FS_OK;
   const int64_t n = ix->n_csr + ix->n_staged;

@@ -62,6 +62,12 @@ struct fs_ivfpq {
 
 namespace fs {
 
+// Stable radix sort of 32-bit keys with their arrival indices (ivfpq.cu): the workspace t holds the keys
+// in its first n words on entry; stable_sort_ws(n) bytes.
+size_t stable_sort_ws(int64_t n);
+int stable_sort_by_key(char* t, int64_t n, int nbits, const uint32_t** keys_sorted, const uint32_t** order,
+                       cudaStream_t s);
+
 // Group staged vectors into the CSR lists (stable: append order kept).
 int ivfpq_finalise(fs_ivfpq* ix, cudaStream_t s);
 
@@ -69,9 +75,10 @@ int ivfpq_finalise(fs_ivfpq* ix, cudaStream_t s);
 int launch_pq_encode(const fs_ivfpq* ix, const float* y, int64_t n, const int64_t* assign,
                      uint8_t* codes_out, uint32_t* list_out, float* s1_out, cudaStream_t s);
 
-// Generic Lloyd k-means on device data x [n][d] -> cent [K][d] (ivfpq_train.cu).
+// Lloyd k-means on device data x [n][d] -> cent [K][d] (ivfpq_train.cu).  init: start from evenly strided
+// input points (else from cent as given); assign_out (or NULL): the assignment the last update used.
 int kmeans_device(const float* x, int64_t n, int d, int K, int niter, uint64_t seed, float* cent,
-                  cudaStream_t s);
+                  cudaStream_t s, bool init = true, int64_t* assign_out = nullptr);
 // Nearest centroid of each x (k = 1 exact search, chunked): assign int64 [n].
 int assign_nearest(const float* x, int64_t n, const float* cent, const float* cent_norm, int K,
                    int d, int64_t* assign, cudaStream_t s);

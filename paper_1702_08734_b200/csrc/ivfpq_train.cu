@@ -1,13 +1,18 @@
-// ivfpq_train.cu -- fs_ivfpq_train: k-means training of the coarse quantizer q1
-// and of the residual product quantizer q2 ("trained via k-means", P:L90;
-// assignment = exact search with k = 1).
+// ivfpq_train.cu -- Lloyd's k-means (fs_kmeans) and fs_ivfpq_train: training of the coarse quantizer
+// q1 and of the residual product quantizer q2 ("trained via k-means"; section 6.2,
+// the assignment step is the exact search with k = 1, whose selection is fused into the
+// distance tiles -- flat_tc.cu -- so no n x K matrix is written).
 //
-// Off the parity path (reading C-11): the oracle and the library share
-// the resulting arrays through fs_ivfpq_get_quantizers.  The paper leaves the
-// initialisation and empty clusters unspecified; here: initial centroids are
-// evenly strided input points, Lloyd iterations assign with the k = 1 exact
-// search (flat.cu) and accumulate the means with float atomics, and an empty
-// cluster is re-seeded from a hashed input point.
+// The paper leaves the initialisation and empty clusters unspecified (reading C-11); here:
+//   init       centroid c = input point floor(c n / K) (evenly strided, distinct for n >= K)
+//   assignment nearest centroid by the k = 1 exact search, ties to the lower centroid
+//   update     DETERMINISTIC: the points are grouped by cluster with the stable radix sort of the
+//              inverted-list builder, and one warp per cluster adds its points in ascending index order
+//              in double precision (no float atomics: the same input gives the same quantizers bit for
+//              bit, and the means match a double-precision reference to fp32 rounding)
+//   empty      cluster c at iteration it is re-seeded from point
+//              mix(mix(seed + 0x9E3779B97F4A7C15 (it + 1)) + c) mod n   (mix = the splitmix64 finaliser)
+// oracle/oracle.cpp restates one step of this (orc_kmeans_step) for the parity test.
 #include "flat.cuh"
 #include "ivfpq.cuh"
 
@@ -25,15 +30,20 @@ __global__ void km_init_kernel(const float* __restrict__ x, int64_t n, int d, in
   cent[e] = x[src * d + j];
 }
 
-__global__ void km_accumulate_kernel(const float* __restrict__ x, int64_t n, int d,
-                                     const int64_t* __restrict__ assign, float* __restrict__ sums,
-                                     unsigned int* __restrict__ counts) {
-  const int lane = threadIdx.x & 31;
-  const int64_t v = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-  if (v >= n) return;
-  const int64_t c = assign[v];
-  for (int j = lane; j < d; j += 32) atomicAdd(&sums[c * d + j], x[v * d + j]);
-  if (lane == 0) atomicAdd(&counts[c], 1u);
+__global__ void km_keys_kernel(const int64_t* __restrict__ assign, int64_t n, uint32_t* __restrict__ keys) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) keys[i] = (uint32_t)assign[i];
+}
+
+// first[c] = position of cluster c's first point in the sorted order (first[K] = n)
+__global__ void km_bounds_kernel(const uint32_t* __restrict__ keys_sorted, int64_t n, int K, int64_t* __restrict__ first) {
+  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= n) return;
+  const int64_t k1 = keys_sorted[p];
+  const int64_t k0 = p > 0 ? (int64_t)keys_sorted[p - 1] : -1;
+  for (int64_t c = k0 + 1; c <= k1; ++c) first[c] = p;
+  if (p == n - 1)
+    for (int64_t c = k1 + 1; c <= K; ++c) first[c] = n;
 }
 
 __device__ __forceinline__ uint64_t km_mix(uint64_t z) {
@@ -42,20 +52,27 @@ __device__ __forceinline__ uint64_t km_mix(uint64_t z) {
   return z ^ (z >> 31);
 }
 
-__global__ void km_update_kernel(const float* __restrict__ x, int64_t n, int d, int K,
-                                 const float* __restrict__ sums,
-                                 const unsigned int* __restrict__ counts, uint64_t seed, int iter,
-                                 float* __restrict__ cent) {
-  const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (e >= (int64_t)K * d) return;
-  const int64_t c = e / d;
-  const int j = (int)(e - c * d);
-  const unsigned int cnt = counts[c];
-  if (cnt > 0) {
-    cent[e] = sums[e] / (float)cnt;
-  } else {
+// One warp per cluster: the mean of its points (ascending point index, double accumulation), or the
+// re-seed point when the cluster is empty.
+__global__ void __launch_bounds__(256)
+    km_update_kernel(const float* __restrict__ x, int64_t n, int d, int K, const uint32_t* __restrict__ order,
+                     const int64_t* __restrict__ first, uint64_t seed, int iter, float* __restrict__ cent) {
+  const int lane = threadIdx.x & 31;
+  const int64_t c = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
+  if (c >= K) return;
+  const int64_t b = first[c], e = first[c + 1];
+  if (e == b) {
     const uint64_t src = km_mix(km_mix(seed + 0x9E3779B97F4A7C15ull * (uint64_t)(iter + 1)) + (uint64_t)c) % (uint64_t)n;
-    cent[e] = x[src * d + j];
+    for (int j = lane; j < d; j += 32) cent[c * d + j] = x[src * d + j];
+    return;
+  }
+  const double inv = 1.0 / (double)(e - b);
+  for (int j0 = 0; j0 < d; j0 += 32) {
+    const int j = j0 + lane;
+    double acc = 0.0;
+    if (j < d)
+      for (int64_t p = b; p < e; ++p) acc += (double)x[(int64_t)order[p] * d + j];
+    if (j < d) cent[c * d + j] = (float)(acc * inv);
   }
 }
 
@@ -72,37 +89,43 @@ __global__ void residual_kernel(const float* __restrict__ x, int64_t n, int d,
 }  // namespace
 
 int kmeans_device(const float* x, int64_t n, int d, int K, int niter, uint64_t seed, float* cent,
-                  cudaStream_t s) {
+                  cudaStream_t s, bool init, int64_t* assign_out) {
   if (n < K) return set_error(FS_EINVAL, "k-means: %lld points for %d centroids", (long long)n, K);
-  DevBuf sums, counts, assign, cnorm;
+  if (n >= (1LL << 32)) return set_error(FS_EUNSUPPORTED, "k-means: more than 2^32-1 points");
+  DevBuf sortws, first, assign, cnorm;
   int rc;
   auto done = [&](int r) {
     cudaStreamSynchronize(s);
-    sums.release();
-    counts.release();
+    sortws.release();
+    first.release();
     assign.release();
     cnorm.release();
     return r;
   };
   const int64_t kd = (int64_t)K * d;
-  if ((rc = sums.ensure((size_t)kd * sizeof(float), 0, s)) != FS_OK ||
-      (rc = counts.ensure((size_t)K * sizeof(unsigned int), 0, s)) != FS_OK ||
+  if ((rc = sortws.ensure(stable_sort_ws(n), 0, s)) != FS_OK ||
+      (rc = first.ensure((size_t)(K + 1) * sizeof(int64_t), 0, s)) != FS_OK ||
       (rc = assign.ensure((size_t)n * sizeof(int64_t), 0, s)) != FS_OK ||
       (rc = cnorm.ensure((size_t)K * sizeof(float), 0, s)) != FS_OK)
     return done(rc);
-  km_init_kernel<<<(unsigned)ceil_div(kd, 256), 256, 0, s>>>(x, n, d, K, cent);
-  ++launch_counter();
+  if (init) {
+    km_init_kernel<<<(unsigned)ceil_div(kd, 256), 256, 0, s>>>(x, n, d, K, cent);
+    ++launch_counter();
+  }
+  int nbits = 0;
+  while ((1LL << nbits) < K) ++nbits;
   for (int it = 0; it < niter; ++it) {
     if ((rc = launch_row_norms(cent, K, d, cnorm.as<float>(), s)) != FS_OK) return done(rc);
     if ((rc = assign_nearest(x, n, cent, cnorm.as<float>(), K, d, assign.as<int64_t>(), s)) != FS_OK)
       return done(rc);
-    cudaMemsetAsync(sums.p, 0, (size_t)kd * sizeof(float), s);
-    cudaMemsetAsync(counts.p, 0, (size_t)K * sizeof(unsigned int), s);
-    km_accumulate_kernel<<<(unsigned)ceil_div(n, 8), 256, 0, s>>>(x, n, d, assign.as<int64_t>(),
-                                                                 sums.as<float>(),
-                                                                 counts.as<unsigned int>());
-    km_update_kernel<<<(unsigned)ceil_div(kd, 256), 256, 0, s>>>(
-        x, n, d, K, sums.as<float>(), counts.as<unsigned int>(), seed, it, cent);
+    if (assign_out && it == niter - 1)
+      cudaMemcpyAsync(assign_out, assign.p, (size_t)n * sizeof(int64_t), cudaMemcpyDeviceToDevice, s);
+    km_keys_kernel<<<(unsigned)ceil_div(n, 256), 256, 0, s>>>(assign.as<int64_t>(), n, sortws.as<uint32_t>());
+    ++launch_counter();
+    const uint32_t *keys_sorted = nullptr, *order = nullptr;
+    if ((rc = stable_sort_by_key(sortws.as<char>(), n, nbits, &keys_sorted, &order, s)) != FS_OK) return done(rc);
+    km_bounds_kernel<<<(unsigned)ceil_div(n, 256), 256, 0, s>>>(keys_sorted, n, K, first.as<int64_t>());
+    km_update_kernel<<<(unsigned)ceil_div(K, 8), 256, 0, s>>>(x, n, d, K, order, first.as<int64_t>(), seed, it, cent);
     launch_counter() += 2;
   }
   cudaError_t e = cudaStreamSynchronize(s);
@@ -112,6 +135,16 @@ int kmeans_device(const float* x, int64_t n, int d, int K, int niter, uint64_t s
 }
 
 }  // namespace fs
+
+extern "C" int fs_kmeans(const float* x, int64_t n, int d, int K, int niter, uint64_t seed, int init,
+                         float* centroids, int64_t* assign, fs_stream stream) {
+  using namespace fs;
+  if (!x || !centroids) return set_error(FS_EINVAL, "fs_kmeans: NULL pointer");
+  if (n < 1 || d < 1 || K < 1 || niter < 0) return set_error(FS_EINVAL, "fs_kmeans: need n, d, K >= 1 and niter >= 0");
+  if (d > 2048) return set_error(FS_EUNSUPPORTED, "fs_kmeans: d > 2048");
+  if (n < K) return set_error(FS_EINVAL, "fs_kmeans: fewer points than centroids");
+  return kmeans_device(x, n, d, K, niter, seed, centroids, static_cast<cudaStream_t>(stream), init != 0, assign);
+}
 
 extern "C" int fs_ivfpq_train(fs_ivfpq* ix, const float* x, int64_t n, int niter, uint64_t seed,
                               fs_stream stream) {
