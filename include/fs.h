@@ -21,6 +21,12 @@
  *    Eq. 7/10).
  *  - Workspaces: if ws == NULL the library allocates and frees a stream-ordered
  *    temporary itself; otherwise ws must hold at least the matching *_ws_bytes.
+ *  - Devices and threads: every call works on the CURRENT device of the calling thread (cudaSetDevice);
+ *    pointers, streams and fs_ivfpq objects belong to the device they were created on.  The device entry
+ *    points (fs_kselect, fs_flat_l2_knn, fs_merge_topk, fs_kmeans, fs_ivfpq_search) may run concurrently
+ *    from several host threads on distinct streams with distinct workspaces; calls on one fs_ivfpq object
+ *    are serialised by the caller (add / train / search change or read its lists and event records); the
+ *    *_host entry points hold a process-wide lock (one staging arena).
  */
 #ifndef FS_H_
 #define FS_H_
@@ -76,6 +82,13 @@ FS_API void fs_reset_launch_count(void);
  * ------------------------------------------------------------------------ */
 FS_API int fs_kselect(const float* rows, int64_t n_rows, int64_t n, int64_t ld, int k, float* out_val,
                int32_t* out_idx, void* ws, size_t ws_bytes, fs_stream stream);
+/* The "other comparator" of P:L48 ("other comparators are sometimes desired"): the k HIGHEST values of
+ * every array, descending, ties broken by LOWER index, -0 == +0, NaN after everything else (so a NaN is
+ * returned only when fewer than k ordinary values exist); k > n pads with (-INF, -1).  Same arguments,
+ * workspace (fs_kselect_ws_bytes) and error behaviour as fs_kselect; the same kernels run on the negated
+ * values. */
+FS_API int fs_kselect_largest(const float* rows, int64_t n_rows, int64_t n, int64_t ld, int k, float* out_val,
+                              int32_t* out_idx, void* ws, size_t ws_bytes, fs_stream stream);
 FS_API size_t fs_kselect_ws_bytes(int64_t n_rows, int64_t n, int k);
 /* Same with HOST buffers (pinned or pageable): rows are copied in, selected and copied out in up to
  * 8 slices on three internal streams (copy-in of a slice overlaps the selection of the previous one and

@@ -62,8 +62,9 @@ def _f32(a):
 _i64 = ctypes.c_int64
 
 
-def kselect(rows: np.ndarray, k: int, n: int | None = None):
-    """k lowest values of each row with indices, ties by lower index.
+def kselect(rows: np.ndarray, k: int, n: int | None = None, largest: bool = False):
+    """k lowest values of each row with indices, ties by lower index
+    (``largest``: the k highest, descending, ties by lower index -- "other comparators").
 
     rows: [n_rows, ld] fp32; only the first ``n`` (default ld) columns belong to
     the arrays.  Returns (values fp32 [n_rows,k], indices int32 [n_rows,k]).
@@ -74,7 +75,8 @@ def kselect(rows: np.ndarray, k: int, n: int | None = None):
     n = ld if n is None else n
     val = np.empty((n_rows, k), np.float32)
     idx = np.empty((n_rows, k), np.int32)
-    lib().orc_kselect(_p(rows), _i64(n_rows), _i64(n), _i64(ld), _i64(k), _p(val), _p(idx))
+    fn = lib().orc_kselect_largest if largest else lib().orc_kselect
+    fn(_p(rows), _i64(n_rows), _i64(n), _i64(ld), _i64(k), _p(val), _p(idx))
     return val, idx
 
 

@@ -11,6 +11,9 @@
 // What each entry point follows:
 //   orc_kselect        P:L48      k lowest values with their indices: the plain
 //                                 definition, by a full sort of (value, index).
+//   orc_kselect_largest P:L48     "other comparators": the k highest values, by a full
+//                                 sort with the value order reversed (ties still to the
+//                                 lower index, NaN still last).
 //   orc_flat_l2_knn    P:L41-57   Eq. (1) with D squared, distances in
 //                                 the DIRECT form sum_c (x_c - y_c)^2 in double
 //                                 (deliberately not Eq. (2), which the GPU uses).
@@ -71,6 +74,18 @@ inline bool pair_less(const Pair<V, I>& a, const Pair<V, I>& b) {
   return a.i < b.i;
 }
 
+// the reversed value order of the k-largest variant: higher value first, NaN last, then index ascending
+template <typename V, typename I>
+inline bool pair_greater(const Pair<V, I>& a, const Pair<V, I>& b) {
+  const bool an = std::isnan(a.v), bn = std::isnan(b.v);
+  if (an != bn) return bn;
+  if (!an) {
+    if (a.v > b.v) return true;
+    if (b.v > a.v) return false;
+  }
+  return a.i < b.i;
+}
+
 }  // namespace
 
 extern "C" {
@@ -101,6 +116,27 @@ void orc_kselect(const float* rows, int64_t n_rows, int64_t n, int64_t ld, int64
         out_idx[r * k + j] = (int32_t)p[(size_t)j].i;
       } else {
         out_val[r * k + j] = std::numeric_limits<float>::infinity();
+        out_idx[r * k + j] = -1;
+      }
+    }
+  }
+}
+
+// P:L48 "other comparators are sometimes desired": the k HIGHEST values, descending.
+void orc_kselect_largest(const float* rows, int64_t n_rows, int64_t n, int64_t ld, int64_t k,
+                         float* out_val, int32_t* out_idx) {
+#pragma omp parallel for schedule(dynamic, 1)
+  for (int64_t r = 0; r < n_rows; ++r) {
+    const float* a = rows + r * ld;
+    std::vector<Pair<float, int64_t>> p((size_t)n);
+    for (int64_t i = 0; i < n; ++i) p[(size_t)i] = {a[i], i};
+    std::sort(p.begin(), p.end(), pair_greater<float, int64_t>);
+    for (int64_t j = 0; j < k; ++j) {
+      if (j < n) {
+        out_val[r * k + j] = a[p[(size_t)j].i];
+        out_idx[r * k + j] = (int32_t)p[(size_t)j].i;
+      } else {
+        out_val[r * k + j] = -std::numeric_limits<float>::infinity();
         out_idx[r * k + j] = -1;
       }
     }

@@ -100,8 +100,10 @@ def kselect_ws_bytes(n_rows: int, n: int, k: int) -> int:
     return int(lib().fs_kselect_ws_bytes(_i64(n_rows), _i64(n), _int(k)))
 
 
-def kselect(rows: torch.Tensor, k: int, n: int | None = None, out_val=None, out_idx=None, ws=None):
-    """fs_kselect: k smallest of each row (ascending, ties by lower index).
+def kselect(rows: torch.Tensor, k: int, n: int | None = None, out_val=None, out_idx=None, ws=None,
+            largest: bool = False):
+    """fs_kselect: k smallest of each row (ascending, ties by lower index); ``largest=True`` calls
+    fs_kselect_largest (k largest, descending, ties by lower index).
 
     rows: CUDA fp32 [n_rows, ld] (row stride ld = rows.stride(0)); n defaults to
     rows.shape[1].  Returns (values fp32 [n_rows,k], indices int32 [n_rows,k]).
@@ -118,9 +120,10 @@ def kselect(rows: torch.Tensor, k: int, n: int | None = None, out_val=None, out_
         out_idx = torch.empty((n_rows, k), dtype=torch.int32, device=rows.device)
     _dev(out_val, torch.float32, "out_val")
     _dev(out_idx, torch.int32, "out_idx")
-    _check(lib().fs_kselect(_ptr(rows), _i64(n_rows), _i64(n), _i64(ld), _int(k), _ptr(out_val),
-                            _ptr(out_idx), _ptr(ws), _sz(0 if ws is None else ws.numel() * ws.element_size()),
-                            _stream()))
+    fn = lib().fs_kselect_largest if largest else lib().fs_kselect
+    _check(fn(_ptr(rows), _i64(n_rows), _i64(n), _i64(ld), _int(k), _ptr(out_val),
+              _ptr(out_idx), _ptr(ws), _sz(0 if ws is None else ws.numel() * ws.element_size()),
+              _stream()))
     return out_val, out_idx
 
 

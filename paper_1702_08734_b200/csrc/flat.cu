@@ -448,14 +448,9 @@ int flat_knn_device(const float* xq, int64_t nq, const float* xb, int64_t nb, in
   const bool vec = (d % 4 == 0) && (((uintptr_t)xq | (uintptr_t)xb) % 16 == 0);
   const dim3 grid((unsigned)ceil_div(nq, TQ), (unsigned)p.S);
   const size_t smem = sizeof(FlatSmem);
-  static bool attr_done = false;
-  if (!attr_done) {
-    FS_CUDA(cudaFuncSetAttribute(flat_tile_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)smem));
-    FS_CUDA(cudaFuncSetAttribute(flat_tile_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)smem));
-    attr_done = true;
-  }
+  // (function attributes are per device: set on every call, it costs about a microsecond)
+  FS_CUDA(cudaFuncSetAttribute(flat_tile_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  FS_CUDA(cudaFuncSetAttribute(flat_tile_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   if (vec)
     flat_tile_kernel<true><<<grid, THREADS, smem, s>>>(xq, nq, xb, nb, d, yn, p.S, p.chunk, p.kclass, Wg);
   else

@@ -618,15 +618,7 @@ bool flat_tc_supported(int d) {
 
 // Every extra split is one more partial queue per query (more survivors in the epilogue,
 // more keys in B4): weigh it against the wave quantisation of the MMA work.
-static double split_penalty(int kclass) {
-  static double forced = -1.0;
-  if (forced < 0.0) {
-    const char* e = getenv("FS_FLAT_SPLIT_PENALTY");  // tuning knob (A/B runs)
-    forced = e ? atof(e) : 0.0;
-  }
-  if (forced > 0.0) return forced;
-  return kclass == 0 ? 0.002 : 0.004;
-}
+static double split_penalty(int kclass) { return kclass == 0 ? 0.002 : 0.004; }
 
 FlatTcPlan flat_tc_plan(int64_t nq, int64_t nb, int d, int k) {
   FlatTcPlan p;
@@ -767,11 +759,7 @@ int flat_knn_tc_device(const float* xq, int64_t nq, const float* xb, int64_t nb,
   a.lo_flag = flag;
   a.dout = dout;
   a.dld = dld;
-  static size_t attr_smem = 0;
-  if (p.smem > attr_smem) {
-    FS_CUDA(cudaFuncSetAttribute(flat_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem));
-    attr_smem = p.smem;
-  }
+  FS_CUDA(cudaFuncSetAttribute(flat_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem));  // per device
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)p.grid);
   cfg.blockDim = dim3(TC_THREADS);

@@ -153,12 +153,7 @@ int launch_pq_encode(const fs_ivfpq* ix, const float* y, int64_t n, const int64_
   if (n == 0) return FS_OK;
   const int dsub = ix->dsub, dsp = dsub | 1;
   const size_t smem = (size_t)(256 * dsp + 2 * ENC_TV * dsub + ENC_TV) * sizeof(float) + (size_t)ENC_TV * ix->M;
-  static size_t attr_smem = 0;
-  if (smem > attr_smem) {
-    FS_CUDA(cudaFuncSetAttribute(pq_encode_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)smem));
-    attr_smem = smem;
-  }
+  FS_CUDA(cudaFuncSetAttribute(pq_encode_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));  // per device
   const int64_t ntiles = ceil_div(n, ENC_TV);
   const int64_t maxg = (int64_t)sm_count() * 8;
   pq_encode_kernel<<<(unsigned)(ntiles < maxg ? ntiles : maxg), ENC_WARPS * 32, smem, s>>>(

@@ -42,7 +42,7 @@ namespace fs {
 // kselect.cu
 size_t kselect_ws_bytes(int64_t n_rows, int64_t n, int k);
 int kselect_device(const float* rows, int64_t n_rows, int64_t n, int64_t ld, int k, float* out_val,
-                   int32_t* out_idx, void* ws, cudaStream_t s);
+                   int32_t* out_idx, void* ws, cudaStream_t s, bool largest);
 
 namespace {
 constexpr int SCAN_WARPS = 8;
@@ -698,7 +698,7 @@ int ivfpq_search_device(fs_ivfpq* ix, const float* xq, int64_t nq, int nprobe, i
       rc = flat_knn_tc_device(xq + q0 * ix->d, n, ix->coarse.as<float>(), ix->nlist, ix->d, 1, nullptr, nullptr, w, s,
                               D, p.c1_ld);
       if (rc != FS_OK) return rc;
-      rc = kselect_device(D, n, ix->nlist, p.c1_ld, nprobe, cval, cidx, w + p.off_ksws, s);
+      rc = kselect_device(D, n, ix->nlist, p.c1_ld, nprobe, cval, cidx, w + p.off_ksws, s, false);
       if (rc != FS_OK) return rc;
       widen_ids_kernel<<<(unsigned)ceil_div(n * nprobe, 256), 256, 0, s>>>(cidx, cval, cids + q0 * nprobe,
                                                                           cdist + q0 * nprobe, n * nprobe);

@@ -21,6 +21,7 @@ struct K1Args {
   float* out_val;     // P == 1: [n_rows]
   int32_t* out_idx;
   uint64_t* out_keys;  // P > 1: [n_rows][P] chunk minima as keys
+  int largest;         // 1: arg max (the kernels reduce -v)
 };
 
 __device__ __forceinline__ float4 ld_stream4(const float* p) {
@@ -31,7 +32,7 @@ __device__ __forceinline__ float4 ld_stream4(const float* p) {
   return r;
 }
 
-template <int WARPS>
+template <int WARPS, bool LG>
 __global__ void __launch_bounds__(WARPS * 32) kselect_k1_kernel(const K1Args a) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int64_t item = (int64_t)blockIdx.x * WARPS + warp;
@@ -48,13 +49,14 @@ __global__ void __launch_bounds__(WARPS * 32) kselect_k1_kernel(const K1Args a) 
   if (head > len) head = len;
   const int64_t nvec = (len - head) >> 2;
   uint64_t best = kSentinelKey;
-  if (lane < head) best = umin64(best, make_key(p[lane], base + lane));
+  if (lane < head) best = umin64(best, make_key(LG ? -p[lane] : p[lane], base + lane));
   const float* pv = p + head;
   const uint32_t vbase = base + (uint32_t)head;
   // Per lane a running float minimum decides whether the exact key compare is
   // needed at all: "!(v > m)" is true for v <= m and for NaN.
   float m = __uint_as_float(0x7FFFFFFFu);
-  auto take = [&](float v, uint32_t idx) {
+  auto take = [&](float raw, uint32_t idx) {
+    const float v = LG ? -raw : raw;  // arg max = arg min of the negated values, ties still to the lower index
     if (!(v > m)) {
       const uint64_t key = make_key(v, idx);
       if (key < best) {
@@ -94,7 +96,7 @@ __global__ void __launch_bounds__(WARPS * 32) kselect_k1_kernel(const K1Args a) 
     if (a.P > 1) {
       a.out_keys[item] = best;
     } else if (best == kSentinelKey) {
-      a.out_val[item] = __uint_as_float(0x7F800000u);
+      a.out_val[item] = __uint_as_float(LG ? 0xFF800000u : 0x7F800000u);
       a.out_idx[item] = -1;
     } else {
       const uint32_t idx = key_idx(best);
@@ -107,7 +109,8 @@ __global__ void __launch_bounds__(WARPS * 32) kselect_k1_kernel(const K1Args a) 
 // The minimum of a row's P chunk minima: one warp per row.
 __global__ void __launch_bounds__(128) kselect_k1_final_kernel(const uint64_t* __restrict__ keys, int64_t n_rows, int P,
                                                                 const float* __restrict__ rows, int64_t ld,
-                                                                float* __restrict__ out_val, int32_t* __restrict__ out_idx) {
+                                                                float* __restrict__ out_val, int32_t* __restrict__ out_idx,
+                                                                int largest) {
   const int lane = threadIdx.x & 31;
   const int64_t row = (int64_t)blockIdx.x * 4 + (threadIdx.x >> 5);
   if (row >= n_rows) return;
@@ -117,7 +120,7 @@ __global__ void __launch_bounds__(128) kselect_k1_final_kernel(const uint64_t* _
   for (int s = 16; s >= 1; s >>= 1) best = umin64(best, shfl_xor64(best, s));
   if (lane == 0) {
     if (best == kSentinelKey) {
-      out_val[row] = __uint_as_float(0x7F800000u);
+      out_val[row] = __uint_as_float(largest ? 0xFF800000u : 0x7F800000u);
       out_idx[row] = -1;
     } else {
       const uint32_t idx = key_idx(best);
@@ -207,7 +210,7 @@ struct HostStage {
 // kselect_row.cu: k >= 2
 size_t kselect_rows_ws_bytes(int64_t n_rows, int64_t n, int k);
 int kselect_rows_device(const float* rows, int64_t n_rows, int64_t n, int64_t ld, int k, float* out_val,
-                        int32_t* out_idx, void* ws, cudaStream_t s);
+                        int32_t* out_idx, void* ws, cudaStream_t s, bool largest);
 
 // Selection over device rows; also used by the flat and IVFPQ drivers.
 size_t kselect_ws_bytes(int64_t n_rows, int64_t n, int k) {
@@ -215,8 +218,8 @@ size_t kselect_ws_bytes(int64_t n_rows, int64_t n, int k) {
 }
 
 int kselect_device(const float* rows, int64_t n_rows, int64_t n, int64_t ld, int k, float* out_val,
-                   int32_t* out_idx, void* ws, cudaStream_t s) {
-  if (k >= 2) return kselect_rows_device(rows, n_rows, n, ld, k, out_val, out_idx, ws, s);
+                   int32_t* out_idx, void* ws, cudaStream_t s, bool largest) {
+  if (k >= 2) return kselect_rows_device(rows, n_rows, n, ld, k, out_val, out_idx, ws, s, largest);
   const Plan p = make_plan(n_rows, n);
   K1Args a;
   a.vals = rows;
@@ -228,15 +231,19 @@ int kselect_device(const float* rows, int64_t n_rows, int64_t n, int64_t ld, int
   a.out_val = out_val;
   a.out_idx = out_idx;
   a.out_keys = p.P > 1 ? reinterpret_cast<uint64_t*>(ws) : nullptr;
+  a.largest = largest ? 1 : 0;
   const int64_t items = n_rows * p.P;
   if (items == 0) return FS_OK;
   const int64_t grid = ceil_div(items, kWarpsPerCtaK1);
   if (grid > 0x7fffffffLL) return set_error(FS_EUNSUPPORTED, "too many rows for one launch");
-  kselect_k1_kernel<kWarpsPerCtaK1><<<(unsigned)grid, kWarpsPerCtaK1 * 32, 0, s>>>(a);
+  if (largest)
+    kselect_k1_kernel<kWarpsPerCtaK1, true><<<(unsigned)grid, kWarpsPerCtaK1 * 32, 0, s>>>(a);
+  else
+    kselect_k1_kernel<kWarpsPerCtaK1, false><<<(unsigned)grid, kWarpsPerCtaK1 * 32, 0, s>>>(a);
   FS_LAUNCHED();
   if (p.P > 1) {
     kselect_k1_final_kernel<<<(unsigned)ceil_div(n_rows, 4), 128, 0, s>>>(a.out_keys, n_rows, p.P, rows, ld, out_val,
-                                                                        out_idx);
+                                                                        out_idx, a.largest);
     FS_LAUNCHED();
   }
   return FS_OK;
@@ -251,8 +258,8 @@ size_t fs_kselect_ws_bytes(int64_t n_rows, int64_t n, int k) {
   return fs::kselect_ws_bytes(n_rows, n, k);
 }
 
-int fs_kselect(const float* rows, int64_t n_rows, int64_t n, int64_t ld, int k, float* out_val,
-               int32_t* out_idx, void* ws, size_t ws_bytes, fs_stream stream) {
+static int kselect_entry(const float* rows, int64_t n_rows, int64_t n, int64_t ld, int k, float* out_val,
+                         int32_t* out_idx, void* ws, size_t ws_bytes, fs_stream stream, bool largest) {
   int rc = fs::validate(rows, n_rows, n, ld, k, out_val, out_idx);
   if (rc != FS_OK) return rc;
   if (n_rows == 0) return FS_OK;
@@ -260,7 +267,17 @@ int fs_kselect(const float* rows, int64_t n_rows, int64_t n, int64_t ld, int k, 
   fs::TempWs t;
   rc = t.acquire(ws, ws_bytes, fs::kselect_ws_bytes(n_rows, n, k), s);
   if (rc != FS_OK) return rc;
-  return fs::kselect_device(rows, n_rows, n, ld, k, out_val, out_idx, t.ptr, s);
+  return fs::kselect_device(rows, n_rows, n, ld, k, out_val, out_idx, t.ptr, s, largest);
+}
+
+int fs_kselect(const float* rows, int64_t n_rows, int64_t n, int64_t ld, int k, float* out_val,
+               int32_t* out_idx, void* ws, size_t ws_bytes, fs_stream stream) {
+  return kselect_entry(rows, n_rows, n, ld, k, out_val, out_idx, ws, ws_bytes, stream, false);
+}
+
+int fs_kselect_largest(const float* rows, int64_t n_rows, int64_t n, int64_t ld, int k, float* out_val,
+                       int32_t* out_idx, void* ws, size_t ws_bytes, fs_stream stream) {
+  return kselect_entry(rows, n_rows, n, ld, k, out_val, out_idx, ws, ws_bytes, stream, true);
 }
 
 int fs_kselect_host(const float* rows_host, int64_t n_rows, int64_t n, int64_t ld, int k,
@@ -301,7 +318,7 @@ int fs_kselect_host(const float* rows_host, int64_t n_rows, int64_t n, int64_t l
                             cudaMemcpyHostToDevice, st.s_in), "cudaMemcpyAsync H2D")) break;
     if (!ck(cudaEventRecord(st.ev_in[slice], st.s_in), "cudaEventRecord")) break;
     if (!ck(cudaStreamWaitEvent(st.s_run, st.ev_in[slice], 0), "cudaStreamWaitEvent")) break;
-    rc = fs::kselect_device(d_rows + r0 * ld, nr, n, ld, k, d_val + r0 * k, d_idx + r0 * k, base + o_ws, st.s_run);
+    rc = fs::kselect_device(d_rows + r0 * ld, nr, n, ld, k, d_val + r0 * k, d_idx + r0 * k, base + o_ws, st.s_run, false);
     if (rc != FS_OK) break;
     if (!ck(cudaEventRecord(st.ev_run[slice], st.s_run), "cudaEventRecord")) break;
     if (!ck(cudaStreamWaitEvent(st.s_out, st.ev_run[slice], 0), "cudaStreamWaitEvent")) break;

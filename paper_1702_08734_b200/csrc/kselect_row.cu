@@ -76,6 +76,7 @@ struct RowArgs {
   float* out_val;           // [n_rows][k]
   int32_t* out_idx;
   unsigned int* work;       // row counter of the persistent CTAs (zero before the launch)
+  int largest;              // 1: the k LARGEST ("other comparators"): the kernels select on -v
 };
 
 struct StageDesc {
@@ -124,6 +125,16 @@ __device__ __forceinline__ void mbar_wait_park(uint64_t* bar, uint32_t parity) {
   while (!mbar_test(bar, parity)) __nanosleep(FS_KROW_POLL_NS);
 }
 
+// The k-largest variant runs the same selection on the negated values (-v < -w <=> v > w; f32_ord folds
+// +-0 and NaN, so NaN still sorts last and ties still go to the lower index).  LG is the kernels'
+// compile-time switch for the streaming loads, sg the run-time sign mask of the rarely taken paths.
+template <bool LG> __device__ __forceinline__ float fl(float v) { return LG ? -v : v; }
+__device__ __forceinline__ float flip(float v, uint32_t sg) { return __uint_as_float(__float_as_uint(v) ^ sg); }
+template <bool LG> __device__ __forceinline__ float4 ldn4(const float4* p) {
+  const float4 x = *p;
+  return make_float4(fl<LG>(x.x), fl<LG>(x.y), fl<LG>(x.z), fl<LG>(x.w));
+}
+
 __device__ __forceinline__ void cbar() { asm volatile("bar.sync 1, %0;" ::"n"(RT) : "memory"); }
 
 // bucket of a key under the monotone map value -> [0, NBK): non-decreasing in the key for any lo, scale >= 0
@@ -155,7 +166,8 @@ __device__ __forceinline__ void emit_out(const RowCtx<CAPT>& c, int64_t row, int
   const uint32_t idx = key_idx(key), o = (uint32_t)(key >> 32);
   // the value is rebuilt from the order image except for the two images that are not injective
   // (+-0 and NaN), which are re-read from the row (original bits, A3)
-  const float v = (o == 0x80000000u || o == 0xFFFFFFFFu) ? a.orig[row * a.orig_ld + idx] : ord_f32(o);
+  const float v = (o == 0x80000000u || o == 0xFFFFFFFFu) ? a.orig[row * a.orig_ld + idx]
+                                                        : flip(ord_f32(o), a.largest ? 0x80000000u : 0u);
   a.out_val[row * a.k + r] = v;
   a.out_idx[row * a.k + r] = (int32_t)idx;
 }
@@ -327,7 +339,7 @@ __device__ void count_select(const RowCtx<CAPT>& c, int64_t row, int m, int want
   if (!RESTORE) {
     const RowArgs& a = *c.a;
     for (int r = want + tid; r < a.k; r += RT) {  // fewer than k elements: (+inf, -1) padding
-      a.out_val[row * a.k + r] = __uint_as_float(0x7F800000u);
+      a.out_val[row * a.k + r] = __uint_as_float(a.largest ? 0xFF800000u : 0x7F800000u);
       a.out_idx[row * a.k + r] = -1;
     }
   }
@@ -358,13 +370,14 @@ __device__ float refilter_row(const RowCtx<CAPT>& c, const float* src, int64_t l
   if (c.tid == 0) s->cnt = 0;
   cbar();
   const unsigned lt = (1u << c.lane) - 1u;
+  const uint32_t sg = c.a->largest ? 0x80000000u : 0u;
   const int64_t n32 = (len + 31) & ~(int64_t)31;
   for (int64_t e0 = (int64_t)c.warp * 32; e0 < n32; e0 += RT) {
     const int64_t e = e0 + c.lane;
     float v = 0.f;
     bool pass = false;
     if (e < len) {
-      v = src[e];
+      v = flip(src[e], sg);
       pass = !(v >= thr_x);
     }
     const unsigned b = __ballot_sync(kFull, pass);
@@ -387,6 +400,7 @@ __device__ void slow_row(const RowCtx<CAPT>& c, int64_t row, const float* src, i
   const RowArgs& a = *c.a;
   const int k = a.k;
   const int want_all = (int64_t)k < len ? k : (int)len;
+  const uint32_t sg = a.largest ? 0x80000000u : 0u;
   zero_hist<CAPT>(c);
   if (c.tid == 0) {
     s->cnt = 0;
@@ -402,7 +416,7 @@ __device__ void slow_row(const RowCtx<CAPT>& c, int64_t row, const float* src, i
     const int64_t e1 = e0 + chunk < len ? e0 + chunk : len;
     const unsigned long long thr = s->thr_key;
     for (int64_t e = e0 + c.tid; e < e1; e += RT) {
-      const uint64_t key = make_key(src[e], map ? map[e] : (uint32_t)e);
+      const uint64_t key = make_key(flip(src[e], sg), map ? map[e] : (uint32_t)e);
       if (key < thr) c.cand[atomicAdd(&s->cnt, 1)] = key;
     }
     cbar();
@@ -428,7 +442,7 @@ __device__ __forceinline__ float sample_target(float z, int k, int S, int64_t le
 
 // The scout warp's job for one row: a bound from the first S = 2 048 (or 1 024) elements of the row's
 // first stage, by a counting search over the sample (interpolation with a bisection safeguard).
-template <int CAPT>
+template <int CAPT, bool LG>
 __device__ __forceinline__ RowBound scout_bound(const float* st, int cnt, int64_t len, int k, int lane) {
   RowBound b;
   b.thr_x = __uint_as_float(0x7FFFFFFFu);
@@ -451,7 +465,7 @@ __device__ __forceinline__ RowBound scout_bound(const float* st, int cnt, int64_
   bool has_nan = false;
 #pragma unroll 4
   for (int j = 0; j < nq; ++j) {
-    const float4 x = s4[j * 32 + lane];
+    const float4 x = ldn4<LG>(s4 + j * 32 + lane);
     mn = fminf(fminf(mn, x.x), fminf(fminf(x.y, x.z), x.w));
     mx = fmaxf(fmaxf(mx, x.x), fmaxf(fmaxf(x.y, x.z), x.w));
     has_nan |= (x.x != x.x) | (x.y != x.y) | (x.z != x.z) | (x.w != x.w);
@@ -485,13 +499,13 @@ __device__ __forceinline__ RowBound scout_bound(const float* st, int cnt, int64_
     if (!snap) {
 #pragma unroll 4
       for (int j = 0; j < nq; ++j) {
-        const float4 x = s4[j * 32 + lane];
+        const float4 x = ldn4<LG>(s4 + j * 32 + lane);
         cme += (x.x <= tf) + (x.y <= tf) + (x.z <= tf) + (x.w <= tf);
       }
     } else {
 #pragma unroll 2
       for (int j = 0; j < nq; ++j) {
-        const float4 x = s4[j * 32 + lane];
+        const float4 x = ldn4<LG>(s4 + j * 32 + lane);
         const float e[4] = {x.x, x.y, x.z, x.w};
 #pragma unroll
         for (int t = 0; t < 4; ++t) {
@@ -530,7 +544,7 @@ __device__ __forceinline__ RowBound scout_bound(const float* st, int cnt, int64_
   return b;
 }
 
-template <int CAPT>
+template <int CAPT, bool LG>
 __global__ void __launch_bounds__(RTHREADS, RowCfg<CAPT>::CTAS) kselect_row_kernel(const RowArgs a) {
   constexpr int NST = RowCfg<CAPT>::NST, SEG = RowCfg<CAPT>::SEG, VPT = SEG / (4 * RT);  // float4 per thread and stage
   using SM = RowSmem<CAPT>;
@@ -624,7 +638,7 @@ __global__ void __launch_bounds__(RTHREADS, RowCfg<CAPT>::CTAS) kselect_row_kern
       const int64_t row = s->desc[slot].row;
       if (row < 0) break;
       if (s->desc[slot].seg == 0) {
-        const RowBound b = scout_bound<CAPT>(c.ring + (size_t)slot * SEG, s->desc[slot].cnt, s->desc[slot].len, a.k, c.lane);
+        const RowBound b = scout_bound<CAPT, LG>(c.ring + (size_t)slot * SEG, s->desc[slot].cnt, s->desc[slot].len, a.k, c.lane);
         if (c.lane == 0) s->bound[slot] = b;
       }
       __syncwarp();
@@ -672,7 +686,7 @@ __global__ void __launch_bounds__(RTHREADS, RowCfg<CAPT>::CTAS) kselect_row_kern
       const int64_t ntail = len - head - body;
       if (tid < head + ntail) {
         const int64_t e = tid < head ? tid : head + body + (tid - head);
-        const float v = p[e];
+        const float v = fl<LG>(p[e]);
         if (!(v >= bd.thr_x)) {
           const int pos = atomicAdd(&s->cnt, 1);
           if (pos < CAPT)
@@ -685,14 +699,20 @@ __global__ void __launch_bounds__(RTHREADS, RowCfg<CAPT>::CTAS) kselect_row_kern
     // ---- A1: first-level filter over this stage (4 VPT elements per thread) ----
     if (dcnt > 0) {
       const int nvec = dcnt >> 2;
-      const float thr_x = bd.thr_x;
+      const float thr_x = fl<LG>(bd.thr_x);  // -v < t  <=>  v > -t
       const uint32_t st_sa = ring_sa + (uint32_t)slot * (SEG * 4u) + (uint32_t)tid * 16u;
       float4 x[VPT];
       uint32_t mask = 0u;
       // pass = !(v >= bound) = "less than or unordered": one FSET and one LOP3 per element
-#define FS_TEST(V, BIT)                                                                                          \
-  asm("{\n\t.reg .b32 t;\n\tset.ltu.u32.f32 t, %1, %2;\n\tlop3.b32 %0, t, %3, %0, 0xEA;\n\t}" : "+r"(mask) : "f"(V), \
-      "f"(thr_x), "r"(BIT))
+#define FS_TEST(V, BIT)                                                                                            \
+  do {                                                                                                             \
+    if (LG)                                                                                                        \
+      asm("{\n\t.reg .b32 t;\n\tset.gtu.u32.f32 t, %1, %2;\n\tlop3.b32 %0, t, %3, %0, 0xEA;\n\t}" : "+r"(mask) : "f"(V), \
+          "f"(thr_x), "r"(BIT));                                                                                   \
+    else                                                                                                           \
+      asm("{\n\t.reg .b32 t;\n\tset.ltu.u32.f32 t, %1, %2;\n\tlop3.b32 %0, t, %3, %0, 0xEA;\n\t}" : "+r"(mask) : "f"(V), \
+          "f"(thr_x), "r"(BIT));                                                                                   \
+  } while (0)
       if (nvec == SEG / 4) {
 #pragma unroll
         for (int u = 0; u < VPT; ++u) {
@@ -751,6 +771,7 @@ __global__ void __launch_bounds__(RTHREADS, RowCfg<CAPT>::CTAS) kselect_row_kern
               const uint32_t off = (uint32_t)(j >> 2) * (RT * 4u) + (uint32_t)(j & 3);
               uint32_t bits;
               asm volatile("ld.shared.u32 %0, [%1];" : "=r"(bits) : "r"(st_sa + off * 4u));
+              if (LG) bits ^= 0x80000000u;
               asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(addr), "r"(bits), "r"(ib + off) : "memory");
               addr += 8u;
             }
@@ -760,7 +781,7 @@ __global__ void __launch_bounds__(RTHREADS, RowCfg<CAPT>::CTAS) kselect_row_kern
       "{\n\t.reg .pred p;\n\t.reg .b32 t;\n\tand.b32 t, %1, %2;\n\tsetp.ne.u32 p, t, 0;\n\t"                 \
       "@p st.shared.u32 [%0], %3;\n\t@p st.shared.u32 [%0+4], %4;\n\t@p add.u32 %0, %0, 8;\n\t}"                   \
       : "+r"(addr)                                                                                            \
-      : "r"(mask), "r"(1u << (4 * (U) + (E))), "r"(__float_as_uint(F)), "r"(ib + (uint32_t)((U)*RT * 4 + (E))) \
+      : "r"(mask), "r"(1u << (4 * (U) + (E))), "r"(__float_as_uint(fl<LG>(F))), "r"(ib + (uint32_t)((U)*RT * 4 + (E))) \
       : "memory")
 #pragma unroll
             for (int u = 0; u < VPT; ++u) {
@@ -817,6 +838,7 @@ constexpr int LS_PIECES = 64, LS_PIECE = 1024, LS_S = LS_PIECES * LS_PIECE;
 constexpr int LS_REG = 32;  // sample values per thread kept in registers; the rest in shared memory ([j][tid])
 constexpr size_t kSampleSmem = (size_t)(LS_PIECES - LS_REG) * LS_PIECE * sizeof(float);
 
+template <bool LG>
 __global__ void __launch_bounds__(1024) kselect_sample_kernel(const float* __restrict__ rows, int64_t n, int64_t ld,
                                                                int k, float* __restrict__ thr_out) {
   extern __shared__ __align__(16) float ls_x[];  // [LS_PIECES - LS_REG][1024]
@@ -827,12 +849,12 @@ __global__ void __launch_bounds__(1024) kselect_sample_kernel(const float* __res
   const int64_t stride = n / LS_PIECES;  // >= LS_PIECE: pieces do not overlap
   float x[LS_REG];
 #pragma unroll
-  for (int j = 0; j < LS_REG; ++j) x[j] = p[j * stride + tid];
+  for (int j = 0; j < LS_REG; ++j) x[j] = fl<LG>(p[j * stride + tid]);
   float mn = x[0], mx = x[0];
   bool has_nan = false;
 #pragma unroll 8
   for (int j = LS_REG; j < LS_PIECES; ++j) {
-    const float v = p[j * stride + tid];
+    const float v = fl<LG>(p[j * stride + tid]);
     ls_x[(j - LS_REG) * LS_PIECE + tid] = v;
     mn = fminf(mn, v);
     mx = fmaxf(mx, v);
@@ -908,6 +930,7 @@ __device__ __forceinline__ float4 ld_stream4(const float* p) {
 
 constexpr int LF_THREADS = 256, LF_UNROLL = 8;
 
+template <bool LG>
 __global__ void __launch_bounds__(LF_THREADS) kselect_filter_kernel(const float* __restrict__ rows, int64_t n, int64_t ld,
                                                                      const float* __restrict__ thr,
                                                                      float* __restrict__ cval, uint32_t* __restrict__ cidx,
@@ -918,7 +941,7 @@ __global__ void __launch_bounds__(LF_THREADS) kselect_filter_kernel(const float*
   float* cv = cval + row * cap;
   uint32_t* ci = cidx + row * cap;
   auto take = [&](float v, int64_t e) {
-    if (!(v >= thr_x)) {
+    if (!(fl<LG>(v) >= thr_x)) {
       const unsigned int pos = atomicAdd(count + row, 1u);
       if ((int64_t)pos < cap) {
         cv[pos] = v;
@@ -944,7 +967,8 @@ __global__ void __launch_bounds__(LF_THREADS) kselect_filter_kernel(const float*
         x[u] = __ldcs(reinterpret_cast<const float4*>(pv + ((v0 + u * LF_THREADS + threadIdx.x) << 2)));
 #pragma unroll
       for (int u = 0; u < LF_UNROLL; ++u) {
-        const bool any = !(x[u].x >= thr_x) | !(x[u].y >= thr_x) | !(x[u].z >= thr_x) | !(x[u].w >= thr_x);
+        const bool any = !(fl<LG>(x[u].x) >= thr_x) | !(fl<LG>(x[u].y) >= thr_x) | !(fl<LG>(x[u].z) >= thr_x) |
+                         !(fl<LG>(x[u].w) >= thr_x);
         if (any) {
           const int64_t e = head + ((v0 + u * LF_THREADS + threadIdx.x) << 2);
           take(x[u].x, e);
@@ -969,29 +993,38 @@ __global__ void __launch_bounds__(LF_THREADS) kselect_filter_kernel(const float*
   }
 }
 
-template <int CAPT>
+template <int CAPT, bool LG>
 int launch_rows_t(const RowArgs& a, cudaStream_t s) {
   using SM = RowSmem<CAPT>;
-  static int occ = 0;
-  if (occ == 0) {
-    FS_CUDA(cudaFuncSetAttribute(kselect_row_kernel<CAPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::total));
-    FS_CUDA(cudaFuncSetAttribute(kselect_row_kernel<CAPT>, cudaFuncAttributePreferredSharedMemoryCarveout,
+  static int occ_of[64] = {};  // per device: function attributes and occupancy belong to the device
+  int dev = 0;
+  FS_CUDA(cudaGetDevice(&dev));
+  const int slot = dev >= 0 && dev < 64 ? dev : 0;
+  int occ = occ_of[slot];
+  if (occ == 0 || slot != dev) {
+    FS_CUDA(cudaFuncSetAttribute(kselect_row_kernel<CAPT, LG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::total));
+    FS_CUDA(cudaFuncSetAttribute(kselect_row_kernel<CAPT, LG>, cudaFuncAttributePreferredSharedMemoryCarveout,
                                  cudaSharedmemCarveoutMaxShared));
     int o = 0;
-    FS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, kselect_row_kernel<CAPT>, RTHREADS, SM::total));
+    FS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, kselect_row_kernel<CAPT, LG>, RTHREADS, SM::total));
     occ = o > 0 ? o : 1;
+    occ_of[slot] = occ;
   }
   int64_t grid = (int64_t)sm_count() * occ;
   if (grid > a.n_rows) grid = a.n_rows;
-  kselect_row_kernel<CAPT><<<(unsigned)grid, RTHREADS, SM::total, s>>>(a);
+  kselect_row_kernel<CAPT, LG><<<(unsigned)grid, RTHREADS, SM::total, s>>>(a);
   FS_LAUNCHED();
   return FS_OK;
 }
 
 int launch_rows(const RowArgs& a, cudaStream_t s) {
   if (a.n_rows == 0) return FS_OK;
-  if (a.map) return launch_rows_t<4096>(a, s);  // one CTA per long row: room for a wide window
-  return a.k <= 256 ? launch_rows_t<1024>(a, s) : launch_rows_t<2048>(a, s);
+  if (a.largest) {
+    if (a.map) return launch_rows_t<4096, true>(a, s);
+    return a.k <= 256 ? launch_rows_t<1024, true>(a, s) : launch_rows_t<2048, true>(a, s);
+  }
+  if (a.map) return launch_rows_t<4096, false>(a, s);  // one CTA per long row: room for a wide window
+  return a.k <= 256 ? launch_rows_t<1024, false>(a, s) : launch_rows_t<2048, false>(a, s);
 }
 
 }  // namespace
@@ -1024,7 +1057,7 @@ size_t kselect_rows_ws_bytes(int64_t n_rows, int64_t n, int k) {
 
 // k >= 2.  ws: kselect_rows_ws_bytes.
 int kselect_rows_device(const float* rows, int64_t n_rows, int64_t n, int64_t ld, int k, float* out_val,
-                        int32_t* out_idx, void* ws, cudaStream_t s) {
+                        int32_t* out_idx, void* ws, cudaStream_t s, bool largest) {
   char* w = static_cast<char*>(ws);
   RowArgs a;
   a.vals = rows;
@@ -1041,6 +1074,7 @@ int kselect_rows_device(const float* rows, int64_t n_rows, int64_t n, int64_t ld
   a.out_val = out_val;
   a.out_idx = out_idx;
   a.work = reinterpret_cast<unsigned int*>(w);
+  a.largest = largest ? 1 : 0;
   if (!kselect_use_long(n_rows, n, k)) {
     FS_CUDA(cudaMemsetAsync(w, 0, 256, s));
     return launch_rows(a, s);
@@ -1056,18 +1090,16 @@ int kselect_rows_device(const float* rows, int64_t n_rows, int64_t n, int64_t ld
   uint32_t* cidx = reinterpret_cast<uint32_t*>(w + o);
   FS_CUDA(cudaMemsetAsync(w, 0, 256 + align_up((size_t)n_rows * sizeof(float), 256) +
                                     align_up((size_t)n_rows * sizeof(unsigned int), 256), s));
-  static bool sample_attr = false;
-  if (!sample_attr) {
-    FS_CUDA(cudaFuncSetAttribute(kselect_sample_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSampleSmem));
-    sample_attr = true;
-  }
-  kselect_sample_kernel<<<(unsigned)n_rows, 1024, kSampleSmem, s>>>(rows, n, ld, k, thr);
+  auto* sample = largest ? kselect_sample_kernel<true> : kselect_sample_kernel<false>;
+  FS_CUDA(cudaFuncSetAttribute(sample, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSampleSmem));  // per device
+  sample<<<(unsigned)n_rows, 1024, kSampleSmem, s>>>(rows, n, ld, k, thr);
   FS_LAUNCHED();
   int64_t gx = (int64_t)sm_count() * 8 / n_rows;
   const int64_t maxg = ceil_div(n / 4, (int64_t)LF_THREADS * LF_UNROLL);
   if (gx > maxg) gx = maxg;
   if (gx < 1) gx = 1;
-  kselect_filter_kernel<<<dim3((unsigned)gx, (unsigned)n_rows), LF_THREADS, 0, s>>>(rows, n, ld, thr, cval, cidx, count, cap);
+  auto* filter = largest ? kselect_filter_kernel<true> : kselect_filter_kernel<false>;
+  filter<<<dim3((unsigned)gx, (unsigned)n_rows), LF_THREADS, 0, s>>>(rows, n, ld, thr, cval, cidx, count, cap);
   FS_LAUNCHED();
   a.vals = cval;
   a.ld = cap;

@@ -108,3 +108,27 @@ def test_host_entry_point():
     gd, gi = fs.flat_l2_knn_host(xq, xb, 10)
     od, oi = oracle.flat_l2_knn(xq, xb, 10)
     assert np.array_equal(gi, oi) and np.array_equal(gd, od)
+
+
+def test_mma_ignores_low_mantissa_bits():
+    """The tensor-core engine reads the caller's fp32 arrays as the TF32 hi plane (DESIGN 5.2): tcgen05.mma
+    kind::tf32 must ignore the 13 low mantissa bits.  FS_TC_PLANES=1 makes the library feed explicitly
+    truncated copies instead; both runs must agree bit for bit on real-valued data."""
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    code = (
+        "import sys, numpy as np, torch; sys.path.insert(0, %r)\n"
+        "import paper_1702_08734_b200 as fs\n"
+        "from datagen import gen_torch as gt\n"
+        "d, i = fs.flat_l2_knn(gt.gaussian_vectors(50000, 300, 128), gt.gaussian_vectors(0, 50000, 128), 10)\n"
+        "torch.cuda.synchronize()\n"
+        "sys.stdout.write(d.cpu().numpy().tobytes().hex() + i.cpu().numpy().tobytes().hex())\n" % root)
+    outs = []
+    for planes in ("0", "1"):
+        env = dict(os.environ, FS_TC_PLANES=planes)
+        r = subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, timeout=600)
+        assert r.returncode == 0, r.stderr[-2000:]
+        outs.append(r.stdout)
+    assert outs[0] == outs[1] and len(outs[0]) > 0

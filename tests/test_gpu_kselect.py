@@ -125,6 +125,52 @@ def test_batch_rows_that_mislead_the_sample(k):
     assert_exact(rows, k)
 
 
+def assert_exact_largest(rows_np, k, n=None):
+    import paper_1702_08734_b200 as fs
+    ev, ei = oracle.kselect(rows_np, k, n=n, largest=True)
+    gv, gi = fs.kselect(torch.from_numpy(rows_np).cuda(), k, n=n, largest=True)
+    torch.cuda.synchronize()
+    gv, gi = gv.cpu().numpy(), gi.cpu().numpy()
+    bad = np.nonzero((gi != ei).any(1) | (gv.view(np.uint32) != ev.view(np.uint32)).any(1))[0]
+    assert bad.size == 0, "rows %s differ (largest, k=%d); first: got %s want %s" % (
+        bad[:5], k, gi[bad[0]][:8], ei[bad[0]][:8])
+
+
+@pytest.mark.parametrize("k", [1, 2, 32, 100, 256, 257, 1024])
+def test_largest_variant(k):
+    """fs_kselect_largest ("other comparators") on every path of the selection: batch rows of cfg2's
+    shape with duplicated runs, ragged short rows with padding, special values, rows that mislead the
+    sample (second filter pass / slow path), and long rows (A4)."""
+    dup, _ = datagen.kselect_dup_rows(0, 10000)
+    sel = list(np.nonzero(dup)[0][:4]) + [0, 1]
+    assert_exact_largest(np.concatenate([datagen.kselect_rows(int(r), 1, 16384) for r in sel]), k)
+    assert_exact_largest(datagen.kselect_rows(3, 21, 2003, duplicates=False), k)
+    rng = np.random.default_rng(k)
+    small = rng.integers(-3, 4, size=(5, 40)).astype(np.float32)
+    for n in (0, 1, 5, 40):
+        assert_exact_largest(small, k, n=n)
+    sp = rng.standard_normal((6, 700)).astype(np.float32)
+    sp[0, ::3] = 0.0
+    sp[0, 1::3] = -0.0
+    sp[1, ::5] = np.inf
+    sp[2, ::4] = -np.inf
+    sp[3, :] = -np.inf
+    sp[4, 10:20] = np.nan
+    sp[5, :] = np.nan
+    assert_exact_largest(sp, k)
+    n = 16384
+    asc = np.sort(rng.random(n, dtype=np.float32))
+    late = rng.random(n, dtype=np.float32)
+    late[-3000:] += 1.0
+    few = rng.integers(0, 3, n).astype(np.float32)
+    rows = np.stack([asc, asc[::-1].copy(), late, few, np.zeros(n, np.float32)])
+    assert_exact_largest(np.concatenate([rows, datagen.kselect_rows(9, 300, n, duplicates=False)[:, :n]]), k)
+    n = 1 << 19
+    a = np.arange(n, dtype=np.float32)
+    lr = datagen.kselect_rows(77, 2, n, duplicates=False)
+    assert_exact_largest(np.concatenate([lr, np.stack([a, a[::-1].copy(), (np.arange(n) % 5).astype(np.float32)])]), k)
+
+
 def test_host_entry_point_and_errors():
     import paper_1702_08734_b200 as fs
     rows = datagen.kselect_rows(7, 5, 3000)

@@ -113,3 +113,34 @@ def test_survey_derived_counts():
     H = np.cumsum(1.0 / np.arange(1, 16385))
     got = [k + k * (H[-1] - H[k - 1]) for k in (1, 32, 128, 1024)]
     assert [round(x) for x in got] == [10, 231, 749, 3863]
+
+
+def test_largest_handworked_and_bruteforce():
+    """The k-largest variant ("other comparators"): hand-worked example, numpy's stable sort of the
+    negated row, special values (NaN last, -0 == +0, ties to the lower index), padding (-inf, -1)."""
+    g = load("kselect_handworked.txt")
+    row = g["row"].astype(np.float32)[None, :]
+    v, i = oracle.kselect(row, 3, largest=True)
+    assert v[0].tolist() == g["top3_val"].tolist() and i[0].tolist() == g["top3_idx"].tolist()
+    v, i = oracle.kselect(row, 8, largest=True)
+    assert i[0].tolist() == g["top8_idx"].tolist()
+    rng = np.random.default_rng(19)
+    for n in (1, 3, 17, 64, 200):
+        rows = rng.integers(-5, 6, size=(10, n)).astype(np.float32) / 4.0
+        for k in sorted({1, min(2, n), n // 2 + 1, n}):
+            v, i = oracle.kselect(rows, k, largest=True)
+            for r in range(rows.shape[0]):
+                order = np.argsort(-rows[r], kind="stable")  # descending value, ties by lower index
+                assert i[r].tolist() == order[:k].tolist()
+                assert v[r].tolist() == rows[r][order[:k]].tolist()
+    row = np.array([[0.0, -0.0, np.inf, -np.inf, np.nan, 1.0, -0.0, np.inf]], np.float32)
+    v, i = oracle.kselect(row, 8, largest=True)
+    assert i[0].tolist() == [2, 7, 5, 0, 1, 6, 3, 4]
+    assert np.isnan(v[0, 7]) and np.signbit(v[0, 4]) and not np.signbit(v[0, 3])
+    v, i = oracle.kselect(np.array([[2.0, 3.0]], np.float32), 4, largest=True)
+    assert i[0].tolist() == [1, 0, -1, -1] and np.all(np.isneginf(v[0, 2:]))
+    # smallest of the negated row selects the same indices
+    rows = rng.standard_normal((4, 500)).astype(np.float32)
+    _, a = oracle.kselect(rows, 40, largest=True)
+    _, b = oracle.kselect(-rows, 40)
+    assert np.array_equal(a, b)
