@@ -267,11 +267,13 @@ def also_flat(fs, gt, pk, cpu=True):
     return out
 
 
-def also_ivfpq(fs, gt, pk, cfg, nb=None, cpu=True):
+def also_ivfpq(fs, gt, pk, cfg, nb=None, cpu=True, graph=False):
     """fs_ivfpq_search on BASELINE.json configs[3] (cfg 4) / configs[4] (cfg 5): build the index, time
     every (nprobe, k), report the whole search and the scan stage (C2-C4: tables + list scan + pass-1
     selection, events inside the library) on code bytes, and time the oracle on the seeded query
-    subset over the GPU-built lists those queries probed (cpu_baseline, with the parity it shows)."""
+    subset over the GPU-built lists those queries probed (cpu_baseline, with the parity it shows).
+    graph: also the all-vs-all 10-NN graph of the stored vectors (f4, section 6.5) with the
+    collection resident in HBM: build (train + add) and fs_ivfpq_knn_graph timed end to end."""
     import math
     import numpy as np
     import torch
@@ -284,22 +286,31 @@ def also_ivfpq(fs, gt, pk, cfg, nb=None, cpu=True):
         c["ntrain"] = min(nb, max(256, min(c["ntrain"], 16 * c["nlist"])))
         c["nb"] = nb
     nb, d, nlist, M, nq = c["nb"], c["d"], c["nlist"], c["M"], c["nq"]
+    chunk = 1 << 22
+    xall = None
+    if graph:  # the collection stays in HBM (38.4 GB at 10^8 x 96): generated before anything is timed
+        xall = torch.empty((nb, d), dtype=torch.float32, device="cuda")
+        for b in range(0, nb, chunk):
+            xall[b:b + chunk] = gt.deep_like(b, min(chunk, nb - b))
+    xtrain = xall[:c["ntrain"]] if graph else gt.deep_like(0, c["ntrain"])
+    torch.cuda.synchronize()
     t0 = time.perf_counter()
     ix = fs.IvfPq(d, nlist, M)
-    ix.train(gt.deep_like(0, c["ntrain"]), niter=10, seed=0)
+    ix.train(xtrain, niter=10, seed=0)
     torch.cuda.synchronize()
     t_train = time.perf_counter() - t0
+    del xtrain
     t0 = time.perf_counter()
-    chunk = 1 << 22
     for b in range(0, nb, chunk):
-        ix.add(gt.deep_like(b, min(chunk, nb - b)))
+        ix.add(xall[b:b + chunk] if graph else gt.deep_like(b, min(chunk, nb - b)))
     xq = gt.deep_like(nb, nq)
     ix.search(xq[:8], 1, 1)  # finalise the lists
     torch.cuda.synchronize()
     t_add = time.perf_counter() - t0
     out = {"workload": "cfg%d%s: nb=%d deep-like d=96, nlist=%d, M=%d, nq=%d"
                        % (cfg, "" if full else "-shaped, REDUCED", nb, nlist, M, nq),
-           "train_s": t_train, "add_s": t_add, "add_vectors_per_s": nb / t_add}
+           "train_s": t_train, "add_s": t_add, "add_vectors_per_s": nb / t_add,
+           "add_s_includes_input_generation": not graph}
     smem_lookups_peak = 148 * 32 * pk["sm_max_mhz"] * 1e6
     sub = datagen.unique_sample_ids(min(c["check_queries"], nq), nq, stream=10 * cfg + 6)
     st = torch.from_numpy(sub).cuda()
@@ -359,8 +370,79 @@ def also_ivfpq(fs, gt, pk, cfg, nb=None, cpu=True):
                                   "queries_identical_frac": float((gi == o["ids"]).all(1).mean()),
                                   "max_rel_dist_err": float(rel.max()) if rel.size else 0.0,
                                   "within_1e-3": bool(rel.size == 0 or rel.max() <= 1e-3)}}
+    if graph:
+        out["knn_graph"] = knn_graph_leg(fs, ix, xall, c, cfg, t_train, t_add, cpu)
     ix.close()
     return out
+
+
+def knn_graph_leg(fs, ix, xall, c, cfg, t_train, t_add, cpu):
+    """All-vs-all 10-NN graph (f4): every stored vector is a query (fs_ivfpq_knn_graph, nprobe 16, k 10).
+    Checked on a seeded subset of rows against the oracle over the GPU-built lists those rows probe, and
+    against the exact 10-NN of those rows (fs_flat_l2_knn over the whole collection) for the graph's
+    accuracy on this synthetic set (the quantity of Fig. 5; not the paper's datasets)."""
+    import numpy as np
+    import torch
+    import datagen
+    nb, d, nlist = c["nb"], c["d"], c["nlist"]
+    nprobe, k = 16, 10
+    gd = torch.empty((nb, k), dtype=torch.float32, device="cuda")
+    gi = torch.empty((nb, k), dtype=torch.int64, device="cuda")
+    warm = min(nb, 65536)
+    ix.knn_graph(xall[:warm], nprobe, k, out_dist=gd[:warm], out_ids=gi[:warm])
+    torch.cuda.synchronize()
+    a, b = event_pair()
+    a.record()
+    ix.knn_graph(xall, nprobe, k, out_dist=gd, out_ids=gi)
+    b.record()
+    torch.cuda.synchronize()
+    t_graph = a.elapsed_time(b) / 1e3
+    res = {"workload": "all-vs-all: the %d stored vectors as queries, nprobe=%d, k=%d, batches of 65536" % (nb, nprobe, k),
+           "graph_search_s": t_graph, "rows_per_s": nb / t_graph, "train_s": t_train, "add_s": t_add,
+           "build_plus_search_s": t_train + t_add + t_graph,
+           "edges": nb * k, "self_in_own_row_frac": None}
+    nsub = min(c["check_queries"], nb)
+    sub = datagen.unique_sample_ids(nsub, nb, stream=10 * cfg + 8)
+    st = torch.from_numpy(sub).cuda()
+    res["self_in_own_row_frac"] = float((gi[st] == st[:, None]).any(1).float().mean().item())
+    try:  # accuracy of the graph rows against the exact neighbours
+        xs_d = xall[st].contiguous()
+        ed, ei = fs.flat_l2_knn(xs_d, xall, k)
+        hit = (gi[st][:, :, None] == ei[:, None, :]).any(2).float().sum(1)
+        res["accuracy_vs_exact_10nn"] = {"rows": int(nsub), "mean_fraction_found": float(hit.mean().item() / k),
+                                         "note": "synthetic deep-like set; exact side = fs_flat_l2_knn over all vectors"}
+        del ed, ei
+    except Exception as e:
+        res["accuracy_vs_exact_10nn"] = {"error": repr(e)}
+    if cpu:
+        import oracle
+        sd, si, sp = ix.knn_graph(xall[st].contiguous(), nprobe, k, want_probed=True)
+        torch.cuda.synchronize()
+        big_d, big_i = gd[st].cpu().numpy(), gi[st].cpu().numpy()
+        sp = sp.cpu().numpy()
+        coarse, pq = (t.cpu().numpy() for t in ix.get_quantizers())
+        lists = np.unique(sp.reshape(-1))
+        so, sc, sids = ix.export_lists(lists)
+        offs = np.zeros(nlist + 1, np.int64)
+        lens = np.zeros(nlist, np.int64)
+        lens[lists] = np.diff(so)
+        np.cumsum(lens, out=offs[1:])
+        xs = xall[st].cpu().numpy()
+        t0 = time.perf_counter()
+        o = oracle.ivfpq_search(coarse, pq, offs, sc.cpu().numpy(), sids.cpu().numpy(), xs, nprobe, k, probed_in=sp)
+        dt = time.perf_counter() - t0
+        fin = np.isfinite(o["dist64"]) & (big_i >= 0)
+        rel = np.abs(big_d[fin] - o["dist64"][fin]) / np.maximum(o["dist64"][fin], 1e-30)
+        res["cpu_baseline"] = {
+            "value": nsub / dt, "unit": "rows/s", "cores": oracle.num_threads(), "kind": "oracle", "seconds": dt,
+            "sample": "oracle.ivfpq_search on a seeded %d-row subset of the graph over the GPU-built lists those rows "
+                      "probed (probed lists from a second run of the same rows); compared with the rows of the "
+                      "full all-vs-all output" % nsub,
+            "gpu_vs_oracle": {"ids_equal_frac": float((big_i == o["ids"]).mean()),
+                              "rows_identical_frac": float((big_i == o["ids"]).all(1).mean()),
+                              "max_rel_dist_err": float(rel.max()) if rel.size else 0.0,
+                              "within_1e-3": bool(rel.size == 0 or rel.max() <= 1e-3)}}
+    return res
 
 
 def run_shard(args):
@@ -446,11 +528,12 @@ def run_ours(args):
     fs.lib()  # fail loudly if libfs.so is missing
     pk = peaks()
 
-    if args.case in ("flat", "ivfpq", "ivfpq5"):  # profiling aid: only that "also" leg
+    if args.case in ("flat", "ivfpq", "ivfpq5", "graph"):  # profiling aid: only that "also" leg
         if args.case == "flat":
             out = also_flat(fs, gt, pk, cpu=not args.no_cpu)
         else:
-            out = also_ivfpq(fs, gt, pk, 5 if args.case == "ivfpq5" else 4, args.ivfpq_nb, cpu=not args.no_cpu)
+            out = also_ivfpq(fs, gt, pk, 5 if args.case == "ivfpq5" else 4, args.ivfpq_nb, cpu=not args.no_cpu,
+                             graph=args.case == "graph")
         print(json.dumps({"case": args.case, **out}))
         return
 
@@ -581,7 +664,8 @@ def run_ours(args):
             torch.cuda.empty_cache()
             also = {}
             for name, fn in (("flat_l2_knn", lambda: also_flat(fs, gt, pk, cpu=not args.no_cpu)),
-                             ("ivfpq_search_cfg4", lambda: also_ivfpq(fs, gt, pk, 4, args.ivfpq_nb, cpu=not args.no_cpu)),
+                             ("ivfpq_search_cfg4", lambda: also_ivfpq(fs, gt, pk, 4, args.ivfpq_nb, cpu=not args.no_cpu,
+                                                                  graph=not args.skip_graph)),
                              ("ivfpq_search_cfg5", lambda: also_ivfpq(fs, gt, pk, 5, None, cpu=not args.no_cpu))):
                 if name == "ivfpq_search_cfg5" and args.skip_cfg5:
                     continue
@@ -637,8 +721,9 @@ def main():
     ap.add_argument("--ivfpq-nb", type=int, default=None,
                     help="cfg4 leg with fewer vectors (profiling aid; default: BASELINE.json's 10^8)")
     ap.add_argument("--skip-cfg5", action="store_true", help="leave out the 10^9-vector leg (about 5 min of index build)")
+    ap.add_argument("--skip-graph", action="store_true", help="leave out the all-vs-all 10-NN graph of the cfg4 leg (about 1 min)")
     ap.add_argument("--no-cpu", action="store_true", help="leave out the oracle timings of the flat / IVFPQ legs")
-    ap.add_argument("--case", default="", help="comma list of k1,k32,k128,k1024,bigrow_k1024 (time only these calls), or flat / ivfpq (only that leg)")
+    ap.add_argument("--case", default="", help="comma list of k1,k32,k128,k1024,bigrow_k1024 (time only these calls), or flat / ivfpq / ivfpq5 / graph (only that leg)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -171,10 +171,11 @@ FS_API int fs_kmeans(const float* x, int64_t n, int d, int K, int niter, uint64_
 FS_API int fs_ivfpq_add(fs_ivfpq* index, const float* xb, int64_t n, const int64_t* ids,
                  fs_stream stream);
 
-/* Search (C1-C5, Alg. 4): coarse top-nprobe (Eq. 5), per-(query,
- * list) lookup tables in shared memory (Eq. 10), inverted-list code
- * scan with fused pass-1 selection, pass-2 merge to k and id
- * resolution for the winners only.
+/* Search (C1-C5, Alg. 4): coarse top-nprobe (Eq. 5); the ADC distance (Eq. 7) in the
+ * decomposition of Eq. 11: term 1 was stored per vector at add time, term 2 = ||x - c_L||^2 is
+ * one number per probed list, term 3 comes from ONE table per query (no per-list tables); inverted-list
+ * code scan with fused pass-1 selection, pass-2 merge to k and id resolution for the winners
+ * only.  Distances agree with Eq. 7 evaluated in double to ~1e-6 relative.
  *   xq device fp32 [nq][d]; 1 <= nprobe <= min(nlist, 1024); 1 <= k <= FS_MAX_K
  *   out_dist device fp32 [nq][k] (squared ADC distance), out_ids device int64 [nq][k]
  *   out_probed device int32 [nq][nprobe] ascending coarse distance, or NULL. */
@@ -185,6 +186,16 @@ FS_API size_t fs_ivfpq_search_ws_bytes(const fs_ivfpq* index, int64_t nq, int np
 FS_API int fs_ivfpq_search_host(fs_ivfpq* index, const float* xq_host, int64_t nq, int nprobe, int k,
                          float* out_dist_host, int64_t* out_ids_host);
 
+/* All-vs-all k-NN graph (section 6.5: "the k-NN graph ... every vector of the collection is a
+ * query"): row i of the output is fs_ivfpq_search's answer for query x_i, computed in batches of `batch`
+ * queries (0: 65 536) with one workspace, all on `stream`.  x are normally the vectors the index holds;
+ * nothing is special-cased for them: x_i's own id is returned like any other neighbour when its
+ * quantised image is among the k nearest (P:L441 does not exclude it either).
+ *   x device fp32 [n][d]; out_dist device fp32 [n][k]; out_ids device int64 [n][k];
+ *   out_probed device int32 [n][nprobe] or NULL.  Arguments checked as in fs_ivfpq_search. */
+FS_API int fs_ivfpq_knn_graph(fs_ivfpq* index, const float* x, int64_t n, int nprobe, int k, int64_t batch,
+                       float* out_dist, int64_t* out_ids, int32_t* out_probed, fs_stream stream);
+
 FS_API int64_t fs_ivfpq_ntotal(const fs_ivfpq* index);
 /* Total code bytes the probed lists of the last fs_ivfpq_search held
  * (sum over (query, list) pairs of len * M): the scan's algorithmic bytes. */
@@ -194,7 +205,10 @@ FS_API int64_t fs_ivfpq_last_scanned_codes(const fs_ivfpq* index);
  * selection: the stage the scan roofline is quoted on), ms[2] = C5 merge + ids.  HOST float
  * [3]; waits for that search to finish. */
 FS_API int fs_ivfpq_last_stage_ms(const fs_ivfpq* index, float* ms);
-/* Read-only device views of one list, valid until the next add/destroy. */
+/* Read-only device views of one list, valid until the next add/destroy.  For M = 8 and 16 the scan's
+ * storage order is what the view shows: byte i of the vector at list position p holds the index of
+ * sub-quantizer i ^ (p mod M) (bank-conflict-free table reads); fs_ivfpq_export and
+ * fs_ivfpq_export_lists return the codes in the paper's order (byte m = sub-quantizer m). */
 FS_API int fs_ivfpq_list(const fs_ivfpq* index, int list_no, const uint8_t** codes, const int64_t** ids,
                   int64_t* len);
 /* The whole inverted file in CSR form, copied to caller buffers (device):

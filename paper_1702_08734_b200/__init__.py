@@ -300,6 +300,22 @@ class IvfPq:
                                      _stream()))
         return (out_dist, out_ids, probed) if want_probed else (out_dist, out_ids)
 
+    def knn_graph(self, x: torch.Tensor, nprobe: int, k: int, batch: int = 0, want_probed: bool = False,
+                  out_dist=None, out_ids=None):
+        """fs_ivfpq_knn_graph: all-vs-all search, row i = the k nearest stored vectors of x[i]."""
+        _dev(x, torch.float32, "x")
+        n = x.shape[0]
+        if out_dist is None:
+            out_dist = torch.empty((n, k), dtype=torch.float32, device=x.device)
+        if out_ids is None:
+            out_ids = torch.empty((n, k), dtype=torch.int64, device=x.device)
+        _dev(out_dist, torch.float32, "out_dist")
+        _dev(out_ids, torch.int64, "out_ids")
+        probed = torch.empty((n, nprobe), dtype=torch.int32, device=x.device) if want_probed else None
+        _check(lib().fs_ivfpq_knn_graph(self._h, _ptr(x), _i64(n), _int(nprobe), _int(k), _i64(batch),
+                                        _ptr(out_dist), _ptr(out_ids), _ptr(probed), _stream()))
+        return (out_dist, out_ids, probed) if want_probed else (out_dist, out_ids)
+
     def search_host(self, xq, nprobe: int, k: int, out_dist=None, out_ids=None):
         import numpy as np
         xq, qp = _host_ptr(xq, np.float32, torch.float32, "xq")

@@ -801,6 +801,39 @@ int fs_ivfpq_search(fs_ivfpq* ix, const float* xq, int64_t nq, int nprobe, int k
   return fs::ivfpq_search_device(ix, xq, nq, nprobe, k, out_dist, out_ids, out_probed, t.ptr, s);
 }
 
+int fs_ivfpq_knn_graph(fs_ivfpq* ix, const float* x, int64_t n, int nprobe, int k, int64_t batch,
+                       float* out_dist, int64_t* out_ids, int32_t* out_probed, fs_stream stream) {
+  if (!ix) return fs::set_error(FS_EINVAL, "fs_ivfpq_knn_graph: NULL index");
+  if (n < 0 || batch < 0 || (n > 0 && (!x || !out_dist || !out_ids)))
+    return fs::set_error(FS_EINVAL, "fs_ivfpq_knn_graph: bad arguments");
+  if (k < 1 || k > FS_MAX_K) return fs::set_error(FS_EINVAL, "fs_ivfpq_knn_graph: k must be in 1..%d", FS_MAX_K);
+  if (nprobe < 1 || nprobe > ix->nlist || nprobe > 1024)
+    return fs::set_error(FS_EINVAL, "fs_ivfpq_knn_graph: nprobe = %d outside 1..min(nlist, 1024)", nprobe);
+  if (!ix->have_quantizers) return fs::set_error(FS_ESTATE, "fs_ivfpq_knn_graph: no quantizers set or trained");
+  if (n == 0) return FS_OK;
+  if (batch == 0) batch = 65536;
+  if (batch > n) batch = n;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  int rc = fs::ivfpq_finalise(ix, s);
+  if (rc != FS_OK) return rc;
+  // one workspace for every batch (the tail batch needs no more than a full one)
+  fs::TempWs t;
+  size_t need = fs::ivfpq_search_ws(ix, batch, nprobe, k);
+  const int64_t tail = n % batch;
+  if (tail) {
+    const size_t nt = fs::ivfpq_search_ws(ix, tail, nprobe, k);
+    need = nt > need ? nt : need;
+  }
+  if ((rc = t.acquire(nullptr, 0, need, s)) != FS_OK) return rc;
+  for (int64_t b = 0; b < n; b += batch) {
+    const int64_t nq = n - b < batch ? n - b : batch;
+    rc = fs::ivfpq_search_device(ix, x + b * ix->d, nq, nprobe, k, out_dist + b * k, out_ids + b * k,
+                                 out_probed ? out_probed + b * nprobe : nullptr, t.ptr, s);
+    if (rc != FS_OK) return rc;
+  }
+  return FS_OK;
+}
+
 int fs_ivfpq_search_host(fs_ivfpq* ix, const float* xq_host, int64_t nq, int nprobe, int k,
                          float* out_dist_host, int64_t* out_ids_host) {
   if (!ix || nq < 0 || (nq > 0 && (!xq_host || !out_dist_host || !out_ids_host)))
