@@ -1,10 +1,13 @@
 // ivfpq_search.cu -- fs_ivfpq_search: Alg. 4, SURVEY 8a rows C1-C5.
 //
 //   C1 coarse quantizer  L_IVF = tau-argmin_c ||x - c||^2 (Eq. 5): the exact-search engine over
-//                        the centroids with k = nprobe; its distances are term 2 of Eq. 11 (P:L308:
-//                        "a by-product of the first-level quantizer")
+//                        the centroids with k = nprobe (P:L308 takes term 2 of Eq. 11 from here, "a
+//                        by-product of the first-level quantizer"; this scan recomputes it, see C2)
 //   C2 lookup tables     Eq. 11 pushed one step further than the paper's table layout:
-//                        ||x - q1(y) - q2(y)||^2 = ||x - q1||^2            term 2: C1's distance, per (query, list)
+//                        ||x - q1(y) - q2(y)||^2 = ||x - q1||^2            term 2: per (query, list), recomputed by the
+//                                                                          scan in the direct form sum (x - c)^2
+//                                                                          (C1's Eq. 2 value loses ~1e-5 relative
+//                                                                          to cancellation; 96 flops per list)
 //                                               + ||q2||^2 + 2 <q1, q2>    term 1: per STORED VECTOR, computed when
 //                                                                          it is added (ivfpq.cu, fs_ivfpq::s1)
 //                                               - 2 <x, q2>                term 3: sum_m T_m[code_m],
