@@ -601,7 +601,7 @@ def run_ours(args):
     call_bytes = {n: b for n, _, b in calls}
     dom = max(call_ms, key=call_ms.get)
     ach = call_bytes[dom] / call_ms[dom] / 1e6
-    roofline = {"bound": "hbm", "kernel": "kselect_stream_kernel (%s call)" % dom, "achieved": ach,
+    roofline = {"bound": "hbm", "kernel": "%s (%s call)" % ("kselect_k1_kernel" if dom == "k1" else "kselect_row_kernel", dom), "achieved": ach,
                 "peak": pk["hbm"], "unit": "GB/s", "frac": ach / pk["hbm"], "traffic": None,
                 "peak_source": pk["source"] + ", burst copy figure",
                 "per_call": {n: {"ms": call_ms[n], "GBps": call_bytes[n] / call_ms[n] / 1e6,

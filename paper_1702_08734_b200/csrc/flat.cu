@@ -237,12 +237,14 @@ __global__ void __launch_bounds__(128) flat_finish_kernel(const uint64_t* __rest
                                                           int64_t nq, int S, int k,
                                                           const float* __restrict__ xnorm,
                                                           float* __restrict__ out_dist,
-                                                          int64_t* __restrict__ out_ids) {
+                                                          int64_t* __restrict__ out_ids, const FinishExtra ex) {
   extern __shared__ __align__(16) uint64_t smem_keys[];
   constexpr int NB = NQ < 4 ? NQ : 4;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int64_t q = (int64_t)blockIdx.x * 4 + warp;
+  if (ex.nq_dev) nq = (int64_t)*ex.nq_dev < nq ? (int64_t)*ex.nq_dev : nq;
   if (q >= nq) return;
+  const int64_t oq = ex.qmap ? (int64_t)ex.qmap[q] : q;  // the query this row belongs to
   constexpr int K = 32 * NQ;
   WarpSelect<NQ, NB> sel;
   sel.init(smem_keys + warp * warp_select_smem_keys<NB>(), lane);
@@ -257,11 +259,25 @@ __global__ void __launch_bounds__(128) flat_finish_kernel(const uint64_t* __rest
     }
     sel.finish();
   }
+  if (ex.bound_out) {  // the sample pass: only the k-th smallest d' is wanted, as a bound
+    sort_blocked<NQ>(sel.W, lane);
+#pragma unroll
+    for (int r = 0; r < NQ; ++r)
+      if (lane * NQ + r == k - 1) ex.bound_out[oq] = (unsigned int)(sel.W[r] >> 32);
+    return;
+  }
+  if (ex.fail_cnt) {  // fewer keys than the query must have: its sampled bound was too tight
+    int have = 0;
+#pragma unroll
+    for (int r = 0; r < NQ; ++r) have += sel.W[r] != kSentinelKey;
+    have = __reduce_add_sync(kFull, have);
+    if (have < ex.need && lane == 0) ex.fail_q[atomicAdd(ex.fail_cnt, 1u)] = (int)q;
+  }
   // Final value = d' + ||x||^2, clamped at 0.  Rounding (and the clamp) can make
   // distinct d' equal, so order again on the final (value, id) keys: ascending,
   // ties by lower id.  The lane-stride registers are read as a blocked array
   // (any bijection is fine before a full sort); sorted element e = lane*NQ + r.
-  const float xn = xnorm ? xnorm[q] : 0.f;
+  const float xn = xnorm ? xnorm[oq] : 0.f;
 #pragma unroll
   for (int r = 0; r < NQ; ++r) {
     const uint64_t key = sel.W[r];
@@ -277,11 +293,11 @@ __global__ void __launch_bounds__(128) flat_finish_kernel(const uint64_t* __rest
     if (i < k) {
       const uint64_t key = sel.W[r];
       if (key == kSentinelKey) {
-        out_dist[q * k + i] = __uint_as_float(0x7F800000u);
-        out_ids[q * k + i] = -1;
+        out_dist[oq * k + i] = __uint_as_float(0x7F800000u);
+        out_ids[oq * k + i] = -1;
       } else {
-        out_dist[q * k + i] = key_val(key);
-        out_ids[q * k + i] = (int64_t)key_idx(key);
+        out_dist[oq * k + i] = key_val(key);
+        out_ids[oq * k + i] = (int64_t)key_idx(key);
       }
     }
   }
@@ -289,11 +305,11 @@ __global__ void __launch_bounds__(128) flat_finish_kernel(const uint64_t* __rest
 
 template <int NQ>
 static int launch_finish_t(const uint64_t* Wg, int64_t nq, int S, int k, const float* xnorm,
-                           float* out_dist, int64_t* out_ids, cudaStream_t s) {
+                           float* out_dist, int64_t* out_ids, cudaStream_t s, const FinishExtra& ex) {
   constexpr int NB = NQ < 4 ? NQ : 4;
   const size_t smem = 4 * warp_select_smem_keys<NB>() * sizeof(uint64_t);
   flat_finish_kernel<NQ><<<(unsigned)ceil_div(nq, 4), 128, smem, s>>>(Wg, nq, S, k, xnorm,
-                                                                      out_dist, out_ids);
+                                                                      out_dist, out_ids, ex);
   FS_LAUNCHED();
   return FS_OK;
 }
@@ -376,15 +392,16 @@ int launch_merge_pack(const float* dist, const int64_t* ids, int64_t nq, int G, 
 }
 
 int launch_flat_finish(const uint64_t* Wg, int64_t nq, int S, int k, const float* xnorm,
-                       float* out_dist, int64_t* out_ids, cudaStream_t s) {
+                       float* out_dist, int64_t* out_ids, cudaStream_t s, const FinishExtra* extra) {
   if (nq == 0) return FS_OK;
+  const FinishExtra ex = extra ? *extra : FinishExtra();
   switch (k_class(k)) {
-    case 0: return launch_finish_t<1>(Wg, nq, S, k, xnorm, out_dist, out_ids, s);
-    case 1: return launch_finish_t<2>(Wg, nq, S, k, xnorm, out_dist, out_ids, s);
-    case 2: return launch_finish_t<4>(Wg, nq, S, k, xnorm, out_dist, out_ids, s);
-    case 3: return launch_finish_t<8>(Wg, nq, S, k, xnorm, out_dist, out_ids, s);
-    case 4: return launch_finish_t<16>(Wg, nq, S, k, xnorm, out_dist, out_ids, s);
-    default: return launch_finish_t<32>(Wg, nq, S, k, xnorm, out_dist, out_ids, s);
+    case 0: return launch_finish_t<1>(Wg, nq, S, k, xnorm, out_dist, out_ids, s, ex);
+    case 1: return launch_finish_t<2>(Wg, nq, S, k, xnorm, out_dist, out_ids, s, ex);
+    case 2: return launch_finish_t<4>(Wg, nq, S, k, xnorm, out_dist, out_ids, s, ex);
+    case 3: return launch_finish_t<8>(Wg, nq, S, k, xnorm, out_dist, out_ids, s, ex);
+    case 4: return launch_finish_t<16>(Wg, nq, S, k, xnorm, out_dist, out_ids, s, ex);
+    default: return launch_finish_t<32>(Wg, nq, S, k, xnorm, out_dist, out_ids, s, ex);
   }
 }
 

@@ -32,6 +32,10 @@ struct FlatTcPlan {
   int64_t chunk, chunk0;
   size_t smem;
   size_t off_ynorm, off_xnorm, off_flag, off_gbound, off_hbound, off_hclaim, off_W, off_cbuf, off_qhi, off_qlo, off_bhi, off_blo, bytes;
+  // sampled bound (k >= 2, large databases): a strided sample of ns rows is searched first for the c-th distance
+  int64_t ns, sstride;
+  int c;
+  size_t off_fail, off_failq, off_qfhi, off_qflo, off_sub;  // fail list, gathered failed queries, the sample pass's own plan
 };
 bool flat_tc_supported(int d);  // d % 32 == 0, 32 <= d <= 128, not disabled by FS_FLAT_ENGINE=ffma
 FlatTcPlan flat_tc_plan(int64_t nq, int64_t nb, int d, int k);
@@ -41,8 +45,17 @@ int flat_knn_tc_device(const float* xq, int64_t nq, const float* xb, int64_t nb,
                        int64_t* out_ids, void* ws, cudaStream_t s, float* dout = nullptr, int64_t dld = 0);
 
 // B4: S partial queues per query -> k results (+||x||^2 if xnorm != NULL).
+// Optional extras of the sampled-bound scheme of the tensor-core engine (flat_tc.cu):
+struct FinishExtra {
+  unsigned int* bound_out = nullptr;       // != NULL: no results; bound_out[q] = order image of the k-th smallest d'
+  unsigned int* fail_cnt = nullptr;        // != NULL: queries whose queues hold fewer than `need` keys are appended
+  int* fail_q = nullptr;                   //          to fail_q (the sampled bound was too tight for them)
+  int need = 0;
+  const unsigned int* nq_dev = nullptr;    // != NULL: number of rows, on the device (<= nq)
+  const int* qmap = nullptr;               // != NULL: row i of Wg is query qmap[i] (xnorm and outputs are indexed by it)
+};
 int launch_flat_finish(const uint64_t* Wg, int64_t nq, int S, int k, const float* xnorm,
-                       float* out_dist, int64_t* out_ids, cudaStream_t s);
+                       float* out_dist, int64_t* out_ids, cudaStream_t s, const FinishExtra* extra = nullptr);
 
 // Positions -> ids: ids_io[q][i] holds a position into table (or < 0); it becomes table[position], and
 // entries of a query with bitwise-equal distance are put in ascending id order.

@@ -24,6 +24,7 @@
 // run at the same time read the same part of the database (L2 reuse), and a query's
 // bound found in earlier splits (gbound) prunes the later ones.
 #include <cuda.h>
+#include <cmath>
 #include <cstdlib>
 #include <cstring>
 
@@ -63,6 +64,8 @@ constexpr int SCRATCH_BYTES = EPI_GROUPS * 4 * ((1 << EPI_RB) * 64 + STAGE_KEYS 
 #endif
 constexpr int EAGER_EXTRA = FS_TC_EAGER;       // idle-time restore of rows holding >= k + max(this, k * FS_TC_EAGER_Q / 4) keys
                                               // (sweep in profiles/r01_flat.md)
+constexpr int KREG = 12;                      // k <= KREG: the row's queue is a sorted array of the thread's own, kept in the
+                                              // warp's selection scratch (3 KB = 12 keys per lane, [slot][lane]: conflict-free)
 constexpr int HB_LEVELS = 3;                  // hierarchical bound: levels 1..3 (2, 4, 8 queues)
 constexpr int HB_SLOTS = 2 + 4 + 8;
 constexpr int SMEM_LIMIT = 227 * 1024;
@@ -85,6 +88,7 @@ struct TcArgs {
   unsigned int* hclaim;        // [nq][HB_LEVELS] slots handed out per level
   uint64_t* cbuf;              // [gridDim.x][EPI_GROUPS][BM][cap]: winners so far, then new candidates
   const unsigned int* lo_flag; // != 0: lo planes are not all zero (3xTF32)
+  const unsigned int* nq_dev;  // != NULL: the number of queries, on the device (<= nq; re-run of the failed queries)
   float* dout;                 // != NULL: no selection, d'(q, j) = ||y_j||^2 - 2 <x_q, y_j> is written to
   int64_t dld;                 //          dout[q * dld + j] (dld % 4 == 0); the launch passes k = 1
 };
@@ -137,6 +141,40 @@ __global__ void __launch_bounds__(256)
 __global__ void __launch_bounds__(256) hi_plane_kernel(const float* __restrict__ x, int64_t n_elems, float* __restrict__ hi) {
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_elems; i += (int64_t)gridDim.x * blockDim.x)
     hi[i] = __uint_as_float(__float_as_uint(x[i]) & 0xFFFFE000u);
+}
+
+// The sample: every stride-th row of the database (and of its lo plane in 3xTF32 mode) with its ||y||^2,
+// copied to a compact array -- one warp per row.
+__global__ void __launch_bounds__(256) gather_sample_kernel(const float* __restrict__ hi, const float* __restrict__ lo,
+                                                            const float* __restrict__ ynorm, int64_t stride, int64_t n, int d,
+                                                            const unsigned int* __restrict__ lo_flag, float* __restrict__ shi,
+                                                            float* __restrict__ slo, float* __restrict__ syn) {
+  const int64_t i = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
+  if (i >= n) return;
+  const int lane = threadIdx.x & 31;
+  const int64_t r = i * stride;
+  const bool split = *lo_flag != 0u;
+  for (int j = lane; j < d; j += 32) {
+    shi[i * d + j] = hi[r * d + j];
+    if (split) slo[i * d + j] = lo[r * d + j];
+  }
+  if (lane == 0) syn[i] = ynorm[r];
+}
+
+// Rows of the queries whose sampled bound failed, gathered for the re-run: one warp per failed query.
+__global__ void __launch_bounds__(256) gather_failed_kernel(const float* __restrict__ hi, const float* __restrict__ lo, int d,
+                                                            const unsigned int* __restrict__ fail_cnt,
+                                                            const int* __restrict__ fail_q, const unsigned int* __restrict__ lo_flag,
+                                                            float* __restrict__ ghi, float* __restrict__ glo) {
+  const int64_t i = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
+  if (i >= (int64_t)*fail_cnt) return;
+  const int lane = threadIdx.x & 31;
+  const int64_t q = fail_q[i];
+  const bool split = *lo_flag != 0u;
+  for (int j = lane; j < d; j += 32) {
+    ghi[i * d + j] = hi[q * d + j];
+    if (split) glo[i * d + j] = lo[q * d + j];
+  }
 }
 
 // ---------------------------------------------------------------------------
@@ -212,7 +250,10 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
   const int64_t cluster_id = blockIdx.x / CLUSTER, n_clusters = gridDim.x / CLUSTER;
   constexpr uint16_t kAllCtas = (uint16_t)((1u << CLUSTER) - 1u);
   const uint32_t tmem_base = *tmem_slot;
-  const int64_t n_items = (int64_t)a.S * a.qgroups;
+  int64_t nq = a.nq;
+  if (a.nq_dev) nq = (int64_t)*a.nq_dev < nq ? (int64_t)*a.nq_dev : nq;
+  const int64_t qgroups = a.nq_dev ? (nq + (int64_t)BM * CLUSTER - 1) / ((int64_t)BM * CLUSTER) : a.qgroups;
+  const int64_t n_items = (int64_t)a.S * qgroups;
 
   if (warp == TMA_WARP) {
     // ===== TMA producer =====
@@ -221,7 +262,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
       int it = 0;
       uint32_t ptile = 0;
       for (int64_t item = cluster_id; item < n_items; item += n_clusters, ++it) {
-        const int s = (int)(item / a.qgroups), qt = (int)(item - (int64_t)s * a.qgroups) * CLUSTER + (int)crank;
+        const int s = (int)(item / qgroups), qt = (int)(item - (int64_t)s * qgroups) * CLUSTER + (int)crank;
         const int64_t b_begin = s == 0 ? 0 : a.chunk0 + (int64_t)(s - 1) * a.chunk;
         const int64_t b_len = s == 0 ? a.chunk0 : a.chunk;
         const int64_t b_end = b_begin + b_len < a.nb ? b_begin + b_len : a.nb;
@@ -267,7 +308,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
       uint32_t tile_count = 0;
       int it = 0;
       for (int64_t item = cluster_id; item < n_items; item += n_clusters, ++it) {
-        const int s = (int)(item / a.qgroups);
+        const int s = (int)(item / qgroups);
         const int64_t b_begin = s == 0 ? 0 : a.chunk0 + (int64_t)(s - 1) * a.chunk;
         const int64_t b_len = s == 0 ? a.chunk0 : a.chunk;
         const int64_t b_end = b_begin + b_len < a.nb ? b_begin + b_len : a.nb;
@@ -316,20 +357,21 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
     const int eg = warp >> 2;  // epilogue group: its own columns, candidate buffers and partial queues
     const int K = a.K, k = a.k, cap = a.cap;
     const int SQ = a.S * EPI_GROUPS;  // partial queues per query
+    const bool rq = k <= KREG;        // thread-private sorted queue: exact bound after every insertion, no restore steps
     uint32_t* scratch = reinterpret_cast<uint32_t*>(scratch_all + (size_t)warp * (sel_scratch_bytes<EPI_RB>() + STAGE_KEYS * 8));
     uint64_t* stage = reinterpret_cast<uint64_t*>(reinterpret_cast<unsigned char*>(scratch) + sel_scratch_bytes<EPI_RB>());
     uint64_t* cb_warp = a.cbuf + (((size_t)blockIdx.x * EPI_GROUPS + eg) * BM + quarter * 32) * cap;
     uint64_t* cb = cb_warp + (size_t)lane * cap;
     uint32_t tile_count = 0;
     for (int64_t item = cluster_id; item < n_items; item += n_clusters) {
-      const int s = (int)(item / a.qgroups), qt = (int)(item - (int64_t)s * a.qgroups) * CLUSTER + (int)crank;
+      const int s = (int)(item / qgroups), qt = (int)(item - (int64_t)s * qgroups) * CLUSTER + (int)crank;
       const int64_t b_begin = s == 0 ? 0 : a.chunk0 + (int64_t)(s - 1) * a.chunk;
       const int64_t b_len = s == 0 ? a.chunk0 : a.chunk;
       const int64_t b_end = b_begin + b_len < a.nb ? b_begin + b_len : a.nb;
       const int ntiles = (int)((b_end - b_begin + BN - 1) / BN);
       const int64_t q_warp = (int64_t)qt * BM + quarter * 32;
       const int64_t q = q_warp + lane;
-      const bool valid = q < a.nq;
+      const bool valid = q < nq;
       // start from the best bound other splits have published (inclusive)
       uint32_t gb = valid ? a.gbound[q] : 0u;
       if (valid && k >= 8) {
@@ -351,6 +393,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
       uint64_t thr_key = thr0;
       float thr_val = valid ? ord_f32((uint32_t)(thr0 >> 32)) : __uint_as_float(0xFF800000u);
       int cnt = 0;  // keys in this row's buffer: the winners so far, then new candidates
+      uint64_t* Rq = reinterpret_cast<uint64_t*>(scratch) + lane;  // rq: the row's cnt <= k smallest keys, ascending, stride 32
       __syncwarp();
 
       // Restore step for the rows that ask for it: the whole warp selects the k
@@ -497,11 +540,23 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
           auto take = [&](float dp, uint32_t col) {  // exact key test, append to the row's buffer
             const uint64_t key = make_key(dp, col);
             if (key < thr_key) {
-              if (k == 1) {  // the queue is one register: the bound is always exact
-                thr_key = key;
-                thr_val = dp;
-                cb[0] = key;
-                cnt = 1;
+              if (rq) {  // sorted insertion (a full queue drops its last key); the bound is the k-th key at once
+                int e = cnt < k ? cnt : k - 1;
+                while (e > 0) {
+                  const uint64_t pk = Rq[(e - 1) * 32];
+                  if (pk < key) break;
+                  Rq[e * 32] = pk;
+                  --e;
+                }
+                Rq[e * 32] = key;
+                if (cnt < k) ++cnt;
+                if (cnt == k) {
+                  const uint64_t t = Rq[(k - 1) * 32];
+                  if (t < thr_key) {
+                    thr_key = t;
+                    thr_val = key_val(t);
+                  }
+                }
               } else {
                 cb[cnt++] = key;
               }
@@ -538,12 +593,18 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
         }
       }
       if (a.dout != nullptr) continue;  // nothing was selected
-      flush_rows(cnt >= k, true);  // establishes the split's k-th distance (published below)
+      // establishes the split's k-th distance (published below); a single split has nobody to publish to and
+      // B4 takes up to K keys per queue as they are
+      if (rq) {  // the thread's queue becomes the row's buffer
+        for (int e = 0; e < cnt; ++e) cb[e] = Rq[e * 32];
+      } else {
+        flush_rows(a.S > 1 ? cnt >= k : cnt > K, true);
+      }
       __syncwarp();
       // the row's partial queue for B4 (unordered, sentinel padded), and this split's k-th
       // distance (when a restore step has established it) as a bound for the splits to come
       for (int r = 0; r < 32; ++r) {
-        if (q_warp + r >= a.nq) break;
+        if (q_warp + r >= nq) break;
         const int m = __shfl_sync(kFull, cnt, r);
         const uint64_t* buf = cb_warp + (size_t)r * cap;
         uint64_t* W = a.Wg + ((q_warp + r) * SQ + s * EPI_GROUPS + eg) * K;
@@ -620,7 +681,80 @@ bool flat_tc_supported(int d) {
 // more keys in B4): weigh it against the wave quantisation of the MMA work.
 static double split_penalty(int kclass) { return kclass == 0 ? 0.002 : 0.004; }
 
+// ---------------------------------------------------------------------------
+// Sampled bound (k >= 8, nb >= 8 192).  Every partial queue of a query pays ~k ln(n / k) candidates when
+// it starts without a bound, and a query has 2 S of them.  Instead a strided sample of
+// ns <= min(8 192, nb / 32) rows is searched first for the query's c-th smallest distance, which
+// then bounds every queue from its first tile on.  c is the smallest rank with
+// P(Poisson(k ns / nb) >= c) <= 1e-7: the bound is below the true k-th distance only if c or more of the
+// sample rows are among the query's k - 1 nearest.  Then fewer than k rows of the whole database pass,
+// B4 sees fewer than k keys, and the query is searched again without a sampled bound (same kernel, the
+// failed queries gathered, their number read on the device): exact in every case, ~c nb / ns candidates
+// per query instead of ~2 S k ln(nb / (2 S k)).  FS_FLAT_SAMPLE=off disables it; =fail makes c = 1 (most
+// queries fail: the tests run the re-run path with it).
+// ---------------------------------------------------------------------------
+static int sample_mode() {
+  static int mode = -1;
+  if (mode < 0) {
+    const char* e = getenv("FS_FLAT_SAMPLE");
+    mode = (e && strcmp(e, "off") == 0) ? 0 : (e && strcmp(e, "fail") == 0) ? 2 : 1;
+  }
+  return mode;
+}
+
+static int poisson_tail_rank(double lambda, double eps) {
+  double term = exp(-lambda), cdf = term;  // P(X <= 0)
+  int c = 1;
+  while (1.0 - cdf > eps && c < 8192) {    // P(X >= c) = 1 - P(X <= c - 1)
+    term *= lambda / (double)c;
+    cdf += term;
+    ++c;
+  }
+  return c;
+}
+
+static FlatTcPlan flat_tc_plan_base(int64_t nq, int64_t nb, int d, int k, bool sample_pass = false);
+
 FlatTcPlan flat_tc_plan(int64_t nq, int64_t nb, int d, int k) {
+  FlatTcPlan p = flat_tc_plan_base(nq, nb, d, k);
+  p.ns = p.sstride = 0;
+  p.c = 0;
+  p.off_fail = p.off_failq = p.off_qfhi = p.off_qflo = p.off_sub = 0;
+  // k < 8: the thread-private queues (k <= KREG) keep exact bounds from the start; nothing to gain
+  if (k < 8 || sample_mode() == 0 || nb < 8192) return p;
+  // Sample size: the pass costs ns / nb of the main one and the main pass sees ~c nb / ns candidates per
+  // query.  ns is taken so that c <= KREG (expected hits k ns / nb <= ~1.5): the sample pass then runs on
+  // the thread-private queues itself, and the candidates stay within ~10 k per query.
+  int64_t ns = (int64_t)(1.5 * (double)nb / (double)k);
+  if (ns > nb / 32) ns = nb / 32;
+  if (ns > 8192) ns = 8192;
+  ns = ns / BN * BN;
+  int c = 0;
+  for (; ns >= BN; ns -= BN) {
+    c = sample_mode() == 2 ? 1 : poisson_tail_rank((double)k * (double)ns / (double)nb, 1e-7);
+    if (c <= KREG) break;
+  }
+  if (ns < BN) return p;
+  const int64_t stride = nb / ns;
+  p.ns = ns;
+  p.sstride = stride;
+  p.c = c;
+  size_t o = p.bytes;
+  auto take = [&](size_t bytes) {
+    const size_t at = o;
+    o += align_up(bytes, 256);
+    return at;
+  };
+  p.off_fail = take(256);
+  p.off_failq = take((size_t)(nq + 1) * sizeof(int));
+  p.off_qfhi = take((size_t)nq * d * sizeof(float));
+  p.off_qflo = take((size_t)nq * d * sizeof(float));
+  p.off_sub = take(flat_tc_plan_base(nq, ns, d, c, true).bytes);
+  p.bytes = o;
+  return p;
+}
+
+static FlatTcPlan flat_tc_plan_base(int64_t nq, int64_t nb, int d, int k, bool sample_pass) {
   FlatTcPlan p;
   p.kclass = k_class(k);
   p.K = 32 << p.kclass;
@@ -639,7 +773,9 @@ FlatTcPlan flat_tc_plan(int64_t nq, int64_t nb, int d, int k) {
     const int64_t items = realS * qgroups;
     const int64_t g = items < ncl ? items : ncl;
     const double eff = (double)items / (double)(ceil_div(items, g) * g) * ((double)g / (double)ncl);
-    const double score = eff - split_penalty(p.kclass) * (double)realS;
+    // the sample pass is short: its items' fixed costs (query tile load, pipeline fill, final restore) outweigh a
+    // half-empty wave, so it takes as few items as possible
+    const double score = eff - (sample_pass ? 0.05 : split_penalty(p.kclass)) * (double)realS;
     if (score > best) {
       best = score;
       best_S = realS;
@@ -735,47 +871,103 @@ int flat_knn_tc_device(const float* xq, int64_t nq, const float* xb, int64_t nb,
       (rc = make_map(&mb_hi, b_hi, nb, d, BN / CLUSTER)) != FS_OK ||
       (rc = make_map(&mb_lo, blo, nb, d, BN / CLUSTER)) != FS_OK)
     return rc;
-  TcArgs a;
-  a.nq = nq;
-  a.nb = nb;
-  a.d = d;
-  a.KB = p.KB;
-  a.k = k;
-  a.kclass = p.kclass;
-  a.K = p.K;
-  a.S = p.S;
-  a.qtiles = p.qtiles;
-  a.qgroups = p.qgroups;
-  a.cap = p.cap;
-  a.smem_bytes = (int)p.smem;
-  a.chunk = p.chunk;
-  a.chunk0 = p.chunk0;
-  a.ynorm = ynorm;
-  a.Wg = reinterpret_cast<uint64_t*>(w + p.off_W);
-  a.gbound = gbound;
-  a.hbound = reinterpret_cast<unsigned int*>(w + p.off_hbound);
-  a.hclaim = reinterpret_cast<unsigned int*>(w + p.off_hclaim);
-  a.cbuf = reinterpret_cast<uint64_t*>(w + p.off_cbuf);
-  a.lo_flag = flag;
-  a.dout = dout;
-  a.dld = dld;
   FS_CUDA(cudaFuncSetAttribute(flat_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem));  // per device
-  cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3((unsigned)p.grid);
-  cfg.blockDim = dim3(TC_THREADS);
-  cfg.dynamicSmemBytes = p.smem;
-  cfg.stream = s;
-  cudaLaunchAttribute attr[1];
-  attr[0].id = cudaLaunchAttributeClusterDimension;
-  attr[0].val.clusterDim.x = CLUSTER;
-  attr[0].val.clusterDim.y = 1;
-  attr[0].val.clusterDim.z = 1;
-  cfg.attrs = attr;
-  cfg.numAttrs = 1;
-  FS_CUDA(cudaLaunchKernelEx(&cfg, flat_tc_kernel, ma_hi, ma_lo, mb_hi, mb_lo, a));
-  FS_LAUNCHED();
+  // one launch of the tile kernel: plan pl over a database of n rows seen through (m_bhi, m_blo), queries
+  // through (m_ahi, m_alo), workspace region wr laid out by pl
+  auto run_tiles = [&](const FlatTcPlan& pl, char* wr, int64_t n, int kk, const float* yn, const CUtensorMap& m_ahi,
+                       const CUtensorMap& m_alo, const CUtensorMap& m_bhi, const CUtensorMap& m_blo,
+                       const unsigned int* nq_dev, unsigned int* gb) -> int {
+    TcArgs a;
+    a.nq = nq;
+    a.nb = n;
+    a.d = d;
+    a.KB = pl.KB;
+    a.k = kk;
+    a.kclass = pl.kclass;
+    a.K = pl.K;
+    a.S = pl.S;
+    a.qtiles = pl.qtiles;
+    a.qgroups = pl.qgroups;
+    a.cap = pl.cap;
+    a.smem_bytes = (int)pl.smem;
+    a.chunk = pl.chunk;
+    a.chunk0 = pl.chunk0;
+    a.ynorm = yn;
+    a.Wg = reinterpret_cast<uint64_t*>(wr + pl.off_W);
+    a.gbound = gb;
+    a.hbound = reinterpret_cast<unsigned int*>(wr + pl.off_hbound);
+    a.hclaim = reinterpret_cast<unsigned int*>(wr + pl.off_hclaim);
+    a.cbuf = reinterpret_cast<uint64_t*>(wr + pl.off_cbuf);
+    a.lo_flag = flag;
+    a.nq_dev = nq_dev;
+    a.dout = dout;
+    a.dld = dld;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)pl.grid);
+    cfg.blockDim = dim3(TC_THREADS);
+    cfg.dynamicSmemBytes = pl.smem;
+    cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = CLUSTER;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    FS_CUDA(cudaLaunchKernelEx(&cfg, flat_tc_kernel, m_ahi, m_alo, m_bhi, m_blo, a));
+    FS_LAUNCHED();
+    return FS_OK;
+  };
+  const bool sampled = p.ns > 0 && dout == nullptr;
+  if (sampled) {
+    // the sample pass: the c-th smallest d' over every sstride-th row becomes gbound[q]
+    const FlatTcPlan sub = flat_tc_plan_base(nq, p.ns, d, p.c, true);
+    char* w2 = w + p.off_sub;
+    float* yn_s = reinterpret_cast<float*>(w2 + sub.off_ynorm);
+    unsigned int* gb_s = reinterpret_cast<unsigned int*>(w2 + sub.off_gbound);
+    float* s_hi = reinterpret_cast<float*>(w2 + sub.off_bhi);
+    float* s_lo = reinterpret_cast<float*>(w2 + sub.off_blo);
+    gather_sample_kernel<<<(unsigned)ceil_div(p.ns, 8), 256, 0, s>>>(b_hi, blo, ynorm, p.sstride, p.ns, d, flag, s_hi, s_lo, yn_s);
+    FS_LAUNCHED();
+    FS_CUDA(cudaMemsetAsync(gb_s, 0xFF, sub.off_hclaim - sub.off_gbound, s));
+    FS_CUDA(cudaMemsetAsync(w2 + sub.off_hclaim, 0, (size_t)(nq + 1) * HB_LEVELS * sizeof(unsigned int), s));
+    CUtensorMap ms_hi, ms_lo;
+    if ((rc = make_map(&ms_hi, s_hi, p.ns, d, BN / CLUSTER)) != FS_OK ||
+        (rc = make_map(&ms_lo, s_lo, p.ns, d, BN / CLUSTER)) != FS_OK)
+      return rc;
+    if ((rc = run_tiles(sub, w2, p.ns, p.c, yn_s, ma_hi, ma_lo, ms_hi, ms_lo, nullptr, gb_s)) != FS_OK) return rc;
+    FinishExtra ex;
+    ex.bound_out = gbound;
+    if ((rc = launch_flat_finish(reinterpret_cast<uint64_t*>(w2 + sub.off_W), nq, sub.S * EPI_GROUPS, p.c, nullptr, nullptr,
+                                 nullptr, s, &ex)) != FS_OK)
+      return rc;
+  }
+  if ((rc = run_tiles(p, w, nb, k, ynorm, ma_hi, ma_lo, mb_hi, mb_lo, nullptr, gbound)) != FS_OK) return rc;
   if (dout != nullptr) return FS_OK;
-  return launch_flat_finish(a.Wg, nq, p.S * EPI_GROUPS, k, xnorm, out_dist, out_ids, s);
+  uint64_t* Wg = reinterpret_cast<uint64_t*>(w + p.off_W);
+  if (!sampled) return launch_flat_finish(Wg, nq, p.S * EPI_GROUPS, k, xnorm, out_dist, out_ids, s);
+  // B4 with the check of the sampled bound, then the failed queries once more without one
+  unsigned int* fail_cnt = reinterpret_cast<unsigned int*>(w + p.off_fail);
+  int* fail_q = reinterpret_cast<int*>(w + p.off_failq);
+  float* qf_hi = reinterpret_cast<float*>(w + p.off_qfhi);
+  float* qf_lo = reinterpret_cast<float*>(w + p.off_qflo);
+  FS_CUDA(cudaMemsetAsync(fail_cnt, 0, 256, s));
+  FinishExtra ex;
+  ex.fail_cnt = fail_cnt;
+  ex.fail_q = fail_q;
+  ex.need = (int)((int64_t)k < nb ? k : nb);
+  if ((rc = launch_flat_finish(Wg, nq, p.S * EPI_GROUPS, k, xnorm, out_dist, out_ids, s, &ex)) != FS_OK) return rc;
+  gather_failed_kernel<<<(unsigned)ceil_div(nq, 8), 256, 0, s>>>(a_hi, qlo, d, fail_cnt, fail_q, flag, qf_hi, qf_lo);
+  FS_LAUNCHED();
+  FS_CUDA(cudaMemsetAsync(gbound, 0xFF, p.off_hclaim - p.off_gbound, s));
+  FS_CUDA(cudaMemsetAsync(w + p.off_hclaim, 0, (size_t)(nq + 1) * HB_LEVELS * sizeof(unsigned int), s));
+  CUtensorMap mf_hi, mf_lo;
+  if ((rc = make_map(&mf_hi, qf_hi, nq, d, BM)) != FS_OK || (rc = make_map(&mf_lo, qf_lo, nq, d, BM)) != FS_OK) return rc;
+  if ((rc = run_tiles(p, w, nb, k, ynorm, mf_hi, mf_lo, mb_hi, mb_lo, fail_cnt, gbound)) != FS_OK) return rc;
+  FinishExtra ex2;
+  ex2.nq_dev = fail_cnt;
+  ex2.qmap = fail_q;
+  return launch_flat_finish(Wg, nq, p.S * EPI_GROUPS, k, xnorm, out_dist, out_ids, s, &ex2);
 }
 
 }  // namespace fs

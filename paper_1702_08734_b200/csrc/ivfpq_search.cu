@@ -550,9 +550,12 @@ bool c1_matrix(int64_t nq, int64_t nlist, int nprobe, int d) {
   if (forced == 1) return false;
   if (forced == 2) return true;
   if (nprobe < 16 || nq < 256) return false;
-  // measured (nq = 10^4, d = 96; search of a tiny index, ms, fused / matrix): nlist 8 192: nprobe 64
-  // 2.79 / 1.95, 256 8.25 / 6.30; nlist 65 536: 16 1.71 / 2.41, 64 2.85 / 2.97, 256 9.24 / 4.93;
-  // nlist 262 144: 64 4.98 / 11.1, 256 14.4 / 13.6
+  // With a sampled bound (flat_tc.cu: k ns / nb small enough for an ns >= 256) the fused engine wins:
+  // C1 stage, nq = 10^4, d = 96, ms fused / matrix: nlist 8 192: nprobe 32 0.58 / 0.73; 16 384: 64 0.68 / 0.97;
+  // 32 768: 128 1.01 / 1.49; 65 536: 16 1.34 / 2.85, 256 1.84 / 3.04; 262 144: 2.7 - 3.2 / > 28.
+  // Without one (large nprobe over a small quantizer) the two-step form does: 8 192: 256 2.45 / 0.79;
+  // 16 384: 128 2.09 / 1.00; 32 768: 256 5.24 / 1.53.
+  if (flat_tc_plan(nq, nlist, d, nprobe).ns > 0) return false;
   return nlist <= 16384 || (nprobe >= 128 && nlist <= 131072) || nprobe >= 256;
 }
 

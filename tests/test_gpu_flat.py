@@ -81,6 +81,36 @@ def test_cfg3_shaped_integer_data_bit_exact(k):
     assert np.array_equal(gd.view(np.uint32), od.view(np.uint32))
 
 
+@pytest.mark.parametrize("k", [2, 10, 100, 1024])
+def test_sampled_bound_integer_data_bit_exact(k):
+    """Databases of >= 32 768 rows take the sampled bound of the tensor-core engine (DESIGN 5.2): a strided
+    sample is searched first and its c-th distance bounds every queue.  Integer data: bit-exact.  The second
+    half of the queries has its nearest rows planted exactly ON the sample positions, so the sampled bound is
+    too tight for them and they must come out of the re-run (B4 sees fewer than k keys)."""
+    nb, nq = 40000, 300
+    xb = datagen.sift_like(0, nb)
+    xq = datagen.sift_like(1_000_000, nq)
+    stride = nb // 4096                       # ns = 4096 for this nb (flat_tc_plan)
+    rng = np.random.default_rng(k)
+    for q in range(nq // 2, nq):              # 160 near-copies of the query at sample positions
+        pos = rng.choice(4096, 160, replace=False) * stride
+        xb[pos] = np.clip(xq[q][None, :] + rng.integers(-2, 3, size=(160, xb.shape[1])), 0, 255).astype(np.float32)
+    od, oi = oracle.flat_l2_knn(xq, xb, k)
+    gd, gi = run(xq, xb, k)
+    assert np.array_equal(gi, oi)
+    assert np.array_equal(gd.view(np.uint32), od.view(np.uint32))
+
+
+def test_sampled_bound_real_valued():
+    xb = datagen.gaussian_vectors(0, 50000, 96)
+    xq = datagen.gaussian_vectors(50000, 200, 96)
+    for k in (5, 100):
+        _, oi, od64 = oracle.flat_l2_knn(xq, xb, k, want64=True)
+        gd, gi = run(xq, xb, k)
+        check_acceptance(xq, xb, k, gd, gi, od64)
+        assert (gi == oi).mean() > 0.999
+
+
 def test_handworked_and_duplicates():
     xb = np.array([[0, 0], [3, 4], [6, 8], [3, 4], [-3, 4]], np.float32)
     xq = np.array([[0, 0], [3, 4]], np.float32)
