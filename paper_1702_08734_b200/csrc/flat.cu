@@ -253,9 +253,15 @@ __global__ void __launch_bounds__(128) flat_finish_kernel(const uint64_t* __rest
 #pragma unroll
     for (int r = 0; r < NQ; ++r) sel.W[r] = src[r * 32 + lane];
   } else {
-    for (int64_t e0 = 0; e0 < (int64_t)S * K; e0 += 32) {
-      const uint64_t key = src[e0 + lane];
-      sel.push(key < sel.thr, key);  // sentinels never pass: thr <= sentinel
+    // ex.packed: a partial queue holds its keys first and sentinels behind them, so the first 32 slots that
+    // hold only sentinels end the queue (with tight bounds most queues are nearly empty)
+    for (int sq = 0; sq < S; ++sq) {
+      const uint64_t* qs = src + (int64_t)sq * K;
+      for (int e0 = 0; e0 < K; e0 += 32) {
+        const uint64_t key = qs[e0 + lane];
+        if (ex.packed && __all_sync(kFull, key == kSentinelKey)) break;
+        sel.push(key < sel.thr, key);  // sentinels never pass: thr <= sentinel
+      }
     }
     sel.finish();
   }

@@ -53,6 +53,7 @@ struct FinishExtra {
   int need = 0;
   const unsigned int* nq_dev = nullptr;    // != NULL: number of rows, on the device (<= nq)
   const int* qmap = nullptr;               // != NULL: row i of Wg is query qmap[i] (xnorm and outputs are indexed by it)
+  bool packed = false;                     // every queue holds its keys first, sentinels behind them: reading stops there
 };
 int launch_flat_finish(const uint64_t* Wg, int64_t nq, int S, int k, const float* xnorm,
                        float* out_dist, int64_t* out_ids, cudaStream_t s, const FinishExtra* extra = nullptr);

@@ -937,6 +937,7 @@ int flat_knn_tc_device(const float* xq, int64_t nq, const float* xb, int64_t nb,
       return rc;
     if ((rc = run_tiles(sub, w2, p.ns, p.c, yn_s, ma_hi, ma_lo, ms_hi, ms_lo, nullptr, gb_s)) != FS_OK) return rc;
     FinishExtra ex;
+    ex.packed = true;
     ex.bound_out = gbound;
     if ((rc = launch_flat_finish(reinterpret_cast<uint64_t*>(w2 + sub.off_W), nq, sub.S * EPI_GROUPS, p.c, nullptr, nullptr,
                                  nullptr, s, &ex)) != FS_OK)
@@ -945,7 +946,9 @@ int flat_knn_tc_device(const float* xq, int64_t nq, const float* xb, int64_t nb,
   if ((rc = run_tiles(p, w, nb, k, ynorm, ma_hi, ma_lo, mb_hi, mb_lo, nullptr, gbound)) != FS_OK) return rc;
   if (dout != nullptr) return FS_OK;
   uint64_t* Wg = reinterpret_cast<uint64_t*>(w + p.off_W);
-  if (!sampled) return launch_flat_finish(Wg, nq, p.S * EPI_GROUPS, k, xnorm, out_dist, out_ids, s);
+  FinishExtra ex0;
+  ex0.packed = true;
+  if (!sampled) return launch_flat_finish(Wg, nq, p.S * EPI_GROUPS, k, xnorm, out_dist, out_ids, s, &ex0);
   // B4 with the check of the sampled bound, then the failed queries once more without one
   unsigned int* fail_cnt = reinterpret_cast<unsigned int*>(w + p.off_fail);
   int* fail_q = reinterpret_cast<int*>(w + p.off_failq);
@@ -953,6 +956,7 @@ int flat_knn_tc_device(const float* xq, int64_t nq, const float* xb, int64_t nb,
   float* qf_lo = reinterpret_cast<float*>(w + p.off_qflo);
   FS_CUDA(cudaMemsetAsync(fail_cnt, 0, 256, s));
   FinishExtra ex;
+  ex.packed = true;
   ex.fail_cnt = fail_cnt;
   ex.fail_q = fail_q;
   ex.need = (int)((int64_t)k < nb ? k : nb);
@@ -965,6 +969,7 @@ int flat_knn_tc_device(const float* xq, int64_t nq, const float* xb, int64_t nb,
   if ((rc = make_map(&mf_hi, qf_hi, nq, d, BM)) != FS_OK || (rc = make_map(&mf_lo, qf_lo, nq, d, BM)) != FS_OK) return rc;
   if ((rc = run_tiles(p, w, nb, k, ynorm, mf_hi, mf_lo, mb_hi, mb_lo, fail_cnt, gbound)) != FS_OK) return rc;
   FinishExtra ex2;
+  ex2.packed = true;
   ex2.nq_dev = fail_cnt;
   ex2.qmap = fail_q;
   return launch_flat_finish(Wg, nq, p.S * EPI_GROUPS, k, xnorm, out_dist, out_ids, s, &ex2);

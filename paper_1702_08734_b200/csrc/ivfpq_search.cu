@@ -774,7 +774,9 @@ int ivfpq_search_device(fs_ivfpq* ix, const float* xq, int64_t nq, int nprobe, i
   if (rc != FS_OK) return rc;
   FS_CUDA(cudaEventRecord(ix->ev[2], s));
   // C5
-  rc = launch_flat_finish(Wg, nq, p.ngroups, k, nullptr, out_dist, out_ids, s);
+  FinishExtra fx;
+  fx.packed = true;  // the scan parks sorted queues: keys first
+  rc = launch_flat_finish(Wg, nq, p.ngroups, k, nullptr, out_dist, out_ids, s, &fx);
   if (rc != FS_OK) return rc;
   if ((rc = launch_resolve_ids(out_dist, out_ids, ix->ids.as<int64_t>(), nq, k, s)) != FS_OK) return rc;
   FS_CUDA(cudaEventRecord(ix->ev[3], s));
