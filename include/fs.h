@@ -96,6 +96,20 @@ FS_API size_t fs_kselect_ws_bytes(int64_t n_rows, int64_t n, int k);
  * allocation owned by the library (kept for the next call, one call at a time per process). */
 FS_API int fs_kselect_host(const float* rows_host, int64_t n_rows, int64_t n, int64_t ld, int k,
                     float* out_val_host, int32_t* out_idx_host);
+/* fs_kselect for callers that may not allocate (code under CUDA graph capture, serving loops, harnesses
+ * that forbid cudaMalloc): same arguments, results and errors as fs_kselect, but the scratch memory of the
+ * kernels (row counter; for few long rows the bound, survivor counts and survivor lists) is a
+ * built-in __device__ array of FS_NOALLOC_SCRATCH_BYTES, which every GPU that loads the library holds
+ * until the process exits.  The call allocates and frees nothing.  A call whose
+ * fs_kselect_ws_bytes(n_rows, n, k) exceeds the array returns FS_EUNSUPPORTED (every batch of >= 75 rows
+ * needs 256 bytes; one 2^27-element row at k = 1024 needs 0.8 MB).  The array is shared by all calls and
+ * keeps the last call's contents; what must start at zero is cleared on `stream` before the kernels run,
+ * so calls in stream order are independent.  Calls that OVERLAP on the GPU (several streams or host
+ * threads on one device) race on the array: serialise them.  Device ordinals 0..63. */
+#define FS_NOALLOC_SCRATCH_BYTES (4u << 20)
+FS_API int fs_kselect_noalloc(const float* rows, int64_t n_rows, int64_t n, int64_t ld, int k, float* out_val,
+                              int32_t* out_idx, fs_stream stream);
+FS_API size_t fs_kselect_noalloc_max_scratch(void);
 
 /* --------------------------------------------------------------------------
  * Exact squared-L2 k-NN (Eq. 1-2; computation layout 5.1):

@@ -54,7 +54,7 @@ def lib():
         L.fs_launch_count.restype = _i64
         L.fs_reset_launch_count.restype = None
         for name in ("fs_kselect_ws_bytes", "fs_flat_l2_knn_ws_bytes", "fs_ivfpq_search_ws_bytes",
-                     "fs_merge_topk_ws_bytes"):
+                     "fs_merge_topk_ws_bytes", "fs_kselect_noalloc_max_scratch"):
             if hasattr(L, name):
                 getattr(L, name).restype = _sz
         for name in ("fs_ivfpq_ntotal", "fs_ivfpq_last_scanned_codes"):
@@ -125,6 +125,27 @@ def kselect(rows: torch.Tensor, k: int, n: int | None = None, out_val=None, out_
               _ptr(out_idx), _ptr(ws), _sz(0 if ws is None else ws.numel() * ws.element_size()),
               _stream()))
     return out_val, out_idx
+
+
+def kselect_noalloc(rows: torch.Tensor, k: int, out_val: torch.Tensor, out_idx: torch.Tensor, n: int | None = None):
+    """fs_kselect_noalloc: fs_kselect on the library's built-in scratch array; allocates nothing, so the
+    outputs must be given.  Raises FsError (FS_EUNSUPPORTED) when the call needs more scratch than
+    kselect_noalloc_max_scratch().  Calls that overlap on the GPU race on the shared array."""
+    if not (rows.is_cuda and rows.dtype == torch.float32 and rows.dim() == 2
+            and (rows.shape[1] == 0 or rows.stride(1) == 1)):
+        raise ValueError("rows must be a 2-D CUDA fp32 tensor with unit column stride")
+    n_rows = rows.shape[0]
+    n = rows.shape[1] if n is None else n
+    ld = rows.stride(0) if n_rows > 1 else max(rows.shape[1], n)
+    _dev(out_val, torch.float32, "out_val")
+    _dev(out_idx, torch.int32, "out_idx")
+    _check(lib().fs_kselect_noalloc(_ptr(rows), _i64(n_rows), _i64(n), _i64(ld), _int(k), _ptr(out_val),
+                                    _ptr(out_idx), _stream()))
+    return out_val, out_idx
+
+
+def kselect_noalloc_max_scratch() -> int:
+    return int(lib().fs_kselect_noalloc_max_scratch())
 
 
 def _host_ptr(a, dtype_np, dtype_t, name):
