@@ -24,10 +24,13 @@
 //       keys on average): rank = bucket start + that count, exact whatever the distribution, ties on the
 //       full 64-bit (value, index) key.  Keys of rank < k go straight to their place in the output.
 //       Skewed buckets (heavy ties) switch to a block-wide bitonic sort of the kept keys.
-//   exactness: if the sampled bound lets fewer than k elements through, or more than the 2 048 slots
-//       (a sample that does not represent the row: sorted rows), the row is done again by the paper's own
-//       scheme -- chunks of the row merged into a running top-k with the exact k-th key as the bound --
-//       using the same counting step as the restore operation.  Slow, rare, exact.
+//   exactness: if the sampled bound lets fewer than k elements through, or more than the candidate slots
+//       (a head of the row that does not represent it: sorted rows, runs of equal values), the row -- still
+//       in L2 -- gets a second look: a STRIDED sample of it is searched the same way and the row filtered
+//       again with that bound (loads batched eight per thread); failing that, two passes with the first
+//       bound rescaled by what was counted; failing that, the paper's own scheme -- chunks of the row merged
+//       into a running top-k with the exact k-th key as the bound -- using the same counting step as the
+//       restore operation.  Rare (5 - 15 of cfg2's 10 000 rows take the second look), exact.
 //   A4  long rows (few rows, n >= 2^18): a 65 536-element strided sample gives a 4-sigma bound
 //       (kselect_sample_kernel), the whole row is streamed once by every SM with that bound and the
 //       few survivors (~40 k of 2^27) are appended to a per-row list (kselect_filter_kernel), which this
@@ -52,16 +55,8 @@ constexpr int RANK_MAX_BUCKET = 512;  // larger buckets among the kept ones -> b
 // Capacity class: CAPT candidate slots and buckets per row, NST ring stages, CTAs per SM.
 template <int CAPT> struct RowCfg;
 template <> struct RowCfg<1024> { static constexpr int SEG = 4096, NST = 3, CTAS = 3; };  // k <= 256: 16 KB stages, 72 KB
-#ifndef FS_KROW_POLL_NS
-#define FS_KROW_POLL_NS 300
-#endif
-#ifndef FS_KROW_2048_SEG
-#define FS_KROW_2048_SEG 2048
-#define FS_KROW_2048_NST 3
-#define FS_KROW_2048_CTAS 3
-#endif
 template <> struct RowCfg<2048> {  // k <= 1 024: 8 KB stages, 72 KB: three CTAs per SM hide the counting step's latency
-  static constexpr int SEG = FS_KROW_2048_SEG, NST = FS_KROW_2048_NST, CTAS = FS_KROW_2048_CTAS;
+  static constexpr int SEG = 2048, NST = 3, CTAS = 3;
 };
 template <> struct RowCfg<4096> { static constexpr int SEG = 4096, NST = 4, CTAS = 1; };  // survivor lists of long rows: 160 KB
 
@@ -100,6 +95,7 @@ struct RowShared {
   uint64_t full[NST], empty[NST], bnd[NST];
   StageDesc desc[NST];
   RowBound bound[NST];
+  RowBound fb;               // bound of a row's second look (strided sample)
   unsigned int redu[2][RW];
   int cnt, ovf;              // candidates appended, overflow flag
   int kb, kept, maxc;        // counting step: boundary bucket, keys in buckets <= kb, largest such bucket
@@ -119,12 +115,10 @@ struct RowSmem {
   static constexpr size_t total = o_sh + sizeof(RowShared<NST>) + 128;
 };
 
-// mbarrier wait for the producer and scout warps: they poll with a sleep in between, so that their
-// waiting stays off the issue slots of the consumer warps (a try_wait loop of two warps per CTA took a
-// sixth of all issued instructions)
-__device__ __forceinline__ void mbar_wait_park(uint64_t* bar, uint32_t parity) {
-  while (!mbar_test(bar, parity)) __nanosleep(FS_KROW_POLL_NS);
-}
+// mbarrier wait of the producer and scout warps: the blocking try_wait form.  (A test_wait + nanosleep poll
+// was measured too: nanosleep(300) returns almost at once, the two warps then issue 18 % of the kernel's
+// instructions, and the calls are 1 - 2 % slower; nanosleep(3000) delays the refills and costs 70 %.)
+__device__ __forceinline__ void mbar_wait_park(uint64_t* bar, uint32_t parity) { mbar_wait(bar, parity); }
 
 // The k-largest variant runs the same selection on the negated values (-v < -w <=> v > w; f32_ord folds
 // +-0 and NaN, so NaN still sorts last and ties still go to the lower index).  LG is the kernels'
@@ -210,7 +204,11 @@ __device__ void count_select(const RowCtx<CAPT>& c, int64_t row, int m, int want
     s->kept = m;
     s->maxc = 0;
   }
-  if (RAW) {  // raw entries -> keys, in place (every thread converts the entries it will histogram)
+  // The passes below are issue-bound, not latency-bound (three CTAs per SM overlap them): U > 1 keys per
+  // thread in flight was measured 7 % (U = 2) and 27 % (U = 4) slower at k = 1 024.
+  constexpr int U = 1;
+  const bool raw = RAW && have_range;  // raw entries become keys inside the histogram pass
+  if (RAW && !have_range) {            // no range given: keys first (the range is taken from them)
     for (int i = tid; i < m; i += RT) {
       const uint64_t e = c.cand[i];
       const uint32_t pos = (uint32_t)(e >> 32);
@@ -242,10 +240,32 @@ __device__ void count_select(const RowCtx<CAPT>& c, int64_t row, int m, int want
   const float span = hi - lo;
   const float scale = (span > 0.f && span < 3.0e38f) ? (float)NBK / span : 0.f;
   // 1. histogram: one shared-memory atomic per key gives the bucket count and the key's slot
-  for (int i = tid; i < m; i += RT) {
-    const int b = bucket_of<NBK>(c.cand[i], lo, scale);
-    const unsigned int slot = atomicAdd(&c.hist[b], 1u);
-    c.bs[i] = (uint32_t)b | (slot << 12);
+  for (int i0 = tid; i0 < m; i0 += U * RT) {
+    uint64_t key[U];
+    int bk[U];
+    unsigned int slot[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) key[u] = i0 + u * RT < m ? c.cand[i0 + u * RT] : 0ull;
+    if (RAW && raw) {
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        const uint32_t pos = (uint32_t)(key[u] >> 32);
+        const uint32_t idx = (mp && i0 + u * RT < m) ? mp[pos] : pos;
+        key[u] = make_key(__uint_as_float((uint32_t)key[u]), idx);
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u) bk[u] = bucket_of<NBK>(key[u], lo, scale);
+#pragma unroll
+    for (int u = 0; u < U; ++u)
+      if (i0 + u * RT < m) slot[u] = atomicAdd(&c.hist[bk[u]], 1u);
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      if (i0 + u * RT < m) {
+        if (RAW && raw) c.cand[i0 + u * RT] = key[u];
+        c.bs[i0 + u * RT] = (uint32_t)bk[u] | (slot[u] << 12);
+      }
+    }
   }
   cbar();
   // 2. exclusive scan of the counts (BPT per thread), boundary bucket, largest kept bucket
@@ -298,26 +318,56 @@ __device__ void count_select(const RowCtx<CAPT>& c, int64_t row, int m, int want
   cbar();
   // 3. scatter the keys of the buckets up to the boundary one, grouped by bucket
   const int kb = s->kb, kept = s->kept;
-  for (int i = tid; i < m; i += RT) {
-    const uint32_t e = c.bs[i];
-    const int b = (int)(e & 0xFFFu);
-    if (b <= kb) c.sorted[c.hist[b] + (e >> 12)] = c.cand[i];
+  for (int i0 = tid; i0 < m; i0 += U * RT) {
+    uint32_t e[U], h[U];
+    uint64_t key[U];
+    bool ok[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const bool in = i0 + u * RT < m;
+      e[u] = in ? c.bs[i0 + u * RT] : 0xFFFu;
+      key[u] = in ? c.cand[i0 + u * RT] : 0ull;
+      ok[u] = in && (int)(e[u] & 0xFFFu) <= kb;
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u) h[u] = ok[u] ? c.hist[e[u] & 0xFFFu] : 0u;
+#pragma unroll
+    for (int u = 0; u < U; ++u)
+      if (ok[u]) c.sorted[h[u] + (e[u] >> 12)] = key[u];
   }
   cbar();
   // 4. rank inside the bucket (or sort everything kept when some bucket is crowded) and emit
   if (s->maxc <= RANK_MAX_BUCKET) {
-    for (int p = tid; p < kept; p += RT) {
-      const uint64_t key = c.sorted[p];
-      const int b = bucket_of<NBK>(key, lo, scale);
-      const int s0 = (int)c.hist[b], e0 = (int)c.hist[b + 1];
-      int r = s0;
-      for (int j = s0; j < e0; ++j) r += c.sorted[j] < key ? 1 : 0;
-      if (r < want) {
-        if (RESTORE) {
-          c.cand[r] = key;
-          if (r == want - 1) s->thr_key = key;
-        } else {
-          emit_out<CAPT>(c, row, r, key);
+    for (int p0 = tid; p0 < kept; p0 += U * RT) {
+      uint64_t key[U];
+      int s0[U], cn[U], r[U], mc = 0;
+#pragma unroll
+      for (int u = 0; u < U; ++u) key[u] = p0 + u * RT < kept ? c.sorted[p0 + u * RT] : 0ull;
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        const int b = bucket_of<NBK>(key[u], lo, scale);
+        const bool in = p0 + u * RT < kept;
+        s0[u] = in ? (int)c.hist[b] : 0;
+        cn[u] = in ? (int)c.hist[b + 1] - s0[u] : 0;
+        r[u] = s0[u];
+        mc = cn[u] > mc ? cn[u] : mc;
+      }
+      if (mc > 1) {  // a key alone in its bucket has its rank already
+        for (int j = 0; j < mc; ++j) {
+#pragma unroll
+          for (int u = 0; u < U; ++u)
+            if (j < cn[u]) r[u] += c.sorted[s0[u] + j] < key[u] ? 1 : 0;
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        if (p0 + u * RT < kept && r[u] < want) {
+          if (RESTORE) {
+            c.cand[r[u]] = key[u];
+            if (r[u] == want - 1) s->thr_key = key[u];
+          } else {
+            emit_out<CAPT>(c, row, r[u], key[u]);
+          }
         }
       }
     }
@@ -355,42 +405,37 @@ __device__ __forceinline__ void zero_hist(const RowCtx<CAPT>& c) {
   if (c.tid < 2) h4[CAPT / 4 + c.tid] = make_uint4(0, 0, 0, 0);
 }
 
-// Second look at a row whose sampled bound let the wrong number of elements through (m_seen of them,
-// counted exactly): the bound is moved along the line through (lo, 0) and (hi, m_seen) to where
-// ~1.3 want elements are expected, and the row (still in L2) is filtered again with plain loads into
-// raw entries.  Returns the new inclusive bound; s->cnt holds the number that passed (entries beyond
-// CAPT are not stored).  The caller decides between the counting step and the exact slow path.
+// Second look at a row whose sampled bound let the wrong number of elements through: the row (still in
+// L2) is filtered again against thr_x (an element enters iff !(v >= thr_x)) into raw entries.  s->cnt
+// holds the number that passed (entries beyond CAPT are not stored); the caller decides what follows.
 template <int CAPT>
-__device__ float refilter_row(const RowCtx<CAPT>& c, const float* src, int64_t len, float lo, float hi, int m_seen,
-                              int want) {
+__device__ void refilter_row(const RowCtx<CAPT>& c, const float* src, int64_t len, float thr_x) {
   auto* s = c.s;
-  float f = 1.3f * (float)want / (float)(m_seen > 0 ? m_seen : 1);
-  f = f > 16.f ? 16.f : f;
-  const float nb = lo + (hi - lo) * f;
-  const float thr_x = ord_f32(f32_ord(nb) + 1u);  // inclusive bound nb
   if (c.tid == 0) s->cnt = 0;
   cbar();
   const unsigned lt = (1u << c.lane) - 1u;
   const uint32_t sg = c.a->largest ? 0x80000000u : 0u;
-  const int64_t n32 = (len + 31) & ~(int64_t)31;
-  for (int64_t e0 = (int64_t)c.warp * 32; e0 < n32; e0 += RT) {
-    const int64_t e = e0 + c.lane;
-    float v = 0.f;
-    bool pass = false;
-    if (e < len) {
-      v = flip(src[e], sg);
-      pass = !(v >= thr_x);
+  constexpr int XU = 8;  // loads in flight per thread: the row comes from L2, one load at a time would cost its latency
+  const int64_t nblk = (len + 32 * XU - 1) / (32 * XU);
+  for (int64_t blk = c.warp; blk < nblk; blk += RW) {
+    const int64_t e0 = blk * (32 * XU) + c.lane;
+    float v[XU];
+#pragma unroll
+    for (int u = 0; u < XU; ++u) v[u] = e0 + 32 * u < len ? flip(__ldg(src + e0 + 32 * u), sg) : 0.f;
+#pragma unroll
+    for (int u = 0; u < XU; ++u) {
+      const int64_t e = e0 + 32 * u;
+      const bool pass = e < len && !(v[u] >= thr_x);
+      const unsigned b = __ballot_sync(kFull, pass);
+      if (b == 0u) continue;
+      int base = 0;
+      if (c.lane == 0) base = atomicAdd(&s->cnt, __popc(b));
+      base = __shfl_sync(kFull, base, 0);
+      const int pos = base + __popc(b & lt);
+      if (pass && pos < CAPT) c.cand[pos] = ((uint64_t)(uint32_t)e << 32) | __float_as_uint(v[u]);
     }
-    const unsigned b = __ballot_sync(kFull, pass);
-    if (b == 0u) continue;
-    int base = 0;
-    if (c.lane == 0) base = atomicAdd(&s->cnt, __popc(b));
-    base = __shfl_sync(kFull, base, 0);
-    const int pos = base + __popc(b & lt);
-    if (pass && pos < CAPT) c.cand[pos] = ((uint64_t)(uint32_t)e << 32) | __float_as_uint(v);
   }
   cbar();
-  return nb;
 }
 
 // Exact selection of one row by the paper's scheme: chunks of the row are merged into a
@@ -779,20 +824,57 @@ __global__ void __launch_bounds__(RTHREADS, RowCfg<CAPT>::CTAS) kselect_row_kern
       cbar();
       const int m = s->cnt;
       const int want = (int64_t)k < len ? k : (int)len;
-      if (dfb) {
-        slow_row<CAPT>(c, row, a.orig + row * a.orig_ld, a.n_orig, nullptr);
+      bool fell_back = false;
+      if constexpr (CAPT == 4096) {  // only survivor lists of long rows can be unusable as a whole
+        if (dfb) {
+          slow_row<CAPT>(c, row, a.orig + row * a.orig_ld, a.n_orig, nullptr);
+          fell_back = true;
+        }
+      }
+      if (fell_back) {
       } else if (s->ovf || m < want || m > CAPT) {
-        // the sample did not represent the row (sorted rows, runs): one more filter pass with the bound
-        // rescaled by what this pass counted, then the exact scheme if that fails too
+        // The sample (the head of the row) did not represent the row: sorted rows, runs of equal values.
+        // Second look: a STRIDED sample of the row (it is in L2) searched the same way, one more filter pass
+        // with its bound; then, if the first bound spanned a range, two passes with that bound rescaled by
+        // what the pass before counted; then the paper's scheme, which needs nothing from the distribution.
         bool done = false;
-        if (bd.sampled && bd.hi > bd.lo) {
-          const float nb = refilter_row<CAPT>(c, p, len, bd.lo, bd.hi, m, want);
-          const int m2 = s->cnt;
-          if (m2 >= want && m2 <= CAPT) {
-            count_select<CAPT, false, true>(c, row, m2, want, false, 0.f, 0.f, mp);
-            done = true;
+        {
+          const int S2 = (CAPT >= 2048 && len > 32768) ? 4096 : 2048;  // what scout_bound takes from 2 CAPT floats
+          const int64_t stride = len / S2;
+          if (stride >= 2) {
+            float* smp = reinterpret_cast<float*>(c.sorted);
+            for (int i = tid; i < S2; i += RT) smp[i] = __ldg(p + (int64_t)i * stride);
+            cbar();
+            if (c.warp == 0) {
+              const RowBound b2 = scout_bound<CAPT, LG>(smp, S2, len, k, lane);
+              if (lane == 0) s->fb = b2;
+            }
+            cbar();
+            const RowBound b2 = s->fb;
+            if (b2.sampled) {
+              refilter_row<CAPT>(c, p, len, b2.thr_x);
+              const int m2 = s->cnt;
+              if (m2 >= want && m2 <= CAPT) {
+                count_select<CAPT, false, true>(c, row, m2, want, true, b2.lo, b2.hi, mp);
+                done = true;
+              }
+            }
           }
-          (void)nb;
+        }
+        if (!done && bd.sampled && bd.hi > bd.lo) {
+          float hi = bd.hi;
+          int seen = m;
+          for (int attempt = 0; attempt < 2 && !done; ++attempt) {
+            float f = 1.3f * (float)want / (float)(seen > 0 ? seen : 1);
+            f = f > 16.f ? 16.f : f;
+            hi = bd.lo + (hi - bd.lo) * f;  // along the line through (lo, 0) and (hi, seen)
+            refilter_row<CAPT>(c, p, len, ord_f32(f32_ord(hi) + 1u));
+            seen = s->cnt;
+            if (seen >= want && seen <= CAPT) {
+              count_select<CAPT, false, true>(c, row, seen, want, false, 0.f, 0.f, mp);
+              done = true;
+            }
+          }
         }
         if (!done) slow_row<CAPT>(c, row, p, len, mp);
       } else {
