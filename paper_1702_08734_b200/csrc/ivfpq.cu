@@ -441,8 +441,8 @@ int ivfpq_finalise(fs_ivfpq* ix, cudaStream_t s) {
       ++launch_counter();
     }
     if (ix->n_staged > 0)
-      cudaMemcpyAsync(kA + ix->n_csr, ix->st_list.p, (size_t)ix->n_staged * sizeof(uint32_t),
-                      cudaMemcpyDeviceToDevice, s);
+      FS_CUDA(cudaMemcpyAsync(kA + ix->n_csr, ix->st_list.p, (size_t)ix->n_staged * sizeof(uint32_t),
+                              cudaMemcpyDeviceToDevice, s));
     const uint32_t* vin = nullptr;
     uint32_t *kin = kA, *kout = kB, *vout = vB, *vother = vA;
     for (int pass = 0; pass < passes; ++pass) {
@@ -566,8 +566,9 @@ static int ivfpq_add_device(fs_ivfpq* ix, const float* xb, int64_t n, const int6
                           ix->st_list.as<uint32_t>() + base, ix->st_s1.as<float>() + base, s);
   if (rc == FS_OK) {
     if (ids) {
-      cudaMemcpyAsync(ix->st_ids.as<int64_t>() + base, ids, (size_t)n * sizeof(int64_t),
-                      cudaMemcpyDeviceToDevice, s);
+      const cudaError_t e = cudaMemcpyAsync(ix->st_ids.as<int64_t>() + base, ids, (size_t)n * sizeof(int64_t),
+                                            cudaMemcpyDeviceToDevice, s);
+      if (e != cudaSuccess) rc = set_error(FS_ECUDA, "fs_ivfpq_add: copy of the ids failed: %s", cudaGetErrorString(e));
     } else {
       iota_ids_kernel<<<(unsigned)ceil_div(n, 256), 256, 0, s>>>(ix->st_ids.as<int64_t>() + base, n,
                                                                 first_id);

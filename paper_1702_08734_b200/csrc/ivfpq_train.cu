@@ -118,8 +118,9 @@ int kmeans_device(const float* x, int64_t n, int d, int K, int niter, uint64_t s
     if ((rc = launch_row_norms(cent, K, d, cnorm.as<float>(), s)) != FS_OK) return done(rc);
     if ((rc = assign_nearest(x, n, cent, cnorm.as<float>(), K, d, assign.as<int64_t>(), s)) != FS_OK)
       return done(rc);
-    if (assign_out && it == niter - 1)
-      cudaMemcpyAsync(assign_out, assign.p, (size_t)n * sizeof(int64_t), cudaMemcpyDeviceToDevice, s);
+    if (assign_out && it == niter - 1 &&
+        cudaMemcpyAsync(assign_out, assign.p, (size_t)n * sizeof(int64_t), cudaMemcpyDeviceToDevice, s) != cudaSuccess)
+      return done(set_error(FS_ECUDA, "fs_kmeans: copy of the assignments failed"));
     km_keys_kernel<<<(unsigned)ceil_div(n, 256), 256, 0, s>>>(assign.as<int64_t>(), n, sortws.as<uint32_t>());
     ++launch_counter();
     const uint32_t *keys_sorted = nullptr, *order = nullptr;
