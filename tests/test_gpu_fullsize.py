@@ -121,6 +121,23 @@ def test_cfg3_full_sampled_queries(k):
     assert np.all(np.diff(d_all, axis=1) >= 0) and i_all.min() >= 0 and i_all.max() < nb
 
 
+def test_cfg3_k100_ten_runs_identical_bits():
+    """The flat engine shares bounds between CTAs while they run (gbound / hbound, sampled bound, re-run of
+    failed queries): whatever the interleaving, the output is one fixed answer.  Ten runs of cfg3 at k = 100
+    on integer data and ten on real-valued data (3xTF32) must give identical bits."""
+    from datagen import gen_torch as gt
+    fs = fsmod()
+    nb, nq, k = 1_000_000, 10_000, 100
+    for gen in (gt.sift_like, lambda r0, n: gt.gaussian_vectors(r0, n, 128)):
+        xb, xq = gen(0, nb), gen(nb, nq)
+        d0, i0 = fs.flat_l2_knn(xq, xb, k)
+        for _ in range(9):
+            d1, i1 = fs.flat_l2_knn(xq, xb, k)
+            assert torch.equal(i0, i1)
+            assert torch.equal(d0.view(torch.int32), d1.view(torch.int32))
+        del xb, xq
+
+
 def test_cfg4_shaped_index():
     from datagen import gen_torch as gt
     from test_gpu_ivfpq import check_search
