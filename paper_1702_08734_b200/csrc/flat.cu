@@ -508,7 +508,7 @@ int flat_validate(const void* xq, int64_t nq, const void* xb, int64_t nb, int d,
 extern "C" {
 
 const char* fs_flat_engine(void) {
-  return fs::flat_tc_supported(128) ? "tcgen05-3xtf32 (d % 32 == 0, d <= 128; ffma-fp32 otherwise)" : "ffma-fp32";
+  return fs::flat_tc_supported(128) ? "tcgen05-3xtf32 (d % 4 == 0, 32 <= d <= 128; ffma-fp32 otherwise)" : "ffma-fp32";
 }
 
 size_t fs_flat_l2_knn_ws_bytes(int64_t nq, int64_t nb, int d, int k) {

@@ -37,7 +37,7 @@ struct FlatTcPlan {
   int c;
   size_t off_fail, off_failq, off_qfhi, off_qflo, off_sub;  // fail list, gathered failed queries, the sample pass's own plan
 };
-bool flat_tc_supported(int d);  // d % 32 == 0, 32 <= d <= 128, not disabled by FS_FLAT_ENGINE=ffma
+bool flat_tc_supported(int d);  // d % 4 == 0, 32 <= d <= 128, not disabled by FS_FLAT_ENGINE=ffma
 FlatTcPlan flat_tc_plan(int64_t nq, int64_t nb, int d, int k);
 // dout != NULL: distance-matrix mode -- no selection, dout[q * dld + j] = ||y_j||^2 - 2 <x_q, y_j>
 // (dld % 4 == 0, dout 16-byte aligned); k, out_dist and out_ids are ignored, the workspace is that of k = 1.

@@ -127,7 +127,11 @@ __global__ void __launch_bounds__(256)
                     const unsigned int* __restrict__ flag) {
   if (*flag == 0u) return;  // every lo is zero: the kernel issues hi * hi only and never reads the plane
   for (int64_t i = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) * 4; i < n_elems; i += (int64_t)gridDim.x * blockDim.x * 4) {
-    const float4 v = *reinterpret_cast<const float4*>(x + i);  // n_elems = rows * d, d % 32 == 0
+    float4 v;  // n_elems = rows * d, d % 4 == 0; x itself may be misaligned (lo is ours: aligned)
+    if ((reinterpret_cast<uintptr_t>(x) & 15u) == 0)
+      v = *reinterpret_cast<const float4*>(x + i);
+    else
+      v = make_float4(x[i], x[i + 1], x[i + 2], x[i + 3]);
     float4 l;
     l.x = __uint_as_float(__float_as_uint(v.x - __uint_as_float(__float_as_uint(v.x) & 0xFFFFE000u)) & 0xFFFFE000u);
     l.y = __uint_as_float(__float_as_uint(v.y - __uint_as_float(__float_as_uint(v.y) & 0xFFFFE000u)) & 0xFFFFE000u);
@@ -674,7 +678,10 @@ bool flat_tc_supported(int d) {
     const char* e = getenv("FS_FLAT_ENGINE");
     forced_off = (e && strcmp(e, "ffma") == 0) ? 1 : 0;
   }
-  return !forced_off && d % BK == 0 && d >= BK && d <= 128;
+  // d need not be a multiple of the 32-column stage: the tensor maps are built on the real d, TMA fills the
+  // columns of the last stage that lie beyond it with zeros, and zeros add nothing to <x, y>.  Rows must be
+  // 16-byte multiples for TMA (d % 4 == 0).
+  return !forced_off && d % 4 == 0 && d >= BK && d <= 128;
 }
 
 // Every extra split is one more partial queue per query (more survivors in the epilogue,
@@ -787,7 +794,7 @@ static FlatTcPlan flat_tc_plan_base(int64_t nq, int64_t nb, int d, int k, bool s
   p.S = (int)ceil_div(nb > 0 ? nb : 1, p.chunk);
   const int64_t items = (int64_t)p.S * qgroups;
   p.grid = (int)(items < ncl ? items : ncl) * CLUSTER;
-  p.KB = d / BK;
+  p.KB = (d + BK - 1) / BK;  // the last stage may be partial (zero-filled by TMA)
   p.cap = p.K + 128;  // the restore step runs when fewer than 64 more keys would fit
   // the kernel carves the ring at run time (the lo plane of the query tile is only
   // resident in 3xTF32 mode); worst case = with the lo plane

@@ -58,6 +58,8 @@ def test_cfg1_tiny_full():
     (1, 1, 1, 1), (3, 5, 2, 3), (65, 129, 3, 7), (70, 1000, 17, 32), (130, 3001, 64, 33),
     (64, 2500, 128, 100), (33, 777, 96, 128), (17, 5000, 100, 1024), (200, 4099, 24, 1),
     (5, 300, 130, 400),
+    # d % 32 != 0 on the tensor-core engine: the last 32-column stage is partly zero-filled by TMA
+    (40, 3000, 36, 10), (128, 2000, 68, 50), (260, 9000, 100, 10), (33, 4000, 124, 1),
 ])
 def test_shapes_real_valued(nq, nb, d, k):
     rng = np.random.default_rng(nq * 7 + nb)
@@ -66,6 +68,42 @@ def test_shapes_real_valued(nq, nb, d, k):
     _, _, od64 = oracle.flat_l2_knn(xq, xb, k, want64=True)
     gd, gi = run(xq, xb, k)
     check_acceptance(xq, xb, k, gd, gi, od64)
+
+
+def test_misaligned_operands():
+    """Operands that start 4 bytes off a 16-byte boundary: TMA cannot read them in place, the engine
+    works on truncated copies; real-valued data so that the lo planes are read too."""
+    import paper_1702_08734_b200 as fs
+    rng = np.random.default_rng(5)
+    nq, nb, d, k = 70, 6000, 96, 10
+    xb = rng.standard_normal((nb, d)).astype(np.float32)
+    xq = rng.standard_normal((nq, d)).astype(np.float32)
+    bb = torch.empty(nb * d + 1, dtype=torch.float32, device="cuda")
+    qq = torch.empty(nq * d + 1, dtype=torch.float32, device="cuda")
+    tb, tq = bb[1:].view(nb, d), qq[1:].view(nq, d)
+    tb.copy_(torch.from_numpy(xb))
+    tq.copy_(torch.from_numpy(xq))
+    assert tb.data_ptr() % 16 == 4 and tq.data_ptr() % 16 == 4
+    gd, gi = fs.flat_l2_knn(tq, tb, k)
+    torch.cuda.synchronize()
+    _, _, od64 = oracle.flat_l2_knn(xq, xb, k, want64=True)
+    check_acceptance(xq, xb, k, gd.cpu().numpy(), gi.cpu().numpy(), od64)
+
+
+@pytest.mark.parametrize("d", [36, 100])
+def test_partial_last_stage_integer_data_bit_exact(d):
+    """d % 32 != 0 through the tensor-core engine (zero-filled tail of the last stage): small-integer data,
+    where every product and partial sum is an exact fp32 integer, must equal the oracle bit for bit."""
+    import paper_1702_08734_b200 as fs
+    assert "d % 4" in fs.flat_engine()
+    rng = np.random.default_rng(d)
+    xb = rng.integers(0, 256, (20000, d)).astype(np.float32)
+    xq = rng.integers(0, 256, (300, d)).astype(np.float32)
+    xb[777] = xq[5]  # an exact duplicate: distance 0
+    for k in (1, 10, 100):
+        od, oi = oracle.flat_l2_knn(xq, xb, k)
+        gd, gi = run(xq, xb, k)
+        assert np.array_equal(gi, oi) and np.array_equal(gd, od)
 
 
 @pytest.mark.parametrize("k", [1, 10, 100])
