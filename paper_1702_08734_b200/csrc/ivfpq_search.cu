@@ -427,16 +427,16 @@ __global__ void __launch_bounds__(SCAN_THREADS, qs_ctas<NQ>())
     __syncthreads();  // C: pass prefix
     if (warp == 0 && prev_item >= 0) {
       // C4, second half: the previous item's eight queues -> one (the other warps are already scanning)
-      WarpSelect<NQ, NB> ms;
-      ms.init(bufs, lane);  // warp 0's own batch area is idle between its items
-      for (int e0 = 0; e0 < SCAN_WARPS * K; e0 += 32) {
-        const uint64_t key = merge[((round - 1) & 1) * (SCAN_WARPS * K) + e0 + lane];
-        ms.push(key < ms.thr, key);
-      }
-      ms.finish();
+      // (every parked queue is sorted: a tree of bitonic merges, not 8 K pushes through a selection queue)
+      const uint64_t* area = merge + ((round - 1) & 1) * (SCAN_WARPS * K);
+      uint64_t Wm[NQ];
+#pragma unroll
+      for (int rr = 0; rr < NQ; ++rr) Wm[rr] = area[rr * 32 + lane];
+#pragma unroll 1
+      for (int w8 = 1; w8 < SCAN_WARPS; ++w8) merge_sorted_queue<NQ>(Wm, area + w8 * K, lane);
       uint64_t* W = a.Wg + prev_item * K;
 #pragma unroll
-      for (int rr = 0; rr < NQ; ++rr) W[rr * 32 + lane] = ms.W[rr];
+      for (int rr = 0; rr < NQ; ++rr) W[rr * 32 + lane] = Wm[rr];
       __syncwarp();
     }
     if (!live) break;

@@ -115,6 +115,16 @@ __device__ __forceinline__ void merge_lane_stride(uint64_t (&W)[NQ], int lane) {
   }
 }
 
+// Merge another ascending queue of 32*NQ keys (lane-stride in memory: element e at other[e]) into the
+// ascending lane-stride queue W, keeping the 32*NQ smallest: half-cleaner against the reversed other
+// queue, then the bitonic merge.  Warp-collective.
+template <int NQ>
+__device__ __forceinline__ void merge_sorted_queue(uint64_t (&W)[NQ], const uint64_t* other, int lane) {
+#pragma unroll
+  for (int r = 0; r < NQ; ++r) W[NQ - 1 - r] = umin64(W[NQ - 1 - r], other[r * 32 + (31 - lane)]);
+  merge_lane_stride<NQ>(W, lane);
+}
+
 // Shared-memory words (uint64) one warp's candidate batch needs.
 template <int NB>
 __host__ __device__ constexpr int warp_select_smem_keys() {
