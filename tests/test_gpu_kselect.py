@@ -125,6 +125,33 @@ def test_batch_rows_that_mislead_the_sample(k):
     assert_exact(rows, k)
 
 
+@pytest.mark.parametrize("n", [8191, 8192, 8193, 8199, 12288 + 5, 16384 + 1, 20000])
+def test_stage_boundaries_of_the_k1024_class(n):
+    """k > 256: rows of >= 8 192 elements keep the counting arrays in the row's last two ring stages (16 KB
+    each), shorter rows in arrays of their own.  Lengths around the switch and around stage ends, a row
+    start that is not 16-byte aligned, more rows than resident CTAs (the ring wraps, stages are held and
+    handed back many times), rows that take the second look / the slow path with the aliased arrays."""
+    import paper_1702_08734_b200 as fs
+    rng = np.random.default_rng(n)
+    nr = 1500
+    big = rng.random((nr, n + 3), dtype=np.float32)
+    big[3, :] = np.sort(big[3, :])                      # ascending: the head misleads the sample
+    big[4, :] = np.sort(big[4, :])[::-1]                # descending
+    big[5, :] = 0.25                                    # constant: everything ties
+    big[6, :] = np.floor(big[6, :] * 4)                 # four distinct values
+    big[7, :n // 2] += 2.0                              # the small values come late
+    t = torch.from_numpy(big).cuda()
+    for off in (0, 1):
+        view = t[:, off:off + n]
+        host = np.ascontiguousarray(big[:, off:off + n])
+        for k in (257, 1024):
+            gv, gi = fs.kselect(view, k)
+            torch.cuda.synchronize()
+            ev, ei = oracle.kselect(host, k)
+            assert np.array_equal(gi.cpu().numpy(), ei), (n, off, k)
+            assert np.array_equal(gv.cpu().numpy().view(np.uint32), ev.view(np.uint32)), (n, off, k)
+
+
 def assert_exact_largest(rows_np, k, n=None):
     import paper_1702_08734_b200 as fs
     ev, ei = oracle.kselect(rows_np, k, n=n, largest=True)
