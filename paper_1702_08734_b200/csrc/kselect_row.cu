@@ -100,6 +100,8 @@ struct RowBound {
 
 struct RowSharedBase {       // what the selection steps use
   RowBound fb;               // bound of a row's second look (strided sample)
+  RowBound cur;              // the bound of the row the consumers are on, and its length: parked here from row
+  long long cur_len;         // begin to row end instead of riding through the stages in five registers
   unsigned int redu[2][RW];
   int cnt, ovf;              // candidates appended, overflow flag
   int kb, kept, maxc;        // counting step: boundary bucket, keys in buckets <= kb, largest such bucket
@@ -733,13 +735,8 @@ __global__ void __launch_bounds__(RTHREADS, RowCfg<CAPT, AL>::CTAS) kselect_row_
   const int k = a.k;
   const uint32_t cnt_addr = smem_addr(&s->cnt), ring_sa = smem_addr(c.ring), cand_sa = smem_addr(c.cand);
   uint32_t stage = 0;
-  RowBound bd;
-  bd.thr_x = 0.f;
-  bd.lo = bd.hi = 0.f;
-  bd.sampled = 0;
-  int64_t len = 0, head = 0;
-  const float* p = nullptr;
-  const uint32_t* mp = nullptr;
+  float row_thr = 0.f;  // the row's bound (RowBound::thr_x)
+  int head = 0;
   for (;;) {
     const int slot = (int)(stage % NST);
     const uint32_t par = (stage / NST) & 1u;
@@ -750,14 +747,18 @@ __global__ void __launch_bounds__(RTHREADS, RowCfg<CAPT, AL>::CTAS) kselect_row_
     const bool held = AL && seg >= s->desc[slot].nseg - HOLD;  // a stage the row's counting step will use
     if (seg == 0) {
       // ---- row begin ----
-      len = s->desc[slot].len;
-      p = a.vals + row * a.ld;
-      mp = a.map ? a.map + row * a.ld : nullptr;
-      head = (4 - (int64_t)(((uintptr_t)p >> 2) & 3)) & 3;
-      if (head > len) head = len;
+      const int64_t len = s->desc[slot].len;
+      const float* p = a.vals + row * a.ld;
+      head = (4 - (int)(((uintptr_t)p >> 2) & 3)) & 3;
+      if (head > len) head = (int)len;
       if (!AL) zero_hist<CAPT>(c);
       mbar_wait(&s->bnd[slot], par);
-      bd = s->bound[slot];
+      const RowBound bd = s->bound[slot];
+      row_thr = bd.thr_x;
+      if (tid == 0) {
+        s->cur = bd;
+        s->cur_len = len;
+      }
       // head and tail scalars around the aligned body (plain loads)
       const int64_t body = ((len - head) >> 2) << 2;
       const int64_t ntail = len - head - body;
@@ -776,7 +777,7 @@ __global__ void __launch_bounds__(RTHREADS, RowCfg<CAPT, AL>::CTAS) kselect_row_
     // ---- A1: first-level filter over this stage (4 VPT elements per thread) ----
     if (dcnt > 0) {
       const int nvec = dcnt >> 2;
-      const float thr_x = fl<LG>(bd.thr_x);  // -v < t  <=>  v > -t
+      const float thr_x = fl<LG>(row_thr);  // -v < t  <=>  v > -t
       const uint32_t st_sa = ring_sa + (uint32_t)slot * STRIDE + (uint32_t)tid * 16u;
       float4 x[VPT];
       uint32_t mask = 0u;
@@ -832,7 +833,7 @@ __global__ void __launch_bounds__(RTHREADS, RowCfg<CAPT, AL>::CTAS) kselect_row_
             s->ovf = 1;
           } else {
             uint32_t addr = cand_sa + (uint32_t)base * 8u;
-            const uint32_t ib = (uint32_t)(head + (int64_t)seg * SEG) + (uint32_t)tid * 4u;
+            const uint32_t ib = (uint32_t)head + (uint32_t)seg * SEG + (uint32_t)tid * 4u;
             while (mask) {
               const int j = __ffs(mask) - 1;
               mask &= mask - 1u;
@@ -863,7 +864,13 @@ __global__ void __launch_bounds__(RTHREADS, RowCfg<CAPT, AL>::CTAS) kselect_row_
         cbar();
       }
       const int m = s->cnt;
+      const RowBound bd = s->cur;
+      const int64_t len = s->cur_len;
       const int want = (int64_t)k < len ? k : (int)len;
+      // the row's base and map again: carried through the stages they cost four registers, and the k <= 1 024
+      // class with 16 KB stages then spills (44 bytes; 3 % of the cfg2 k = 1 024 call)
+      const float* p = a.vals + row * a.ld;
+      const uint32_t* mp = a.map ? a.map + row * a.ld : nullptr;
       bool fell_back = false;
       if constexpr (CAPT == 4096) {  // only survivor lists of long rows can be unusable as a whole
         if (dfb) {
