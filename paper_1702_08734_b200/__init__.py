@@ -54,7 +54,7 @@ def lib():
         L.fs_launch_count.restype = _i64
         L.fs_reset_launch_count.restype = None
         for name in ("fs_kselect_ws_bytes", "fs_flat_l2_knn_ws_bytes", "fs_ivfpq_search_ws_bytes",
-                     "fs_merge_topk_ws_bytes", "fs_kselect_noalloc_max_scratch"):
+                     "fs_merge_topk_ws_bytes", "fs_kselect_noalloc_max_scratch", "fs_flat_prepare_bytes"):
             if hasattr(L, name):
                 getattr(L, name).restype = _sz
         for name in ("fs_ivfpq_ntotal", "fs_ivfpq_last_scanned_codes"):
@@ -178,8 +178,9 @@ def flat_l2_knn_ws_bytes(nq: int, nb: int, d: int, k: int) -> int:
     return int(lib().fs_flat_l2_knn_ws_bytes(_i64(nq), _i64(nb), _int(d), _int(k)))
 
 
-def flat_l2_knn(xq: torch.Tensor, xb: torch.Tensor, k: int, out_dist=None, out_ids=None, ws=None):
-    """fs_flat_l2_knn: exact squared-L2 k-NN; returns (dist fp32 [nq,k], ids int64 [nq,k])."""
+def flat_l2_knn(xq: torch.Tensor, xb: torch.Tensor, k: int, out_dist=None, out_ids=None, ws=None, prep=None):
+    """fs_flat_l2_knn (prep given: fs_flat_l2_knn_prepared, prep from flat_prepare(xb)): exact squared-L2
+    k-NN; returns (dist fp32 [nq,k], ids int64 [nq,k])."""
     _dev(xq, torch.float32, "xq")
     _dev(xb, torch.float32, "xb")
     nq, d = xq.shape
@@ -190,10 +191,28 @@ def flat_l2_knn(xq: torch.Tensor, xb: torch.Tensor, k: int, out_dist=None, out_i
         out_dist = torch.empty((nq, k), dtype=torch.float32, device=xq.device)
     if out_ids is None:
         out_ids = torch.empty((nq, k), dtype=torch.int64, device=xq.device)
+    wsz = _sz(0 if ws is None else ws.numel() * ws.element_size())
+    if prep is not None:
+        _check(lib().fs_flat_l2_knn_prepared(_ptr(xq), _i64(nq), _ptr(xb), _ptr(prep),
+                                             _sz(prep.numel() * prep.element_size()), _i64(nb), _int(d), _int(k),
+                                             _ptr(out_dist), _ptr(out_ids), _ptr(ws), wsz, _stream()))
+        return out_dist, out_ids
     _check(lib().fs_flat_l2_knn(_ptr(xq), _i64(nq), _ptr(xb), _i64(nb), _int(d), _int(k),
-                                _ptr(out_dist), _ptr(out_ids), _ptr(ws),
-                                _sz(0 if ws is None else ws.numel() * ws.element_size()), _stream()))
+                                _ptr(out_dist), _ptr(out_ids), _ptr(ws), wsz, _stream()))
     return out_dist, out_ids
+
+
+def flat_prepare(xb: torch.Tensor, prep: torch.Tensor | None = None) -> torch.Tensor:
+    """fs_flat_prepare: the database's share of the pre-pass (norms, operand split), once.  Returns the
+    prepared block (a uint8 CUDA tensor of fs_flat_prepare_bytes) for flat_l2_knn(..., prep=...)."""
+    _dev(xb, torch.float32, "xb")
+    nb, d = xb.shape
+    need = int(lib().fs_flat_prepare_bytes(_i64(nb), _int(d)))
+    if prep is None:
+        prep = torch.empty(need, dtype=torch.uint8, device=xb.device)
+    _check(lib().fs_flat_prepare(_ptr(xb), _i64(nb), _int(d), _ptr(prep), _sz(prep.numel() * prep.element_size()),
+                                 _stream()))
+    return prep
 
 
 def flat_l2_knn_host(xq, xb, k: int, out_dist=None, out_ids=None):

@@ -454,8 +454,9 @@ FlatPlan flat_plan(int64_t nq, int64_t nb, int d, int k) {
 
 int flat_knn_device(const float* xq, int64_t nq, const float* xb, int64_t nb, int d, int k,
                     const float* ynorm_opt, float* out_dist, int64_t* out_ids, void* ws,
-                    cudaStream_t s) {
-  if (flat_tc_supported(d)) return flat_knn_tc_device(xq, nq, xb, nb, d, k, out_dist, out_ids, ws, s);
+                    cudaStream_t s, const FlatPrep* prep) {
+  if (flat_tc_supported(d)) return flat_knn_tc_device(xq, nq, xb, nb, d, k, out_dist, out_ids, ws, s, nullptr, 0, prep);
+  if (prep != nullptr && ynorm_opt == nullptr) ynorm_opt = prep->ynorm;
   const FlatPlan p = flat_plan(nq, nb, d, k);
   char* w = static_cast<char*>(ws);
   float* ynorm = reinterpret_cast<float*>(w + p.off_ynorm);
@@ -516,8 +517,8 @@ size_t fs_flat_l2_knn_ws_bytes(int64_t nq, int64_t nb, int d, int k) {
   return fs::flat_plan(nq, nb, d, k).bytes;
 }
 
-int fs_flat_l2_knn(const float* xq, int64_t nq, const float* xb, int64_t nb, int d, int k,
-                   float* out_dist, int64_t* out_ids, void* ws, size_t ws_bytes, fs_stream stream) {
+static int flat_l2_knn_entry(const float* xq, int64_t nq, const float* xb, int64_t nb, int d, int k, float* out_dist,
+                             int64_t* out_ids, void* ws, size_t ws_bytes, fs_stream stream, const void* prep) {
   int rc = fs::flat_validate(xq, nq, xb, nb, d, k, out_dist, out_ids);
   if (rc != FS_OK) return rc;
   if (nq == 0) return FS_OK;
@@ -531,7 +532,41 @@ int fs_flat_l2_knn(const float* xq, int64_t nq, const float* xb, int64_t nb, int
   fs::TempWs t;
   rc = t.acquire(ws, ws_bytes, fs::flat_plan(nq, nb, d, k).bytes, s);
   if (rc != FS_OK) return rc;
-  return fs::flat_knn_device(xq, nq, xb, nb, d, k, nullptr, out_dist, out_ids, t.ptr, s);
+  fs::FlatPrep view;
+  if (prep) view = fs::flat_prep_view(prep, nb, d);
+  return fs::flat_knn_device(xq, nq, xb, nb, d, k, nullptr, out_dist, out_ids, t.ptr, s, prep ? &view : nullptr);
+}
+
+int fs_flat_l2_knn(const float* xq, int64_t nq, const float* xb, int64_t nb, int d, int k,
+                   float* out_dist, int64_t* out_ids, void* ws, size_t ws_bytes, fs_stream stream) {
+  return flat_l2_knn_entry(xq, nq, xb, nb, d, k, out_dist, out_ids, ws, ws_bytes, stream, nullptr);
+}
+
+size_t fs_flat_prepare_bytes(int64_t nb, int d) {
+  if (nb < 0 || d < 1 || d > 2048 || nb >= (1LL << 31)) return 0;
+  return fs::flat_prep_bytes(nb, d);
+}
+
+int fs_flat_prepare(const float* xb, int64_t nb, int d, void* prep, size_t prep_bytes, fs_stream stream) {
+  if (nb < 0 || d < 1) return fs::set_error(FS_EINVAL, "fs_flat_prepare: nb >= 0 and d >= 1");
+  if (d > 2048 || nb >= (1LL << 31)) return fs::set_error(FS_EUNSUPPORTED, "fs_flat_prepare: d <= 2048, nb < 2^31");
+  if (!prep || (nb > 0 && !xb)) return fs::set_error(FS_EINVAL, "fs_flat_prepare: NULL pointer");
+  if ((reinterpret_cast<uintptr_t>(prep) & 255u) != 0) return fs::set_error(FS_EINVAL, "fs_flat_prepare: prep must be 256-byte aligned");
+  if (prep_bytes < fs::flat_prep_bytes(nb, d))
+    return fs::set_error(FS_EINVAL, "fs_flat_prepare: prep holds %zu bytes, %zu needed", prep_bytes, fs::flat_prep_bytes(nb, d));
+  return fs::flat_prepare_device(xb, nb, d, prep, static_cast<cudaStream_t>(stream));
+}
+
+int fs_flat_l2_knn_prepared(const float* xq, int64_t nq, const float* xb, const void* prep, size_t prep_bytes, int64_t nb,
+                            int d, int k, float* out_dist, int64_t* out_ids, void* ws, size_t ws_bytes,
+                            fs_stream stream) {
+  if (!prep) return fs::set_error(FS_EINVAL, "fs_flat_l2_knn_prepared: prep is NULL");
+  if ((reinterpret_cast<uintptr_t>(prep) & 255u) != 0)
+    return fs::set_error(FS_EINVAL, "fs_flat_l2_knn_prepared: prep must be 256-byte aligned");
+  if (nb >= 0 && d >= 1 && d <= 2048 && nb < (1LL << 31) && prep_bytes < fs::flat_prep_bytes(nb, d))
+    return fs::set_error(FS_EINVAL, "fs_flat_l2_knn_prepared: prep holds %zu bytes, %zu needed", prep_bytes,
+                         fs::flat_prep_bytes(nb, d));
+  return flat_l2_knn_entry(xq, nq, xb, nb, d, k, out_dist, out_ids, ws, ws_bytes, stream, prep);
 }
 
 size_t fs_merge_topk_ws_bytes(int64_t nq, int G, int k) {

@@ -20,11 +20,23 @@ FlatPlan flat_plan(int64_t nq, int64_t nb, int d, int k);
 // ||row||^2 for n rows of x [n][d] (B1).
 int launch_row_norms(const float* x, int64_t n, int d, float* out, cudaStream_t s);
 
-// Exact k-NN on device buffers.  ynorm_opt: precomputed ||y||^2 [nb] or NULL.
-// ws must hold flat_plan(...).bytes.  nq > 0, nb > 0.
+// The database side of B1 done once (fs_flat_prepare; the ||y_j||^2 do not depend on the queries):
+// views into the caller's prepared block.  Layout (flat_tc.cu): 256-byte header (word 0: some lo of the database
+// is non-zero) | ||y||^2 with the tile padding of the tensor-core engine | tensor-core engine: the lo plane.
+struct FlatPrep {
+  const float* ynorm;        // [nb] (+ padding)
+  const unsigned int* flag;  // tensor-core engine: the database's lo flag; NULL on the FFMA engine
+  const float* blo;          // tensor-core engine: lo plane [nb][d] (zeros where x is a TF32 number)
+};
+size_t flat_prep_bytes(int64_t nb, int d);
+int flat_prepare_device(const float* xb, int64_t nb, int d, void* prep, cudaStream_t s);
+FlatPrep flat_prep_view(const void* prep, int64_t nb, int d);
+
+// Exact k-NN on device buffers.  ynorm_opt: precomputed ||y||^2 [nb] or NULL (FFMA engine); prep: the
+// prepared database or NULL (both engines).  ws must hold flat_plan(...).bytes.  nq > 0, nb > 0.
 int flat_knn_device(const float* xq, int64_t nq, const float* xb, int64_t nb, int d, int k,
                     const float* ynorm_opt, float* out_dist, int64_t* out_ids, void* ws,
-                    cudaStream_t s);
+                    cudaStream_t s, const FlatPrep* prep = nullptr);
 
 // Tensor-core engine (flat_tc.cu): tcgen05 / TMEM / TMA, 3xTF32 split operands.
 struct FlatTcPlan {
@@ -42,7 +54,8 @@ FlatTcPlan flat_tc_plan(int64_t nq, int64_t nb, int d, int k);
 // dout != NULL: distance-matrix mode -- no selection, dout[q * dld + j] = ||y_j||^2 - 2 <x_q, y_j>
 // (dld % 4 == 0, dout 16-byte aligned); k, out_dist and out_ids are ignored, the workspace is that of k = 1.
 int flat_knn_tc_device(const float* xq, int64_t nq, const float* xb, int64_t nb, int d, int k, float* out_dist,
-                       int64_t* out_ids, void* ws, cudaStream_t s, float* dout = nullptr, int64_t dld = 0);
+                       int64_t* out_ids, void* ws, cudaStream_t s, float* dout = nullptr, int64_t dld = 0,
+                       const FlatPrep* prep = nullptr);
 
 // B4: S partial queues per query -> k results (+||x||^2 if xnorm != NULL).
 // Optional extras of the sampled-bound scheme of the tensor-core engine (flat_tc.cu):

@@ -37,6 +37,14 @@ def test_argument_validation_needs_no_gpu(L):
     assert L.fs_flat_l2_knn(one, i64(1), one, i64(1), ci(0), ci(1), one, one, vp(0), sz(0), vp(0)) == 1
     assert L.fs_flat_l2_knn(one, i64(1), one, i64(1), ci(4), ci(5000), one, one, vp(0), sz(0), vp(0)) == 2
     assert L.fs_flat_l2_knn(one, i64(-1), one, i64(1), ci(4), ci(1), one, one, vp(0), sz(0), vp(0)) == 1
+    # prepared database: NULL / misaligned / too small block, sizes
+    L.fs_flat_prepare_bytes.restype = sz
+    assert L.fs_flat_prepare_bytes(i64(-1), ci(4)) == 0 and L.fs_flat_prepare_bytes(i64(1000), ci(64)) >= 1000 * 4
+    assert L.fs_flat_prepare(one, i64(10), ci(4), vp(0), sz(1 << 20), vp(0)) == 1
+    assert L.fs_flat_prepare(one, i64(10), ci(4), vp(256 + 16), sz(1 << 20), vp(0)) == 1
+    assert L.fs_flat_prepare(one, i64(10), ci(4), vp(256), sz(8), vp(0)) == 1
+    assert L.fs_flat_l2_knn_prepared(one, i64(1), one, vp(0), sz(0), i64(1), ci(4), ci(1), one, one, vp(0), sz(0), vp(0)) == 1
+    assert L.fs_flat_l2_knn_prepared(one, i64(1), one, vp(256), sz(8), i64(1), ci(4), ci(1), one, one, vp(0), sz(0), vp(0)) == 1
     h = vp()
     assert L.fs_ivfpq_create(ctypes.byref(h), ci(96), ci(16), ci(7)) == 1    # d % M != 0
     assert L.fs_ivfpq_create(ctypes.byref(h), ci(256), ci(16), ci(128)) == 2  # M > 64

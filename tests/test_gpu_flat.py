@@ -200,3 +200,76 @@ def test_mma_ignores_low_mantissa_bits():
         assert r.returncode == 0, r.stderr[-2000:]
         outs.append(r.stdout)
     assert outs[0] == outs[1] and len(outs[0]) > 0
+
+
+def _both(xq, xb, k, view_off=0):
+    """(unprepared, prepared) results of the same search; xb may be a column-offset view start (misaligned)."""
+    import paper_1702_08734_b200 as fs
+    q = torch.from_numpy(xq).cuda()
+    if view_off:
+        flat = torch.zeros(xb.size + view_off, dtype=torch.float32, device="cuda")
+        flat[view_off:] = torch.from_numpy(xb).cuda().reshape(-1)
+        b = flat[view_off:].view(xb.shape)
+    else:
+        b = torch.from_numpy(xb).cuda()
+    d0, i0 = fs.flat_l2_knn(q, b, k)
+    prep = fs.flat_prepare(b)
+    d1, i1 = fs.flat_l2_knn(q, b, k, prep=prep)
+    d2, i2 = fs.flat_l2_knn(q, b, k, prep=prep)  # the block is only read: a second call sees the same
+    torch.cuda.synchronize()
+    assert torch.equal(d1, d2) and torch.equal(i1, i2)
+    return (d0.cpu().numpy(), i0.cpu().numpy()), (d1.cpu().numpy(), i1.cpu().numpy())
+
+
+@pytest.mark.parametrize("k", [1, 10, 100])
+def test_prepared_database_integer_data_bit_exact(k):
+    """fs_flat_prepare + fs_flat_l2_knn_prepared (the ||y||^2 of Eq. 2 computed once): the oracle's
+    result bit for bit on integer data, on a database large enough for the sampled bound."""
+    xb = datagen.sift_like(0, 40000)
+    xq = datagen.sift_like(1_000_000, 150)
+    xb[5000:5040] = xb[100:140]
+    od, oi = oracle.flat_l2_knn(xq, xb, k)
+    (d0, i0), (d1, i1) = _both(xq, xb, k)
+    assert np.array_equal(i1, oi) and np.array_equal(d1.view(np.uint32), od.view(np.uint32))
+    assert np.array_equal(i0, i1) and np.array_equal(d0.view(np.uint32), d1.view(np.uint32))
+
+
+@pytest.mark.parametrize("case", ["real", "int_db_real_q", "real_db_int_q", "ffma_d30", "ffma_d200", "misaligned"])
+def test_prepared_database_equals_the_plain_call(case):
+    """Same bits as fs_flat_l2_knn in every operand-split situation: both sides real-valued (3xTF32), only
+    the queries (the database's lo plane is zeros but is read), only the database, dimensions of the FFMA
+    engine (the block holds the norms only), a database TMA cannot read in place (the block is not used)."""
+    rng = np.random.default_rng(7)
+    d = {"ffma_d30": 30, "ffma_d200": 200}.get(case, 96)
+    nb, nq = 20000, 70
+    xb = rng.standard_normal((nb, d)).astype(np.float32)
+    xq = rng.standard_normal((nq, d)).astype(np.float32)
+    if case == "int_db_real_q":
+        xb = np.rint(xb * 8).astype(np.float32)
+    if case == "real_db_int_q":
+        xq = np.rint(xq * 8).astype(np.float32)
+    for k in (1, 10, 100):
+        (d0, i0), (d1, i1) = _both(xq, xb, k, view_off=1 if case == "misaligned" else 0)
+        assert np.array_equal(i0, i1) and np.array_equal(d0.view(np.uint32), d1.view(np.uint32)), (case, k)
+    _, _, od64 = oracle.flat_l2_knn(xq, xb, 10, want64=True)
+    (_, _), (d1, i1) = _both(xq, xb, 10)
+    check_acceptance(xq, xb, 10, d1, i1, od64)
+
+
+def test_prepared_database_errors_and_empty():
+    import paper_1702_08734_b200 as fs
+    xb = torch.zeros((100, 64), device="cuda")
+    xq = torch.zeros((4, 64), device="cuda")
+    prep = fs.flat_prepare(xb)
+    assert prep.numel() == fs.lib().fs_flat_prepare_bytes(100, 64) > 100 * 4
+    with pytest.raises(fs.FsError):
+        fs.flat_l2_knn(xq, xb, 3, prep=prep[:256])          # too small
+    with pytest.raises(fs.FsError):
+        fs.flat_l2_knn(xq, xb, 3, prep=prep[16:])           # misaligned (and too small)
+    with pytest.raises(fs.FsError):
+        fs.flat_prepare(xb, prep=torch.empty(64, dtype=torch.uint8, device="cuda"))
+    e = torch.zeros((0, 64), device="cuda")
+    d, i = fs.flat_l2_knn(xq, e, 3, prep=fs.flat_prepare(e))
+    assert np.all(i.cpu().numpy() == -1) and np.all(np.isposinf(d.cpu().numpy()))
+    d, i = fs.flat_l2_knn(xq, xb, 3, prep=prep)             # all-zero data: every distance 0, ids 0..2
+    assert i.cpu().numpy().tolist() == [[0, 1, 2]] * 4 and np.all(d.cpu().numpy() == 0)
