@@ -188,6 +188,11 @@ __global__ void pq_bmax_kernel(const float* __restrict__ pq, float* __restrict__
 // (c % REP) * M + m, REP = 32 / M, so that a warp reads 32 consecutive words and its stores of the
 // replicated table are conflict-free.
 // ---------------------------------------------------------------------------
+#ifndef FS_QT_QPB
+#define FS_QT_QPB 8
+#endif
+constexpr int QT_QPB = FS_QT_QPB;  // queries per block of ivfpq_qtable_kernel
+
 struct QMeta {
   float inv_scale;  // 2^-se
   uint32_t isum;    // sum_m b_m * 2^se (exact integer)
@@ -198,13 +203,20 @@ struct QMeta {
 template <int M>
 __global__ void __launch_bounds__(256) ivfpq_qtable_kernel(const float* __restrict__ xq, const float* __restrict__ pq,
                                                            const float* __restrict__ bmax, int d, int dsub,
-                                                           uint32_t* __restrict__ Tq, QMeta* __restrict__ meta) {
+                                                           uint32_t* __restrict__ Tq, QMeta* __restrict__ meta,
+                                                           int64_t nq, int qpb) {
   constexpr int REP = 32 / M;
   __shared__ float x[2048];
   __shared__ float bm[M];
   __shared__ float xn_s;
-  const int64_t q = blockIdx.x;
+  // the table is staged in shared memory (word o at o + o / 32: the stores of a warp -- 32 entries c of one m,
+  // 16 words apart -- fall in 32 different banks) and leaves in whole 128-byte lines; a block takes qpb queries
+  // one after the other, so that the codebook (M x 256 x dsub floats) is read from L2 once per block
+  __shared__ uint32_t stg[256 * M + 8 * M];
   const int tid = threadIdx.x, lane = tid & 31;
+  for (int qi = 0; qi < qpb; ++qi) {
+  const int64_t q = (int64_t)blockIdx.x * qpb + qi;
+  if (q >= nq) break;
   for (int j = tid; j < d; j += 256) x[j] = xq[q * d + j];
   __syncthreads();
   if (tid < 32) {  // warp 0: ||x^m|| for m = lane (< M), ||x||^2
@@ -240,7 +252,8 @@ __global__ void __launch_bounds__(256) ivfpq_qtable_kernel(const float* __restri
     float acc = 0.f;
     for (int j = 0; j < dsub; ++j) acc = fmaf(x[m * dsub + j], b[j], acc);
     const float t = -2.f * acc * scale + (float)bi[m];  // exact for integer-valued inputs
-    Tq[q * (256 * M) + (c / REP) * 32 + (c % REP) * M + m] = __float2uint_rn(fmaxf(t, 0.f));
+    const int o = (c / REP) * 32 + (c % REP) * M + m;
+    stg[o + (o >> 5)] = __float2uint_rn(fmaxf(t, 0.f));
   }
   if (tid == 0) {
     QMeta mt;
@@ -249,6 +262,10 @@ __global__ void __launch_bounds__(256) ivfpq_qtable_kernel(const float* __restri
     mt.xnorm = xn_s;
     mt.pad = 0.f;
     meta[q] = mt;
+  }
+  __syncthreads();
+  for (int o = tid; o < 256 * M; o += 256) Tq[q * (256 * M) + o] = stg[o + (o >> 5)];
+  __syncthreads();  // the next query overwrites x, bm and the staged table
   }
 }
 
@@ -746,9 +763,9 @@ int ivfpq_search_device(fs_ivfpq* ix, const float* xq, int64_t nq, int nprobe, i
     pq_bmax_kernel<<<ix->M, 32, 0, s>>>(a.pq, bmax, ix->dsub);
     FS_LAUNCHED();
     if (ix->M == 16)
-      ivfpq_qtable_kernel<16><<<(unsigned)nq, 256, 0, s>>>(xq, a.pq, bmax, ix->d, ix->dsub, Tq, meta);
+      ivfpq_qtable_kernel<16><<<(unsigned)ceil_div(nq, (int64_t)QT_QPB), 256, 0, s>>>(xq, a.pq, bmax, ix->d, ix->dsub, Tq, meta, nq, QT_QPB);
     else
-      ivfpq_qtable_kernel<8><<<(unsigned)nq, 256, 0, s>>>(xq, a.pq, bmax, ix->d, ix->dsub, Tq, meta);
+      ivfpq_qtable_kernel<8><<<(unsigned)ceil_div(nq, (int64_t)QT_QPB), 256, 0, s>>>(xq, a.pq, bmax, ix->d, ix->dsub, Tq, meta, nq, QT_QPB);
     FS_LAUNCHED();
 #define FS_QS(NQ)                                                                          \
   (ix->M == 16 ? launch_scan_q<NQ, 16>(a, nq, Tq, meta, work, s) : launch_scan_q<NQ, 8>(a, nq, Tq, meta, work, s))
