@@ -89,6 +89,8 @@ struct TcArgs {
   uint64_t* cbuf;              // [gridDim.x][EPI_GROUPS][BM][cap]: winners so far, then new candidates
   const unsigned int* lo_flag; // != 0: lo planes are not all zero (3xTF32)
   const unsigned int* nq_dev;  // != NULL: the number of queries, on the device (<= nq; re-run of the failed queries)
+  int lazy_final;              // != 0: the queues start from a sampled bound; a queue is not restored at the end of its
+                               // item just to publish its k-th distance (only if it holds more than K keys)
   float* dout;                 // != NULL: no selection, d'(q, j) = ||y_j||^2 - 2 <x_q, y_j> is written to
   int64_t dld;                 //          dout[q * dld + j] (dld % 4 == 0); the launch passes k = 1
 };
@@ -602,7 +604,11 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
       if (rq) {  // the thread's queue becomes the row's buffer
         for (int e = 0; e < cnt; ++e) cb[e] = Rq[e * 32];
       } else {
-        flush_rows(a.S > 1 ? cnt >= k : cnt > K, true);
+        // With a sampled bound every queue already starts tight and holds ~c nb / (ns 2 S) keys at the end, about k
+        // for k just above KREG: restoring half the rows of every warp (a radix selection plus three more for the
+        // hierarchical bounds, row after row) to publish bounds nobody needs cost 0.3 ms of a 1.3 ms search
+        // (nb = 65 536, k = 13 .. 16: slower than k = 64).  B4 takes up to K keys per queue as they are.
+        flush_rows((a.S > 1 && !a.lazy_final) ? cnt >= k : cnt > K, true);
       }
       __syncwarp();
       // the row's partial queue for B4 (unordered, sentinel padded), and this split's k-th
@@ -956,6 +962,7 @@ int flat_knn_tc_device(const float* xq, int64_t nq, const float* xb, int64_t nb,
     a.hclaim = reinterpret_cast<unsigned int*>(wr + pl.off_hclaim);
     a.cbuf = reinterpret_cast<uint64_t*>(wr + pl.off_cbuf);
     a.lo_flag = flag;
+    a.lazy_final = (p.ns > 0 && dout == nullptr && &pl == &p && nq_dev == nullptr) ? 1 : 0;  // main pass over a sampled bound
     a.nq_dev = nq_dev;
     a.dout = dout;
     a.dld = dld;
