@@ -517,9 +517,17 @@ int ivfpq_finalise(fs_ivfpq* ix, cudaStream_t s) {
 // ---------------------------------------------------------------------------
 // D1: nearest centroid (k = 1 exact search), in chunks that bound the workspace.
 // ---------------------------------------------------------------------------
+int ivfpq_prepare_coarse(fs_ivfpq* ix, cudaStream_t s) {
+  int rc = launch_row_norms(ix->coarse.as<float>(), ix->nlist, ix->d, ix->cnorm.as<float>(), s);
+  if (rc != FS_OK) return rc;
+  return flat_prepare_device(ix->coarse.as<float>(), ix->nlist, ix->d, ix->cprep.p, s);
+}
+
 int assign_nearest(const float* x, int64_t n, const float* cent, const float* cent_norm, int K,
-                   int d, int64_t* assign, cudaStream_t s) {
+                   int d, int64_t* assign, cudaStream_t s, const void* cent_prep) {
   if (n == 0) return FS_OK;
+  FlatPrep view;
+  if (cent_prep) view = flat_prep_view(cent_prep, K, d);
   const int64_t chunk = n < (1 << 20) ? n : (1 << 20);
   size_t need = flat_plan(chunk, K, d, 1).bytes;
   if (n % chunk != 0) {  // the smaller last chunk has its own plan
@@ -536,7 +544,7 @@ int assign_nearest(const float* x, int64_t n, const float* cent, const float* ce
   for (int64_t b = 0; b < n && rc == FS_OK; b += chunk) {
     const int64_t m = (n - b) < chunk ? (n - b) : chunk;
     rc = flat_knn_device(x + b * d, m, cent, K, d, 1, cent_norm, dist.as<float>(), assign + b,
-                         ws.p, s);
+                         ws.p, s, cent_prep ? &view : nullptr);
   }
   cudaStreamSynchronize(s);
   ws.release();
@@ -560,7 +568,7 @@ static int ivfpq_add_device(fs_ivfpq* ix, const float* xb, int64_t n, const int6
   DevBuf assign;
   if ((rc = assign.ensure((size_t)n * sizeof(int64_t), 0, s)) != FS_OK) return rc;
   rc = assign_nearest(xb, n, ix->coarse.as<float>(), ix->cnorm.as<float>(), ix->nlist, ix->d,
-                      assign.as<int64_t>(), s);
+                      assign.as<int64_t>(), s, ix->cprep.p);
   if (rc == FS_OK)
     rc = launch_pq_encode(ix, xb, n, assign.as<int64_t>(), ix->st_codes.as<uint8_t>() + base * M,
                           ix->st_list.as<uint32_t>() + base, ix->st_s1.as<float>() + base, s);
@@ -607,6 +615,7 @@ int fs_ivfpq_create(fs_ivfpq** out, int d, int nlist, int M) {
   int rc;
   if ((rc = ix->coarse.ensure((size_t)nlist * d * sizeof(float), 0, nullptr)) != FS_OK ||
       (rc = ix->cnorm.ensure((size_t)nlist * sizeof(float), 0, nullptr)) != FS_OK ||
+      (rc = ix->cprep.ensure(fs::flat_prep_bytes(nlist, d), 0, nullptr)) != FS_OK ||
       (rc = ix->pq.ensure((size_t)256 * d * sizeof(float), 0, nullptr)) != FS_OK ||
       (rc = ix->scanned.ensure(sizeof(unsigned long long), 0, nullptr)) != FS_OK) {
     fs_ivfpq_destroy(ix);
@@ -625,7 +634,7 @@ int fs_ivfpq_create(fs_ivfpq** out, int d, int nlist, int M) {
 int fs_ivfpq_destroy(fs_ivfpq* ix) {
   if (!ix) return FS_OK;
   cudaDeviceSynchronize();
-  fs::DevBuf* bufs[] = {&ix->coarse, &ix->cnorm, &ix->pq, &ix->offsets, &ix->codes, &ix->ids,
+  fs::DevBuf* bufs[] = {&ix->coarse, &ix->cnorm, &ix->cprep, &ix->pq, &ix->offsets, &ix->codes, &ix->ids,
                         &ix->st_list, &ix->st_codes, &ix->st_ids, &ix->scanned, &ix->s1, &ix->st_s1};
   for (fs::DevBuf* b : bufs) b->release();
   for (cudaEvent_t e : ix->ev)
@@ -642,7 +651,7 @@ int fs_ivfpq_set_quantizers(fs_ivfpq* ix, const float* coarse, const float* pq, 
   FS_CUDA(cudaMemcpyAsync(ix->coarse.p, coarse, (size_t)ix->nlist * ix->d * sizeof(float),
                           cudaMemcpyDeviceToDevice, s));
   FS_CUDA(cudaMemcpyAsync(ix->pq.p, pq, (size_t)256 * ix->d * sizeof(float), cudaMemcpyDeviceToDevice, s));
-  int rc = fs::launch_row_norms(ix->coarse.as<float>(), ix->nlist, ix->d, ix->cnorm.as<float>(), s);
+  int rc = fs::ivfpq_prepare_coarse(ix, s);
   if (rc != FS_OK) return rc;
   ix->have_quantizers = true;
   return FS_OK;

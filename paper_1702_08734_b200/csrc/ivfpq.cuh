@@ -30,6 +30,8 @@ struct fs_ivfpq {
   bool have_quantizers = false;
   fs::DevBuf coarse;  // [nlist][d] fp32
   fs::DevBuf cnorm;   // [nlist] fp32: ||c||^2 (B1 of the coarse search, precomputed)
+  fs::DevBuf cprep;   // the centroids as a prepared database of the exact search (flat.cuh FlatPrep: norms, lo flag,
+                      // lo plane), written whenever the centroids are: C1 and D1 skip that pass on every call
   fs::DevBuf pq;      // [M][256][dsub] fp32
   // Finalised inverted file, CSR over list number (codes and
   // ids in separate arrays, each list contiguous, append order kept).
@@ -81,7 +83,9 @@ int kmeans_device(const float* x, int64_t n, int d, int K, int niter, uint64_t s
                   cudaStream_t s, bool init = true, int64_t* assign_out = nullptr);
 // Nearest centroid of each x (k = 1 exact search, chunked): assign int64 [n].
 int assign_nearest(const float* x, int64_t n, const float* cent, const float* cent_norm, int K,
-                   int d, int64_t* assign, cudaStream_t s);
+                   int d, int64_t* assign, cudaStream_t s, const void* cent_prep = nullptr);
+// ||c||^2 and the prepared block of the index's centroids (after every change of them)
+int ivfpq_prepare_coarse(fs_ivfpq* ix, cudaStream_t s);
 
 int ivfpq_search_device(fs_ivfpq* ix, const float* xq, int64_t nq, int nprobe, int k,
                         float* out_dist, int64_t* out_ids, int32_t* out_probed, void* ws,

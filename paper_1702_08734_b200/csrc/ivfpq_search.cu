@@ -711,7 +711,8 @@ int ivfpq_search_device(fs_ivfpq* ix, const float* xq, int64_t nq, int nprobe, i
   int rc;
   ix->ev_valid = false;
   FS_CUDA(cudaEventRecord(ix->ev[0], s));
-  // C1
+  // C1 (the centroids are a prepared database: their norms and operand split were made when they were set)
+  const FlatPrep cview = flat_prep_view(ix->cprep.p, ix->nlist, ix->d);
   if (p.c1_chunk > 0) {
     float* D = reinterpret_cast<float*>(w + p.off_D);
     float* cval = reinterpret_cast<float*>(w + p.off_cval);
@@ -719,7 +720,7 @@ int ivfpq_search_device(fs_ivfpq* ix, const float* xq, int64_t nq, int nprobe, i
     for (int64_t q0 = 0; q0 < nq; q0 += p.c1_chunk) {
       const int64_t n = nq - q0 < p.c1_chunk ? nq - q0 : p.c1_chunk;
       rc = flat_knn_tc_device(xq + q0 * ix->d, n, ix->coarse.as<float>(), ix->nlist, ix->d, 1, nullptr, nullptr, w, s,
-                              D, p.c1_ld);
+                              D, p.c1_ld, &cview);
       if (rc != FS_OK) return rc;
       rc = kselect_device(D, n, ix->nlist, p.c1_ld, nprobe, cval, cidx, w + p.off_ksws, s, false);
       if (rc != FS_OK) return rc;
@@ -729,7 +730,7 @@ int ivfpq_search_device(fs_ivfpq* ix, const float* xq, int64_t nq, int nprobe, i
     }
   } else {
     rc = flat_knn_device(xq, nq, ix->coarse.as<float>(), ix->nlist, ix->d, nprobe,
-                         ix->cnorm.as<float>(), cdist, cids, w, s);
+                         ix->cnorm.as<float>(), cdist, cids, w, s, &cview);
     if (rc != FS_OK) return rc;
   }
   FS_CUDA(cudaEventRecord(ix->ev[1], s));

@@ -159,8 +159,7 @@ extern "C" int fs_ivfpq_train(fs_ivfpq* ix, const float* x, int64_t n, int niter
   const int d = ix->d, M = ix->M, dsub = ix->dsub;
   int rc = kmeans_device(x, n, d, ix->nlist, niter, seed, ix->coarse.as<float>(), s);
   if (rc != FS_OK) return rc;
-  if ((rc = launch_row_norms(ix->coarse.as<float>(), ix->nlist, d, ix->cnorm.as<float>(), s)) != FS_OK)
-    return rc;
+  if ((rc = ivfpq_prepare_coarse(ix, s)) != FS_OK) return rc;
   DevBuf assign, sub;
   if ((rc = assign.ensure((size_t)n * sizeof(int64_t), 0, s)) != FS_OK) return rc;
   if ((rc = sub.ensure((size_t)n * dsub * sizeof(float), 0, s)) != FS_OK) {
@@ -168,7 +167,7 @@ extern "C" int fs_ivfpq_train(fs_ivfpq* ix, const float* x, int64_t n, int niter
     return rc;
   }
   rc = assign_nearest(x, n, ix->coarse.as<float>(), ix->cnorm.as<float>(), ix->nlist, d,
-                      assign.as<int64_t>(), s);
+                      assign.as<int64_t>(), s, ix->cprep.p);
   for (int m = 0; m < M && rc == FS_OK; ++m) {
     residual_kernel<<<(unsigned)ceil_div(n * dsub, 256), 256, 0, s>>>(
         x, n, d, ix->coarse.as<float>(), assign.as<int64_t>(), m * dsub, dsub, sub.as<float>());
