@@ -119,7 +119,7 @@ def test_cfg3_shaped_integer_data_bit_exact(k):
     assert np.array_equal(gd.view(np.uint32), od.view(np.uint32))
 
 
-@pytest.mark.parametrize("k", [2, 10, 100, 1024])
+@pytest.mark.parametrize("k", [2, 10, 13, 16, 40, 100, 1024])
 def test_sampled_bound_integer_data_bit_exact(k):
     """Databases of >= 32 768 rows take the sampled bound of the tensor-core engine (DESIGN 5.2): a strided
     sample is searched first and its c-th distance bounds every queue.  Integer data: bit-exact.  The second
