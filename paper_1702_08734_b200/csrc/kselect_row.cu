@@ -72,6 +72,7 @@ struct RowArgs {
   int64_t n_rows, n, ld;
   int k;
   const unsigned int* len;  // per-row length (long rows: survivors of the filter pass) or NULL: n
+  const unsigned int* len_nan;  // with len: how many of them are NaN (they pass every bound)
   int64_t len_cap;          // rows with len[row] > len_cap or < min(k, n_orig) take the exact slow path on orig
   const uint32_t* map;      // [n_rows][ld] index of vals[row][i] in the original row, or NULL: i
   const float* orig;        // original rows (ties of +-0 / NaN re-read their bits here; slow path of mapped rows)
@@ -105,6 +106,7 @@ struct RowSharedBase {       // what the selection steps use
   unsigned int redu[2][RW];
   int cnt, ovf;              // candidates appended, overflow flag
   int kb, kept, maxc;        // counting step: boundary bucket, keys in buckets <= kb, largest such bucket
+  int nan_cnt;               // counting step: NaN keys among the candidates (counted only when rank k is in their bucket)
   unsigned long long thr_key;  // slow path: exact k-th key so far
   int wsum[RW];
 };
@@ -219,9 +221,14 @@ __device__ void block_bitonic(const RowCtx<CAPT>& c, int n2) {
 // filter wrote them (position in vals, translated through mp when the row is a survivor list);
 // otherwise keys.  lo / hi: value range of the map (have_range), else taken from the candidates.
 // The histogram must be zero on entry and is left dirty.  All consumer threads; ends with a barrier.
+// bounded: the candidates are what a bound let through, not the whole row.  NaN passes every bound (the
+// filters test "less than or unordered"), so m >= want does not yet mean that the `want` smallest keys of the
+// ROW are among the candidates: if fewer than `want` of them are real values, elements above the bound would
+// have come before the NaNs.  The step then returns false before it writes anything (the caller goes on to
+// its next, wider method); the check costs nothing unless rank `want` falls into the bucket NaN lives in.
 template <int CAPT, bool RESTORE, bool RAW>
-__device__ void count_select(const RowCtx<CAPT>& c, int64_t row, int m, int want, bool have_range, float lo, float hi,
-                             const uint32_t* mp) {
+__device__ bool count_select(const RowCtx<CAPT>& c, int64_t row, int m, int want, bool have_range, float lo, float hi,
+                             const uint32_t* mp, bool bounded = false) {
   constexpr int NBK = CAPT, BPT = NBK / RT;  // buckets per thread in the scan
   auto* s = c.s;
   const int tid = c.tid, lane = c.lane, warp = c.warp;
@@ -229,6 +236,7 @@ __device__ void count_select(const RowCtx<CAPT>& c, int64_t row, int m, int want
     s->kb = NBK - 1;
     s->kept = m;
     s->maxc = 0;
+    s->nan_cnt = 0;
   }
   // The passes below are issue-bound, not latency-bound (three CTAs per SM overlap them): U > 1 keys per
   // thread in flight was measured 7 % (U = 2) and 27 % (U = 4) slower at k = 1 024.
@@ -345,6 +353,14 @@ __device__ void count_select(const RowCtx<CAPT>& c, int64_t row, int m, int want
     if (lane == 0 && mxc > 0) atomicMax(&s->maxc, (int)mxc);
   }
   cbar();
+  if (bounded && s->kb == NBK - 1) {  // (uniform) rank `want` is in the last bucket: count the NaN keys
+    int nn = 0;
+    for (int i = tid; i < m; i += RT) nn += (uint32_t)(c.cand[i] >> 32) == 0xFFFFFFFFu ? 1 : 0;
+    nn = __reduce_add_sync(kFull, nn);
+    if (lane == 0 && nn) atomicAdd(&s->nan_cnt, nn);
+    cbar();
+    if (m - s->nan_cnt < want) return false;
+  }
   // 3. scatter the keys of the buckets up to the boundary one, grouped by bucket
   const int kb = s->kb, kept = s->kept;
   for (int i0 = tid; i0 < m; i0 += U * RT) {
@@ -424,6 +440,7 @@ __device__ void count_select(const RowCtx<CAPT>& c, int64_t row, int m, int want
     }
   }
   cbar();
+  return true;
 }
 
 template <int CAPT>
@@ -668,7 +685,9 @@ __global__ void __launch_bounds__(RTHREADS, RowCfg<CAPT, AL>::CTAS) kselect_row_
       if (a.len) {
         const int64_t l = (int64_t)a.len[row];
         const int64_t need = (int64_t)a.k < a.n_orig ? a.k : a.n_orig;
-        if (l > a.len_cap || l < need) {
+        // NaNs pass the long-row bound too: only the real values of the list count towards the k it must hold
+        const int64_t real = l - (a.len_nan ? (int64_t)a.len_nan[row] : 0);
+        if (l > a.len_cap || real < need) {
           fallback = 1;
           len = 0;
         } else {
@@ -878,13 +897,25 @@ __global__ void __launch_bounds__(RTHREADS, RowCfg<CAPT, AL>::CTAS) kselect_row_
           fell_back = true;
         }
       }
-      if (fell_back) {
-      } else if (s->ovf || m < want || m > CAPT) {
-        // The sample (the head of the row) did not represent the row: sorted rows, runs of equal values.
+      // One counting step over what a bound let through.  It refuses (false, nothing written) when the
+      // candidates hold fewer than `want` real values and NaNs -- which pass every bound -- made up the number;
+      // the histogram it leaves behind is cleared before the next attempt.
+      bool done = false, dirty = false;
+      auto select = [&](int mm, bool have_range, float lo, float hi, bool bounded) {
+        if (dirty) {
+          zero_hist<CAPT>(c);
+          cbar();
+        }
+        dirty = true;
+        return count_select<CAPT, false, true>(c, row, mm, want, have_range, lo, hi, mp, bounded);
+      };
+      if (!fell_back && !(s->ovf || m < want || m > CAPT))
+        done = select(m, bd.sampled != 0, bd.lo, bd.hi, bd.sampled != 0);
+      if (!fell_back && !done) {
+        // The sample (the head of the row) did not represent the row: sorted rows, runs of equal values, NaNs.
         // Second look: a STRIDED sample of the row (it is in L2) searched the same way, one more filter pass
         // with its bound; then, if the first bound spanned a range, two passes with that bound rescaled by
         // what the pass before counted; then the paper's scheme, which needs nothing from the distribution.
-        bool done = false;
         {
           const int S2 = (CAPT >= 2048 && len > 32768) ? 4096 : 2048;  // what scout_bound takes from 2 CAPT floats
           const int64_t stride = len / S2;
@@ -901,10 +932,7 @@ __global__ void __launch_bounds__(RTHREADS, RowCfg<CAPT, AL>::CTAS) kselect_row_
             if (b2.sampled) {
               refilter_row<CAPT>(c, p, len, b2.thr_x);
               const int m2 = s->cnt;
-              if (m2 >= want && m2 <= CAPT) {
-                count_select<CAPT, false, true>(c, row, m2, want, true, b2.lo, b2.hi, mp);
-                done = true;
-              }
+              if (m2 >= want && m2 <= CAPT) done = select(m2, true, b2.lo, b2.hi, true);
             }
           }
         }
@@ -917,15 +945,10 @@ __global__ void __launch_bounds__(RTHREADS, RowCfg<CAPT, AL>::CTAS) kselect_row_
             hi = bd.lo + (hi - bd.lo) * f;  // along the line through (lo, 0) and (hi, seen)
             refilter_row<CAPT>(c, p, len, ord_f32(f32_ord(hi) + 1u));
             seen = s->cnt;
-            if (seen >= want && seen <= CAPT) {
-              count_select<CAPT, false, true>(c, row, seen, want, false, 0.f, 0.f, mp);
-              done = true;
-            }
+            if (seen >= want && seen <= CAPT) done = select(seen, false, 0.f, 0.f, true);
           }
         }
         if (!done) slow_row<CAPT>(c, row, p, len, mp);
-      } else {
-        count_select<CAPT, false, true>(c, row, m, want, bd.sampled != 0, bd.lo, bd.hi, mp);
       }
       if (tid == 0) {
         s->cnt = 0;
@@ -1043,7 +1066,8 @@ template <bool LG>
 __global__ void __launch_bounds__(LF_THREADS) kselect_filter_kernel(const float* __restrict__ rows, int64_t n, int64_t ld,
                                                                      const float* __restrict__ thr,
                                                                      float* __restrict__ cval, uint32_t* __restrict__ cidx,
-                                                                     unsigned int* __restrict__ count, int64_t cap) {
+                                                                     unsigned int* __restrict__ count,
+                                                                     unsigned int* __restrict__ nan_count, int64_t cap) {
   const int64_t row = blockIdx.y;
   const float* p = rows + row * ld;
   const float thr_x = thr[row];
@@ -1051,6 +1075,7 @@ __global__ void __launch_bounds__(LF_THREADS) kselect_filter_kernel(const float*
   uint32_t* ci = cidx + row * cap;
   auto take = [&](float v, int64_t e) {
     if (!(fl<LG>(v) >= thr_x)) {
+      if (v != v) atomicAdd(nan_count + row, 1u);
       const unsigned int pos = atomicAdd(count + row, 1u);
       if ((int64_t)pos < cap) {
         cv[pos] = v;
@@ -1167,7 +1192,7 @@ size_t kselect_rows_ws_bytes(int64_t n_rows, int64_t n, int k) {
   size_t b = 256;  // work counter
   if (kselect_use_long(n_rows, n, k)) {
     const int64_t cap = kselect_long_cap(n, k);
-    b += align_up((size_t)n_rows * sizeof(float), 256) + align_up((size_t)n_rows * sizeof(unsigned int), 256) +
+    b += align_up((size_t)n_rows * sizeof(float), 256) + 2 * align_up((size_t)n_rows * sizeof(unsigned int), 256) +
          align_up((size_t)n_rows * cap * sizeof(float), 256) + align_up((size_t)n_rows * cap * sizeof(uint32_t), 256);
   }
   return b;
@@ -1184,6 +1209,7 @@ int kselect_rows_device(const float* rows, int64_t n_rows, int64_t n, int64_t ld
   a.ld = ld;
   a.k = k;
   a.len = nullptr;
+  a.len_nan = nullptr;
   a.len_cap = 0;
   a.map = nullptr;
   a.orig = rows;
@@ -1203,11 +1229,13 @@ int kselect_rows_device(const float* rows, int64_t n_rows, int64_t n, int64_t ld
   o += align_up((size_t)n_rows * sizeof(float), 256);
   unsigned int* count = reinterpret_cast<unsigned int*>(w + o);
   o += align_up((size_t)n_rows * sizeof(unsigned int), 256);
+  unsigned int* nan_count = reinterpret_cast<unsigned int*>(w + o);
+  o += align_up((size_t)n_rows * sizeof(unsigned int), 256);
   float* cval = reinterpret_cast<float*>(w + o);
   o += align_up((size_t)n_rows * cap * sizeof(float), 256);
   uint32_t* cidx = reinterpret_cast<uint32_t*>(w + o);
   FS_CUDA(cudaMemsetAsync(w, 0, 256 + align_up((size_t)n_rows * sizeof(float), 256) +
-                                    align_up((size_t)n_rows * sizeof(unsigned int), 256), s));
+                                    2 * align_up((size_t)n_rows * sizeof(unsigned int), 256), s));
   auto* sample = largest ? kselect_sample_kernel<true> : kselect_sample_kernel<false>;
   FS_CUDA(cudaFuncSetAttribute(sample, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSampleSmem));  // per device
   sample<<<(unsigned)n_rows, 1024, kSampleSmem, s>>>(rows, n, ld, k, thr);
@@ -1217,12 +1245,13 @@ int kselect_rows_device(const float* rows, int64_t n_rows, int64_t n, int64_t ld
   if (gx > maxg) gx = maxg;
   if (gx < 1) gx = 1;
   auto* filter = largest ? kselect_filter_kernel<true> : kselect_filter_kernel<false>;
-  filter<<<dim3((unsigned)gx, (unsigned)n_rows), LF_THREADS, 0, s>>>(rows, n, ld, thr, cval, cidx, count, cap);
+  filter<<<dim3((unsigned)gx, (unsigned)n_rows), LF_THREADS, 0, s>>>(rows, n, ld, thr, cval, cidx, count, nan_count, cap);
   FS_LAUNCHED();
   a.vals = cval;
   a.ld = cap;
   a.n = cap;
   a.len = count;
+  a.len_nan = nan_count;
   a.len_cap = cap;
   a.map = cidx;
   return launch_rows(a, s);

@@ -140,6 +140,13 @@ def test_stage_boundaries_of_the_k1024_class(n):
     big[5, :] = 0.25                                    # constant: everything ties
     big[6, :] = np.floor(big[6, :] * 4)                 # four distinct values
     big[7, :n // 2] += 2.0                              # the small values come late
+    big[8, ::3] = 0.0                                   # +-0, infinities and NaN in rows of this class
+    big[8, 1::3] = -0.0
+    big[9, ::5] = np.inf
+    big[10, ::4] = -np.inf
+    big[11, :] = np.inf
+    big[12, 100:1500] = np.nan
+    big[13, :] = np.nan
     t = torch.from_numpy(big).cuda()
     for off in (0, 1):
         view = t[:, off:off + n]
@@ -150,6 +157,35 @@ def test_stage_boundaries_of_the_k1024_class(n):
             ev, ei = oracle.kselect(host, k)
             assert np.array_equal(gi.cpu().numpy(), ei), (n, off, k)
             assert np.array_equal(gv.cpu().numpy().view(np.uint32), ev.view(np.uint32)), (n, off, k)
+
+
+@pytest.mark.parametrize("k", [2, 100, 300, 1024])
+def test_rows_with_many_nans(k):
+    """NaN sorts last but passes every bound (the filters test "less than or unordered"): a row whose
+    candidates reach k only through NaNs must not be answered from them.  Blocks of NaN in the sampled head,
+    NaN scattered through the row, rows with fewer than k real values (there NaNs do belong in the output),
+    at row lengths of every class, and as long rows (A4)."""
+    rng = np.random.default_rng(k)
+    for n in (700, 5000, 8191, 16384, 40000):
+        rows = rng.random((12, n), dtype=np.float32)
+        rows[0, 100:100 + n // 6] = np.nan          # a block inside the head the scout samples
+        rows[1, : n // 2] = np.nan                  # the whole head
+        rows[2, ::3] = np.nan                       # scattered
+        rows[3, 10:] = np.nan                       # ten real values
+        rows[4, : n - 1500] = np.nan                # 1 500 real values at the end
+        rows[5, :] = np.nan
+        rows[6, n // 3:] = np.nan                   # NaN tail
+        rows[7, ::2] = np.inf
+        rows[7, 1::4] = np.nan
+        rows = np.concatenate([rows, rng.random((300, n), dtype=np.float32)])   # and a GPU's worth of plain rows
+        assert_exact(rows, k)
+    n = 1 << 19
+    long = rng.random((4, n), dtype=np.float32)
+    long[0, 1000:200000] = np.nan
+    long[1, ::3] = np.nan
+    long[2, 700:] = np.nan
+    long[3, : n - 5000] = np.nan
+    assert_exact(long, k)
 
 
 def assert_exact_largest(rows_np, k, n=None):
