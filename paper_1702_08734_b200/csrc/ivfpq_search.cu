@@ -188,10 +188,7 @@ __global__ void pq_bmax_kernel(const float* __restrict__ pq, float* __restrict__
 // (c % REP) * M + m, REP = 32 / M, so that a warp reads 32 consecutive words and its stores of the
 // replicated table are conflict-free.
 // ---------------------------------------------------------------------------
-#ifndef FS_QT_QPB
-#define FS_QT_QPB 8
-#endif
-constexpr int QT_QPB = FS_QT_QPB;  // queries per block of ivfpq_qtable_kernel
+constexpr int QT_QPB = 8;  // queries per block of ivfpq_qtable_kernel
 
 struct QMeta {
   float inv_scale;  // 2^-se

@@ -1154,14 +1154,9 @@ int launch_rows_t(const RowArgs& a, cudaStream_t s) {
 template <bool LG>
 int launch_rows_l(const RowArgs& a, cudaStream_t s) {
   if (a.map) return launch_rows_t<4096, false, LG>(a, s);  // one CTA per long row: room for a wide window
-  static int al = -1;  // FS_KSELECT_ALIAS=0: the classes with counting arrays of their own (A/B runs, tests)
-  if (al < 0) {
-    const char* e = getenv("FS_KSELECT_ALIAS");
-    al = (e && e[0] == '0') ? 0 : 1;
-  }
   if (a.k <= 256) return launch_rows_t<1024, false, LG>(a, s);
   // two held stages: every row must span at least two (head and tail scalars are at most 6 elements)
-  const bool two = al && a.n >= 2 * (int64_t)RowCfg<2048, true>::SEG;
+  const bool two = a.n >= 2 * (int64_t)RowCfg<2048, true>::SEG;
   return two ? launch_rows_t<2048, true, LG>(a, s) : launch_rows_t<2048, false, LG>(a, s);
 }
 
