@@ -73,8 +73,10 @@ FS_API void fs_reset_launch_count(void);
  * k-selection (WarpSelect, section 4.2; k = 1 is a
  * reduction; long rows by decomposition).
  * For each of n_rows arrays [a_i], i = 0..n-1, the k lowest values ascending
- * with their indices; ties broken by lower index, -0 == +0, NaN (not expected)
- * orders after +INF.  Bit-exact: out_val holds the original fp32 bits.
+ * with their indices; ties broken by lower index, -0 == +0, NaN orders after
+ * +INF (a NaN is returned only when fewer than k other values exist; rows with many
+ * NaNs are answered exactly but by slower passes).  Bit-exact: out_val holds the
+ * original fp32 bits.
  *   rows     device fp32 [n_rows][ld], row-major, ld >= n
  *   out_val  device fp32 [n_rows][k];  out_idx device int32 [n_rows][k]
  *   1 <= k <= FS_MAX_K; n < 2^31; k > n pads with (+INF, -1).
